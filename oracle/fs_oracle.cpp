@@ -1,0 +1,703 @@
+// fs_oracle.cpp -- CPU ORACLE (test infrastructure, NOT the product; see fs_oracle.h).
+//
+// Plain single-threaded fp64 restatement of one fractional step of Diff-FlowFSI's fluid solver
+// (section 2.3.1, Eq. 4-10) with marker-based direct-forcing IBM (Eq. 3, 5, 20-22) and
+// the rigid-body oscillator (Eq. 12), following SURVEY.md 8(c) steps O1..O9 in that order.
+// Triple loops, explicit index wrapping, sums in index order, no blocking / fusion / threads.
+// Compile: g++ -O2 -ffp-contract=off (no FMA contraction, so index arithmetic is reproducible).
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): P1..P15 of SURVEY.md 8(c).
+// Parity unpinned (readings of formulas the paper does not give):
+//   convective outflow update, outflow flux correction, inflow noise  -- only mass balance is pinned.
+#include "fs_oracle.h"
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include <algorithm>
+
+typedef std::vector<double> vec;
+
+struct orc_sim {
+  orc_params P;
+  int nx, ny, nz, bx, by, bz;          // bounded flags
+  int nxu, nyv, nzw;                   // stored extent of each component along its own normal
+  double hx, hy, hz;
+  bool uniform_y;
+  vec yf, dy, yc;                      // faces (ny+1), cell heights (ny), centres (ny)
+  vec u, v, w, p, hu, hv, hw, divu;
+  bool have_hist; long long step;
+  // markers (always fp64)
+  int nl; vec X, Ub, dV, Fl, Ul;       // positions, target vel, volumes, force, interpolated vel
+  std::vector<int> base, perm, keys, seg; int nseg;
+  // body (Eq. 12)
+  bool has_body; double bm, bc_, bk; int dof; double bdisp[3], bvel[3], bforce[3];
+  // GMG levels
+  int nlev;
+};
+
+static inline int wrapi(int i, int n) { i %= n; return i < 0 ? i + n : i; }
+
+// ---- grid metrics (SURVEY 8(c) "Grid") -------------------------------------------------
+// DY(j) for j in [-1, ny]: mirrored ghost at a bounded end, wrapped when periodic.
+static inline double DY(const orc_sim* s, int j) {
+  if (j < 0)       return s->by ? s->dy[0]         : s->dy[wrapi(j, s->ny)];
+  if (j >= s->ny)  return s->by ? s->dy[s->ny - 1] : s->dy[wrapi(j, s->ny)];
+  return s->dy[j];
+}
+// distance between centres j-1 and j (across face j), j in [0, ny]
+static inline double DYC(const orc_sim* s, int j) { return 0.5 * (DY(s, j - 1) + DY(s, j)); }
+
+// ---- O1: velocity access with boundary rules ----------------------------------------------
+// comp c (0=u,1=v,2=w); index (i,j,k) may be one layer outside in a tangential direction.
+// Periodic: wrap.  Own normal direction, bounded: faces 0..n are stored.  Tangential, bounded:
+// ghost = A*interior + B  with  no-slip/inflow: (-1, 2*bc_vel)  slip/outflow: (+1, 0).
+static double getvel(const orc_sim* s, const vec& f, int c, int i, int j, int k) {
+  const int n[3] = {s->nx, s->ny, s->nz};
+  const int bd[3] = {s->bx, s->by, s->bz};
+  int idx[3] = {i, j, k};
+  double A = 1.0, B = 0.0;
+  for (int d = 0; d < 3; ++d) {
+    if (!bd[d]) { idx[d] = wrapi(idx[d], n[d]); continue; }
+    if (d == c) continue;                       // stored 0..n
+    int face = -1;
+    if (idx[d] < 0)       { face = 2 * d;     idx[d] = -1 - idx[d]; }
+    else if (idx[d] >= n[d]) { face = 2 * d + 1; idx[d] = 2 * n[d] - 1 - idx[d]; }
+    if (face >= 0) {
+      int t = s->P.bc[face];
+      if (t == ORC_BC_NOSLIP || t == ORC_BC_INFLOW) { B = B * -1.0 + 2.0 * s->P.bc_vel[face][c]; A = -A; }
+      // slip / outflow: zero gradient, A,B unchanged
+    }
+  }
+  int ex = s->nx + (c == 0 ? s->bx : 0), ey = s->ny + (c == 1 ? s->by : 0);
+  return A * f[(size_t)idx[0] + (size_t)ex * (idx[1] + (size_t)ey * idx[2])] + B;
+}
+#define U_(i,j,k) getvel(s, uu, 0, i, j, k)
+#define V_(i,j,k) getvel(s, vv, 1, i, j, k)
+#define W_(i,j,k) getvel(s, ww, 2, i, j, k)
+
+static inline size_t IU(const orc_sim* s, int i, int j, int k) { return (size_t)i + (size_t)s->nxu * (j + (size_t)s->ny * k); }
+static inline size_t IV(const orc_sim* s, int i, int j, int k) { return (size_t)i + (size_t)s->nx * (j + (size_t)s->nyv * k); }
+static inline size_t IW(const orc_sim* s, int i, int j, int k) { return (size_t)i + (size_t)s->nx * (j + (size_t)s->ny * k); }
+static inline size_t IP(const orc_sim* s, int i, int j, int k) { return (size_t)i + (size_t)s->nx * (j + (size_t)s->ny * k); }
+
+// linear interpolation in y to face jf from centre values a (at jf-1) and b (at jf)   [O2]
+static inline double interpY(const orc_sim* s, double a, double b, int jf) {
+  double dm = DY(s, jf - 1), dp = DY(s, jf);
+  return (dp * a + dm * b) / (dm + dp);
+}
+
+// ---- O2: momentum right-hand side H = -C + nu*Lap(u) + g -----------------------------------
+// (Eq. 4: divergence form; central convection and diffusion, L100)
+static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& ww,
+                     double nu, const double g[3], vec& HU, vec& HV, vec& HW) {
+  const int nx = s->nx, ny = s->ny, nz = s->nz;
+  const double hx = s->hx, hz = s->hz;
+  std::fill(HU.begin(), HU.end(), 0.0); std::fill(HV.begin(), HV.end(), 0.0); std::fill(HW.begin(), HW.end(), 0.0);
+  // u faces (boundary-normal faces i=0, nx of a bounded direction are prescribed, not advanced)
+  for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = s->bx; i < nx; ++i) {
+    double uc = U_(i, j, k);
+    double ue = 0.5 * (uc + U_(i + 1, j, k)), uw = 0.5 * (U_(i - 1, j, k) + uc);
+    double cx = (ue * ue - uw * uw) / hx;
+    double vn = 0.5 * (V_(i - 1, j + 1, k) + V_(i, j + 1, k)), un = interpY(s, uc, U_(i, j + 1, k), j + 1);
+    double vs = 0.5 * (V_(i - 1, j, k) + V_(i, j, k)),         us = interpY(s, U_(i, j - 1, k), uc, j);
+    double cy = (vn * un - vs * us) / s->dy[j];
+    double wt = 0.5 * (W_(i - 1, j, k + 1) + W_(i, j, k + 1)), ut = 0.5 * (uc + U_(i, j, k + 1));
+    double wb = 0.5 * (W_(i - 1, j, k) + W_(i, j, k)),         ub = 0.5 * (U_(i, j, k - 1) + uc);
+    double cz = (wt * ut - wb * ub) / hz;
+    double dxx = (U_(i + 1, j, k) - 2.0 * uc + U_(i - 1, j, k)) / (hx * hx);
+    double dyy = ((U_(i, j + 1, k) - uc) / DYC(s, j + 1) - (uc - U_(i, j - 1, k)) / DYC(s, j)) / s->dy[j];
+    double dzz = (U_(i, j, k + 1) - 2.0 * uc + U_(i, j, k - 1)) / (hz * hz);
+    HU[IU(s, i, j, k)] = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + g[0];
+  }
+  // v faces (control volume between y_c(j-1) and y_c(j), height DYC(j))
+  for (int k = 0; k < nz; ++k) for (int j = s->by; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+    double vc = V_(i, j, k);
+    double ue = interpY(s, U_(i + 1, j - 1, k), U_(i + 1, j, k), j), ve = 0.5 * (vc + V_(i + 1, j, k));
+    double uw = interpY(s, U_(i, j - 1, k), U_(i, j, k), j),         vw = 0.5 * (V_(i - 1, j, k) + vc);
+    double cx = (ue * ve - uw * vw) / hx;
+    double vn = 0.5 * (vc + V_(i, j + 1, k)), vs = 0.5 * (V_(i, j - 1, k) + vc);
+    double cy = (vn * vn - vs * vs) / DYC(s, j);
+    double wt = interpY(s, W_(i, j - 1, k + 1), W_(i, j, k + 1), j), vt = 0.5 * (vc + V_(i, j, k + 1));
+    double wb = interpY(s, W_(i, j - 1, k), W_(i, j, k), j),         vb = 0.5 * (V_(i, j, k - 1) + vc);
+    double cz = (wt * vt - wb * vb) / hz;
+    double dxx = (V_(i + 1, j, k) - 2.0 * vc + V_(i - 1, j, k)) / (hx * hx);
+    double dyy = ((V_(i, j + 1, k) - vc) / DY(s, j) - (vc - V_(i, j - 1, k)) / DY(s, j - 1)) / DYC(s, j);
+    double dzz = (V_(i, j, k + 1) - 2.0 * vc + V_(i, j, k - 1)) / (hz * hz);
+    HV[IV(s, i, j, k)] = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + g[1];
+  }
+  // w faces
+  for (int k = s->bz; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+    double wc = W_(i, j, k);
+    double ue = 0.5 * (U_(i + 1, j, k - 1) + U_(i + 1, j, k)), we = 0.5 * (wc + W_(i + 1, j, k));
+    double uw = 0.5 * (U_(i, j, k - 1) + U_(i, j, k)),         wwst = 0.5 * (W_(i - 1, j, k) + wc);
+    double cx = (ue * we - uw * wwst) / hx;
+    double vn = 0.5 * (V_(i, j + 1, k - 1) + V_(i, j + 1, k)), wn = interpY(s, wc, W_(i, j + 1, k), j + 1);
+    double vs = 0.5 * (V_(i, j, k - 1) + V_(i, j, k)),         ws = interpY(s, W_(i, j - 1, k), wc, j);
+    double cy = (vn * wn - vs * ws) / s->dy[j];
+    double wt = 0.5 * (wc + W_(i, j, k + 1)), wb = 0.5 * (W_(i, j, k - 1) + wc);
+    double cz = (wt * wt - wb * wb) / hz;
+    double dxx = (W_(i + 1, j, k) - 2.0 * wc + W_(i - 1, j, k)) / (hx * hx);
+    double dyy = ((W_(i, j + 1, k) - wc) / DYC(s, j + 1) - (wc - W_(i, j - 1, k)) / DYC(s, j)) / s->dy[j];
+    double dzz = (W_(i, j, k + 1) - 2.0 * wc + W_(i, j, k - 1)) / (hz * hz);
+    HW[IW(s, i, j, k)] = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + g[2];
+  }
+}
+
+// ---- counter-based inflow noise (O1; the GPU path implements the same generator independently) --
+static inline uint64_t sm64(uint64_t z) {
+  z += 0x9E3779B97F4A7C15ULL;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  return z ^ (z >> 31);
+}
+extern "C" double orc_inflow_rand(uint64_t seed, long long step, int face, int a, int b) {
+  uint64_t h = sm64(seed + 0x632BE59BD9B4E019ULL * (uint64_t)(face + 1));
+  h = sm64(h + (uint64_t)step);
+  h = sm64(h + (((uint64_t)(uint32_t)b << 32) | (uint64_t)(uint32_t)a));
+  return (double)(h >> 11) * (1.0 / 9007199254740992.0);   // [0,1), exact
+}
+
+// ---- O3 (boundary part): prescribed boundary-normal faces of the predicted field -------------
+// us/vs/ws hold u~; un* hold u^n (needed by the convective outflow update).
+static void set_boundary_normal(const orc_sim* s, vec& us, vec& vs, vec& ws,
+                                const vec& un, const vec& vn, const vec& wn) {
+  const int n[3] = {s->nx, s->ny, s->nz};
+  const int bd[3] = {s->bx, s->by, s->bz};
+  const double h[3] = {s->hx, s->hy, s->hz};
+  for (int d = 0; d < 3; ++d) {
+    if (!bd[d]) continue;
+    vec& dst = d == 0 ? us : d == 1 ? vs : ws;
+    const vec& old = d == 0 ? un : d == 1 ? vn : wn;
+    int d1 = (d + 1) % 3, d2 = (d + 2) % 3;           // tangential directions
+    if (d1 > d2) std::swap(d1, d2);                   // (a,b) = lower, higher axis
+    for (int side = 0; side < 2; ++side) {
+      int face = 2 * d + side, t = s->P.bc[face];
+      int fidx = side ? n[d] : 0, inner = side ? n[d] - 1 : 1;
+      double Ub = s->P.bc_vel[face][d];
+      for (int b = 0; b < n[d2]; ++b) for (int a = 0; a < n[d1]; ++a) {
+        int id[3], in[3]; id[d] = fidx; id[d1] = a; id[d2] = b; in[d] = inner; in[d1] = a; in[d2] = b;
+        size_t q, qi;
+        if (d == 0) { q = IU(s, id[0], id[1], id[2]); qi = IU(s, in[0], in[1], in[2]); }
+        else if (d == 1) { q = IV(s, id[0], id[1], id[2]); qi = IV(s, in[0], in[1], in[2]); }
+        else { q = IW(s, id[0], id[1], id[2]); qi = IW(s, in[0], in[1], in[2]); }
+        double val;
+        if (t == ORC_BC_NOSLIP) val = Ub;
+        else if (t == ORC_BC_SLIP) val = 0.0;
+        else if (t == ORC_BC_INFLOW) {
+          double r = orc_inflow_rand(s->P.seed, s->step, face, a, b);
+          val = Ub * (1.0 + s->P.inflow_noise * (2.0 * r - 1.0));
+        } else {  // convective outflow (reading): d(u)/dt + Uc d(u)/dn = 0, first-order upwind
+          double dn = d == 1 ? (side ? s->dy[s->ny - 1] : s->dy[0]) : h[d];
+          double grad = side ? (old[q] - old[qi]) / dn : (old[qi] - old[q]) / dn;
+          val = old[q] - Ub * s->P.dt * grad;
+        }
+        dst[q] = val;
+      }
+    }
+  }
+}
+
+// ---- O4: IBM -----------------------------------------------------------------------------------
+// 1-D kernels with h factored out.  Roma 3-point and the paper's 4-point Eq. 22 (L204).
+extern "C" double orc_delta_phi(int kind, double r) {
+  double a = std::fabs(r);
+  if (kind == ORC_DELTA_ROMA3) {
+    if (a <= 0.5) return (1.0 + std::sqrt(1.0 - 3.0 * a * a)) / 3.0;
+    if (a <= 1.5) { double q = 1.0 - a; return (5.0 - 3.0 * a - std::sqrt(1.0 - 3.0 * q * q)) / 6.0; }
+    return 0.0;
+  }
+  if (a <= 1.0) return (3.0 - 2.0 * a + std::sqrt(1.0 + 4.0 * a - 4.0 * a * a)) / 8.0;
+  if (a <= 2.0) return (5.0 - 2.0 * a - std::sqrt(-7.0 + 12.0 * a - 4.0 * a * a)) / 8.0;
+  return 0.0;
+}
+
+// node offset of component c along direction d: faces for d==c, centres otherwise
+static inline double node_origin(const orc_sim* s, int c, int d) {
+  const double o[3] = {s->P.x0, s->P.y0, s->P.z0}, h[3] = {s->hx, s->hy, s->hz};
+  return d == c ? o[d] : o[d] + 0.5 * h[d];
+}
+static inline int support_width(const orc_sim* s) { return s->P.delta == ORC_DELTA_ROMA3 ? 3 : 4; }
+
+// I-1: scaled coordinate and lowest support index (operations individually rounded; build uses
+// -ffp-contract=off so no FMA is formed).
+static inline double scaled_coord(const orc_sim* s, double X, int c, int d) {
+  const double inv[3] = {1.0 / s->hx, 1.0 / s->hy, 1.0 / s->hz};
+  double t = X - node_origin(s, c, d);
+  return t * inv[d];
+}
+static inline int support_base(const orc_sim* s, double sc) {
+  if (s->P.delta == ORC_DELTA_ROMA3) { double q = sc + 0.5; return (int)std::floor(q) - 1; }
+  return (int)std::floor(sc) - 1;
+}
+// map a support node index to a storage index, or -1 if it must be skipped:
+// periodic: wrap; bounded face-located: only interior faces 1..n-1; bounded centre-located: 0..n-1
+static inline int node_index(const orc_sim* s, int m, int c, int d) {
+  const int n[3] = {s->nx, s->ny, s->nz}; const int bd[3] = {s->bx, s->by, s->bz};
+  if (!bd[d]) return wrapi(m, n[d]);
+  if (d == c) return (m >= 1 && m <= n[d] - 1) ? m : -1;
+  return (m >= 0 && m <= n[d] - 1) ? m : -1;
+}
+
+extern "C" void orc_ibm_index(orc_sim* s) {
+  const int nl = s->nl;
+  const int n[3] = {s->nx, s->ny, s->nz}; const int bd[3] = {s->bx, s->by, s->bz};
+  const double o[3] = {s->P.x0, s->P.y0, s->P.z0};
+  const double inv[3] = {1.0 / s->hx, 1.0 / s->hy, 1.0 / s->hz};
+  s->base.assign((size_t)9 * nl, 0); s->keys.assign(nl, 0); s->perm.assign(nl, 0);
+  std::vector<int> key_of(nl);
+  for (int l = 0; l < nl; ++l) {
+    for (int c = 0; c < 3; ++c) for (int d = 0; d < 3; ++d)
+      s->base[((size_t)c * nl + l) * 3 + d] = support_base(s, scaled_coord(s, s->X[3 * l + d], c, d));
+    int ic[3];
+    for (int d = 0; d < 3; ++d) {
+      double t = s->X[3 * l + d] - o[d];
+      int q = (int)std::floor(t * inv[d]);
+      ic[d] = bd[d] ? std::min(std::max(q, 0), n[d] - 1) : wrapi(q, n[d]);
+    }
+    key_of[l] = ic[0] + s->nx * (ic[1] + s->ny * ic[2]);
+    s->perm[l] = l;
+  }
+  std::stable_sort(s->perm.begin(), s->perm.end(), [&](int a, int b) { return key_of[a] < key_of[b]; });
+  s->seg.assign(nl + 1, 0); s->nseg = 0;
+  for (int r = 0; r < nl; ++r) {
+    s->keys[r] = key_of[s->perm[r]];
+    if (r == 0 || s->keys[r] != s->keys[r - 1]) s->seg[s->nseg++] = r;
+  }
+  s->seg[s->nseg] = nl;
+}
+
+// weight of support node (a,b,cc) offsets for marker l / component c; returns storage index or -1
+static inline long long ibm_node(const orc_sim* s, int l, int c, int a, int b, int cc, double* wgt) {
+  int off[3] = {a, b, cc}, id[3]; double wt = 1.0;
+  for (int d = 0; d < 3; ++d) {
+    double sc = scaled_coord(s, s->X[3 * l + d], c, d);
+    int m = s->base[((size_t)c * s->nl + l) * 3 + d] + off[d];
+    double r = sc - (double)m;
+    wt *= orc_delta_phi(s->P.delta, r);
+    id[d] = node_index(s, m, c, d);
+    if (id[d] < 0) return -1;
+  }
+  *wgt = wt;
+  if (c == 0) return (long long)IU(s, id[0], id[1], id[2]);
+  if (c == 1) return (long long)IV(s, id[0], id[1], id[2]);
+  return (long long)IW(s, id[0], id[1], id[2]);
+}
+
+// I-2: U_l = sum_x u(x) delta_h(x - X_l) dv  = sum u * phi phi phi   (Eq. 3b / Eq. 20 operator)
+static void interpolate(const orc_sim* s, const vec& us, const vec& vs, const vec& ws, vec& out) {
+  const int sw = support_width(s);
+  for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) {
+    const vec& f = c == 0 ? us : c == 1 ? vs : ws;
+    double acc = 0.0;
+    for (int cc = 0; cc < sw; ++cc) for (int b = 0; b < sw; ++b) for (int a = 0; a < sw; ++a) {
+      double wt; long long q = ibm_node(s, l, c, a, b, cc, &wt);
+      if (q >= 0) acc += f[(size_t)q] * wt;
+    }
+    out[3 * l + c] = acc;
+  }
+}
+// I-4: f(x) += F_l delta_h(x - X_l) dV_l  (Eq. 3a), markers visited in cell-list (perm) order
+static void spread(const orc_sim* s, const vec& F, vec& fu, vec& fv, vec& fw) {
+  const int sw = support_width(s);
+  const double ivol = 1.0 / (s->hx * s->hy * s->hz);
+  for (int r = 0; r < s->nl; ++r) { int l = s->perm[r];
+    for (int c = 0; c < 3; ++c) {
+      vec& f = c == 0 ? fu : c == 1 ? fv : fw;
+      for (int cc = 0; cc < sw; ++cc) for (int b = 0; b < sw; ++b) for (int a = 0; a < sw; ++a) {
+        double wt; long long q = ibm_node(s, l, c, a, b, cc, &wt);
+        if (q >= 0) f[(size_t)q] += F[3 * l + c] * wt * s->dV[l] * ivol;
+      }
+    }
+  }
+}
+
+// ---- O5: outflow flux correction (reading; paper silent) ---------------------------------------
+// net outward flux Phi through all boundary-normal faces is removed by a uniform shift of the
+// outflow faces:  u_n(out) -= Phi / A_out.
+static void flux_correction(const orc_sim* s, vec& us, vec& vs, vec& ws) {
+  const int n[3] = {s->nx, s->ny, s->nz}; const int bd[3] = {s->bx, s->by, s->bz};
+  double Phi = 0.0, Aout = 0.0; bool any = false;
+  for (int pass = 0; pass < 2; ++pass) {
+    for (int d = 0; d < 3; ++d) {
+      if (!bd[d]) continue;
+      vec& f = d == 0 ? us : d == 1 ? vs : ws;
+      int d1 = (d + 1) % 3, d2 = (d + 2) % 3; if (d1 > d2) std::swap(d1, d2);
+      for (int side = 0; side < 2; ++side) {
+        int face = 2 * d + side; bool out = s->P.bc[face] == ORC_BC_OUTFLOW;
+        double sgn = side ? 1.0 : -1.0;
+        for (int b = 0; b < n[d2]; ++b) for (int a = 0; a < n[d1]; ++a) {
+          int id[3]; id[d] = side ? n[d] : 0; id[d1] = a; id[d2] = b;
+          double area = d == 0 ? s->dy[id[1]] * s->hz : d == 1 ? s->hx * s->hz : s->hx * s->dy[id[1]];
+          size_t q = d == 0 ? IU(s, id[0], id[1], id[2]) : d == 1 ? IV(s, id[0], id[1], id[2]) : IW(s, id[0], id[1], id[2]);
+          if (pass == 0) { Phi += sgn * f[q] * area; if (out) { Aout += area; any = true; } }
+          else if (out) f[q] -= sgn * Phi / Aout;
+        }
+      }
+    }
+    if (!any) return;
+  }
+}
+
+// ---- O6: staggered divergence, gradient, Laplacian -------------------------------------------
+static void divergence(const orc_sim* s, const vec& uu, const vec& vv, const vec& ww, vec& out) {
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i) {
+    double ue = uu[IU(s, s->bx ? i + 1 : wrapi(i + 1, s->nx), j, k)], uw = uu[IU(s, i, j, k)];
+    double vn = vv[IV(s, i, s->by ? j + 1 : wrapi(j + 1, s->ny), k)], vs = vv[IV(s, i, j, k)];
+    double wt = ww[IW(s, i, j, s->bz ? k + 1 : wrapi(k + 1, s->nz))], wb = ww[IW(s, i, j, k)];
+    out[IP(s, i, j, k)] = (ue - uw) / s->hx + (vn - vs) / s->dy[j] + (wt - wb) / s->hz;
+  }
+}
+// L p with the flux through every non-periodic boundary face dropped (homogeneous Neumann)
+static void laplacian(const orc_sim* s, const double* p, double* out) {
+  const int nx = s->nx, ny = s->ny, nz = s->nz;
+  for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+    double pc = p[IP(s, i, j, k)], acc = 0.0;
+    if (!s->bx || i + 1 < nx) acc += (p[IP(s, wrapi(i + 1, nx), j, k)] - pc) / (s->hx * s->hx);
+    if (!s->bx || i > 0)      acc -= (pc - p[IP(s, wrapi(i - 1, nx), j, k)]) / (s->hx * s->hx);
+    double fy = 0.0;
+    if (!s->by || j + 1 < ny) fy += (p[IP(s, i, wrapi(j + 1, ny), k)] - pc) / DYC(s, j + 1);
+    if (!s->by || j > 0)      fy -= (pc - p[IP(s, i, wrapi(j - 1, ny), k)]) / DYC(s, j);
+    acc += fy / s->dy[j];
+    if (!s->bz || k + 1 < nz) acc += (p[IP(s, i, j, wrapi(k + 1, nz))] - pc) / (s->hz * s->hz);
+    if (!s->bz || k > 0)      acc -= (pc - p[IP(s, i, j, wrapi(k - 1, nz))]) / (s->hz * s->hz);
+    out[IP(s, i, j, k)] = acc;
+  }
+}
+// A = -dy_j * L  (symmetric positive semi-definite, null space = constants)
+static void apply_A(const orc_sim* s, const double* x, double* out) {
+  laplacian(s, x, out);
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i)
+    out[IP(s, i, j, k)] *= -s->dy[j];
+}
+static void jacobi_diag(const orc_sim* s, double* dg) {
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i) {
+    double a = 0.0;
+    if (!s->bx || i + 1 < s->nx) a += 1.0 / (s->hx * s->hx);
+    if (!s->bx || i > 0)         a += 1.0 / (s->hx * s->hx);
+    double fy = 0.0;
+    if (!s->by || j + 1 < s->ny) fy += 1.0 / DYC(s, j + 1);
+    if (!s->by || j > 0)         fy += 1.0 / DYC(s, j);
+    a += fy / s->dy[j];
+    if (!s->bz || k + 1 < s->nz) a += 1.0 / (s->hz * s->hz);
+    if (!s->bz || k > 0)         a += 1.0 / (s->hz * s->hz);
+    dg[IP(s, i, j, k)] = a * s->dy[j];
+  }
+}
+
+// ---- O7g: geometric multigrid V-cycle on (-L) e = g, all-periodic uniform isotropic grids --------
+// level arrays are n^3-shaped with spacing h; operator rediscretised on every level.
+static void mg_neg_lap(int nx, int ny, int nz, double h, const vec& e, vec& out) {
+  double ih2 = 1.0 / (h * h);
+  for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+    size_t c = (size_t)i + (size_t)nx * (j + (size_t)ny * k);
+    double nb = e[(size_t)wrapi(i + 1, nx) + (size_t)nx * (j + (size_t)ny * k)] + e[(size_t)wrapi(i - 1, nx) + (size_t)nx * (j + (size_t)ny * k)]
+              + e[(size_t)i + (size_t)nx * (wrapi(j + 1, ny) + (size_t)ny * k)] + e[(size_t)i + (size_t)nx * (wrapi(j - 1, ny) + (size_t)ny * k)]
+              + e[(size_t)i + (size_t)nx * (j + (size_t)ny * wrapi(k + 1, nz))] + e[(size_t)i + (size_t)nx * (j + (size_t)ny * wrapi(k - 1, nz))];
+    out[c] = (6.0 * e[c] - nb) * ih2;
+  }
+}
+// one damped-Jacobi sweep  e <- e + omega D^-1 (g - (-L) e),  D = 6/h^2
+static void mg_sweep(int nx, int ny, int nz, double h, double omega, const vec& g, vec& e, vec& tmp, bool zero_guess) {
+  double c = omega * h * h / 6.0;
+  size_t N = (size_t)nx * ny * nz;
+  if (zero_guess) { for (size_t q = 0; q < N; ++q) e[q] = c * g[q]; return; }
+  mg_neg_lap(nx, ny, nz, h, e, tmp);
+  for (size_t q = 0; q < N; ++q) e[q] = e[q] + c * (g[q] - tmp[q]);
+}
+static int mg_levels(int nx, int ny, int nz) {
+  int L = 1;
+  while (nx % 2 == 0 && ny % 2 == 0 && nz % 2 == 0 && std::min(nx, std::min(ny, nz)) / 2 >= 4) { nx /= 2; ny /= 2; nz /= 2; ++L; }
+  return L;
+}
+static void mg_vcycle(const orc_sim* s, int lev, int nx, int ny, int nz, double h, const vec& g, vec& e) {
+  size_t N = (size_t)nx * ny * nz; vec tmp(N);
+  e.assign(N, 0.0);
+  if (lev == s->nlev - 1) {                                    // coarsest: fixed sweeps from zero
+    for (int it = 0; it < s->P.mg_coarse_sweeps; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, g, e, tmp, it == 0);
+    return;
+  }
+  for (int it = 0; it < s->P.mg_nu1; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, g, e, tmp, it == 0);
+  vec res(N);
+  if (s->P.mg_nu1 > 0) { mg_neg_lap(nx, ny, nz, h, e, tmp); for (size_t q = 0; q < N; ++q) res[q] = g[q] - tmp[q]; }
+  else res = g;
+  int cx = nx / 2, cy = ny / 2, cz = nz / 2; size_t Nc = (size_t)cx * cy * cz;
+  vec gc(Nc), ec;
+  for (int k = 0; k < cz; ++k) for (int j = 0; j < cy; ++j) for (int i = 0; i < cx; ++i) {   // restriction: mean of 8 children
+    double a = 0.0;
+    for (int dk = 0; dk < 2; ++dk) for (int dj = 0; dj < 2; ++dj) for (int di = 0; di < 2; ++di)
+      a += res[(size_t)(2 * i + di) + (size_t)nx * ((2 * j + dj) + (size_t)ny * (2 * k + dk))];
+    gc[(size_t)i + (size_t)cx * (j + (size_t)cy * k)] = 0.125 * a;
+  }
+  mg_vcycle(s, lev + 1, cx, cy, cz, 2.0 * h, gc, ec);
+  for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i)      // piecewise-constant prolongation
+    e[(size_t)i + (size_t)nx * (j + (size_t)ny * k)] += ec[(size_t)(i / 2) + (size_t)cx * ((j / 2) + (size_t)cy * (k / 2))];
+  for (int it = 0; it < s->P.mg_nu2; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, g, e, tmp, false);
+}
+// z = M^-1 r : A = -h L = h(-L)  =>  z = Vcycle(r / h)
+static void precond_gmg(const orc_sim* s, const vec& r, vec& z) {
+  vec g(r.size());
+  for (size_t q = 0; q < r.size(); ++q) g[q] = r[q] / s->hy;
+  mg_vcycle(s, 0, s->nx, s->ny, s->nz, s->hx, g, z);
+}
+
+// ---- O7: preconditioned conjugate gradients (textbook Hestenes-Stiefel) -----------------------
+static double dot(const vec& a, const vec& b) { double t = 0.0; for (size_t q = 0; q < a.size(); ++q) t += a[q] * b[q]; return t; }
+static void apply_precond(const orc_sim* s, const vec& dg, const vec& r, vec& z) {
+  if (s->P.precond == ORC_PC_NONE) z = r;
+  else if (s->P.precond == ORC_PC_JACOBI) { for (size_t q = 0; q < r.size(); ++q) z[q] = r[q] / dg[q]; }
+  else precond_gmg(s, r, z);
+}
+// solves A x = bh (bh already compatible); x holds the initial guess
+static void pcg(const orc_sim* s, const vec& bh, vec& x, orc_info* info) {
+  size_t N = bh.size(); vec r(N), z(N), d(N), q(N), dg;
+  if (s->P.precond == ORC_PC_JACOBI) { dg.resize(N); jacobi_diag(s, dg.data()); }
+  apply_A(s, x.data(), q.data());
+  for (size_t i = 0; i < N; ++i) r[i] = bh[i] - q[i];
+  double bnorm = std::sqrt(dot(bh, bh)), rnorm = std::sqrt(dot(r, r));
+  int it = 0, conv = 0;
+  if (bnorm == 0.0 || rnorm <= s->P.rtol * bnorm) conv = 1;
+  else {
+    apply_precond(s, dg, r, z); d = z; double rho = dot(r, z);
+    for (it = 1; it <= s->P.max_iter; ++it) {
+      apply_A(s, d.data(), q.data());
+      double alpha = rho / dot(d, q);
+      for (size_t i = 0; i < N; ++i) x[i] += alpha * d[i];
+      for (size_t i = 0; i < N; ++i) r[i] -= alpha * q[i];
+      rnorm = std::sqrt(dot(r, r));
+      if (rnorm <= s->P.rtol * bnorm) { conv = 1; break; }
+      if (it == s->P.max_iter) break;
+      apply_precond(s, dg, r, z);
+      double rho2 = dot(r, z), beta = rho2 / rho;
+      for (size_t i = 0; i < N; ++i) d[i] = z[i] + beta * d[i];
+      rho = rho2;
+    }
+  }
+  info->pcg_iters = it > s->P.max_iter ? s->P.max_iter : it; info->converged = conv;
+  info->rel_residual = bnorm > 0.0 ? rnorm / bnorm : 0.0;
+  apply_A(s, x.data(), q.data());
+  double t = 0.0; for (size_t i = 0; i < N; ++i) { double e = bh[i] - q[i]; t += e * e; }
+  info->true_rel_residual = bnorm > 0.0 ? std::sqrt(t) / bnorm : 0.0;
+}
+// O6: rhs = Laplacian right-hand side b (Eq. 7);  solves L p = b  as  A p = -dy*b, zero-mean p
+static void poisson(const orc_sim* s, const vec& b, vec& p, orc_info* info) {
+  size_t N = b.size(); vec bh(N);
+  double sb = 0.0, sd = 0.0;
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i) {
+    size_t q = IP(s, i, j, k); bh[q] = -s->dy[j] * b[q]; sb += bh[q]; sd += s->dy[j];
+  }
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i)
+    bh[IP(s, i, j, k)] -= (sb / sd) * s->dy[j];
+  if (!s->P.warm_start) std::fill(p.begin(), p.end(), 0.0);
+  pcg(s, bh, p, info);
+  double sp = 0.0;
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i) sp += p[IP(s, i, j, k)] * s->dy[j];
+  double mean = sp / sd;
+  for (size_t q = 0; q < N; ++q) p[q] -= mean;
+}
+
+// ---- O8: projection  u = u* - (dt/rho) G p  at non-boundary faces (Eq. 10) ---------------
+static void gradient(const orc_sim* s, const vec& p, vec& gu, vec& gv, vec& gw) {
+  std::fill(gu.begin(), gu.end(), 0.0); std::fill(gv.begin(), gv.end(), 0.0); std::fill(gw.begin(), gw.end(), 0.0);
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = s->bx; i < s->nx; ++i)
+    gu[IU(s, i, j, k)] = (p[IP(s, i, j, k)] - p[IP(s, wrapi(i - 1, s->nx), j, k)]) / s->hx;
+  for (int k = 0; k < s->nz; ++k) for (int j = s->by; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i)
+    gv[IV(s, i, j, k)] = (p[IP(s, i, j, k)] - p[IP(s, i, wrapi(j - 1, s->ny), k)]) / DYC(s, j);
+  for (int k = s->bz; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i)
+    gw[IW(s, i, j, k)] = (p[IP(s, i, j, k)] - p[IP(s, i, j, wrapi(k - 1, s->nz))]) / s->hz;
+}
+
+// ---- O9: rigid body, one classical RK4 step of  m w'' + c w' + k w = F  (Eq. 12), F frozen ------
+extern "C" void orc_rk4_body(double m, double c, double k, double F, double dt, double* w, double* wd) {
+  double y0 = *w, y1 = *wd;
+  #define ACC(a, b) ((F - c * (b) - k * (a)) / m)
+  double k1a = y1,                   k1b = ACC(y0, y1);
+  double k2a = y1 + 0.5 * dt * k1b,  k2b = ACC(y0 + 0.5 * dt * k1a, y1 + 0.5 * dt * k1b);
+  double k3a = y1 + 0.5 * dt * k2b,  k3b = ACC(y0 + 0.5 * dt * k2a, y1 + 0.5 * dt * k2b);
+  double k4a = y1 + dt * k3b,        k4b = ACC(y0 + dt * k3a, y1 + dt * k3b);
+  #undef ACC
+  *w  = y0 + dt / 6.0 * (k1a + 2.0 * k2a + 2.0 * k3a + k4a);
+  *wd = y1 + dt / 6.0 * (k1b + 2.0 * k2b + 2.0 * k3b + k4b);
+}
+
+// ---- one fractional step (O1..O9 in order) -----------------------------------------------------
+static void one_step(orc_sim* s, orc_info* info) {
+  const double dt = s->P.dt, rho = s->P.rho;
+  vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size());
+  momentum(s, s->u, s->v, s->w, s->P.nu, s->P.body_force, HU, HV, HW);                 // O1+O2
+  double a0 = 1.0, a1 = 0.0;
+  if (s->P.time_scheme == ORC_TIME_AB2 && s->have_hist) { a0 = 1.5; a1 = -0.5; }
+  vec us = s->u, vs = s->v, ws = s->w;                                                 // O3
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = s->bx; i < s->nx; ++i) {
+    size_t q = IU(s, i, j, k); us[q] = s->u[q] + dt * (a0 * HU[q] + a1 * s->hu[q]); }
+  for (int k = 0; k < s->nz; ++k) for (int j = s->by; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i) {
+    size_t q = IV(s, i, j, k); vs[q] = s->v[q] + dt * (a0 * HV[q] + a1 * s->hv[q]); }
+  for (int k = s->bz; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i) {
+    size_t q = IW(s, i, j, k); ws[q] = s->w[q] + dt * (a0 * HW[q] + a1 * s->hw[q]); }
+  set_boundary_normal(s, us, vs, ws, s->u, s->v, s->w);
+  for (int c = 0; c < 3; ++c) s->bforce[c] = 0.0;
+  if (s->nl > 0) {                                                                     // O4
+    orc_ibm_index(s);                                                                  // I-1
+    interpolate(s, us, vs, ws, s->Ul);                                                 // I-2
+    for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c)                        // I-3 (Eq. 5 at markers)
+      s->Fl[3 * l + c] = (s->Ub[3 * l + c] - s->Ul[3 * l + c]) / dt;
+    for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) s->bforce[c] += s->Fl[3 * l + c] * s->dV[l];
+    for (int c = 0; c < 3; ++c) s->bforce[c] *= -rho;
+    vec fu(us.size(), 0.0), fv(vs.size(), 0.0), fw(ws.size(), 0.0);
+    spread(s, s->Fl, fu, fv, fw);                                                      // I-4
+    for (size_t q = 0; q < us.size(); ++q) us[q] += dt * fu[q];
+    for (size_t q = 0; q < vs.size(); ++q) vs[q] += dt * fv[q];
+    for (size_t q = 0; q < ws.size(); ++q) ws[q] += dt * fw[q];
+  }
+  flux_correction(s, us, vs, ws);                                                      // O5
+  vec b(s->p.size());
+  divergence(s, us, vs, ws, b);                                                        // O6
+  for (size_t q = 0; q < b.size(); ++q) b[q] *= rho / dt;
+  poisson(s, b, s->p, info);                                                           // O7
+  vec gu(us.size()), gv(vs.size()), gw(ws.size());
+  gradient(s, s->p, gu, gv, gw);                                                       // O8
+  for (size_t q = 0; q < us.size(); ++q) s->u[q] = us[q] - dt / rho * gu[q];
+  for (size_t q = 0; q < vs.size(); ++q) s->v[q] = vs[q] - dt / rho * gv[q];
+  for (size_t q = 0; q < ws.size(); ++q) s->w[q] = ws[q] - dt / rho * gw[q];
+  divergence(s, s->u, s->v, s->w, s->divu);
+  double md = 0.0; int nan = 0;
+  for (size_t q = 0; q < s->divu.size(); ++q) { double a = std::fabs(s->divu[q]); if (a > md) md = a; if (a != a) nan = 1; }
+  info->max_abs_div = md; info->nan_flag = nan;
+  if (s->has_body) {                                                                   // O9
+    for (int c = 0; c < 3; ++c) if (s->dof & (1 << c)) {
+      double w0 = s->bdisp[c];
+      orc_rk4_body(s->bm, s->bc_, s->bk, s->bforce[c], dt, &s->bdisp[c], &s->bvel[c]);
+      double dw = s->bdisp[c] - w0;
+      for (int l = 0; l < s->nl; ++l) s->X[3 * l + c] += dw;
+    }
+    for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) s->Ub[3 * l + c] = s->bvel[c];
+  }
+  s->hu = HU; s->hv = HV; s->hw = HW; s->have_hist = true; s->step += 1;
+  for (int c = 0; c < 3; ++c) { info->body_force[c] = s->bforce[c]; info->body_disp[c] = s->bdisp[c]; info->body_vel[c] = s->bvel[c]; }
+  info->step = s->step;
+}
+
+// ---- C interface --------------------------------------------------------------------------------
+extern "C" orc_sim* orc_create(const orc_params* p) {
+  if (!p || p->nx < 2 || p->ny < 2 || p->nz < 2 || p->dt <= 0 || p->rho <= 0 || p->lx <= 0 || p->ly <= 0 || p->lz <= 0) return nullptr;
+  for (int d = 0; d < 3; ++d) {
+    bool a = p->bc[2 * d] == ORC_BC_PERIODIC, b = p->bc[2 * d + 1] == ORC_BC_PERIODIC;
+    if (a != b) return nullptr;
+  }
+  orc_sim* s = new orc_sim();
+  s->P = *p; s->nx = p->nx; s->ny = p->ny; s->nz = p->nz;
+  s->bx = p->bc[0] != ORC_BC_PERIODIC; s->by = p->bc[2] != ORC_BC_PERIODIC; s->bz = p->bc[4] != ORC_BC_PERIODIC;
+  s->nxu = s->nx + s->bx; s->nyv = s->ny + s->by; s->nzw = s->nz + s->bz;
+  s->hx = p->lx / p->nx; s->hy = p->ly / p->ny; s->hz = p->lz / p->nz;
+  s->yf.resize(s->ny + 1); s->dy.resize(s->ny); s->yc.resize(s->ny);
+  s->uniform_y = (p->yf == nullptr);
+  for (int j = 0; j <= s->ny; ++j) s->yf[j] = p->yf ? p->yf[j] : p->y0 + j * s->hy;
+  for (int j = 0; j < s->ny; ++j) {
+    s->dy[j] = p->yf ? s->yf[j + 1] - s->yf[j] : s->hy;
+    s->yc[j] = 0.5 * (s->yf[j] + s->yf[j + 1]);
+    if (!(s->dy[j] > 0)) { delete s; return nullptr; }
+  }
+  s->P.yf = nullptr;
+  if (p->precond == ORC_PC_GMG) {
+    bool ok = !s->bx && !s->by && !s->bz && s->uniform_y &&
+              std::fabs(s->hx - s->hy) <= 1e-12 * s->hx && std::fabs(s->hx - s->hz) <= 1e-12 * s->hx;
+    if (!ok) { delete s; return nullptr; }
+    s->nlev = mg_levels(s->nx, s->ny, s->nz);
+  } else s->nlev = 0;
+  size_t N = (size_t)s->nx * s->ny * s->nz;
+  s->u.assign((size_t)s->nxu * s->ny * s->nz, 0.0); s->v.assign((size_t)s->nx * s->nyv * s->nz, 0.0);
+  s->w.assign((size_t)s->nx * s->ny * s->nzw, 0.0); s->p.assign(N, 0.0); s->divu.assign(N, 0.0);
+  s->hu = s->u; s->hv = s->v; s->hw = s->w;
+  s->have_hist = false; s->step = 0; s->nl = 0; s->nseg = 0; s->has_body = false; s->dof = 0;
+  for (int c = 0; c < 3; ++c) s->bdisp[c] = s->bvel[c] = s->bforce[c] = 0.0;
+  return s;
+}
+extern "C" void orc_destroy(orc_sim* s) { delete s; }
+static vec* field_ptr(orc_sim* s, int f) {
+  switch (f) { case ORC_U: return &s->u; case ORC_V: return &s->v; case ORC_W: return &s->w; case ORC_P: return &s->p;
+    case ORC_HU: return &s->hu; case ORC_HV: return &s->hv; case ORC_HW: return &s->hw; case ORC_DIV: return &s->divu; }
+  return nullptr;
+}
+extern "C" long long orc_field_size(orc_sim* s, int f) { vec* v = field_ptr(s, f); return v ? (long long)v->size() : -1; }
+extern "C" int orc_set_field(orc_sim* s, int f, const double* src) { vec* v = field_ptr(s, f); if (!v || !src) return 1; std::copy(src, src + v->size(), v->begin()); return 0; }
+extern "C" int orc_get_field(orc_sim* s, int f, double* dst) { vec* v = field_ptr(s, f); if (!v || !dst) return 1; std::copy(v->begin(), v->end(), dst); return 0; }
+extern "C" int orc_set_history(orc_sim* s, int have, long long step) { s->have_hist = have != 0; s->step = step; return 0; }
+extern "C" int orc_set_markers(orc_sim* s, int n, const double* xyz, const double* vel, const double* dvol) {
+  if (n < 0 || (n > 0 && !xyz)) return 1;
+  if (n > 0 && (!s->uniform_y)) return 1;   // IBM needs uniform spacing
+  s->nl = n; s->X.assign(xyz, xyz + (size_t)3 * n);
+  s->Ub.assign((size_t)3 * n, 0.0); if (vel) s->Ub.assign(vel, vel + (size_t)3 * n);
+  s->dV.assign(n, s->hx * s->hy * s->hz); if (dvol) s->dV.assign(dvol, dvol + n);
+  s->Fl.assign((size_t)3 * n, 0.0); s->Ul.assign((size_t)3 * n, 0.0);
+  orc_ibm_index(s);
+  return 0;
+}
+extern "C" int orc_set_body(orc_sim* s, double m, double c, double k, int dof) {
+  if (!(m > 0)) return 1;
+  s->has_body = true; s->bm = m; s->bc_ = c; s->bk = k; s->dof = dof; return 0;
+}
+extern "C" int orc_step(orc_sim* s, int nsteps, orc_info* last, int* iters) {
+  orc_info info; std::memset(&info, 0, sizeof info);
+  for (int n = 0; n < nsteps; ++n) { one_step(s, &info); if (iters) iters[n] = info.pcg_iters; }
+  if (last) *last = info;
+  return 0;
+}
+extern "C" int orc_poisson_solve(orc_sim* s, const double* rhs, double* p, orc_info* info) {
+  size_t N = s->p.size(); vec b(rhs, rhs + N), x(p, p + N); orc_info I; std::memset(&I, 0, sizeof I);
+  poisson(s, b, x, &I); std::copy(x.begin(), x.end(), p); if (info) *info = I; return 0;
+}
+extern "C" void orc_laplacian(orc_sim* s, const double* p, double* out) { laplacian(s, p, out); }
+extern "C" void orc_apply_A(orc_sim* s, const double* x, double* out) { apply_A(s, x, out); }
+extern "C" void orc_jacobi_diag(orc_sim* s, double* d) { jacobi_diag(s, d); }
+extern "C" void orc_divergence(orc_sim* s, const double* u, const double* v, const double* w, double* out) {
+  vec uu(u, u + s->u.size()), vv(v, v + s->v.size()), ww(w, w + s->w.size()), o(s->p.size());
+  divergence(s, uu, vv, ww, o); std::copy(o.begin(), o.end(), out);
+}
+extern "C" void orc_gradient(orc_sim* s, const double* p, double* gu, double* gv, double* gw) {
+  vec pp(p, p + s->p.size()), a(s->u.size()), b(s->v.size()), c(s->w.size());
+  gradient(s, pp, a, b, c);
+  std::copy(a.begin(), a.end(), gu); std::copy(b.begin(), b.end(), gv); std::copy(c.begin(), c.end(), gw);
+}
+extern "C" void orc_momentum_rhs(orc_sim* s, double* hu, double* hv, double* hw) {
+  vec a(s->u.size()), b(s->v.size()), c(s->w.size());
+  momentum(s, s->u, s->v, s->w, s->P.nu, s->P.body_force, a, b, c);
+  std::copy(a.begin(), a.end(), hu); std::copy(b.begin(), b.end(), hv); std::copy(c.begin(), c.end(), hw);
+}
+extern "C" void orc_convection(orc_sim* s, double* cu, double* cv, double* cw) {
+  vec a(s->u.size()), b(s->v.size()), c(s->w.size()); const double g0[3] = {0, 0, 0};
+  momentum(s, s->u, s->v, s->w, 0.0, g0, a, b, c);
+  for (size_t q = 0; q < a.size(); ++q) cu[q] = -a[q];
+  for (size_t q = 0; q < b.size(); ++q) cv[q] = -b[q];
+  for (size_t q = 0; q < c.size(); ++q) cw[q] = -c[q];
+}
+extern "C" void orc_vcycle(orc_sim* s, const double* r, double* z) {
+  vec rr(r, r + s->p.size()), zz(s->p.size()); precond_gmg(s, rr, zz); std::copy(zz.begin(), zz.end(), z);
+}
+extern "C" int orc_marker_count(orc_sim* s) { return s->nl; }
+extern "C" void orc_get_cell_list(orc_sim* s, int* base, int* perm, int* keys, int* seg, int* nseg) {
+  if (base) std::copy(s->base.begin(), s->base.end(), base);
+  if (perm) std::copy(s->perm.begin(), s->perm.end(), perm);
+  if (keys) std::copy(s->keys.begin(), s->keys.end(), keys);
+  if (seg)  std::copy(s->seg.begin(), s->seg.end(), seg);
+  if (nseg) *nseg = s->nseg;
+}
+extern "C" void orc_interpolate(orc_sim* s, const double* u, const double* v, const double* w, double* out) {
+  vec uu(u, u + s->u.size()), vv(v, v + s->v.size()), ww(w, w + s->w.size()), o((size_t)3 * s->nl);
+  interpolate(s, uu, vv, ww, o); std::copy(o.begin(), o.end(), out);
+}
+extern "C" void orc_spread(orc_sim* s, const double* F, double* fu, double* fv, double* fw) {
+  vec FF(F, F + (size_t)3 * s->nl), a(fu, fu + s->u.size()), b(fv, fv + s->v.size()), c(fw, fw + s->w.size());
+  spread(s, FF, a, b, c);
+  std::copy(a.begin(), a.end(), fu); std::copy(b.begin(), b.end(), fv); std::copy(c.begin(), c.end(), fw);
+}
+extern "C" void orc_get_markers(orc_sim* s, double* xyz, double* vel, double* force) {
+  if (xyz) std::copy(s->X.begin(), s->X.end(), xyz);
+  if (vel) std::copy(s->Ub.begin(), s->Ub.end(), vel);
+  if (force) std::copy(s->Fl.begin(), s->Fl.end(), force);
+}
+extern "C" void orc_set_body_state(orc_sim* s, const double* disp, const double* vel) {
+  for (int c = 0; c < 3; ++c) { s->bdisp[c] = disp[c]; s->bvel[c] = vel[c]; }
+}
+extern "C" void orc_get_body_state(orc_sim* s, double* disp, double* vel, double* force) {
+  for (int c = 0; c < 3; ++c) { disp[c] = s->bdisp[c]; vel[c] = s->bvel[c]; if (force) force[c] = s->bforce[c]; }
+}

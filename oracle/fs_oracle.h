@@ -1,0 +1,91 @@
+/*
+ * fs_oracle.h -- C interface of the CPU ORACLE (test infrastructure, NOT the product).
+ *
+ * A plain, slow, single-threaded fp64 implementation of one fractional step of the
+ * incompressible Navier-Stokes finite-volume solver of Diff-FlowFSI (arxiv 2505.23940,
+ * /root/reference/PAPER.md section 2.3: Eq. 3-10, 12, 20-22) written from the paper and from
+ * SURVEY.md section 8(c) (steps O1..O9).  It shares no code, header, table or helper with
+ * the CUDA path under paper_2505_23940_b200/csrc and must never be imported by the product.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs use it.
+ *
+ * Array conventions (all fp64, x fastest, then y, then z):
+ *   p, div   : nz * ny * nx
+ *   u        : nz * ny * (nx+bx)      bx = 1 when the x direction is bounded (non-periodic)
+ *   v        : nz * (ny+by) * nx
+ *   w        : (nz+bz) * ny * nx
+ *   u(i,j,k) sits at (x_f(i), y_c(j), z_c(k)) etc. (staggered grid).
+ */
+#ifndef FS_ORACLE_H
+#define FS_ORACLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ORC_BC_PERIODIC = 0, ORC_BC_NOSLIP = 1, ORC_BC_SLIP = 2, ORC_BC_INFLOW = 3, ORC_BC_OUTFLOW = 4 };
+enum { ORC_TIME_EULER = 0, ORC_TIME_AB2 = 1 };
+enum { ORC_PC_NONE = 0, ORC_PC_JACOBI = 1, ORC_PC_GMG = 2 };
+enum { ORC_DELTA_ROMA3 = 0, ORC_DELTA_PESKIN4 = 1 };
+enum { ORC_U = 0, ORC_V, ORC_W, ORC_P, ORC_HU, ORC_HV, ORC_HW, ORC_DIV };
+
+typedef struct {
+  int nx, ny, nz;
+  double x0, y0, z0, lx, ly, lz;
+  const double* yf;          /* ny+1 face coordinates or NULL (uniform) */
+  int bc[6];                 /* -x,+x,-y,+y,-z,+z */
+  double bc_vel[6][3];
+  double nu, rho, dt, body_force[3];
+  int time_scheme;
+  int precond; double rtol; int max_iter; int warm_start;
+  int mg_nu1, mg_nu2, mg_coarse_sweeps; double mg_omega;
+  int delta;
+  uint64_t seed; double inflow_noise;
+} orc_params;
+
+typedef struct {
+  int pcg_iters, converged, nan_flag;
+  double rel_residual, true_rel_residual, max_abs_div;
+  double body_force[3], body_disp[3], body_vel[3];
+  long long step;
+} orc_info;
+
+typedef struct orc_sim orc_sim;
+
+orc_sim* orc_create(const orc_params* p);           /* NULL on invalid parameters */
+void     orc_destroy(orc_sim*);
+long long orc_field_size(orc_sim*, int field);
+int  orc_set_field(orc_sim*, int field, const double* src);
+int  orc_get_field(orc_sim*, int field, double* dst);
+int  orc_set_markers(orc_sim*, int n, const double* xyz, const double* vel, const double* dvol);
+int  orc_set_body(orc_sim*, double m, double c, double k, int dof_mask);
+int  orc_step(orc_sim*, int nsteps, orc_info* last, int* iters_per_step /* nsteps ints or NULL */);
+int  orc_poisson_solve(orc_sim*, const double* rhs, double* p_inout, orc_info* info);
+int  orc_set_history(orc_sim*, int have_history, long long step);   /* restart support */
+
+/* pieces exposed so the tests can pin them one by one */
+double orc_delta_phi(int kind, double r);                       /* Eq. 22 / Roma kernel, h factored out */
+void orc_laplacian(orc_sim*, const double* p, double* out);     /* L p  (O6) */
+void orc_apply_A(orc_sim*, const double* x, double* out);       /* A x = -dy_j L x */
+void orc_divergence(orc_sim*, const double* u, const double* v, const double* w, double* out);
+void orc_gradient(orc_sim*, const double* p, double* gu, double* gv, double* gw); /* 0 on boundary faces */
+void orc_momentum_rhs(orc_sim*, double* hu, double* hv, double* hw); /* H^n of current u,v,w */
+void orc_convection(orc_sim*, double* cu, double* cv, double* cw);   /* C only (nu=0, g=0) */
+void orc_vcycle(orc_sim*, const double* r, double* z);          /* z = M^-1 r, GMG */
+void orc_jacobi_diag(orc_sim*, double* diag);
+/* IBM pieces: arrays sized by the current marker count n */
+int  orc_marker_count(orc_sim*);
+void orc_ibm_index(orc_sim*);                                   /* I-1: (re)build indices + cell list */
+void orc_get_cell_list(orc_sim*, int* base /*3*n*3*/, int* perm /*n*/, int* keys /*n*/,
+                       int* seg_start /*n+1*/, int* nseg);
+void orc_interpolate(orc_sim*, const double* u, const double* v, const double* w, double* out /*n*3*/);
+void orc_spread(orc_sim*, const double* F /*n*3*/, double* fu, double* fv, double* fw); /* adds f */
+void orc_get_markers(orc_sim*, double* xyz, double* vel, double* force);
+void orc_set_body_state(orc_sim*, const double* disp, const double* vel);
+void orc_get_body_state(orc_sim*, double* disp, double* vel, double* force);
+double orc_inflow_rand(uint64_t seed, long long step, int face, int a, int b);
+void orc_rk4_body(double m, double c, double k, double F, double dt, double* w, double* wdot);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
