@@ -1,0 +1,157 @@
+/*
+ * fs.h -- C ABI of the B200-native fractional-step Navier-Stokes / immersed-boundary library.
+ *
+ * One call of fs_step advances the incompressible Navier-Stokes finite-volume solver of
+ * Diff-FlowFSI (arxiv 2505.23940; section 2.3.1) by one fractional step on a
+ * staggered Cartesian grid (pressure at cell centres, velocity components on their faces, PAPER.md
+ * L100):
+ *
+ *   predictor   u~ = u^n + dt (a0 H^n + a1 H^{n-1}),  H = -div(u u) + nu lap(u) + g   (Eq. 4)
+ *   IBM         U_l = sum_x u~(x) delta_h(x - X_l) dv            (Eq. 3b; operator of Eq. 20)
+ *               F_l = (U^b_l - U_l)/dt                           (Eq. 5, at the markers)
+ *               u*  = u~ + dt sum_l F_l delta_h(x - X_l) dV_l    (Eq. 3a; Eq. 4)
+ *   Poisson     lap p = (rho/dt) div u*                          (Eq. 7; Eq. 9 with eps = 0, L127-129)
+ *   projection  u^{n+1} = u* - (dt/rho) grad p                   (Eq. 6/10, L114, L131)
+ *   rigid body  m w'' + c w' + k w = F  by RK4                   (Eq. 12)
+ *
+ * All of it runs in hand-written CUDA kernels for sm_100a, replayed as one CUDA graph per step
+ * (the PCG loop is a device-controlled conditional WHILE node).  There is no CPU fallback.
+ *
+ * Conventions
+ *  - Every pointer argument says whether it is a HOST or a DEVICE pointer.  No torch types.
+ *  - Eulerian arrays: x fastest, then y, then z; structure of arrays.  Extents:
+ *        p, div       : nz * ny * nx
+ *        u, hu        : nz * ny * (nx+bx)     bx = 1 if the x direction is bounded (non-periodic)
+ *        v, hv        : nz * (ny+by) * nx
+ *        w, hw        : (nz+bz) * ny * nx
+ *    u(i,j,k) sits at (x_f(i), y_c(j), z_c(k)), v at (x_c, y_f(j), z_c), w at (x_c, y_c, z_f(k)).
+ *  - Marker arrays are always fp64 (positions decide integer indices; see fs_set_ibm_markers).
+ *  - Ownership: the library never allocates device memory.  The caller passes one workspace of
+ *    fs_workspace_bytes() bytes (256-byte aligned) and the CUDA stream everything runs on; both
+ *    must outlive the fs_grid.  The fs_grid host object (and its CUDA graphs) belongs to the
+ *    library and is released by fs_grid_destroy.  All set calls copy; all get calls copy out.
+ *  - Errors: every call returns fs_status; nothing throws or aborts across the ABI; out-parameters
+ *    are untouched on failure.
+ */
+#ifndef FS_H
+#define FS_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fs_grid fs_grid;   /* opaque */
+
+typedef enum { FS_OK = 0, FS_ERR_INVALID_ARG, FS_ERR_BAD_STATE, FS_ERR_OOM, FS_ERR_CUDA,
+               FS_ERR_NOT_CONVERGED, FS_ERR_UNSUPPORTED } fs_status;
+typedef enum { FS_F32 = 0, FS_F64 = 1 } fs_dtype;
+/* Boundary types of PAPER.md Table 1 (L429, L454-456). */
+typedef enum { FS_BC_PERIODIC = 0, FS_BC_NOSLIP = 1, FS_BC_SLIP = 2, FS_BC_INFLOW = 3,
+               FS_BC_OUTFLOW_CONVECTIVE = 4 } fs_bc;
+typedef enum { FS_TIME_EULER = 0, FS_TIME_AB2 = 1 } fs_time;               /* Eq. 4 / configs */
+typedef enum { FS_PC_NONE = 0, FS_PC_JACOBI = 1, FS_PC_GMG = 2 } fs_precond; /* CG: L449, L686 */
+typedef enum { FS_DELTA_ROMA3 = 0, FS_DELTA_PESKIN4 = 1 } fs_delta;        /* Eq. 21-22 */
+typedef enum { FS_EXEC_GRAPH = 0,   /* one CUDA-graph replay per step, PCG loop = conditional WHILE node */
+               FS_EXEC_STREAM = 1   /* same kernels launched directly; host polls the PCG flag (debug) */
+             } fs_exec;
+typedef enum { FS_U = 0, FS_V, FS_W, FS_P, FS_HU, FS_HV, FS_HW, FS_DIV,
+               FS_MARKER_X,      /* n*3 fp64 positions */
+               FS_MARKER_U,      /* n*3 fp64 target velocities U^b */
+               FS_MARKER_F,      /* n*3 fp64 forces F_l of the last step */
+               FS_MARKER_BASE,   /* 3*n*3 int32: lowest support index [component][marker][direction] */
+               FS_MARKER_PERM,   /* n int32: marker ids sorted by (cell key, id) */
+               FS_MARKER_KEYS,   /* n int32: sorted cell keys */
+               FS_MARKER_SEG,    /* nseg+1 int32 segment starts (call fs_marker_segments for nseg) */
+               FS_BODY_STATE     /* 9 fp64: displacement[3], velocity[3], force[3] */
+             } fs_field;
+
+typedef struct {
+  int nx, ny, nz;
+  double x0, y0, z0, lx, ly, lz;
+  const double* yf;            /* HOST, ny+1 face coordinates; NULL = uniform (stretching is y-only) */
+  fs_dtype dtype;              /* arithmetic / storage type of all Eulerian fields */
+  fs_bc bc[6];                 /* -x,+x,-y,+y,-z,+z ; both faces of a direction periodic or neither */
+  double bc_vel[6][3];         /* wall / inflow velocity; [outflow][normal] = convective speed U_c */
+  double nu, rho, dt, body_force[3];
+  fs_time time_scheme;
+  fs_precond precond; double rtol; int max_iter; int warm_start;
+  int mg_nu1, mg_nu2, mg_coarse_sweeps; double mg_omega;   /* GMG V(nu1,nu2), damped Jacobi */
+  fs_delta delta; int max_markers;
+  uint64_t seed; double inflow_noise;
+  fs_exec exec_mode;
+} fs_params;
+
+typedef struct {
+  int pcg_iters; int converged; int nan_flag;
+  double rel_residual;        /* recurrence residual ||r|| / ||b|| that the stopping test used */
+  double true_rel_residual;   /* ||b - A p|| / ||b|| recomputed from the projected field */
+  double max_abs_div;         /* max |D u^{n+1}| */
+  double body_force[3], body_disp[3], body_vel[3];
+  long long step;
+} fs_step_info;
+typedef struct { int iters; int converged; double rel_residual, true_rel_residual; } fs_poisson_info;
+
+/* Bytes of device workspace fs_grid_create needs for these parameters.  HOST pointers. */
+fs_status fs_workspace_bytes(const fs_params* params, size_t* bytes);
+
+/* Creates a grid.  params: HOST.  workspace: DEVICE, >= fs_workspace_bytes, 256-byte aligned, owned
+ * by the caller, zeroed by this call.  cuda_stream: a cudaStream_t (NULL = legacy default stream).
+ * FS_ERR_UNSUPPORTED: GMG on a grid that is not uniform/isotropic/all-periodic. */
+fs_status fs_grid_create(const fs_params* params, void* workspace, size_t bytes, void* cuda_stream,
+                         fs_grid** out);
+fs_status fs_grid_destroy(fs_grid* g);
+
+/* Number of elements of a field (HOST out pointer). */
+fs_status fs_field_size(fs_grid* g, fs_field f, long long* count);
+
+/* Copy a whole field in / out.  src/dst is a HOST pointer when *_on_device == 0, else a DEVICE
+ * pointer.  dtype applies to FS_U..FS_DIV (converted if it differs from the grid's); marker fields
+ * are fp64 / int32 regardless.  Synchronises the stream.  FS_DIV is computed on demand (get only). */
+fs_status fs_fields_set(fs_grid* g, fs_field f, const void* src, fs_dtype dtype, int src_on_device);
+fs_status fs_fields_get(fs_grid* g, fs_field f, void* dst, fs_dtype dtype, int dst_on_device);
+
+/* Restart support: whether H^{n-1} is valid (AB2) and the step counter (inflow-noise hash). */
+fs_status fs_set_history(fs_grid* g, int have_history, long long step);
+
+/* Lagrangian markers (Eq. 18 notation: X_l, velocity, volume element dV_l; L183-185).  HOST
+ * pointers, fp64: xyz n*3, vel n*3 (NULL = 0), dvol n (NULL = hx*hy*hz).  n = 0 removes them.
+ * Rebuilds indices and the cell list.  FS_ERR_UNSUPPORTED on a y-stretched grid, n > max_markers
+ * is FS_ERR_INVALID_ARG. */
+fs_status fs_set_ibm_markers(fs_grid* g, int n, const double* xyz, const double* vel, const double* dvol);
+fs_status fs_marker_segments(fs_grid* g, int* nseg);
+
+/* Rigid body of Eq. 12 (L144-147): mass, damping, stiffness given directly; dof_mask bit0=x,1=y,2=z.
+ * All markers translate with the body. */
+fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask);
+fs_status fs_set_body_state(fs_grid* g, const double* disp3, const double* vel3);   /* HOST */
+
+/* Advance nsteps fractional steps.  last == NULL: fully asynchronous on the grid's stream.
+ * last != NULL (HOST): synchronises and reports the final step; FS_ERR_NOT_CONVERGED if that
+ * step's PCG hit max_iter. */
+fs_status fs_step(fs_grid* g, int nsteps, fs_step_info* last);
+
+/* Solves lap p = rhs (Eq. 7 form; homogeneous Neumann on bounded faces, zero-mean solution) with
+ * the grid's PCG.  rhs and p_inout: nz*ny*nx elements of `dtype`, HOST or DEVICE by on_device;
+ * p_inout holds the initial guess when warm_start != 0.  Synchronises. */
+fs_status fs_poisson_solve(fs_grid* g, const void* rhs, void* p_inout, fs_dtype dtype, int on_device,
+                           fs_poisson_info* info);
+
+/* Pieces of the path exposed for element-wise parity tests (DEVICE work, HOST pointers, fp64):
+ *   fs_ibm_interpolate: out[n*3] = interpolation of the current u,v,w at the markers (Eq. 3b)
+ *   fs_ibm_spread:      u,v,w += spread of F[n*3] (Eq. 3a, f = sum_l F_l delta_h dV_l, no dt) */
+fs_status fs_ibm_interpolate(fs_grid* g, double* out);
+fs_status fs_ibm_spread(fs_grid* g, const double* F);
+/*   fs_gmg_vcycle: z = M^-1 r, one V-cycle of the GMG preconditioner (r, z: nz*ny*nx fp64, HOST);
+ *   FS_ERR_BAD_STATE unless precond == FS_PC_GMG.  Clobbers the PCG scratch fields only. */
+fs_status fs_gmg_vcycle(fs_grid* g, const double* r, double* z);
+
+/* Number of kernel launches (graph kernel nodes incl. loop-body replays) issued so far. */
+fs_status fs_launch_count(fs_grid* g, long long* launches);
+
+const char* fs_status_string(fs_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,668 @@
+// fs_api.cu -- the C ABI of include/fs.h: parameter validation, workspace carving, host-side metric
+// tables, CUDA-graph capture of one fractional step (PCG loop = conditional WHILE node) and the
+// field I/O calls.  No torch types; the caller owns device memory and the stream.
+#include "fs_internal.cuh"
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace fs;
+
+#define CK(x)                                                              \
+  do {                                                                     \
+    cudaError_t e_ = (x);                                                  \
+    if (e_ != cudaSuccess) {                                               \
+      std::fprintf(stderr, "libfs: CUDA error %s at %s:%d (%s)\n", cudaGetErrorString(e_), __FILE__, __LINE__, #x); \
+      return FS_ERR_CUDA;                                                  \
+    }                                                                      \
+  } while (0)
+
+struct fs_grid {
+  fs_params P;
+  std::vector<double> yf;
+  bool f64 = true;
+  int bx = 0, by = 0, bz = 0, nxu = 0, nyv = 0, nzw = 0;
+  double hx = 0, hy = 0, hz = 0;
+  bool uniform_y = true;
+  cudaStream_t stream = nullptr, cap = nullptr, cap2 = nullptr;
+  char* ws = nullptr; size_t ws_bytes = 0;
+  Ctx<float> cf; Ctx<double> cd;
+  MgCtx<float> mf; MgCtx<double> md;
+  IbmCtx ib;
+  Scalars* S = nullptr;
+  size_t nU = 0, nV = 0, nW = 0, nP = 0;
+  void* fld[8] = {nullptr};           // device pointers of FS_U..FS_HW (+ none for FS_DIV)
+  // graphs
+  cudaGraphExec_t step_exec = nullptr, poisson_exec = nullptr;
+  int step_fixed = 0, step_body = 0, poisson_fixed = 0, poisson_body = 0;
+  long long fixed_launches = 0, body_iters_poisson = 0;
+  int nl = 0; bool indexed = false;
+};
+
+namespace {
+
+struct Bump {
+  char* base; size_t off;
+  template <class T> T* take(size_t n) {
+    off = (off + 255) & ~size_t(255);
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += n * sizeof(T);
+    return p;
+  }
+};
+
+int mg_levels(int nx, int ny, int nz) {
+  int L = 1;
+  while (nx % 2 == 0 && ny % 2 == 0 && nz % 2 == 0 && std::min(nx, std::min(ny, nz)) / 2 >= 4) { nx /= 2; ny /= 2; nz /= 2; ++L; }
+  return L;
+}
+
+fs_status validate(const fs_params* p) {
+  if (!p) return FS_ERR_INVALID_ARG;
+  if (p->nx < 2 || p->ny < 2 || p->nz < 2) return FS_ERR_INVALID_ARG;
+  if (!(p->dt > 0) || !(p->rho > 0) || !(p->lx > 0) || !(p->ly > 0) || !(p->lz > 0) || !(p->nu >= 0)) return FS_ERR_INVALID_ARG;
+  if (p->dtype != FS_F32 && p->dtype != FS_F64) return FS_ERR_INVALID_ARG;
+  if (p->max_markers < 0 || p->max_iter < 0 || !(p->rtol >= 0)) return FS_ERR_INVALID_ARG;
+  for (int f = 0; f < 6; ++f) if ((int)p->bc[f] < 0 || (int)p->bc[f] > 4) return FS_ERR_INVALID_ARG;
+  for (int d = 0; d < 3; ++d)
+    if ((p->bc[2 * d] == FS_BC_PERIODIC) != (p->bc[2 * d + 1] == FS_BC_PERIODIC)) return FS_ERR_INVALID_ARG;
+  if ((long long)p->nx * p->ny * p->nz > (1LL << 31) - 1) return FS_ERR_UNSUPPORTED;   // int32 cell keys
+  if (p->yf) for (int j = 0; j < p->ny; ++j) if (!(p->yf[j + 1] > p->yf[j])) return FS_ERR_INVALID_ARG;
+  if ((int)p->precond < 0 || (int)p->precond > 2 || (int)p->delta < 0 || (int)p->delta > 1) return FS_ERR_INVALID_ARG;
+  if (p->precond == FS_PC_GMG) {
+    const double hx = p->lx / p->nx, hy = p->ly / p->ny, hz = p->lz / p->nz;
+    const bool periodic = p->bc[0] == FS_BC_PERIODIC && p->bc[2] == FS_BC_PERIODIC && p->bc[4] == FS_BC_PERIODIC;
+    if (!periodic || p->yf || std::fabs(hx - hy) > 1e-12 * hx || std::fabs(hx - hz) > 1e-12 * hx) return FS_ERR_UNSUPPORTED;
+    if (p->mg_nu1 < 0 || p->mg_nu2 < 0 || p->mg_coarse_sweeps < 0) return FS_ERR_INVALID_ARG;
+    if (mg_levels(p->nx, p->ny, p->nz) > kMaxLevels) return FS_ERR_UNSUPPORTED;
+  }
+  return FS_OK;
+}
+
+template <class T> Ctx<T>& ctx(fs_grid* g);
+template <> Ctx<float>& ctx<float>(fs_grid* g) { return g->cf; }
+template <> Ctx<double>& ctx<double>(fs_grid* g) { return g->cd; }
+template <class T> MgCtx<T>& mgc(fs_grid* g);
+template <> MgCtx<float>& mgc<float>(fs_grid* g) { return g->mf; }
+template <> MgCtx<double>& mgc<double>(fs_grid* g) { return g->md; }
+
+// Carves the workspace (base == nullptr: size pass only).
+template <class T> size_t carve(fs_grid* g, char* base) {
+  const fs_params& P = g->P;
+  Ctx<T>& c = ctx<T>(g);
+  MgCtx<T>& mg = mgc<T>(g);
+  Bump b{base, 0};
+  const int ny = P.ny;
+  g->S = b.take<Scalars>(1);
+  c.S = g->S;
+  c.partials = b.take<double>((size_t)kRedSlots * kMaxPartials);
+  T* dy = b.take<T>(ny + 2); T* idy = b.take<T>(ny + 2); T* idyc = b.take<T>(ny + 1);
+  T* wyl = b.take<T>(ny + 1); T* wyh = b.take<T>(ny + 1); T* cyl = b.take<T>(ny); T* cyh = b.take<T>(ny);
+  double* dy64 = b.take<double>(ny);
+  c.dy = dy; c.idy = idy; c.idyc = idyc; c.wyl = wyl; c.wyh = wyh; c.cyl = cyl; c.cyh = cyh; c.dy64 = dy64;
+  c.u = b.take<T>(g->nU); c.v = b.take<T>(g->nV); c.w = b.take<T>(g->nW);
+  c.us = b.take<T>(g->nU); c.vs = b.take<T>(g->nV); c.ws = b.take<T>(g->nW);
+  c.hu = b.take<T>(g->nU); c.hv = b.take<T>(g->nV); c.hw = b.take<T>(g->nW);
+  c.p = b.take<T>(g->nP); c.r = b.take<T>(g->nP); c.d = b.take<T>(g->nP); c.q = b.take<T>(g->nP); c.bh = b.take<T>(g->nP);
+  c.z = nullptr;
+  mg.nlev = 0;
+  if (P.precond == FS_PC_GMG) {
+    c.z = b.take<T>(g->nP);
+    mg.nlev = mg_levels(P.nx, P.ny, P.nz);
+    mg.nu1 = P.mg_nu1; mg.nu2 = P.mg_nu2; mg.coarse_sweeps = P.mg_coarse_sweeps; mg.omega = P.mg_omega;
+    int nx = P.nx, nyy = P.ny, nz = P.nz; double h = g->hx;
+    for (int l = 0; l < mg.nlev; ++l) {
+      MgLevel& V = mg.lev[l];
+      V.nx = nx; V.ny = nyy; V.nz = nz; V.h = h;
+      const size_t N = (size_t)nx * nyy * nz;
+      V.t = b.take<T>(N);
+      V.e = l == 0 ? nullptr : (void*)b.take<T>(N);
+      V.g = l == 0 ? nullptr : (void*)b.take<T>(N);
+      nx /= 2; nyy /= 2; nz /= 2; h *= 2.0;
+    }
+  }
+  IbmCtx& ib = g->ib;
+  const size_t M = (size_t)P.max_markers;
+  ib.X = b.take<double>(3 * M); ib.Ub = b.take<double>(3 * M); ib.dV = b.take<double>(M);
+  ib.Fl = b.take<double>(3 * M); ib.Ul = b.take<double>(3 * M); ib.wts = b.take<double>(36 * M);
+  ib.base = b.take<int>(9 * M); ib.perm = b.take<int>(M); ib.keys = b.take<int>(M); ib.keys_raw = b.take<int>(M);
+  ib.seg = b.take<int>(M + 1); ib.flags = b.take<int>(M);
+  return (b.off + 255) & ~size_t(255);
+}
+
+void init_dims(fs_grid* g) {
+  const fs_params& P = g->P;
+  g->f64 = P.dtype == FS_F64;
+  g->bx = P.bc[0] != FS_BC_PERIODIC; g->by = P.bc[2] != FS_BC_PERIODIC; g->bz = P.bc[4] != FS_BC_PERIODIC;
+  g->nxu = P.nx + g->bx; g->nyv = P.ny + g->by; g->nzw = P.nz + g->bz;
+  g->hx = P.lx / P.nx; g->hy = P.ly / P.ny; g->hz = P.lz / P.nz;
+  g->uniform_y = P.yf == nullptr;
+  g->nU = (size_t)g->nxu * P.ny * P.nz; g->nV = (size_t)P.nx * g->nyv * P.nz; g->nW = (size_t)P.nx * P.ny * g->nzw;
+  g->nP = (size_t)P.nx * P.ny * P.nz;
+}
+
+// Host-side metric tables (SURVEY 8(c) "Grid"), uploaded once.
+template <class T> fs_status upload_metrics(fs_grid* g) {
+  const fs_params& P = g->P;
+  Ctx<T>& c = ctx<T>(g);
+  const int ny = P.ny;
+  std::vector<double> dy(ny);
+  for (int j = 0; j < ny; ++j) dy[j] = g->uniform_y ? g->hy : g->yf[j + 1] - g->yf[j];
+  auto DY = [&](int j) {            // mirrored ghost at a bounded end, wrapped when periodic
+    if (j < 0) return g->by ? dy[0] : dy[(j % ny + ny) % ny];
+    if (j >= ny) return g->by ? dy[ny - 1] : dy[j % ny];
+    return dy[j];
+  };
+  auto DYC = [&](int j) { return 0.5 * (DY(j - 1) + DY(j)); };
+  std::vector<T> hdy(ny + 2), hidy(ny + 2), hidyc(ny + 1), hwl(ny + 1), hwh(ny + 1), hcl(ny), hch(ny);
+  for (int j = -1; j <= ny; ++j) { hdy[j + 1] = (T)DY(j); hidy[j + 1] = (T)(1.0 / DY(j)); }
+  for (int j = 0; j <= ny; ++j) {
+    hidyc[j] = (T)(1.0 / DYC(j));
+    const double dm = DY(j - 1), dp = DY(j);
+    hwl[j] = (T)(dp / (dm + dp)); hwh[j] = (T)(dm / (dm + dp));
+  }
+  double sdy = 0.0;
+  for (int j = 0; j < ny; ++j) {
+    hcl[j] = (g->by && j == 0) ? (T)0 : (T)(1.0 / DYC(j));
+    hch[j] = (g->by && j == ny - 1) ? (T)0 : (T)(1.0 / DYC(j + 1));
+    sdy += dy[j];
+  }
+  CK(cudaMemcpyAsync((void*)c.dy, hdy.data(), sizeof(T) * (ny + 2), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync((void*)c.idy, hidy.data(), sizeof(T) * (ny + 2), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync((void*)c.idyc, hidyc.data(), sizeof(T) * (ny + 1), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync((void*)c.wyl, hwl.data(), sizeof(T) * (ny + 1), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync((void*)c.wyh, hwh.data(), sizeof(T) * (ny + 1), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync((void*)c.cyl, hcl.data(), sizeof(T) * ny, cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync((void*)c.cyh, hch.data(), sizeof(T) * ny, cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync((void*)c.dy64, dy.data(), sizeof(double) * ny, cudaMemcpyHostToDevice, g->stream));
+  Scalars hs; std::memset(&hs, 0, sizeof hs);
+  hs.sum_dy = sdy * (double)P.nx * (double)P.nz;
+  hs.max_iter = P.max_iter; hs.rtol = P.rtol; hs.rho_prev = 1.0; hs.dq = 1.0;
+  CK(cudaMemcpyAsync(g->S, &hs, sizeof hs, cudaMemcpyHostToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  // constants
+  c.nx = P.nx; c.ny = P.ny; c.nz = P.nz; c.bx = g->bx; c.by = g->by; c.bz = g->bz;
+  c.nxu = g->nxu; c.nyv = g->nyv; c.nzw = g->nzw;
+  for (int f = 0; f < 6; ++f) { c.bc[f] = (int)P.bc[f]; for (int a = 0; a < 3; ++a) c.bcv[f][a] = P.bc_vel[f][a]; }
+  c.hx = g->hx; c.hy = g->hy; c.hz = g->hz; c.dt = P.dt; c.rho = P.rho; c.nu = P.nu;
+  for (int a = 0; a < 3; ++a) c.g[a] = P.body_force[a];
+  c.x0 = P.x0; c.y0 = P.y0; c.z0 = P.z0;
+  c.ihx = (T)(1.0 / g->hx); c.ihz = (T)(1.0 / g->hz);
+  c.ihx2 = (T)(1.0 / (g->hx * g->hx)); c.ihz2 = (T)(1.0 / (g->hz * g->hz));
+  c.time_scheme = (int)P.time_scheme; c.precond = (int)P.precond; c.warm_start = P.warm_start; c.delta = (int)P.delta;
+  c.uniform_y = g->uniform_y; c.seed = P.seed; c.inflow_noise = P.inflow_noise;
+  return FS_OK;
+}
+
+void init_ibm(fs_grid* g) {
+  const fs_params& P = g->P;
+  IbmCtx& ib = g->ib;
+  ib.n = 0; ib.delta = (int)P.delta; ib.sw = P.delta == FS_DELTA_ROMA3 ? 3 : 4;
+  const double o[3] = {P.x0, P.y0, P.z0}, h[3] = {g->hx, g->hy, g->hz};
+  for (int d = 0; d < 3; ++d) {
+    ib.o[d] = o[d]; ib.inv[d] = 1.0 / h[d];
+    for (int c = 0; c < 3; ++c) ib.org[c][d] = d == c ? o[d] : o[d] + 0.5 * h[d];
+  }
+  ib.ivol = 1.0 / (g->hx * g->hy * g->hz);
+  ib.has_body = 0; ib.dof = 0; ib.bm = 1.0; ib.bc = 0.0; ib.bk = 0.0;
+}
+
+
+// ---- the step as three kernel sequences: before the PCG loop, the loop body, after the loop ---------
+template <class T> int enqueue_pre(fs_grid* g, const Launch& L, bool poisson) {
+  Ctx<T>& c = ctx<T>(g);
+  int n = 0;
+  if (poisson) {
+    n += launch_rhs_from_b<T>(c, c.vs, L);
+  } else {
+    n += launch_momentum<T>(c, L);
+    if (g->ib.n > 0) {
+      if (g->ib.has_body || !g->indexed) n += launch_ibm_index<T>(c, g->ib, L);
+      n += launch_ibm_interpolate<T>(c, g->ib, c.us, c.vs, c.ws, g->ib.Ul, L);
+      n += launch_ibm_force<T>(c, g->ib, L);
+      n += launch_ibm_spread<T>(c, g->ib, g->ib.Fl, c.us, c.vs, c.ws, c.dt, L);
+    }
+    n += launch_flux_correction<T>(c, L);
+    n += launch_div_rhs<T>(c, L);
+  }
+  n += launch_pcg_init<T>(c, L);
+  return n;
+}
+template <class T> int enqueue_body(fs_grid* g, const Launch& L) { return launch_pcg_body<T>(ctx<T>(g), mgc<T>(g), L); }
+template <class T> int enqueue_post(fs_grid* g, const Launch& L, bool poisson) {
+  Ctx<T>& c = ctx<T>(g);
+  int n = launch_pcg_finish<T>(c, L);
+  if (poisson) n += launch_true_residual<T>(c, L);
+  else { n += launch_project<T>(c, L); n += launch_step_end<T>(c, g->ib, L); }
+  return n;
+}
+
+template <class T> fs_status build_graph(fs_grid* g, bool poisson, cudaGraphExec_t* out, int* n_fixed, int* n_body) {
+  cudaStream_t s = g->cap;
+  cudaStreamCaptureStatus st; cudaGraph_t graph = nullptr; const cudaGraphNode_t* deps = nullptr; size_t nd = 0;
+  CK(cudaStreamBeginCapture(s, cudaStreamCaptureModeRelaxed));
+  CK(cudaStreamGetCaptureInfo_v2(s, &st, nullptr, &graph, &deps, &nd));
+  cudaGraphConditionalHandle h;
+  CK(cudaGraphConditionalHandleCreate(&h, graph, 0, cudaGraphCondAssignDefault));
+  Launch L{s, h, 1};
+  const int npre = enqueue_pre<T>(g, L, poisson);
+  CK(cudaGetLastError());
+  CK(cudaStreamGetCaptureInfo_v2(s, &st, nullptr, &graph, &deps, &nd));
+  cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+  np.conditional.handle = h; np.conditional.type = cudaGraphCondTypeWhile; np.conditional.size = 1;
+  cudaGraphNode_t node;
+  CK(cudaGraphAddNode(&node, graph, deps, nd, &np));
+  cudaGraph_t body = np.conditional.phGraph_out[0];
+  CK(cudaStreamBeginCaptureToGraph(g->cap2, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+  Launch Lb{g->cap2, h, 1};
+  const int nbody = enqueue_body<T>(g, Lb);
+  CK(cudaGetLastError());
+  cudaGraph_t tmp = nullptr;
+  CK(cudaStreamEndCapture(g->cap2, &tmp));
+  CK(cudaStreamUpdateCaptureDependencies(s, &node, 1, cudaStreamSetCaptureDependencies));
+  const int npost = enqueue_post<T>(g, L, poisson);
+  CK(cudaGetLastError());
+  CK(cudaStreamEndCapture(s, &graph));
+  if (*out) { cudaGraphExecDestroy(*out); *out = nullptr; }
+  CK(cudaGraphInstantiate(out, graph, 0));
+  CK(cudaGraphDestroy(graph));
+  *n_fixed = npre + npost; *n_body = nbody;
+  return FS_OK;
+}
+
+// FS_EXEC_STREAM: same kernels, launched directly; the host polls the done flag between chunks.
+template <class T> fs_status run_stream(fs_grid* g, bool poisson, int* n_fixed, int* n_body) {
+  Launch L{g->stream, 0, 0};
+  const int npre = enqueue_pre<T>(g, L, poisson);
+  int nbody = 0;
+  for (;;) {
+    int done = 0;
+    CK(cudaMemcpyAsync(&done, &g->S->done, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
+    CK(cudaStreamSynchronize(g->stream));
+    if (done) break;
+    for (int a = 0; a < 4; ++a) nbody = enqueue_body<T>(g, L);
+  }
+  const int npost = enqueue_post<T>(g, L, poisson);
+  CK(cudaGetLastError());
+  *n_fixed = npre + npost; *n_body = nbody;
+  return FS_OK;
+}
+
+template <class T> fs_status run_once(fs_grid* g, bool poisson) {
+  if (g->P.exec_mode == FS_EXEC_STREAM) {
+    int nf = 0, nb = 0;
+    fs_status st = run_stream<T>(g, poisson, &nf, &nb);
+    if (st != FS_OK) return st;
+    (poisson ? g->poisson_fixed : g->step_fixed) = nf; (poisson ? g->poisson_body : g->step_body) = nb;
+  } else {
+    cudaGraphExec_t* ex = poisson ? &g->poisson_exec : &g->step_exec;
+    if (!*ex) {
+      fs_status st = build_graph<T>(g, poisson, ex, poisson ? &g->poisson_fixed : &g->step_fixed, poisson ? &g->poisson_body : &g->step_body);
+      if (st != FS_OK) return st;
+    }
+    CK(cudaGraphLaunch(*ex, g->stream));
+  }
+  g->fixed_launches += poisson ? g->poisson_fixed : g->step_fixed;
+  if (!poisson && g->ib.n > 0) g->indexed = true;
+  return FS_OK;
+}
+
+void invalidate(fs_grid* g) {
+  if (g->step_exec) { cudaGraphExecDestroy(g->step_exec); g->step_exec = nullptr; }
+}
+
+fs_status read_scalars(fs_grid* g, Scalars* hs) {
+  CK(cudaMemcpyAsync(hs, g->S, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+// copy a T-typed device field to / from a user buffer of `dtype`, host or device
+template <class T> fs_status copy_out(fs_grid* g, const T* dev, size_t n, void* dst, fs_dtype dtype, int on_device) {
+  const bool same = (dtype == FS_F64) == (sizeof(T) == 8);
+  if (on_device) {
+    if (same) CK(cudaMemcpyAsync(dst, dev, n * sizeof(T), cudaMemcpyDeviceToDevice, g->stream));
+    else if (dtype == FS_F64) launch_convert<T, double>(dev, (double*)dst, (long long)n, g->stream);
+    else launch_convert<T, float>(dev, (float*)dst, (long long)n, g->stream);
+    CK(cudaStreamSynchronize(g->stream));
+    return FS_OK;
+  }
+  if (same) { CK(cudaMemcpyAsync(dst, dev, n * sizeof(T), cudaMemcpyDeviceToHost, g->stream)); CK(cudaStreamSynchronize(g->stream)); return FS_OK; }
+  std::vector<T> tmp(n);
+  CK(cudaMemcpyAsync(tmp.data(), dev, n * sizeof(T), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  if (dtype == FS_F64) { double* o = (double*)dst; for (size_t q = 0; q < n; ++q) o[q] = (double)tmp[q]; }
+  else { float* o = (float*)dst; for (size_t q = 0; q < n; ++q) o[q] = (float)tmp[q]; }
+  return FS_OK;
+}
+template <class T> fs_status copy_in(fs_grid* g, T* dev, size_t n, const void* src, fs_dtype dtype, int on_device) {
+  const bool same = (dtype == FS_F64) == (sizeof(T) == 8);
+  if (on_device) {
+    if (same) CK(cudaMemcpyAsync(dev, src, n * sizeof(T), cudaMemcpyDeviceToDevice, g->stream));
+    else if (dtype == FS_F64) launch_convert<double, T>((const double*)src, dev, (long long)n, g->stream);
+    else launch_convert<float, T>((const float*)src, dev, (long long)n, g->stream);
+    CK(cudaStreamSynchronize(g->stream));
+    return FS_OK;
+  }
+  if (same) { CK(cudaMemcpyAsync(dev, src, n * sizeof(T), cudaMemcpyHostToDevice, g->stream)); CK(cudaStreamSynchronize(g->stream)); return FS_OK; }
+  std::vector<T> tmp(n);
+  if (dtype == FS_F64) { const double* i = (const double*)src; for (size_t q = 0; q < n; ++q) tmp[q] = (T)i[q]; }
+  else { const float* i = (const float*)src; for (size_t q = 0; q < n; ++q) tmp[q] = (T)i[q]; }
+  CK(cudaMemcpyAsync(dev, tmp.data(), n * sizeof(T), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+template <class T> T* field_ptr(fs_grid* g, fs_field f, size_t* n) {
+  Ctx<T>& c = ctx<T>(g);
+  switch (f) {
+    case FS_U: *n = g->nU; return c.u;   case FS_V: *n = g->nV; return c.v;   case FS_W: *n = g->nW; return c.w;
+    case FS_P: *n = g->nP; return c.p;
+    case FS_HU: *n = g->nU; return c.hu; case FS_HV: *n = g->nV; return c.hv; case FS_HW: *n = g->nW; return c.hw;
+    case FS_DIV: *n = g->nP; return c.q;
+    default: *n = 0; return nullptr;
+  }
+}
+
+template <class T> fs_status fields_io(fs_grid* g, fs_field f, void* buf, fs_dtype dtype, int on_device, bool set) {
+  size_t n; T* dev = field_ptr<T>(g, f, &n);
+  if (!dev) return FS_ERR_INVALID_ARG;
+  if (set) {
+    if (f == FS_DIV) return FS_ERR_INVALID_ARG;
+    return copy_in<T>(g, dev, n, buf, dtype, on_device);
+  }
+  if (f == FS_DIV) {
+    Ctx<T>& c = ctx<T>(g);
+    Launch L{g->stream, 0, 0};
+    launch_divergence<T>(c, c.u, c.v, c.w, c.q, L);
+    CK(cudaGetLastError());
+  }
+  return copy_out<T>(g, dev, n, buf, dtype, on_device);
+}
+
+template <class T> fs_status poisson_impl(fs_grid* g, const void* rhs, void* p_inout, fs_dtype dtype, int on_device, fs_poisson_info* info) {
+  Ctx<T>& c = ctx<T>(g);
+  const size_t N = g->nP;
+  // the flow state's pressure is parked in us (scratch between steps); rhs goes to vs
+  CK(cudaMemcpyAsync(c.us, c.p, N * sizeof(T), cudaMemcpyDeviceToDevice, g->stream));
+  fs_status st = copy_in<T>(g, c.vs, N, rhs, dtype, on_device); if (st != FS_OK) return st;
+  st = copy_in<T>(g, c.p, N, p_inout, dtype, on_device); if (st != FS_OK) return st;
+  st = run_once<T>(g, true); if (st != FS_OK) return st;
+  Scalars hs; st = read_scalars(g, &hs); if (st != FS_OK) return st;
+  g->body_iters_poisson += hs.iter;
+  st = copy_out<T>(g, c.p, N, p_inout, dtype, on_device); if (st != FS_OK) return st;
+  CK(cudaMemcpyAsync(c.p, c.us, N * sizeof(T), cudaMemcpyDeviceToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  if (info) {
+    info->iters = hs.iter; info->converged = hs.converged;
+    info->rel_residual = hs.bnorm2 > 0 ? std::sqrt(hs.rr / hs.bnorm2) : 0.0;
+    info->true_rel_residual = hs.bnorm2 > 0 ? std::sqrt(hs.true_rr / hs.bnorm2) : 0.0;
+  }
+  return hs.converged ? FS_OK : FS_ERR_NOT_CONVERGED;
+}
+
+}  // namespace
+
+// ======================================================================================================
+extern "C" {
+
+const char* fs_status_string(fs_status s) {
+  switch (s) {
+    case FS_OK: return "ok"; case FS_ERR_INVALID_ARG: return "invalid argument"; case FS_ERR_BAD_STATE: return "bad state";
+    case FS_ERR_OOM: return "out of memory"; case FS_ERR_CUDA: return "CUDA error"; case FS_ERR_NOT_CONVERGED: return "PCG not converged";
+    case FS_ERR_UNSUPPORTED: return "unsupported configuration";
+  }
+  return "unknown";
+}
+
+fs_status fs_workspace_bytes(const fs_params* params, size_t* bytes) {
+  if (!bytes) return FS_ERR_INVALID_ARG;
+  fs_status st = validate(params); if (st != FS_OK) return st;
+  fs_grid tmp; tmp.P = *params; init_dims(&tmp);
+  *bytes = tmp.f64 ? carve<double>(&tmp, nullptr) : carve<float>(&tmp, nullptr);
+  return FS_OK;
+}
+
+fs_status fs_grid_create(const fs_params* params, void* workspace, size_t bytes, void* cuda_stream, fs_grid** out) {
+  if (!out || !workspace) return FS_ERR_INVALID_ARG;
+  fs_status st = validate(params); if (st != FS_OK) return st;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return FS_ERR_INVALID_ARG;
+  fs_grid* g = new (std::nothrow) fs_grid();
+  if (!g) return FS_ERR_OOM;
+  g->P = *params;
+  if (params->yf) { g->yf.assign(params->yf, params->yf + params->ny + 1); }
+  g->P.yf = params->yf ? g->yf.data() : nullptr;
+  init_dims(g);
+  const size_t need = g->f64 ? carve<double>(g, nullptr) : carve<float>(g, nullptr);
+  if (bytes < need) { delete g; return FS_ERR_INVALID_ARG; }
+  g->stream = (cudaStream_t)cuda_stream; g->ws = (char*)workspace; g->ws_bytes = bytes;
+  if (g->f64) carve<double>(g, g->ws); else carve<float>(g, g->ws);
+  auto fail = [&](fs_status s) { fs_grid_destroy(g); return s; };
+  if (cudaStreamCreateWithFlags(&g->cap, cudaStreamNonBlocking) != cudaSuccess) return fail(FS_ERR_CUDA);
+  if (cudaStreamCreateWithFlags(&g->cap2, cudaStreamNonBlocking) != cudaSuccess) return fail(FS_ERR_CUDA);
+  if (cudaMemsetAsync(g->ws, 0, need, g->stream) != cudaSuccess) return fail(FS_ERR_CUDA);
+  init_ibm(g);
+  st = g->f64 ? upload_metrics<double>(g) : upload_metrics<float>(g);
+  if (st != FS_OK) return fail(st);
+  *out = g;
+  return FS_OK;
+}
+
+fs_status fs_grid_destroy(fs_grid* g) {
+  if (!g) return FS_ERR_INVALID_ARG;
+  if (g->stream || g->cap) cudaStreamSynchronize(g->stream);
+  if (g->step_exec) cudaGraphExecDestroy(g->step_exec);
+  if (g->poisson_exec) cudaGraphExecDestroy(g->poisson_exec);
+  if (g->cap) cudaStreamDestroy(g->cap);
+  if (g->cap2) cudaStreamDestroy(g->cap2);
+  delete g;
+  return FS_OK;
+}
+
+fs_status fs_field_size(fs_grid* g, fs_field f, long long* count) {
+  if (!g || !count) return FS_ERR_INVALID_ARG;
+  const long long n = g->ib.n;
+  switch (f) {
+    case FS_U: case FS_HU: *count = (long long)g->nU; break;
+    case FS_V: case FS_HV: *count = (long long)g->nV; break;
+    case FS_W: case FS_HW: *count = (long long)g->nW; break;
+    case FS_P: case FS_DIV: *count = (long long)g->nP; break;
+    case FS_MARKER_X: case FS_MARKER_U: case FS_MARKER_F: *count = 3 * n; break;
+    case FS_MARKER_BASE: *count = 9 * n; break;
+    case FS_MARKER_PERM: case FS_MARKER_KEYS: *count = n; break;
+    case FS_MARKER_SEG: *count = n + 1; break;
+    case FS_BODY_STATE: *count = 9; break;
+    default: return FS_ERR_INVALID_ARG;
+  }
+  return FS_OK;
+}
+
+fs_status fs_fields_set(fs_grid* g, fs_field f, const void* src, fs_dtype dtype, int src_on_device) {
+  if (!g || !src) return FS_ERR_INVALID_ARG;
+  if (f <= FS_DIV) return g->f64 ? fields_io<double>(g, f, const_cast<void*>(src), dtype, src_on_device, true)
+                                 : fields_io<float>(g, f, const_cast<void*>(src), dtype, src_on_device, true);
+  const cudaMemcpyKind kind = src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  const size_t n = (size_t)g->ib.n;
+  if (f == FS_MARKER_X) { CK(cudaMemcpyAsync(g->ib.X, src, 3 * n * sizeof(double), kind, g->stream)); g->indexed = false; invalidate(g); }
+  else if (f == FS_MARKER_U) CK(cudaMemcpyAsync(g->ib.Ub, src, 3 * n * sizeof(double), kind, g->stream));
+  else if (f == FS_BODY_STATE) {
+    CK(cudaMemcpyAsync(g->S->body_disp, src, 3 * sizeof(double), kind, g->stream));
+    CK(cudaMemcpyAsync(g->S->body_vel, (const double*)src + 3, 3 * sizeof(double), kind, g->stream));
+  } else return FS_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+fs_status fs_fields_get(fs_grid* g, fs_field f, void* dst, fs_dtype dtype, int dst_on_device) {
+  if (!g || !dst) return FS_ERR_INVALID_ARG;
+  if (f <= FS_DIV) return g->f64 ? fields_io<double>(g, f, dst, dtype, dst_on_device, false)
+                                 : fields_io<float>(g, f, dst, dtype, dst_on_device, false);
+  const cudaMemcpyKind kind = dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  const size_t n = (size_t)g->ib.n;
+  const void* src = nullptr; size_t bytes = 0;
+  switch (f) {
+    case FS_MARKER_X: src = g->ib.X; bytes = 3 * n * sizeof(double); break;
+    case FS_MARKER_U: src = g->ib.Ub; bytes = 3 * n * sizeof(double); break;
+    case FS_MARKER_F: src = g->ib.Fl; bytes = 3 * n * sizeof(double); break;
+    case FS_MARKER_BASE: src = g->ib.base; bytes = 9 * n * sizeof(int); break;
+    case FS_MARKER_PERM: src = g->ib.perm; bytes = n * sizeof(int); break;
+    case FS_MARKER_KEYS: src = g->ib.keys; bytes = n * sizeof(int); break;
+    case FS_MARKER_SEG: src = g->ib.seg; bytes = (n + 1) * sizeof(int); break;
+    case FS_BODY_STATE: {
+      CK(cudaMemcpyAsync(dst, g->S->body_disp, 3 * sizeof(double), kind, g->stream));
+      CK(cudaMemcpyAsync((double*)dst + 3, g->S->body_vel, 3 * sizeof(double), kind, g->stream));
+      CK(cudaMemcpyAsync((double*)dst + 6, g->S->body_force, 3 * sizeof(double), kind, g->stream));
+      CK(cudaStreamSynchronize(g->stream));
+      return FS_OK;
+    }
+    default: return FS_ERR_INVALID_ARG;
+  }
+  if (bytes) CK(cudaMemcpyAsync(dst, src, bytes, kind, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+fs_status fs_set_history(fs_grid* g, int have_history, long long step) {
+  if (!g) return FS_ERR_INVALID_ARG;
+  const int hh = have_history != 0;
+  CK(cudaMemcpyAsync(&g->S->have_hist, &hh, sizeof(int), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(&g->S->step, &step, sizeof(long long), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+fs_status fs_set_ibm_markers(fs_grid* g, int n, const double* xyz, const double* vel, const double* dvol) {
+  if (!g || n < 0 || (n > 0 && !xyz)) return FS_ERR_INVALID_ARG;
+  if (n > g->P.max_markers) return FS_ERR_INVALID_ARG;
+  if (n > 0 && !g->uniform_y) return FS_ERR_UNSUPPORTED;
+  IbmCtx& ib = g->ib;
+  ib.n = n; g->nl = n; g->indexed = false;
+  invalidate(g);
+  if (n == 0) {
+    double z[3] = {0, 0, 0};
+    CK(cudaMemcpyAsync(g->S->body_force, z, sizeof z, cudaMemcpyHostToDevice, g->stream));
+    CK(cudaStreamSynchronize(g->stream));
+    return FS_OK;
+  }
+  CK(cudaMemcpyAsync(ib.X, xyz, 3 * (size_t)n * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  if (vel) CK(cudaMemcpyAsync(ib.Ub, vel, 3 * (size_t)n * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  else CK(cudaMemsetAsync(ib.Ub, 0, 3 * (size_t)n * sizeof(double), g->stream));
+  std::vector<double> dv;
+  if (dvol) dv.assign(dvol, dvol + n); else dv.assign(n, g->hx * g->hy * g->hz);
+  CK(cudaMemcpyAsync(ib.dV, dv.data(), (size_t)n * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemsetAsync(ib.Fl, 0, 3 * (size_t)n * sizeof(double), g->stream));
+  CK(cudaMemsetAsync(ib.Ul, 0, 3 * (size_t)n * sizeof(double), g->stream));
+  Launch L{g->stream, 0, 0};
+  g->fixed_launches += g->f64 ? launch_ibm_index<double>(g->cd, ib, L) : launch_ibm_index<float>(g->cf, ib, L);
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(g->stream));
+  g->indexed = true;
+  return FS_OK;
+}
+
+fs_status fs_marker_segments(fs_grid* g, int* nseg) {
+  if (!g || !nseg) return FS_ERR_INVALID_ARG;
+  if (g->ib.n == 0) { *nseg = 0; return FS_OK; }
+  int v = 0;
+  CK(cudaMemcpyAsync(&v, &g->S->nseg, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  *nseg = v;
+  return FS_OK;
+}
+
+fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask) {
+  if (!g || !(m > 0)) return FS_ERR_INVALID_ARG;
+  g->ib.has_body = 1; g->ib.bm = m; g->ib.bc = c; g->ib.bk = k; g->ib.dof = dof_mask;
+  invalidate(g);
+  return FS_OK;
+}
+
+fs_status fs_set_body_state(fs_grid* g, const double* disp3, const double* vel3) {
+  if (!g || !disp3 || !vel3) return FS_ERR_INVALID_ARG;
+  CK(cudaMemcpyAsync(g->S->body_disp, disp3, 3 * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(g->S->body_vel, vel3, 3 * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+fs_status fs_step(fs_grid* g, int nsteps, fs_step_info* last) {
+  if (!g || nsteps < 0) return FS_ERR_INVALID_ARG;
+  for (int s = 0; s < nsteps; ++s) {
+    fs_status st = g->f64 ? run_once<double>(g, false) : run_once<float>(g, false);
+    if (st != FS_OK) return st;
+  }
+  if (!last) return FS_OK;
+  Scalars hs; fs_status st = read_scalars(g, &hs); if (st != FS_OK) return st;
+  fs_step_info I;
+  I.pcg_iters = hs.iter; I.converged = hs.converged; I.nan_flag = hs.nan_flag;
+  I.rel_residual = hs.bnorm2 > 0 ? std::sqrt(hs.rr / hs.bnorm2) : 0.0;
+  I.true_rel_residual = hs.bnorm2 > 0 ? std::sqrt(hs.true_rr / hs.bnorm2) : 0.0;
+  I.max_abs_div = hs.max_div;
+  for (int a = 0; a < 3; ++a) { I.body_force[a] = hs.body_force[a]; I.body_disp[a] = hs.body_disp[a]; I.body_vel[a] = hs.body_vel[a]; }
+  I.step = hs.step;
+  *last = I;
+  return (nsteps > 0 && !hs.converged) ? FS_ERR_NOT_CONVERGED : FS_OK;
+}
+
+fs_status fs_poisson_solve(fs_grid* g, const void* rhs, void* p_inout, fs_dtype dtype, int on_device, fs_poisson_info* info) {
+  if (!g || !rhs || !p_inout) return FS_ERR_INVALID_ARG;
+  return g->f64 ? poisson_impl<double>(g, rhs, p_inout, dtype, on_device, info) : poisson_impl<float>(g, rhs, p_inout, dtype, on_device, info);
+}
+
+fs_status fs_ibm_interpolate(fs_grid* g, double* out) {
+  if (!g || !out) return FS_ERR_INVALID_ARG;
+  if (g->ib.n == 0) return FS_ERR_BAD_STATE;
+  Launch L{g->stream, 0, 0};
+  if (g->f64) g->fixed_launches += launch_ibm_interpolate<double>(g->cd, g->ib, g->cd.u, g->cd.v, g->cd.w, g->ib.Ul, L);
+  else g->fixed_launches += launch_ibm_interpolate<float>(g->cf, g->ib, g->cf.u, g->cf.v, g->cf.w, g->ib.Ul, L);
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, g->ib.Ul, 3 * (size_t)g->ib.n * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+fs_status fs_ibm_spread(fs_grid* g, const double* F) {
+  if (!g || !F) return FS_ERR_INVALID_ARG;
+  if (g->ib.n == 0) return FS_ERR_BAD_STATE;
+  CK(cudaMemcpyAsync(g->ib.Fl, F, 3 * (size_t)g->ib.n * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  Launch L{g->stream, 0, 0};
+  if (g->f64) g->fixed_launches += launch_ibm_spread<double>(g->cd, g->ib, g->ib.Fl, g->cd.u, g->cd.v, g->cd.w, 1.0, L);
+  else g->fixed_launches += launch_ibm_spread<float>(g->cf, g->ib, g->ib.Fl, g->cf.u, g->cf.v, g->cf.w, 1.0, L);
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+fs_status fs_gmg_vcycle(fs_grid* g, const double* r, double* z) {
+  if (!g || !r || !z) return FS_ERR_INVALID_ARG;
+  if (g->P.precond != FS_PC_GMG) return FS_ERR_BAD_STATE;
+  const int zero = 0;
+  CK(cudaMemcpyAsync(&g->S->done, &zero, sizeof(int), cudaMemcpyHostToDevice, g->stream));
+  Launch L{g->stream, 0, 0};
+  fs_status st;
+  if (g->f64) {
+    st = copy_in<double>(g, g->cd.r, g->nP, r, FS_F64, 0); if (st != FS_OK) return st;
+    g->fixed_launches += launch_vcycle<double>(g->cd, g->md, g->cd.r, g->cd.z, L);
+    launch_scale<double>(g->cd.z, 1.0 / g->hy, (long long)g->nP, g->stream);   // A = h (-L)  =>  M^-1 r = V(r) / h
+    CK(cudaGetLastError());
+    st = copy_out<double>(g, g->cd.z, g->nP, z, FS_F64, 0); if (st != FS_OK) return st;
+  } else {
+    st = copy_in<float>(g, g->cf.r, g->nP, r, FS_F64, 0); if (st != FS_OK) return st;
+    g->fixed_launches += launch_vcycle<float>(g->cf, g->mf, g->cf.r, g->cf.z, L);
+    launch_scale<float>(g->cf.z, 1.0 / g->hy, (long long)g->nP, g->stream);
+    CK(cudaGetLastError());
+    st = copy_out<float>(g, g->cf.z, g->nP, z, FS_F64, 0); if (st != FS_OK) return st;
+  }
+  return FS_OK;
+}
+
+fs_status fs_launch_count(fs_grid* g, long long* launches) {
+  if (!g || !launches) return FS_ERR_INVALID_ARG;
+  Scalars hs; fs_status st = read_scalars(g, &hs); if (st != FS_OK) return st;
+  *launches = g->fixed_launches + hs.total_iters * (long long)g->step_body + g->body_iters_poisson * (long long)g->poisson_body;
+  return FS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,177 @@
+// fs_internal.cuh -- device-side data structures and launcher declarations shared by the CUDA
+// translation units of libfs (the product).  Nothing here is shared with oracle/.
+//
+// Layout in HBM: structure of arrays, x fastest, then y, then z;
+// a velocity component has n+1 entries along its own normal when that direction is bounded.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/fs.h"
+
+namespace fs {
+
+constexpr int kMaxLevels = 12;
+constexpr int kMaxPartials = 16384;   // partial sums per reduction slot (>= blocks of any reducing kernel)
+constexpr int kRedSlots = 4;          // values reduced at once by one kernel
+
+// Scalars that live in device memory so that a captured step never needs the host.
+struct Scalars {
+  // Poisson / PCG
+  double mean_coef;      // sum(bhat_raw) / sum(dy)      (compatibility shift)
+  double bnorm2, rr;     // ||bhat||^2, ||r||^2 (recurrence residual)
+  double rho_cur, rho_prev, dq;
+  double pmean;
+  double sum_dy;         // sum over all cells of dy_j
+  int iter, done, converged, first;
+  int max_iter, pad0;
+  double rtol;
+  // step control
+  long long step; int have_hist; int nan_flag;
+  double max_div, true_rr;
+  long long total_iters;
+  // open-boundary flux correction (O5)
+  double flux_phi, flux_aout;
+  // IBM
+  int nseg; int bbox_lo[3], bbox_hi[3]; int pad1;
+  double body_force[3], body_disp[3], body_vel[3];
+  // tickets for last-block reductions
+  unsigned int ticket[8];
+};
+
+template <class T> struct Ctx {
+  int nx, ny, nz, bx, by, bz, nxu, nyv, nzw;
+  int bc[6];
+  double bcv[6][3];
+  double hx, hy, hz, dt, rho, nu, g[3];
+  double x0, y0, z0;
+  T ihx, ihz, ihx2, ihz2;
+  int time_scheme, precond, warm_start, delta, uniform_y;
+  uint64_t seed; double inflow_noise;
+  // y metrics (device arrays of T unless noted)
+  const T* dy;     // [ny+2]: dy[j+1] = DY(j), j in [-1, ny] (mirrored ghost at walls, wrapped if periodic)
+  const T* idy;    // [ny+2] idy[j+1] = 1/DY(j)
+  const T* idyc;   // [ny+1] 1/DYC(j): centre-to-centre distance across face j
+  const T* wyl;    // [ny+1] weight of the value below face j in the linear interpolation to the face
+  const T* wyh;    // [ny+1] weight of the value above
+  const T* cyl;    // [ny]   Laplacian coefficient towards j-1 (0 at a bounded end)
+  const T* cyh;    // [ny]   towards j+1
+  const double* dy64;  // [ny] fp64 cell heights (reductions, flux areas)
+  // fields
+  T *u, *v, *w, *p, *us, *vs, *ws, *hu, *hv, *hw;
+  T *r, *d, *q, *z, *bh;
+  Scalars* S;
+  double* partials;     // [kRedSlots][kMaxPartials]
+};
+
+struct MgLevel { int nx, ny, nz; double h; void *e, *g, *t; };
+template <class T> struct MgCtx {
+  int nlev, nu1, nu2, coarse_sweeps; double omega;
+  MgLevel lev[kMaxLevels];
+};
+
+struct IbmCtx {
+  int n, sw, delta;            // markers, support width (3 or 4)
+  double org[3][3];            // node origin of component c along direction d
+  double inv[3];               // 1/h per direction
+  double o[3];                 // domain origin
+  double ivol;                 // 1/(hx hy hz)
+  double *X, *Ub, *dV, *Fl, *Ul, *wts;   // wts: [3][n][3][4]
+  int *base, *perm, *keys, *keys_raw, *seg, *flags;
+  // body (Eq. 12)
+  int has_body, dof; double bm, bc, bk;
+};
+
+struct Launch { cudaStream_t s; cudaGraphConditionalHandle cond; int use_cond; };
+
+// ---- launchers (one per kernel family; each returns the number of kernels it enqueued) ----------
+template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L);
+template <class T> int launch_flux_correction(const Ctx<T>& c, const Launch& L);
+template <class T> int launch_div_rhs(const Ctx<T>& c, const Launch& L);
+template <class T> int launch_rhs_from_b(const Ctx<T>& c, const T* b, const Launch& L);
+template <class T> int launch_project(const Ctx<T>& c, const Launch& L);
+template <class T> int launch_divergence(const Ctx<T>& c, const T* u, const T* v, const T* w, T* out, const Launch& L);
+template <class T> int launch_step_end(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
+template <class TS, class TD> void launch_convert(const TS* src, TD* dst, long long n, cudaStream_t s);
+template <class T> void launch_scale(T* x, double a, long long n, cudaStream_t s);
+
+template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L);
+template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, const Launch& L);
+template <class T> int launch_pcg_finish(const Ctx<T>& c, const Launch& L);
+template <class T> int launch_true_residual(const Ctx<T>& c, const Launch& L);
+template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L);
+
+template <class T> int launch_ibm_index(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
+template <class T> int launch_ibm_interpolate(const Ctx<T>& c, const IbmCtx& ib, const T* u, const T* v, const T* w, double* out, const Launch& L);
+template <class T> int launch_ibm_force(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
+template <class T> int launch_ibm_spread(const Ctx<T>& c, const IbmCtx& ib, const double* F, T* u, T* v, T* w, double scale, const Launch& L);
+
+// ---- device helpers ---------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ int wrapi(int i, int n) { i %= n; return i < 0 ? i + n : i; }
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// Block-wide sum of NV values; result valid in thread 0.  blockDim (flattened) <= 1024.
+template <int NV> __device__ __forceinline__ void block_sum(double (&v)[NV], double* sh /*[NV*32]*/) {
+  const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+  const int nth = blockDim.x * blockDim.y * blockDim.z;
+  const int lane = tid & 31, wid = tid >> 5, nw = (nth + 31) >> 5;
+#pragma unroll
+  for (int a = 0; a < NV; ++a) v[a] = warp_sum(v[a]);
+  __syncthreads();
+  if (lane == 0) {
+#pragma unroll
+    for (int a = 0; a < NV; ++a) sh[a * 32 + wid] = v[a];
+  }
+  __syncthreads();
+  if (wid == 0) {
+#pragma unroll
+    for (int a = 0; a < NV; ++a) {
+      double t = lane < nw ? sh[a * 32 + lane] : 0.0;
+      v[a] = warp_sum(t);
+    }
+  }
+}
+
+// Deterministic grid-wide sum: every block stores its partial, the last block to arrive (ticket)
+// adds the partials in a fixed order.  Returns true in ALL threads of that last block; v holds the
+// totals in its thread 0.  No floating-point atomics, so results do not depend on block scheduling.
+template <int NV> __device__ __forceinline__ bool grid_sum(double (&v)[NV], double* partials, unsigned int* ticket,
+                                                          double* sh /*[NV*32]*/, int* sh_flag) {
+  const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+  const int nth = blockDim.x * blockDim.y * blockDim.z;
+  const int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+  const int nblk = gridDim.x * gridDim.y * gridDim.z;
+  block_sum<NV>(v, sh);
+  if (tid == 0) {
+#pragma unroll
+    for (int a = 0; a < NV; ++a) __stcg(&partials[a * kMaxPartials + bid], v[a]);
+    __threadfence();
+    unsigned int t = atomicAdd(ticket, 1u);
+    *sh_flag = (t == (unsigned int)(nblk - 1));
+  }
+  __syncthreads();
+  if (!*sh_flag) return false;
+  __threadfence();
+#pragma unroll
+  for (int a = 0; a < NV; ++a) {
+    double t = 0.0;
+    for (int b = tid; b < nblk; b += nth) t += __ldcg(&partials[a * kMaxPartials + b]);
+    v[a] = t;
+  }
+  block_sum<NV>(v, sh);
+  if (tid == 0) *ticket = 0u;
+  return true;
+}
+#endif
+
+}  // namespace fs

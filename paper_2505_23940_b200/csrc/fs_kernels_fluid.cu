@@ -1,0 +1,501 @@
+// fs_kernels_fluid.cu -- momentum RHS + predictor (S0+S1), open-boundary flux correction (O5),
+// Poisson right-hand side (S6), projection + divergence diagnostics (S8), step bookkeeping (S9/S10).
+// Hand-written for sm_100a; shares nothing with oracle/.
+#include "fs_internal.cuh"
+
+namespace fs {
+
+// ---------------------------------------------------------------------------------------------------
+// Boundary-aware velocity access (S0).
+// Component C at (i,j,k), at most one layer outside the stored range in a direction tangential to C:
+//   periodic      : index wrap
+//   no-slip/inflow: ghost = 2*u_wall - u_interior      slip/outflow: ghost = u_interior
+// Along its own normal a bounded component stores faces 0..n, so no ghost is needed there.
+// ---------------------------------------------------------------------------------------------------
+template <class T, int C> __device__ __forceinline__ T ldv(const Ctx<T>& c, const T* __restrict__ f, int i, int j, int k) {
+  T A = T(1), B = T(0);
+  // x
+  if (!c.bx) { i = i < 0 ? i + c.nx : (i >= c.nx ? i - c.nx : i); }
+  else if (C != 0) {
+    int face = -1;
+    if (i < 0) { face = 0; i = -1 - i; } else if (i >= c.nx) { face = 1; i = 2 * c.nx - 1 - i; }
+    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
+  }
+  // y
+  if (!c.by) { j = j < 0 ? j + c.ny : (j >= c.ny ? j - c.ny : j); }
+  else if (C != 1) {
+    int face = -1;
+    if (j < 0) { face = 2; j = -1 - j; } else if (j >= c.ny) { face = 3; j = 2 * c.ny - 1 - j; }
+    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
+  }
+  // z
+  if (!c.bz) { k = k < 0 ? k + c.nz : (k >= c.nz ? k - c.nz : k); }
+  else if (C != 2) {
+    int face = -1;
+    if (k < 0) { face = 4; k = -1 - k; } else if (k >= c.nz) { face = 5; k = 2 * c.nz - 1 - k; }
+    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
+  }
+  const int ex = C == 0 ? c.nxu : c.nx, ey = C == 1 ? c.nyv : c.ny;
+  return A * f[(size_t)i + (size_t)ex * ((size_t)j + (size_t)ey * (size_t)k)] + B;
+}
+
+// Counter-based inflow noise (O1): SplitMix64 finaliser chained over (seed, face, step, a, b) and
+// mapped to [0,1) by (x >> 11) * 2^-53.  The oracle implements the same generator independently.
+__device__ __forceinline__ uint64_t mix64(uint64_t z) {
+  z += 0x9E3779B97F4A7C15ULL;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  return z ^ (z >> 31);
+}
+__device__ __forceinline__ double inflow_rand(uint64_t seed, long long step, int face, int a, int b) {
+  uint64_t h = mix64(seed + 0x632BE59BD9B4E019ULL * (uint64_t)(face + 1));
+  h = mix64(h + (uint64_t)step);
+  h = mix64(h + (((uint64_t)(uint32_t)b << 32) | (uint64_t)(uint32_t)a));
+  return (double)(h >> 11) * (1.0 / 9007199254740992.0);
+}
+
+// Value of a prescribed boundary-normal face of the predicted field (O1/O3).
+//   old = u^n of that component, q = index of the face, qi = index of its interior neighbour face.
+template <class T> __device__ __forceinline__ T boundary_normal(const Ctx<T>& c, const T* __restrict__ old, int d, int side,
+                                                               int a, int b, size_t q, size_t qi, int jedge) {
+  const int face = 2 * d + side, t = c.bc[face];
+  const double Ub = c.bcv[face][d];
+  if (t == FS_BC_NOSLIP) return T(Ub);
+  if (t == FS_BC_SLIP) return T(0);
+  if (t == FS_BC_INFLOW) {
+    double r = inflow_rand(c.seed, c.S->step, face, a, b);
+    return T(Ub * (1.0 + c.inflow_noise * (2.0 * r - 1.0)));
+  }
+  // convective outflow (reading): du/dt + Uc du/dn = 0, first-order upwind
+  const double dn = d == 0 ? c.hx : (d == 1 ? (double)c.dy64[jedge] : c.hz);
+  const double o = (double)old[q], oi = (double)old[qi];
+  const double grad = side ? (o - oi) / dn : (oi - o) / dn;
+  return T(o - Ub * c.dt * grad);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// S1: H^n = -div(u u) + nu lap(u) + g (central / central, Eq. 4) and the explicit
+// predictor u~ = u^n + dt (a0 H^n + a1 H^{n-1}); prescribed boundary-normal faces get their O1 values.
+// One thread per cell of the extended box (nxu x nyv x nzw); it owns the three faces u,v,w(i,j,k).
+// ---------------------------------------------------------------------------------------------------
+template <class T> __global__ void __launch_bounds__(256) k_momentum(const Ctx<T> c) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i >= c.nxu || j >= c.nyv || k >= c.nzw) return;
+  const bool ab2 = c.time_scheme == FS_TIME_AB2 && c.S->have_hist;
+  const T a0 = ab2 ? T(1.5) : T(1), a1 = ab2 ? T(-0.5) : T(0);
+  const T dt = T(c.dt), nu = T(c.nu);
+  const T* __restrict__ U = c.u; const T* __restrict__ V = c.v; const T* __restrict__ W = c.w;
+#define U_(a, b, cc) ldv<T, 0>(c, U, a, b, cc)
+#define V_(a, b, cc) ldv<T, 1>(c, V, a, b, cc)
+#define W_(a, b, cc) ldv<T, 2>(c, W, a, b, cc)
+  // ---- u face ----
+  if (j < c.ny && k < c.nz) {
+    const size_t q = (size_t)i + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k);
+    if (c.bx && (i == 0 || i == c.nx)) {
+      const int side = i == 0 ? 0 : 1;
+      const size_t qi = side ? q - 1 : q + 1;
+      c.us[q] = boundary_normal<T>(c, U, 0, side, j, k, q, qi, 0);
+      c.hu[q] = T(0);
+    } else {
+      const T uc = U[q];
+      const T uE = U_(i + 1, j, k), uW = U_(i - 1, j, k), uN = U_(i, j + 1, k), uS = U_(i, j - 1, k);
+      const T uT = U_(i, j, k + 1), uB = U_(i, j, k - 1);
+      const T ue = T(0.5) * (uc + uE), uw = T(0.5) * (uW + uc);
+      const T cx = (ue * ue - uw * uw) * c.ihx;
+      const T vn = T(0.5) * (V_(i - 1, j + 1, k) + V_(i, j + 1, k)), un = c.wyl[j + 1] * uc + c.wyh[j + 1] * uN;
+      const T vs = T(0.5) * (V_(i - 1, j, k) + V_(i, j, k)),         us = c.wyl[j] * uS + c.wyh[j] * uc;
+      const T cy = (vn * un - vs * us) * c.idy[j + 1];
+      const T wt = T(0.5) * (W_(i - 1, j, k + 1) + W_(i, j, k + 1)), ut = T(0.5) * (uc + uT);
+      const T wb = T(0.5) * (W_(i - 1, j, k) + W_(i, j, k)),         ub = T(0.5) * (uB + uc);
+      const T cz = (wt * ut - wb * ub) * c.ihz;
+      const T dxx = (uE - T(2) * uc + uW) * c.ihx2;
+      const T dyy = ((uN - uc) * c.idyc[j + 1] - (uc - uS) * c.idyc[j]) * c.idy[j + 1];
+      const T dzz = (uT - T(2) * uc + uB) * c.ihz2;
+      const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[0]);
+      c.us[q] = uc + dt * (a0 * H + a1 * c.hu[q]);
+      c.hu[q] = H;
+    }
+  }
+  // ---- v face (control volume between y_c(j-1) and y_c(j)) ----
+  if (i < c.nx && k < c.nz) {
+    const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.nyv * k);
+    if (c.by && (j == 0 || j == c.ny)) {
+      const int side = j == 0 ? 0 : 1;
+      const size_t qi = side ? q - c.nx : q + c.nx;
+      c.vs[q] = boundary_normal<T>(c, V, 1, side, i, k, q, qi, side ? c.ny - 1 : 0);
+      c.hv[q] = T(0);
+    } else {
+      const T vc = V[q];
+      const T vE = V_(i + 1, j, k), vW = V_(i - 1, j, k), vN = V_(i, j + 1, k), vS = V_(i, j - 1, k);
+      const T vT = V_(i, j, k + 1), vB = V_(i, j, k - 1);
+      const T wl = c.wyl[j], wh = c.wyh[j];
+      const T ue = wl * U_(i + 1, j - 1, k) + wh * U_(i + 1, j, k), ve = T(0.5) * (vc + vE);
+      const T uw = wl * U_(i, j - 1, k) + wh * U_(i, j, k),         vw = T(0.5) * (vW + vc);
+      const T cx = (ue * ve - uw * vw) * c.ihx;
+      const T vn = T(0.5) * (vc + vN), vs = T(0.5) * (vS + vc);
+      const T cy = (vn * vn - vs * vs) * c.idyc[j];
+      const T wt = wl * W_(i, j - 1, k + 1) + wh * W_(i, j, k + 1), vt = T(0.5) * (vc + vT);
+      const T wb = wl * W_(i, j - 1, k) + wh * W_(i, j, k),         vb = T(0.5) * (vB + vc);
+      const T cz = (wt * vt - wb * vb) * c.ihz;
+      const T dxx = (vE - T(2) * vc + vW) * c.ihx2;
+      const T dyy = ((vN - vc) * c.idy[j + 1] - (vc - vS) * c.idy[j]) * c.idyc[j];
+      const T dzz = (vT - T(2) * vc + vB) * c.ihz2;
+      const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[1]);
+      c.vs[q] = vc + dt * (a0 * H + a1 * c.hv[q]);
+      c.hv[q] = H;
+    }
+  }
+  // ---- w face ----
+  if (i < c.nx && j < c.ny) {
+    const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k);
+    if (c.bz && (k == 0 || k == c.nz)) {
+      const int side = k == 0 ? 0 : 1;
+      const size_t pl = (size_t)c.nx * c.ny;
+      const size_t qi = side ? q - pl : q + pl;
+      c.ws[q] = boundary_normal<T>(c, W, 2, side, i, j, q, qi, 0);
+      c.hw[q] = T(0);
+    } else {
+      const T wc = W[q];
+      const T wE = W_(i + 1, j, k), wW = W_(i - 1, j, k), wN = W_(i, j + 1, k), wS = W_(i, j - 1, k);
+      const T wT = W_(i, j, k + 1), wB = W_(i, j, k - 1);
+      const T ue = T(0.5) * (U_(i + 1, j, k - 1) + U_(i + 1, j, k)), we = T(0.5) * (wc + wE);
+      const T uw = T(0.5) * (U_(i, j, k - 1) + U_(i, j, k)),         ww = T(0.5) * (wW + wc);
+      const T cx = (ue * we - uw * ww) * c.ihx;
+      const T vn = T(0.5) * (V_(i, j + 1, k - 1) + V_(i, j + 1, k)), wn = c.wyl[j + 1] * wc + c.wyh[j + 1] * wN;
+      const T vs = T(0.5) * (V_(i, j, k - 1) + V_(i, j, k)),         ws = c.wyl[j] * wS + c.wyh[j] * wc;
+      const T cy = (vn * wn - vs * ws) * c.idy[j + 1];
+      const T wt = T(0.5) * (wc + wT), wb = T(0.5) * (wB + wc);
+      const T cz = (wt * wt - wb * wb) * c.ihz;
+      const T dxx = (wE - T(2) * wc + wW) * c.ihx2;
+      const T dyy = ((wN - wc) * c.idyc[j + 1] - (wc - wS) * c.idyc[j]) * c.idy[j + 1];
+      const T dzz = (wT - T(2) * wc + wB) * c.ihz2;
+      const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[2]);
+      c.ws[q] = wc + dt * (a0 * H + a1 * c.hw[q]);
+      c.hw[q] = H;
+    }
+  }
+#undef U_
+#undef V_
+#undef W_
+}
+
+template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
+  dim3 b(32, 4, 2), g((c.nxu + 31) / 32, (c.nyv + 3) / 4, (c.nzw + 1) / 2);
+  k_momentum<T><<<g, b, 0, L.s>>>(c);
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// O5 outflow flux correction (reading; the paper is silent): the net outward flux Phi through all
+// boundary-normal faces is removed by a uniform shift of the outflow faces, u_n(out) -= Phi / A_out.
+// ---------------------------------------------------------------------------------------------------
+template <class T> struct FaceIt {   // enumerates the boundary-normal faces of the bounded directions
+  const Ctx<T>& c;
+  __device__ FaceIt(const Ctx<T>& cc) : c(cc) {}
+  __device__ long long count() const {
+    long long n = 0;
+    if (c.bx) n += 2LL * c.ny * c.nz;
+    if (c.by) n += 2LL * c.nx * c.nz;
+    if (c.bz) n += 2LL * c.nx * c.ny;
+    return n;
+  }
+  // decode face id -> (d, side, a, b); returns the storage index, area, outward sign, and field
+  __device__ void decode(long long f, int& d, int& side, size_t& q, double& area, T*& fld) const {
+    long long nxf = c.bx ? 2LL * c.ny * c.nz : 0, nyf = c.by ? 2LL * c.nx * c.nz : 0;
+    if (f < nxf) {
+      d = 0; long long pl = (long long)c.ny * c.nz; side = f >= pl; long long r = f - side * pl;
+      int j = (int)(r % c.ny), k = (int)(r / c.ny);
+      q = (size_t)(side ? c.nx : 0) + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k);
+      area = c.dy64[j] * c.hz; fld = c.us;
+    } else if (f < nxf + nyf) {
+      f -= nxf; d = 1; long long pl = (long long)c.nx * c.nz; side = f >= pl; long long r = f - side * pl;
+      int i = (int)(r % c.nx), k = (int)(r / c.nx);
+      q = (size_t)i + (size_t)c.nx * ((size_t)(side ? c.ny : 0) + (size_t)c.nyv * k);
+      area = c.hx * c.hz; fld = c.vs;
+    } else {
+      f -= nxf + nyf; d = 2; long long pl = (long long)c.nx * c.ny; side = f >= pl; long long r = f - side * pl;
+      int i = (int)(r % c.nx), j = (int)(r / c.nx);
+      q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * (size_t)(side ? c.nz : 0));
+      area = c.hx * c.dy64[j]; fld = c.ws;
+    }
+  }
+};
+
+template <class T> __global__ void __launch_bounds__(256) k_flux_sum(const Ctx<T> c) {
+  __shared__ double sh[2 * 32]; __shared__ int flag;
+  FaceIt<T> it(c);
+  const long long nf = it.count();
+  double v[2] = {0.0, 0.0};
+  for (long long f = blockIdx.x * (long long)blockDim.x + threadIdx.x; f < nf; f += (long long)gridDim.x * blockDim.x) {
+    int d, side; size_t q; double area; T* fld;
+    it.decode(f, d, side, q, area, fld);
+    const double sgn = side ? 1.0 : -1.0;
+    v[0] += sgn * (double)fld[q] * area;
+    if (c.bc[2 * d + side] == FS_BC_OUTFLOW_CONVECTIVE) v[1] += area;
+  }
+  if (grid_sum<2>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0) { c.S->flux_phi = v[0]; c.S->flux_aout = v[1]; }
+  }
+}
+template <class T> __global__ void __launch_bounds__(256) k_flux_apply(const Ctx<T> c) {
+  FaceIt<T> it(c);
+  const long long nf = it.count();
+  const double shift = c.S->flux_phi / c.S->flux_aout;
+  for (long long f = blockIdx.x * (long long)blockDim.x + threadIdx.x; f < nf; f += (long long)gridDim.x * blockDim.x) {
+    int d, side; size_t q; double area; T* fld;
+    it.decode(f, d, side, q, area, fld);
+    if (c.bc[2 * d + side] == FS_BC_OUTFLOW_CONVECTIVE) {
+      const double sgn = side ? 1.0 : -1.0;
+      fld[q] = T((double)fld[q] - sgn * shift);
+    }
+  }
+}
+template <class T> int launch_flux_correction(const Ctx<T>& c, const Launch& L) {
+  bool any = false;
+  for (int f = 0; f < 6; ++f) any |= c.bc[f] == FS_BC_OUTFLOW_CONVECTIVE;
+  if (!any) return 0;
+  k_flux_sum<T><<<64, 256, 0, L.s>>>(c);
+  k_flux_apply<T><<<64, 256, 0, L.s>>>(c);
+  return 2;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// S6: raw right-hand side of the symmetrised system, bhat_raw = -dy_j (rho/dt) D(u*)  (Eq. 7;
+// SURVEY O6), and its sum for the compatibility shift.  Written into r; pcg_init finishes the job.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kFlatBlocks = 148 * 8;
+
+template <class T> __global__ void __launch_bounds__(256) k_div_rhs(const Ctx<T> c, const T* __restrict__ bsrc) {
+  __shared__ double sh[32]; __shared__ int flag;
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  const T sc = T(c.rho / c.dt);
+  double v[1] = {0.0};
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
+    T b;
+    if (bsrc) b = bsrc[q];
+    else {
+      const int ip = c.bx ? i + 1 : (i + 1 == c.nx ? 0 : i + 1);
+      const int jp = c.by ? j + 1 : (j + 1 == c.ny ? 0 : j + 1);
+      const int kp = c.bz ? k + 1 : (k + 1 == c.nz ? 0 : k + 1);
+      const T ue = c.us[(size_t)ip + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k)], uw = c.us[(size_t)i + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k)];
+      const T vn = c.vs[(size_t)i + (size_t)c.nx * ((size_t)jp + (size_t)c.nyv * k)], vs = c.vs[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.nyv * k)];
+      const T wt = c.ws[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * kp)], wb = c.ws[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k)];
+      const T div = (ue - uw) * c.ihx + (vn - vs) * c.idy[j + 1] + (wt - wb) * c.ihz;
+      b = div * sc;
+    }
+    const T bh = -c.dy[j + 1] * b;
+    c.r[q] = bh;
+    v[0] += (double)bh;
+  }
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0) {
+      c.S->mean_coef = v[0] / c.S->sum_dy;
+      c.S->max_div = 0.0; c.S->nan_flag = 0; c.S->true_rr = 0.0;
+    }
+  }
+}
+static inline int flat_blocks(long long n) { long long b = (n + 255) / 256; return (int)(b < kFlatBlocks ? (b < 1 ? 1 : b) : kFlatBlocks); }
+
+template <class T> int launch_div_rhs(const Ctx<T>& c, const Launch& L) {
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, nullptr);
+  return 1;
+}
+template <class T> int launch_rhs_from_b(const Ctx<T>& c, const T* b, const Launch& L) {
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, b);
+  return 1;
+}
+
+// plain staggered divergence of (u,v,w) (FS_DIV on demand)
+template <class T> __global__ void __launch_bounds__(256) k_divergence(const Ctx<T> c, const T* __restrict__ u, const T* __restrict__ v,
+                                                                     const T* __restrict__ w, T* __restrict__ out) {
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
+    const int ip = c.bx ? i + 1 : (i + 1 == c.nx ? 0 : i + 1);
+    const int jp = c.by ? j + 1 : (j + 1 == c.ny ? 0 : j + 1);
+    const int kp = c.bz ? k + 1 : (k + 1 == c.nz ? 0 : k + 1);
+    const T ue = u[(size_t)ip + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k)], uw = u[(size_t)i + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k)];
+    const T vn = v[(size_t)i + (size_t)c.nx * ((size_t)jp + (size_t)c.nyv * k)], vs = v[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.nyv * k)];
+    const T wt = w[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * kp)], wb = w[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k)];
+    out[q] = (ue - uw) * c.ihx + (vn - vs) * c.idy[j + 1] + (wt - wb) * c.ihz;
+  }
+}
+template <class T> int launch_divergence(const Ctx<T>& c, const T* u, const T* v, const T* w, T* out, const Launch& L) {
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  k_divergence<T><<<flat_blocks(N), 256, 0, L.s>>>(c, u, v, w, out);
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// S8: projection u^{n+1} = u* - (dt/rho) G p at non-boundary faces (Eq. 6/10, L114, L131), fused with
+// the diagnostics of the projected field: max |D u^{n+1}|, NaN flag, and the true Poisson residual
+// (since D G = L:  bhat - A p = -dy_j (rho/dt) D u^{n+1} - mean_coef dy_j).
+// One thread per cell of the extended box.
+// ---------------------------------------------------------------------------------------------------
+template <class T> __device__ __forceinline__ T proj_u(const Ctx<T>& c, int i, int j, int k, T dtr) {
+  const size_t q = (size_t)i + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k);
+  if (c.bx && (i == 0 || i == c.nx)) return c.us[q];
+  const int im = i == 0 ? c.nx - 1 : i - 1;
+  const size_t row = (size_t)c.nx * ((size_t)j + (size_t)c.ny * k);
+  return c.us[q] - dtr * ((c.p[row + i] - c.p[row + im]) * c.ihx);
+}
+template <class T> __device__ __forceinline__ T proj_v(const Ctx<T>& c, int i, int j, int k, T dtr) {
+  const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.nyv * k);
+  if (c.by && (j == 0 || j == c.ny)) return c.vs[q];
+  const int jm = j == 0 ? c.ny - 1 : j - 1;
+  return c.vs[q] - dtr * ((c.p[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k)] -
+                           c.p[(size_t)i + (size_t)c.nx * ((size_t)jm + (size_t)c.ny * k)]) * c.idyc[j]);
+}
+template <class T> __device__ __forceinline__ T proj_w(const Ctx<T>& c, int i, int j, int k, T dtr) {
+  const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k);
+  if (c.bz && (k == 0 || k == c.nz)) return c.ws[q];
+  const int km = k == 0 ? c.nz - 1 : k - 1;
+  return c.ws[q] - dtr * ((c.p[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k)] -
+                           c.p[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * km)]) * c.ihz);
+}
+
+template <class T> __global__ void __launch_bounds__(256) k_project(const Ctx<T> c, int kz) {
+  __shared__ double sh[32]; __shared__ int flag;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k0 = blockIdx.z * kz;
+  const T dtr = T(c.dt / c.rho);
+  const double sc = c.rho / c.dt, mc = c.S->mean_coef;
+  double v[1] = {0.0}; double md = 0.0; int nan = 0;
+  if (i < c.nxu && j < c.nyv) {
+    const int k1 = min(k0 + kz, c.nzw);
+    for (int k = k0; k < k1; ++k) {
+      T un = T(0), vn = T(0), wn = T(0);
+      if (j < c.ny && k < c.nz) { un = proj_u<T>(c, i, j, k, dtr); c.u[(size_t)i + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k)] = un; }
+      if (i < c.nx && k < c.nz) { vn = proj_v<T>(c, i, j, k, dtr); c.v[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.nyv * k)] = vn; }
+      if (i < c.nx && j < c.ny) { wn = proj_w<T>(c, i, j, k, dtr); c.w[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k)] = wn; }
+      if (i < c.nx && j < c.ny && k < c.nz) {
+        const T ue = proj_u<T>(c, c.bx ? i + 1 : (i + 1 == c.nx ? 0 : i + 1), j, k, dtr);
+        const T vt = proj_v<T>(c, i, c.by ? j + 1 : (j + 1 == c.ny ? 0 : j + 1), k, dtr);
+        const T wt = proj_w<T>(c, i, j, c.bz ? k + 1 : (k + 1 == c.nz ? 0 : k + 1), dtr);
+        const T div = (ue - un) * c.ihx + (vt - vn) * c.idy[j + 1] + (wt - wn) * c.ihz;
+        const double a = fabs((double)div);
+        if (a != a) nan = 1;
+        md = fmax(md, a);
+        const double dyj = c.dy64[j];
+        const double e = -dyj * sc * (double)div - mc * dyj;
+        v[0] += e * e;
+      }
+    }
+  }
+  // max and NaN flag are order-independent: plain atomics keep them deterministic
+  md = warp_max(md);
+  nan = __any_sync(0xffffffffu, nan);
+  if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0) {
+    if (md > 0.0) atomicMax((unsigned long long*)&c.S->max_div, (unsigned long long)__double_as_longlong(md));
+    if (nan) atomicOr(&c.S->nan_flag, 1);
+  }
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0 && threadIdx.y == 0) c.S->true_rr = v[0];
+  }
+}
+
+struct ColGeom { dim3 grid, block; int kz; };
+ColGeom col_geom(int nx, int ny, int nz);
+ColGeom col_geom(int nx, int ny, int nz) {
+  ColGeom g;
+  const int tx = nx >= 64 ? 64 : 32, ty = 256 / tx;
+  g.block = dim3(tx, ty, 1);
+  const int bxn = (nx + tx - 1) / tx, byn = (ny + ty - 1) / ty;
+  // z chunk: aim at >= 4 waves of 148 blocks but keep chunks >= 8 planes and partials <= kMaxPartials
+  int kz = nz;
+  while (kz > 8 && (long long)bxn * byn * ((nz + kz - 1) / kz) < 4 * 148) kz = (kz + 1) / 2;
+  while ((long long)bxn * byn * ((nz + kz - 1) / kz) > kMaxPartials) kz *= 2;
+  g.kz = kz;
+  g.grid = dim3(bxn, byn, (nz + kz - 1) / kz);
+  return g;
+}
+
+template <class T> int launch_project(const Ctx<T>& c, const Launch& L) {
+  ColGeom g = col_geom(c.nxu, c.nyv, c.nzw);
+  k_project<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz);
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// S9 + S10: rigid-body oscillator m w'' + c w' + k w = F (Eq. 12) advanced by one classical
+// RK4 step with the force frozen over the step (weak coupling, L212); markers translate with the body;
+// AB2 history flag and step counter.  One block.
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double body_acc(double F, double cc, double kk, double m, double a, double b) { return (F - cc * b - kk * a) / m; }
+
+template <class T> __global__ void k_step_end(const Ctx<T> c, const IbmCtx ib) {
+  __shared__ double dw[3], nv[3];
+  Scalars* S = c.S;
+  if (threadIdx.x == 0) {
+    for (int a = 0; a < 3; ++a) { dw[a] = 0.0; nv[a] = S->body_vel[a]; }
+    if (ib.has_body) {
+      const double dt = c.dt, m = ib.bm, cc = ib.bc, kk = ib.bk;
+      for (int a = 0; a < 3; ++a) if (ib.dof & (1 << a)) {
+        const double F = S->body_force[a], y0 = S->body_disp[a], y1 = S->body_vel[a];
+        const double k1a = y1,                  k1b = body_acc(F, cc, kk, m, y0, y1);
+        const double k2a = y1 + 0.5 * dt * k1b, k2b = body_acc(F, cc, kk, m, y0 + 0.5 * dt * k1a, y1 + 0.5 * dt * k1b);
+        const double k3a = y1 + 0.5 * dt * k2b, k3b = body_acc(F, cc, kk, m, y0 + 0.5 * dt * k2a, y1 + 0.5 * dt * k2b);
+        const double k4a = y1 + dt * k3b,       k4b = body_acc(F, cc, kk, m, y0 + dt * k3a, y1 + dt * k3b);
+        const double w1 = y0 + dt / 6.0 * (k1a + 2.0 * k2a + 2.0 * k3a + k4a);
+        const double v1 = y1 + dt / 6.0 * (k1b + 2.0 * k2b + 2.0 * k3b + k4b);
+        dw[a] = w1 - y0; nv[a] = v1;
+        S->body_disp[a] = w1; S->body_vel[a] = v1;
+      }
+    }
+    S->have_hist = 1; S->step += 1; S->total_iters += S->iter;
+  }
+  __syncthreads();
+  if (ib.has_body) {
+    for (int l = threadIdx.x; l < ib.n; l += blockDim.x)
+      for (int a = 0; a < 3; ++a) {
+        if (ib.dof & (1 << a)) ib.X[3 * l + a] = __dadd_rn(ib.X[3 * l + a], dw[a]);
+        ib.Ub[3 * l + a] = nv[a];
+      }
+  }
+}
+template <class T> int launch_step_end(const Ctx<T>& c, const IbmCtx& ib, const Launch& L) {
+  k_step_end<T><<<1, 256, 0, L.s>>>(c, ib);
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// dtype conversion / constant shift helpers for fs_fields_set / fs_fields_get
+// ---------------------------------------------------------------------------------------------------
+template <class TS, class TD> __global__ void k_convert(const TS* __restrict__ s, TD* __restrict__ d, long long n) {
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n; q += (long long)gridDim.x * blockDim.x) d[q] = (TD)s[q];
+}
+template <class TS, class TD> void launch_convert(const TS* src, TD* dst, long long n, cudaStream_t s) {
+  if (n <= 0) return;
+  k_convert<TS, TD><<<flat_blocks(n), 256, 0, s>>>(src, dst, n);
+}
+template <class T> __global__ void k_scale(T* __restrict__ x, T a, long long n) {
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n; q += (long long)gridDim.x * blockDim.x) x[q] *= a;
+}
+template <class T> void launch_scale(T* x, double a, long long n, cudaStream_t s) {
+  if (n <= 0) return;
+  k_scale<T><<<flat_blocks(n), 256, 0, s>>>(x, (T)a, n);
+}
+
+#define INST(T)                                                                                        \
+  template int launch_momentum<T>(const Ctx<T>&, const Launch&);                                       \
+  template int launch_flux_correction<T>(const Ctx<T>&, const Launch&);                                \
+  template int launch_div_rhs<T>(const Ctx<T>&, const Launch&);                                        \
+  template int launch_rhs_from_b<T>(const Ctx<T>&, const T*, const Launch&);                           \
+  template int launch_project<T>(const Ctx<T>&, const Launch&);                                        \
+  template int launch_divergence<T>(const Ctx<T>&, const T*, const T*, const T*, T*, const Launch&);   \
+  template int launch_step_end<T>(const Ctx<T>&, const IbmCtx&, const Launch&);                        \
+  template void launch_scale<T>(T*, double, long long, cudaStream_t);
+INST(float)
+INST(double)
+template void launch_convert<float, double>(const float*, double*, long long, cudaStream_t);
+template void launch_convert<double, float>(const double*, float*, long long, cudaStream_t);
+template void launch_convert<float, float>(const float*, float*, long long, cudaStream_t);
+template void launch_convert<double, double>(const double*, double*, long long, cudaStream_t);
+
+}  // namespace fs

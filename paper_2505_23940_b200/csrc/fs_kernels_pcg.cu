@@ -1,0 +1,245 @@
+// fs_kernels_pcg.cu -- pressure Poisson solve (S6 tail, S7): matrix-free 7-point operator
+// A = -dy_j L (symmetric positive semi-definite) and textbook preconditioned CG (O7;
+// solver family PAPER.md L449, CG L686).  The Laplacian apply is fused with the d.q dot product and
+// the x/r update with the residual norm; all sums are deterministic (fs_internal.cuh grid_sum).
+// Loop control lives in device memory: the last block of k_pcg_update decides whether the CUDA-graph
+// WHILE node runs another iteration.
+#include "fs_internal.cuh"
+
+namespace fs {
+
+struct ColGeom { dim3 grid, block; int kz; };
+ColGeom col_geom(int nx, int ny, int nz);
+constexpr int kFlatBlocks = 148 * 8;
+static inline int flat_blocks(long long n) { long long b = (n + 255) / 256; return (int)(b < kFlatBlocks ? (b < 1 ? 1 : b) : kFlatBlocks); }
+
+// Jacobi diagonal of A at (i,j,k): dy_j * (sum of the face coefficients that exist).
+template <class T> __device__ __forceinline__ T diag_A(const Ctx<T>& c, int i, int j, int k) {
+  const T cx = T((c.bx && i == 0 ? 0 : 1) + (c.bx && i == c.nx - 1 ? 0 : 1)) * c.ihx2;
+  const T cz = T((c.bz && k == 0 ? 0 : 1) + (c.bz && k == c.nz - 1 ? 0 : 1)) * c.ihz2;
+  const T cy = (c.cyh[j] + c.cyl[j]) * c.idy[j + 1];
+  return (cx + cy + cz) * c.dy[j + 1];
+}
+// z = M^-1 r for the point preconditioners
+template <class T> __device__ __forceinline__ T precond_point(const Ctx<T>& c, T r, int i, int j, int k) {
+  return c.precond == FS_PC_JACOBI ? r / diag_A<T>(c, i, j, k) : r;
+}
+
+// Column-marching application of A: thread (i,j) walks k0..k1-1 keeping x(k-1), x(k), x(k+1) in
+// registers; x+-1 / y+-1 neighbours come through L1.  Neighbour indices wrap (periodic) or clamp
+// (bounded: the clamped difference is exactly zero = homogeneous Neumann flux dropped).
+template <class T, class F> __device__ __forceinline__ void march_A(const Ctx<T>& c, const T* __restrict__ x, int i, int j, int k0, int k1, F&& f) {
+  const int im = i > 0 ? i - 1 : (c.bx ? 0 : c.nx - 1), ip = i + 1 < c.nx ? i + 1 : (c.bx ? i : 0);
+  const int jm = j > 0 ? j - 1 : (c.by ? 0 : c.ny - 1), jp = j + 1 < c.ny ? j + 1 : (c.by ? j : 0);
+  const size_t pl = (size_t)c.nx * c.ny;
+  const size_t oc = (size_t)i + (size_t)c.nx * j, ow = (size_t)im + (size_t)c.nx * j, oe = (size_t)ip + (size_t)c.nx * j;
+  const size_t os = (size_t)i + (size_t)c.nx * jm, on = (size_t)i + (size_t)c.nx * jp;
+  const T cyl = c.cyl[j], cyh = c.cyh[j], idy = c.idy[j + 1], ndy = -c.dy[j + 1];
+  const int kb = k0 > 0 ? k0 - 1 : (c.bz ? 0 : c.nz - 1);
+  T xb = x[oc + pl * kb], xc = x[oc + pl * k0];
+  for (int k = k0; k < k1; ++k) {
+    const int kt = k + 1 < c.nz ? k + 1 : (c.bz ? k : 0);
+    const T xt = x[oc + pl * kt];
+    const size_t o = pl * k;
+    const T xw = x[ow + o], xe = x[oe + o], xs = x[os + o], xn = x[on + o];
+    T acc = (xe - xc) * c.ihx2 - (xc - xw) * c.ihx2;
+    const T fy = (xn - xc) * cyh - (xc - xs) * cyl;
+    acc += fy * idy;
+    acc += (xt - xc) * c.ihz2 - (xc - xb) * c.ihz2;
+    f(k, oc + o, xc, acc * ndy);
+    xb = xc; xc = xt;
+  }
+}
+
+// ---- PCG start: r = (bhat_raw - mean_coef dy_j) - A x0 ; ||bhat||^2, ||r||^2, r.z -------------------
+template <class T> __global__ void __launch_bounds__(256) k_pcg_init(const Ctx<T> c, int kz, Launch L) {
+  __shared__ double sh[3 * 32]; __shared__ int flag;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  double v[3] = {0.0, 0.0, 0.0};
+  if (i < c.nx && j < c.ny) {
+    const T shift = T(c.S->mean_coef) * c.dy[j + 1];
+    march_A<T>(c, c.p, i, j, k0, k1, [&](int k, size_t q, T xc, T Ax) {
+      const T bh = c.r[q] - shift;
+      const T r = bh - Ax;
+      c.r[q] = r;
+      c.bh[q] = bh;
+      const T z = precond_point<T>(c, r, i, j, k);
+      v[0] += (double)bh * (double)bh; v[1] += (double)r * (double)r; v[2] += (double)r * (double)z;
+    });
+  }
+  if (grid_sum<3>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0 && threadIdx.y == 0) {
+      Scalars* S = c.S;
+      S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
+      S->iter = 0; S->first = 1;
+      const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
+      S->converged = conv; S->done = conv || S->max_iter <= 0;
+      if (L.use_cond) cudaGraphSetConditional(L.cond, S->done ? 0u : 1u);
+    }
+  }
+}
+
+// ---- K4: d = z + beta d  (z from the point preconditioner, or the V-cycle output scaled by zs) -----
+template <class T> __global__ void __launch_bounds__(256) k_pcg_dir(const Ctx<T> c, T zs) {
+  const Scalars* S = c.S;
+  if (S->done) return;
+  const bool first = S->first != 0;
+  const T beta = first ? T(0) : T(S->rho_cur / S->rho_prev);
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  const bool gmg = c.precond == FS_PC_GMG;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+    T z;
+    if (gmg) z = c.z[q] * zs;
+    else {
+      const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
+      z = precond_point<T>(c, c.r[q], i, j, k);
+    }
+    c.d[q] = first ? z : z + beta * c.d[q];
+  }
+}
+
+// ---- K1: q = A d fused with d.q ------------------------------------------------------------------------
+template <class T> __global__ void __launch_bounds__(256) k_pcg_apply(const Ctx<T> c, int kz) {
+  __shared__ double sh[32]; __shared__ int flag;
+  if (c.S->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  double v[1] = {0.0};
+  if (i < c.nx && j < c.ny) {
+    march_A<T>(c, c.d, i, j, k0, k1, [&](int k, size_t q, T xc, T Ax) {
+      c.q[q] = Ax;
+      v[0] += (double)xc * (double)Ax;
+    });
+  }
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0 && threadIdx.y == 0) c.S->dq = v[0];
+  }
+}
+
+// ---- K2: x += alpha d, r -= alpha q fused with ||r||^2 and r.z; loop control -------------------------
+template <class T> __global__ void __launch_bounds__(256) k_pcg_update(const Ctx<T> c, Launch L) {
+  __shared__ double sh[2 * 32]; __shared__ int flag;
+  Scalars* S = c.S;
+  if (S->done) return;
+  const T alpha = T(S->rho_cur / S->dq);
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  const bool gmg = c.precond == FS_PC_GMG;
+  double v[2] = {0.0, 0.0};
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+    c.p[q] += alpha * c.d[q];
+    const T r = c.r[q] - alpha * c.q[q];
+    c.r[q] = r;
+    v[0] += (double)r * (double)r;
+    if (!gmg) {
+      const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
+      v[1] += (double)r * (double)precond_point<T>(c, r, i, j, k);
+    }
+  }
+  if (grid_sum<2>(v, c.partials, &S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0) {
+      S->rr = v[0];
+      S->iter += 1; S->first = 0;
+      S->rho_prev = S->rho_cur;
+      if (!gmg) S->rho_cur = v[1];
+      const int conv = sqrt(v[0]) <= S->rtol * sqrt(S->bnorm2);
+      S->converged = conv;
+      S->done = conv || S->iter >= S->max_iter;
+      if (L.use_cond) cudaGraphSetConditional(L.cond, S->done ? 0u : 1u);
+    }
+  }
+}
+
+// ---- GMG: rho = r . (zs z') after the V-cycle ----------------------------------------------------------
+template <class T> __global__ void __launch_bounds__(256) k_dot_rz(const Ctx<T> c, T zs) {
+  __shared__ double sh[32]; __shared__ int flag;
+  if (c.S->done) return;
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  double v[1] = {0.0};
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x)
+    v[0] += (double)c.r[q] * (double)(c.z[q] * zs);
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0) c.S->rho_cur = v[0];
+  }
+}
+
+template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L) {
+  ColGeom g = col_geom(c.nx, c.ny, c.nz);
+  int n = 0;
+  if (!c.warm_start) { cudaMemsetAsync(c.p, 0, sizeof(T) * (size_t)c.nx * c.ny * c.nz, L.s); ++n; }
+  k_pcg_init<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz, L);
+  return n + 1;
+}
+
+template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, const Launch& L) {
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  ColGeom g = col_geom(c.nx, c.ny, c.nz);
+  int n = 0;
+  T zs = T(1);
+  if (c.precond == FS_PC_GMG) {
+    zs = T(1.0 / c.hy);
+    n += launch_vcycle<T>(c, mg, c.r, c.z, L);
+    k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs); ++n;
+  }
+  k_pcg_dir<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs); ++n;
+  k_pcg_apply<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz); ++n;
+  k_pcg_update<T><<<flat_blocks(N), 256, 0, L.s>>>(c, L); ++n;
+  return n;
+}
+
+// ---- after the loop: zero-mean pressure (volume-weighted), SURVEY O6 ---------------------------------
+template <class T> __global__ void __launch_bounds__(256) k_pmean(const Ctx<T> c) {
+  __shared__ double sh[32]; __shared__ int flag;
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  double v[1] = {0.0};
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+    const int j = (int)((q / c.nx) % c.ny);
+    v[0] += (double)c.p[q] * c.dy64[j];
+  }
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0) c.S->pmean = v[0] / c.S->sum_dy;
+  }
+}
+template <class T> __global__ void __launch_bounds__(256) k_pshift(const Ctx<T> c) {
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  const T m = T(c.S->pmean);
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) c.p[q] -= m;
+}
+template <class T> int launch_pcg_finish(const Ctx<T>& c, const Launch& L) {
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  k_pmean<T><<<flat_blocks(N), 256, 0, L.s>>>(c);
+  k_pshift<T><<<flat_blocks(N), 256, 0, L.s>>>(c);
+  return 2;
+}
+
+// ---- true residual ||bhat - A p||^2 (fs_poisson_solve; fs_step gets it from the projection) ---------
+template <class T> __global__ void __launch_bounds__(256) k_true_res(const Ctx<T> c, int kz) {
+  __shared__ double sh[32]; __shared__ int flag;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  double v[1] = {0.0};
+  if (i < c.nx && j < c.ny) {
+    march_A<T>(c, c.p, i, j, k0, k1, [&](int k, size_t q, T xc, T Ax) {
+      const double e = (double)c.bh[q] - (double)Ax;
+      v[0] += e * e;
+    });
+  }
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0 && threadIdx.y == 0) c.S->true_rr = v[0];
+  }
+}
+template <class T> int launch_true_residual(const Ctx<T>& c, const Launch& L) {
+  ColGeom g = col_geom(c.nx, c.ny, c.nz);
+  k_true_res<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz);
+  return 1;
+}
+
+#define INST(T)                                                                   \
+  template int launch_pcg_init<T>(const Ctx<T>&, const Launch&);                  \
+  template int launch_pcg_body<T>(const Ctx<T>&, const MgCtx<T>&, const Launch&); \
+  template int launch_pcg_finish<T>(const Ctx<T>&, const Launch&);                \
+  template int launch_true_residual<T>(const Ctx<T>&, const Launch&);
+INST(float)
+INST(double)
+
+}  // namespace fs
