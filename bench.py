@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of one full fractional step (all rows of SURVEY.md 8(a)) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--n 512]
+    python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
+
+Workload (BASELINE.json configs[4], the case north_star's target is stated on): decaying homogeneous
+isotropic turbulence, triply periodic n^3 (default 512^3), random-phase solenoidal field with
+E(k) ~ k^4 exp(-2 (k/4)^2), u_rms = 1, nu = 1e-3, dt = 5e-4, AB2, GMG-preconditioned CG to rel tol
+1e-8.  Synthetic, seeded (fs_workloads.hit).  One "step" = one fs_step = momentum RHS + predictor,
+(IBM: none in c5), Poisson RHS, PCG with one V(2,2) cycle per iteration, projection.
+
+Prints ONE JSON line (contract in the task statement): metric Mcell-steps/s, `roofline` for the
+dominant kernel (event-timed through fs_profile_step), `cpu_baseline` (oracle on a bounded sample),
+`e2e` (host buffers in and out through the C ABI every step), `clocks`, `gpu_launches`.
+Multi-GPU: the path does not shard (replicas only) -- every rank advances
+its own independent grid, no collective on the data path; timing = max over ranks.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Mcell-steps/s per full fractional step"
+UNIT = "Mcell-steps/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--n", type=int, default=512, help="cells per direction of the HIT box (c5: 512)")
+    ap.add_argument("--ref-n", type=int, default=128, help="replica size the CPU oracle is timed on")
+    ap.add_argument("--exec", dest="exec_mode", default="graph", choices=["graph", "stream"],
+                    help="graph: one CUDA-graph replay per step (default); stream: same kernels launched directly (for ncu)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-profile", action="store_true")
+    return ap.parse_args()
+
+
+# ----------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------------------------------- reference arm
+def oracle_sample(n, steps, dtype_unused=None):
+    """The CPU oracle as it stands (single thread, fp64) on an n^3 replica of the workload."""
+    import fs_workloads as W
+    from oracle import Oracle
+    cfg = W.hit(n=n)
+    o = Oracle(cfg)
+    for c in "uvw":
+        o.set(c, cfg["init"][c])
+    t0 = time.perf_counter()
+    info = o.step(steps)
+    dt = time.perf_counter() - t0
+    return n ** 3 * steps / dt / 1e6, dt, info["iters_per_step"]
+
+
+def run_reference(a):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = a.ref_n
+    # warm-up on a tiny replica (library load, page-in), then K timed steps of the bounded sample
+    oracle_sample(32, max(1, min(a.warmup, 2)))
+    v, dt, iters = oracle_sample(n, a.steps)
+    sample = "c5 HIT replica %d^3 (same recipe, seed, nu, dt, GMG-PCG rtol 1e-8), %d steps, %.1f s" % (n, a.steps, dt)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+            "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "c5 decaying HIT, GMG-PCG; CPU oracle timed on a %d^3 replica" % n,
+                       "cells": n ** 3, "pcg_iters_per_step": iters},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------- our arm
+def run_ours(a):
+    import numpy as np
+    import torch
+    import fs_workloads as W
+    import paper_2505_23940_b200 as fs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    fs.lib()
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    n = a.n
+    cells = n ** 3
+    wbytes = 8 if a.dtype == "f64" else 4
+    cfg = W.hit(n=n, dtype=a.dtype, device=dev, exec_mode=a.exec_mode)   # seeded IC, built with torch FFT on the device
+    g = fs.from_workload(cfg, device=dev)
+    cfg["init"] = None
+    torch.cuda.empty_cache()
+    stream = g.stream
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events ----
+    for _ in range(a.warmup):
+        g.step(1, sync=False)
+    info_w = g.step(0)
+    l0 = g.launch_count()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    g.step(a.steps, sync=False)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    info = g.step(0)
+    launches = g.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    if dist is not None:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * cells * a.steps / (ms * 1e-3) / 1e6
+    iters_total = None
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): per step H2D of u,v,w, fs_step,
+    #      D2H of u,v,w,p ----
+    e2e = None
+    if not a.no_e2e:
+        tdt = torch.float64 if a.dtype == "f64" else torch.float32
+        host = {c: torch.empty(g.shape[c], dtype=tdt).pin_memory() for c in "uvwp"}
+        npv = {c: host[c].numpy() for c in "uvwp"}
+        for c in "uvwp":
+            g.get(c, dtype=a.dtype, out=npv[c])
+        ke = max(2, min(a.steps, 3))
+
+        def e2e_step():
+            for c in "uvw":
+                g.set(c, npv[c])
+            g.step(1, sync=False)
+            for c in "uvwp":
+                g.get(c, dtype=a.dtype, out=npv[c])
+
+        e2e_step()                                        # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            e2e_step()
+        barrier()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * cells * ke / dt / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": 3 * cells * wbytes, "d2h_bytes_per_step": 4 * cells * wbytes,
+               "steps": ke, "ms_per_step": 1e3 * dt / ke,
+               "api": "fs_fields_set(u,v,w: pinned host) -> fs_step(1) -> fs_fields_get(u,v,w,p: pinned host)"}
+        del host, npv
+
+    # ---- per-kernel event timing (same kernels, stream launches) -> roofline of the dominant kernel ----
+    roof, kernels = None, None
+    if not a.no_profile and rank == 0:
+        peak, peak_src = peaks()
+        ksteps = 2
+        prof = g.profile_step(ksteps)
+        tot = sum(v["ms"] for v in prof.values())
+        kernels = {k: {"launches_per_step": v["launches"] / ksteps, "ms_per_step": v["ms"] / ksteps,
+                       "share": v["ms"] / tot if tot else 0.0,
+                       "algorithmic_GBps": (v["bytes"] / (v["ms"] * 1e-3) / 1e9) if v["ms"] > 0 else None}
+                   for k, v in sorted(prof.items(), key=lambda kv: -kv[1]["ms"])}
+        top = max(prof.items(), key=lambda kv: kv[1]["ms"])
+        ach = top[1]["bytes"] / (top[1]["ms"] * 1e-3) / 1e9
+        step_bytes = sum(v["bytes"] for v in prof.values()) / ksteps
+        roof = {"bound": "hbm", "kernel": top[0], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": top[1]["bytes"] / top[1]["launches"],
+                "avg_launch_ms": top[1]["ms"] / top[1]["launches"], "share_of_step": top[1]["ms"] / tot,
+                "step": {"algorithmic_bytes": step_bytes, "achieved": step_bytes / (ms / a.steps * 1e-3) / 1e9,
+                         "frac": step_bytes / (ms / a.steps * 1e-3) / 1e9 / peak,
+                         "note": "sum of per-kernel algorithmic bytes of one step / graph-replay step time"}}
+    if dist is not None:
+        dist.barrier()
+
+    # ---- CPU oracle on a bounded sample (rank 0, N=1 only) ----
+    cpu = None
+    if not a.no_cpu and rank == 0 and world == 1:
+        v, dt, _ = oracle_sample(a.ref_n, 3)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "c5 HIT replica %d^3, 3 steps, %.1f s (single-threaded fp64 C++ oracle)" % (a.ref_n, dt)}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+                "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": a.dtype, "data": "synthetic",
+                "config": {"workload": "c5 decaying HIT %d^3 triply periodic, AB2, GMG-PCG rtol 1e-8 (BASELINE.json configs[4])" % n,
+                           "cells": cells, "parallelism": "replicas x%d (no sharding)" % world,
+                           "l2": "inputs larger than L2 (each field %.0f MB vs 126 MB L2)" % (cells * wbytes / 1e6),
+                           "pcg_iters_last_step": info["pcg_iters"], "rel_residual": info["rel_residual"],
+                           "true_rel_residual": info["true_rel_residual"], "max_abs_div": info["max_abs_div"],
+                           "converged": info["converged"], "nan_flag": info["nan_flag"],
+                           "exec": ("one CUDA graph replay per step, PCG loop = conditional WHILE node" if a.exec_mode == "graph"
+                                    else "stream launches, host polls the PCG flag")},
+                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
+                "gpu_launches": int(launches), "kernels": kernels}
+        print(json.dumps(line), flush=True)
+    g.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
+
+
+if __name__ == "__main__":
+    main()

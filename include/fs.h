@@ -145,6 +145,19 @@ fs_status fs_ibm_spread(fs_grid* g, const double* F);
 /*   fs_gmg_vcycle: z = M^-1 r, one V-cycle of the GMG preconditioner (r, z: nz*ny*nx fp64, HOST);
  *   FS_ERR_BAD_STATE unless precond == FS_PC_GMG.  Clobbers the PCG scratch fields only. */
 fs_status fs_gmg_vcycle(fs_grid* g, const double* r, double* z);
+/*   fs_momentum_rhs: runs the S1 kernel alone on the current u,v,w: FS_HU/HV/HW := H^n (Eq. 4),
+ *   overwriting the stored H^{n-1}; u,v,w,p are untouched (the predicted field goes to scratch). */
+fs_status fs_momentum_rhs(fs_grid* g);
+
+/* Per-kernel timing (measurement aid for bench.py's roofline block).  fs_profile_step advances nsteps
+ * steps with the SAME kernels launched directly on the grid's stream (not the graph), each bracketed by
+ * a CUDA event pair, and accumulates per kernel name: launches, milliseconds, and ALGORITHMIC bytes
+ * (the field words that pass must move).  Synchronises.  Entries are read back
+ * one by one (name: library-owned static string; all out pointers HOST). */
+fs_status fs_profile_step(fs_grid* g, int nsteps);
+fs_status fs_profile_count(fs_grid* g, int* n);
+fs_status fs_profile_entry(fs_grid* g, int idx, const char** name, long long* launches, double* ms, double* bytes);
+fs_status fs_profile_reset(fs_grid* g);
 
 /* Number of kernel launches (graph kernel nodes incl. loop-body replays) issued so far. */
 fs_status fs_launch_count(fs_grid* g, long long* launches);

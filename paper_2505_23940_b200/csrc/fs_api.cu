@@ -19,8 +19,35 @@ using namespace fs;
     }                                                                      \
   } while (0)
 
+// ---- per-kernel timing (fs_profile_step / fs_profile_entry) ---------------------------------------------
+namespace fs {
+struct ProfRec { const char* name; double bytes; cudaEvent_t e0, e1; };
+struct ProfAgg { const char* name; long long launches; double ms, bytes; };
+struct Prof { std::vector<ProfRec> recs; std::vector<ProfAgg> agg; };
+void prof_begin(Prof* p, const char* name, double bytes, cudaStream_t s) {
+  ProfRec r{name, bytes, nullptr, nullptr};
+  cudaEventCreate(&r.e0); cudaEventCreate(&r.e1);
+  cudaEventRecord(r.e0, s);
+  p->recs.push_back(r);
+}
+void prof_end(Prof* p, cudaStream_t s) { cudaEventRecord(p->recs.back().e1, s); }
+static void prof_collect(Prof* p) {     // caller has synchronised the stream
+  for (ProfRec& r : p->recs) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, r.e0, r.e1);
+    cudaEventDestroy(r.e0); cudaEventDestroy(r.e1);
+    ProfAgg* a = nullptr;
+    for (ProfAgg& x : p->agg) if (std::strcmp(x.name, r.name) == 0) { a = &x; break; }
+    if (!a) { p->agg.push_back(ProfAgg{r.name, 0, 0.0, 0.0}); a = &p->agg.back(); }
+    a->launches += 1; a->ms += ms; a->bytes += r.bytes;
+  }
+  p->recs.clear();
+}
+}  // namespace fs
+
 struct fs_grid {
   fs_params P;
+  fs::Prof prof; bool profiling = false;
   std::vector<double> yf;
   bool f64 = true;
   int bx = 0, by = 0, bz = 0, nxu = 0, nyv = 0, nzw = 0;
@@ -274,7 +301,7 @@ template <class T> fs_status build_graph(fs_grid* g, bool poisson, cudaGraphExec
 
 // FS_EXEC_STREAM: same kernels, launched directly; the host polls the done flag between chunks.
 template <class T> fs_status run_stream(fs_grid* g, bool poisson, int* n_fixed, int* n_body) {
-  Launch L{g->stream, 0, 0};
+  Launch L{g->stream, 0, 0, g->profiling ? &g->prof : nullptr};
   const int npre = enqueue_pre<T>(g, L, poisson);
   int nbody = 0;
   for (;;) {
@@ -291,7 +318,7 @@ template <class T> fs_status run_stream(fs_grid* g, bool poisson, int* n_fixed, 
 }
 
 template <class T> fs_status run_once(fs_grid* g, bool poisson) {
-  if (g->P.exec_mode == FS_EXEC_STREAM) {
+  if (g->P.exec_mode == FS_EXEC_STREAM || g->profiling) {
     int nf = 0, nb = 0;
     fs_status st = run_stream<T>(g, poisson, &nf, &nb);
     if (st != FS_OK) return st;
@@ -655,6 +682,47 @@ fs_status fs_gmg_vcycle(fs_grid* g, const double* r, double* z) {
     CK(cudaGetLastError());
     st = copy_out<float>(g, g->cf.z, g->nP, z, FS_F64, 0); if (st != FS_OK) return st;
   }
+  return FS_OK;
+}
+
+fs_status fs_momentum_rhs(fs_grid* g) {
+  if (!g) return FS_ERR_INVALID_ARG;
+  Launch L{g->stream, 0, 0};
+  g->fixed_launches += g->f64 ? launch_momentum<double>(g->cd, L) : launch_momentum<float>(g->cf, L);
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+fs_status fs_profile_step(fs_grid* g, int nsteps) {
+  if (!g || nsteps < 0) return FS_ERR_INVALID_ARG;
+  g->profiling = true;
+  fs_status st = FS_OK;
+  for (int s = 0; s < nsteps && st == FS_OK; ++s) {
+    st = g->f64 ? run_once<double>(g, false) : run_once<float>(g, false);
+    if (st == FS_OK && cudaStreamSynchronize(g->stream) != cudaSuccess) st = FS_ERR_CUDA;
+    prof_collect(&g->prof);
+  }
+  g->profiling = false;
+  return st;
+}
+
+fs_status fs_profile_count(fs_grid* g, int* n) {
+  if (!g || !n) return FS_ERR_INVALID_ARG;
+  *n = (int)g->prof.agg.size();
+  return FS_OK;
+}
+
+fs_status fs_profile_entry(fs_grid* g, int idx, const char** name, long long* launches, double* ms, double* bytes) {
+  if (!g || idx < 0 || idx >= (int)g->prof.agg.size() || !name || !launches || !ms || !bytes) return FS_ERR_INVALID_ARG;
+  const ProfAgg& a = g->prof.agg[idx];
+  *name = a.name; *launches = a.launches; *ms = a.ms; *bytes = a.bytes;
+  return FS_OK;
+}
+
+fs_status fs_profile_reset(fs_grid* g) {
+  if (!g) return FS_ERR_INVALID_ARG;
+  g->prof.agg.clear();
   return FS_OK;
 }
 

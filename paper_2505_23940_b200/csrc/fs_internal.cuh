@@ -21,6 +21,7 @@ struct Scalars {
   double bnorm2, rr;     // ||bhat||^2, ||r||^2 (recurrence residual)
   double rho_cur, rho_prev, dq;
   double pmean;
+  double rmean;         // fp32 only: mean of the recurrence residual, removed with one iteration of lag (null-space deflation)
   double sum_dy;         // sum over all cells of dy_j
   int iter, done, converged, first;
   int max_iter, pad0;
@@ -81,7 +82,19 @@ struct IbmCtx {
   int has_body, dof; double bm, bc, bk;
 };
 
-struct Launch { cudaStream_t s; cudaGraphConditionalHandle cond; int use_cond; };
+// Per-kernel timing (measurement aid, fs_profile_step): when prof != nullptr every launch is bracketed
+// by a CUDA event pair on the launching stream and tagged with its name and ALGORITHMIC bytes (the
+// field words the pass must move; not what the hardware happened to move).
+struct Prof;
+void prof_begin(Prof* p, const char* name, double bytes, cudaStream_t s);
+void prof_end(Prof* p, cudaStream_t s);
+struct Launch { cudaStream_t s; cudaGraphConditionalHandle cond; int use_cond; Prof* prof; };
+#define FS_LAUNCH(L, name, bytes, ...)                              \
+  do {                                                              \
+    if ((L).prof) prof_begin((L).prof, name, (double)(bytes), (L).s); \
+    __VA_ARGS__;                                                    \
+    if ((L).prof) prof_end((L).prof, (L).s);                        \
+  } while (0)
 
 // ---- launchers (one per kernel family; each returns the number of kernels it enqueued) ----------
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L);

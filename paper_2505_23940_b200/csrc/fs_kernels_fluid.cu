@@ -183,7 +183,7 @@ template <class T> __global__ void __launch_bounds__(256) k_momentum(const Ctx<T
 
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
   dim3 b(32, 4, 2), g((c.nxu + 31) / 32, (c.nyv + 3) / 4, (c.nzw + 1) / 2);
-  k_momentum<T><<<g, b, 0, L.s>>>(c);
+  FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T><<<g, b, 0, L.s>>>(c));
   return 1;
 }
 
@@ -256,8 +256,8 @@ template <class T> int launch_flux_correction(const Ctx<T>& c, const Launch& L) 
   bool any = false;
   for (int f = 0; f < 6; ++f) any |= c.bc[f] == FS_BC_OUTFLOW_CONVECTIVE;
   if (!any) return 0;
-  k_flux_sum<T><<<64, 256, 0, L.s>>>(c);
-  k_flux_apply<T><<<64, 256, 0, L.s>>>(c);
+  FS_LAUNCH(L, "flux_sum", 0.0, k_flux_sum<T><<<64, 256, 0, L.s>>>(c));
+  FS_LAUNCH(L, "flux_apply", 0.0, k_flux_apply<T><<<64, 256, 0, L.s>>>(c));
   return 2;
 }
 
@@ -301,12 +301,12 @@ static inline int flat_blocks(long long n) { long long b = (n + 255) / 256; retu
 
 template <class T> int launch_div_rhs(const Ctx<T>& c, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;
-  k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, nullptr);
+  FS_LAUNCH(L, "div_rhs", 4.0 * sizeof(T) * N, k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, nullptr));
   return 1;
 }
 template <class T> int launch_rhs_from_b(const Ctx<T>& c, const T* b, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;
-  k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, b);
+  FS_LAUNCH(L, "div_rhs", 2.0 * sizeof(T) * N, k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, b));
   return 1;
 }
 
@@ -327,7 +327,7 @@ template <class T> __global__ void __launch_bounds__(256) k_divergence(const Ctx
 }
 template <class T> int launch_divergence(const Ctx<T>& c, const T* u, const T* v, const T* w, T* out, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;
-  k_divergence<T><<<flat_blocks(N), 256, 0, L.s>>>(c, u, v, w, out);
+  FS_LAUNCH(L, "divergence", 4.0 * sizeof(T) * N, k_divergence<T><<<flat_blocks(N), 256, 0, L.s>>>(c, u, v, w, out));
   return 1;
 }
 
@@ -418,7 +418,7 @@ ColGeom col_geom(int nx, int ny, int nz) {
 
 template <class T> int launch_project(const Ctx<T>& c, const Launch& L) {
   ColGeom g = col_geom(c.nxu, c.nyv, c.nzw);
-  k_project<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz);
+  FS_LAUNCH(L, "project", 7.0 * sizeof(T) * c.nx * c.ny * c.nz, k_project<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz));
   return 1;
 }
 
@@ -460,7 +460,7 @@ template <class T> __global__ void k_step_end(const Ctx<T> c, const IbmCtx ib) {
   }
 }
 template <class T> int launch_step_end(const Ctx<T>& c, const IbmCtx& ib, const Launch& L) {
-  k_step_end<T><<<1, 256, 0, L.s>>>(c, ib);
+  FS_LAUNCH(L, "step_end", 0.0, k_step_end<T><<<1, 256, 0, L.s>>>(c, ib));
   return 1;
 }
 

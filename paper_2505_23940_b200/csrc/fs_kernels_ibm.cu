@@ -132,9 +132,9 @@ template <class T> __global__ void __launch_bounds__(1024) k_ibm_segments(const 
 template <class T> int launch_ibm_index(const Ctx<T>& c, const IbmCtx& ib, const Launch& L) {
   if (ib.n <= 0) return 0;
   const int nb = (ib.n + 255) / 256;
-  k_ibm_index<T><<<nb, 256, 0, L.s>>>(c, ib);
-  k_ibm_rank<<<nb, 256, 0, L.s>>>(ib);
-  k_ibm_segments<T><<<1, 1024, 0, L.s>>>(c, ib);
+  FS_LAUNCH(L, "ibm_index", 0.0, k_ibm_index<T><<<nb, 256, 0, L.s>>>(c, ib));
+  FS_LAUNCH(L, "ibm_rank", 0.0, k_ibm_rank<<<nb, 256, 0, L.s>>>(ib));
+  FS_LAUNCH(L, "ibm_segments", 0.0, k_ibm_segments<T><<<1, 1024, 0, L.s>>>(c, ib));
   return 3;
 }
 
@@ -164,7 +164,7 @@ template <class T> __global__ void __launch_bounds__(128) k_ibm_interp(const Ctx
 }
 template <class T> int launch_ibm_interpolate(const Ctx<T>& c, const IbmCtx& ib, const T* u, const T* v, const T* w, double* out, const Launch& L) {
   if (ib.n <= 0) return 0;
-  k_ibm_interp<T><<<(3 * ib.n + 127) / 128, 128, 0, L.s>>>(c, ib, u, v, w, out);
+  FS_LAUNCH(L, "ibm_interpolate", 3.0 * ib.sw * ib.sw * ib.sw * ib.n * sizeof(T), k_ibm_interp<T><<<(3 * ib.n + 127) / 128, 128, 0, L.s>>>(c, ib, u, v, w, out));
   return 1;
 }
 
@@ -183,7 +183,7 @@ template <class T> __global__ void __launch_bounds__(1024) k_ibm_force(const Ctx
 }
 template <class T> int launch_ibm_force(const Ctx<T>& c, const IbmCtx& ib, const Launch& L) {
   if (ib.n <= 0) return 0;
-  k_ibm_force<T><<<1, 1024, 0, L.s>>>(c, ib);
+  FS_LAUNCH(L, "ibm_force", 0.0, k_ibm_force<T><<<1, 1024, 0, L.s>>>(c, ib));
   return 1;
 }
 
@@ -261,7 +261,7 @@ template <class T> __global__ void __launch_bounds__(128) k_ibm_spread(const Ctx
 }
 template <class T> int launch_ibm_spread(const Ctx<T>& c, const IbmCtx& ib, const double* F, T* u, T* v, T* w, double scale, const Launch& L) {
   if (ib.n <= 0) return 0;
-  k_ibm_spread<T><<<148 * 4, 128, 0, L.s>>>(c, ib, F, u, v, w, scale);
+  FS_LAUNCH(L, "ibm_spread", 6.0 * ib.sw * ib.sw * ib.sw * ib.n * sizeof(T), k_ibm_spread<T><<<148 * 4, 128, 0, L.s>>>(c, ib, F, u, v, w, scale));
   return 1;
 }
 

@@ -88,19 +88,19 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     T* a = (swaps % 2 == 0) ? el[l] : tl[l];          // so that the level's final iterate lands in el[l]
     T* b = (swaps % 2 == 0) ? tl[l] : el[l];
     if (pre > 0) {
-      k_mg_first<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, cw, N); ++n;
+      FS_LAUNCH(L, l == 0 ? "mg_first_l0" : "mg_coarse", 2.0 * sizeof(T) * N, k_mg_first<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, cw, N)); ++n;
       for (int it = 1; it < pre; ++it) {
-        k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, b, V.nx, V.ny, V.nz, ih2, cw); ++n;
+        FS_LAUNCH(L, l == 0 ? "mg_sweep_l0" : "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, b, V.nx, V.ny, V.nz, ih2, cw)); ++n;
         T* t = a; a = b; b = t;
       }
       cur[l] = a;
     } else {
       cur[l] = nullptr;                                // e = 0
-      if (coarsest) { cudaMemsetAsync(el[l], 0, sizeof(T) * (size_t)N, L.s); ++n; cur[l] = el[l]; }
+      if (coarsest) { FS_LAUNCH(L, "mg_coarse", 1.0 * sizeof(T) * N, cudaMemsetAsync(el[l], 0, sizeof(T) * (size_t)N, L.s)); ++n; cur[l] = el[l]; }
     }
     if (!coarsest) {
       const long long Nc = N / 8;
-      k_mg_restrict<T><<<flat_blocks(Nc), 256, 0, L.s>>>(done, gl[l], cur[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, ih2); ++n;
+      FS_LAUNCH(L, l == 0 ? "mg_restrict_l0" : "mg_coarse", (cur[l] ? 2.125 : 1.125) * sizeof(T) * N, k_mg_restrict<T><<<flat_blocks(Nc), 256, 0, L.s>>>(done, gl[l], cur[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, ih2)); ++n;
     }
   }
   // upward leg
@@ -110,11 +110,11 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     const T ih2 = T(1.0 / (V.h * V.h)), cw = T(mg.omega * V.h * V.h / 6.0);
     T* a = cur[l];
     T* dst = a ? a : ((mg.nu2 % 2 == 0) ? el[l] : tl[l]);
-    k_mg_prolong<T><<<flat_blocks(N), 256, 0, L.s>>>(done, el[l + 1], a, dst, V.nx, V.ny, V.nz); ++n;
+    FS_LAUNCH(L, l == 0 ? "mg_prolong_l0" : "mg_coarse", (a ? 2.125 : 1.125) * sizeof(T) * N, k_mg_prolong<T><<<flat_blocks(N), 256, 0, L.s>>>(done, el[l + 1], a, dst, V.nx, V.ny, V.nz)); ++n;
     a = dst;
     T* b = a == el[l] ? tl[l] : el[l];
     for (int it = 0; it < mg.nu2; ++it) {
-      k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, b, V.nx, V.ny, V.nz, ih2, cw); ++n;
+      FS_LAUNCH(L, l == 0 ? "mg_sweep_l0" : "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, b, V.nx, V.ny, V.nz, ih2, cw)); ++n;
       T* t = a; a = b; b = t;
     }
     // a == el[l] by construction of the swap parity

@@ -53,10 +53,10 @@ template <class T, class F> __device__ __forceinline__ void march_A(const Ctx<T>
 
 // ---- PCG start: r = (bhat_raw - mean_coef dy_j) - A x0 ; ||bhat||^2, ||r||^2, r.z -------------------
 template <class T> __global__ void __launch_bounds__(256) k_pcg_init(const Ctx<T> c, int kz, Launch L) {
-  __shared__ double sh[3 * 32]; __shared__ int flag;
+  __shared__ double sh[4 * 32]; __shared__ int flag;
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
-  double v[3] = {0.0, 0.0, 0.0};
+  double v[4] = {0.0, 0.0, 0.0, 0.0};
   if (i < c.nx && j < c.ny) {
     const T shift = T(c.S->mean_coef) * c.dy[j + 1];
     march_A<T>(c, c.p, i, j, k0, k1, [&](int k, size_t q, T xc, T Ax) {
@@ -65,14 +65,15 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_init(const Ctx<T
       c.r[q] = r;
       c.bh[q] = bh;
       const T z = precond_point<T>(c, r, i, j, k);
-      v[0] += (double)bh * (double)bh; v[1] += (double)r * (double)r; v[2] += (double)r * (double)z;
+      v[0] += (double)bh * (double)bh; v[1] += (double)r * (double)r; v[2] += (double)r * (double)z; v[3] += (double)r;
     });
   }
-  if (grid_sum<3>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+  if (grid_sum<4>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
     if (threadIdx.x == 0 && threadIdx.y == 0) {
       Scalars* S = c.S;
       S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
       S->iter = 0; S->first = 1;
+      S->rmean = v[3] / ((double)c.nx * c.ny * c.nz);
       const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
       S->converged = conv; S->done = conv || S->max_iter <= 0;
       if (L.use_cond) cudaGraphSetConditional(L.cond, S->done ? 0u : 1u);
@@ -118,27 +119,33 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_apply(const Ctx<
 }
 
 // ---- K2: x += alpha d, r -= alpha q fused with ||r||^2 and r.z; loop control -------------------------
+// fp32 only: rounding makes sum(q) != 0, so r slowly acquires a component along the null space of A
+// (constants) that CG can never remove; once it dominates r the fp32 stencil differences lose all
+// accuracy and the iteration diverges.  The mean of r measured by the previous pass is subtracted here
+// (one iteration of lag; exactly zero in exact arithmetic, where sum(r) = 0).  fp64 follows O7 literally.
 template <class T> __global__ void __launch_bounds__(256) k_pcg_update(const Ctx<T> c, Launch L) {
-  __shared__ double sh[2 * 32]; __shared__ int flag;
+  __shared__ double sh[3 * 32]; __shared__ int flag;
   Scalars* S = c.S;
   if (S->done) return;
   const T alpha = T(S->rho_cur / S->dq);
   const long long N = (long long)c.nx * c.ny * c.nz;
   const bool gmg = c.precond == FS_PC_GMG;
-  double v[2] = {0.0, 0.0};
+  const T rm = sizeof(T) == 4 ? T(S->rmean) : T(0);
+  double v[3] = {0.0, 0.0, 0.0};
   for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
     c.p[q] += alpha * c.d[q];
-    const T r = c.r[q] - alpha * c.q[q];
+    T r = c.r[q] - alpha * c.q[q];
+    if (sizeof(T) == 4) r -= rm;
     c.r[q] = r;
-    v[0] += (double)r * (double)r;
+    v[0] += (double)r * (double)r; v[2] += (double)r;
     if (!gmg) {
       const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
       v[1] += (double)r * (double)precond_point<T>(c, r, i, j, k);
     }
   }
-  if (grid_sum<2>(v, c.partials, &S->ticket[0], sh, &flag)) {
+  if (grid_sum<3>(v, c.partials, &S->ticket[0], sh, &flag)) {
     if (threadIdx.x == 0) {
-      S->rr = v[0];
+      S->rr = v[0]; S->rmean = v[2] / (double)N;
       S->iter += 1; S->first = 0;
       S->rho_prev = S->rho_cur;
       if (!gmg) S->rho_cur = v[1];
@@ -166,8 +173,8 @@ template <class T> __global__ void __launch_bounds__(256) k_dot_rz(const Ctx<T> 
 template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L) {
   ColGeom g = col_geom(c.nx, c.ny, c.nz);
   int n = 0;
-  if (!c.warm_start) { cudaMemsetAsync(c.p, 0, sizeof(T) * (size_t)c.nx * c.ny * c.nz, L.s); ++n; }
-  k_pcg_init<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz, L);
+  if (!c.warm_start) { FS_LAUNCH(L, "memset_p", 1.0 * sizeof(T) * c.nx * c.ny * c.nz, cudaMemsetAsync(c.p, 0, sizeof(T) * (size_t)c.nx * c.ny * c.nz, L.s)); ++n; }
+  FS_LAUNCH(L, "pcg_init", 4.0 * sizeof(T) * c.nx * c.ny * c.nz, k_pcg_init<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz, L));
   return n + 1;
 }
 
@@ -179,11 +186,11 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
   if (c.precond == FS_PC_GMG) {
     zs = T(1.0 / c.hy);
     n += launch_vcycle<T>(c, mg, c.r, c.z, L);
-    k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs); ++n;
+    FS_LAUNCH(L, "pcg_dot_rz", 2.0 * sizeof(T) * N, k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n;
   }
-  k_pcg_dir<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs); ++n;
-  k_pcg_apply<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz); ++n;
-  k_pcg_update<T><<<flat_blocks(N), 256, 0, L.s>>>(c, L); ++n;
+  FS_LAUNCH(L, "pcg_dir", 3.0 * sizeof(T) * N, k_pcg_dir<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n;
+  FS_LAUNCH(L, "pcg_apply_dot", 2.0 * sizeof(T) * N, k_pcg_apply<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz)); ++n;
+  FS_LAUNCH(L, "pcg_update_norm", 6.0 * sizeof(T) * N, k_pcg_update<T><<<flat_blocks(N), 256, 0, L.s>>>(c, L)); ++n;
   return n;
 }
 
@@ -207,8 +214,8 @@ template <class T> __global__ void __launch_bounds__(256) k_pshift(const Ctx<T> 
 }
 template <class T> int launch_pcg_finish(const Ctx<T>& c, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;
-  k_pmean<T><<<flat_blocks(N), 256, 0, L.s>>>(c);
-  k_pshift<T><<<flat_blocks(N), 256, 0, L.s>>>(c);
+  FS_LAUNCH(L, "p_mean", 1.0 * sizeof(T) * N, k_pmean<T><<<flat_blocks(N), 256, 0, L.s>>>(c));
+  FS_LAUNCH(L, "p_shift", 2.0 * sizeof(T) * N, k_pshift<T><<<flat_blocks(N), 256, 0, L.s>>>(c));
   return 2;
 }
 
@@ -230,7 +237,7 @@ template <class T> __global__ void __launch_bounds__(256) k_true_res(const Ctx<T
 }
 template <class T> int launch_true_residual(const Ctx<T>& c, const Launch& L) {
   ColGeom g = col_geom(c.nx, c.ny, c.nz);
-  k_true_res<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz);
+  FS_LAUNCH(L, "true_residual", 2.0 * sizeof(T) * c.nx * c.ny * c.nz, k_true_res<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz));
   return 1;
 }
 

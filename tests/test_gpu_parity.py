@@ -1,0 +1,377 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle on the
+same seeded inputs, element by element.  Acceptance (BASELINE.json north_star):
+fp64 fields <= 1e-9 max relative error (per field, ||gpu - oracle||_inf / ||oracle||_inf) after the
+config's steps with PCG iteration counts within +-1 per step; fp32 fields <= 1e-4 of the fp64 oracle
+over 5 steps; marker indices / perm / keys / seg_start bit-exact."""
+import math
+
+import numpy as np
+import pytest
+
+import fs_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-9     # north_star: fp64 fields within 1e-9 max relative error
+TOL32 = 1e-4     # north_star: fp32 fields within 1e-4 of the fp64 oracle over 5 steps
+
+
+@pytest.fixture(scope="module")
+def fs():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2505_23940_b200 as fs
+    fs.lib()
+    return fs
+
+
+def _oracle(cfg):
+    from oracle import Oracle
+    o = Oracle(cfg)
+    for c, a in cfg.get("init", {}).items():
+        o.set(c, a)
+    if cfg.get("markers") is not None:
+        o.set_markers(*cfg["markers"])
+    if cfg.get("body") is not None:
+        o.set_body(*cfg["body"])
+    return o
+
+
+def relerr(a, b):
+    """A9 norm: max |a-b| / max |b| (absolute when the reference is identically zero)."""
+    d = float(np.abs(np.asarray(a, dtype=np.float64) - b).max())
+    s = float(np.abs(b).max())
+    return d / s if s > 0 else d
+
+
+def _rand_fields(cfg, seed, solenoidal_bc=True):
+    rng = np.random.default_rng(seed)
+    sh = W.shapes(cfg)
+    f = {c: rng.standard_normal(sh[c]) for c in "uvw"}
+    # boundary-normal faces of bounded directions carry the prescribed values
+    if cfg["bc"][0] != "periodic":
+        f["u"][:, :, 0] = cfg["bc_vel"][0][0]; f["u"][:, :, -1] = cfg["bc_vel"][1][0]
+    if cfg["bc"][2] != "periodic":
+        f["v"][:, 0, :] = 0.0; f["v"][:, -1, :] = 0.0
+    if cfg["bc"][4] != "periodic":
+        f["w"][0] = 0.0; f["w"][-1] = 0.0
+    return f
+
+
+def _cfg_periodic(nx, ny, nz, **kw):
+    h = 2 * math.pi / nx
+    return W._base(nx=nx, ny=ny, nz=nz, lx=nx * h, ly=ny * h, lz=nz * h, nu=0.01, dt=1e-3, **kw)
+
+
+def _cfg_channel(nx, ny, nz, **kw):
+    j = np.arange(ny + 1)
+    yf = np.tanh(2.0 * (2.0 * j / ny - 1.0)) / math.tanh(2.0)
+    yf[0], yf[-1] = -1.0, 1.0
+    c = W._base(nx=nx, ny=ny, nz=nz, lx=2 * math.pi, ly=2.0, lz=math.pi, y0=-1.0, yf=yf, nu=1 / 180.0, dt=2e-4,
+                body_force=[1.0, 0.0, 0.0], **kw)
+    c["bc"] = ["periodic", "periodic", "noslip", "noslip", "periodic", "periodic"]
+    c["bc_vel"][3] = [0.3, 0.0, -0.2]      # moving lid exercises the 2*u_wall - u ghost
+    return c
+
+
+def _cfg_open(nx, ny, nz, **kw):
+    h = 1.0 / 16
+    c = W._base(nx=nx, ny=ny, nz=nz, lx=nx * h, ly=ny * h, lz=nz * h, nu=1 / 300.0, dt=5e-3, **kw)
+    c["bc"] = ["inflow", "outflow", "slip", "slip", "noslip", "slip"]
+    c["bc_vel"][0] = [1.0, 0.0, 0.0]
+    c["bc_vel"][1] = [1.0, 0.0, 0.0]
+    return c
+
+
+# ------------------------------------------------------------------------------------ S1 momentum kernel
+@pytest.mark.parametrize("kind", ["periodic", "channel", "open"])
+def test_momentum_rhs_elementwise(fs, kind):
+    # sizes span several 32x4x2 tiles with ragged tails in every direction
+    cfg = {"periodic": _cfg_periodic(72, 38, 21), "channel": _cfg_channel(40, 50, 19),
+           "open": _cfg_open(70, 27, 22, inflow_noise=0.05, seed=3)}[kind]
+    cfg["init"] = _rand_fields(cfg, 11)
+    o = _oracle(cfg)
+    ref = o.momentum_rhs()
+    g = fs.from_workload(cfg)
+    got = g.momentum_rhs()
+    for c, a, b in zip("uvw", got, ref):
+        assert relerr(a, b) < 1e-12, (kind, c, relerr(a, b))
+    g.close()
+
+
+# ------------------------------------------------------------------------------------ S6/S7 Poisson
+@pytest.mark.parametrize("kind,pc", [("periodic", "none"), ("periodic", "jacobi"), ("periodic", "gmg"),
+                                     ("channel", "jacobi"), ("open", "jacobi"), ("open", "none")])
+def test_poisson_solve_matches_oracle(fs, kind, pc):
+    if kind == "periodic":
+        n = (48, 32, 40) if pc == "gmg" else (44, 30, 37)
+        cfg = _cfg_periodic(*n, precond=pc, rtol=1e-10, warm_start=0)
+        if pc == "gmg":
+            h = 2 * math.pi / 48
+            cfg.update(lx=48 * h, ly=32 * h, lz=40 * h)
+    elif kind == "channel":
+        cfg = _cfg_channel(36, 42, 20, precond=pc, rtol=1e-10, warm_start=0)
+    else:
+        cfg = _cfg_open(50, 23, 18, precond=pc, rtol=1e-10, warm_start=0)
+    rng = np.random.default_rng(5)
+    rhs = rng.standard_normal(W.shapes(cfg)["p"])
+    o = _oracle(cfg)
+    p_ref, iref = o.poisson_solve(rhs)
+    g = fs.Grid(cfg)
+    p, info = g.poisson_solve(rhs)
+    assert info["converged"] == 1 and iref["converged"] == 1
+    assert abs(info["iters"] - iref["pcg_iters"]) <= 1, (info, iref)
+    assert relerr(p, p_ref) < TOL64, relerr(p, p_ref)
+    assert info["true_rel_residual"] < 1e-8
+    # warm start from the solution: 0 iterations
+    cfg2 = dict(cfg, warm_start=1)
+    g2 = fs.Grid(cfg2)
+    p2, info2 = g2.poisson_solve(rhs, p0=p)
+    assert info2["iters"] <= 1
+    g.close(); g2.close()
+
+
+def test_poisson_zero_rhs_and_max_iter(fs):
+    cfg = _cfg_periodic(32, 32, 32, precond="jacobi", rtol=1e-12, warm_start=0, max_iter=3)
+    g = fs.Grid(cfg)
+    p, info = g.poisson_solve(np.zeros(W.shapes(cfg)["p"]))
+    assert info["iters"] == 0 and info["converged"] == 1 and np.all(p == 0.0)
+    rng = np.random.default_rng(1)
+    p, info = g.poisson_solve(rng.standard_normal(W.shapes(cfg)["p"]))
+    assert info["iters"] == 3 and info["converged"] == 0
+    g.close()
+
+
+def test_gmg_vcycle_elementwise(fs):
+    cfg = _cfg_periodic(48, 32, 40, precond="gmg")
+    rng = np.random.default_rng(2)
+    r = rng.standard_normal(W.shapes(cfg)["p"])
+    z_ref = _oracle(cfg).vcycle(r)
+    g = fs.Grid(cfg)
+    z = g.gmg_vcycle(r)
+    assert relerr(z, z_ref) < 1e-12, relerr(z, z_ref)
+    g.close()
+
+
+# ------------------------------------------------------------------------------------ S2-S5 IBM
+def _markers(cfg, n, seed, spread_cells=6.0):
+    rng = np.random.default_rng(seed)
+    h = cfg["lx"] / cfg["nx"]
+    lo = np.array([cfg["x0"], cfg["y0"], cfg["z0"]])
+    L = np.array([cfg["lx"], cfg["ly"], cfg["lz"]])
+    centre = lo + 0.5 * L
+    xyz = centre + spread_cells * h * (rng.random((n, 3)) - 0.5) * 2.0
+    # some markers exactly on faces / centres (floor ties) and coincident pairs (sort stability)
+    xyz[0] = lo + h * np.array([5.0, 7.0, 6.0])
+    xyz[1] = lo + h * np.array([5.5, 7.5, 6.5])
+    xyz[2] = xyz[1]
+    xyz[3] = xyz[7]
+    vel = rng.standard_normal((n, 3))
+    dvol = h ** 3 * (0.5 + rng.random(n))
+    return xyz, vel, dvol
+
+
+@pytest.mark.parametrize("delta", ["roma3", "peskin4"])
+@pytest.mark.parametrize("kind", ["periodic", "open"])
+def test_ibm_cell_list_bit_exact_and_interp_spread_elementwise(fs, kind, delta):
+    n = 700
+    if kind == "periodic":
+        cfg = _cfg_periodic(24, 20, 16, delta=delta, max_markers=n)
+        cfg["markers"] = _markers(cfg, n, 9, spread_cells=14.0)       # supports wrap around the box
+    else:
+        cfg = _cfg_open(40, 30, 28, delta=delta, max_markers=n)
+        cfg["markers"] = _markers(cfg, n, 9, spread_cells=8.0)
+    cfg["init"] = _rand_fields(cfg, 4)
+    o = _oracle(cfg)
+    g = fs.from_workload(cfg)
+    a, b = g.cell_list(), o.cell_list()
+    assert a["nseg"] == b["nseg"]
+    for k in ("base", "perm", "keys", "seg_start"):
+        assert np.array_equal(a[k], b[k]), k
+    U_ref = o.interpolate(*[cfg["init"][c] for c in "uvw"])
+    U = g.ibm_interpolate()
+    assert relerr(U, U_ref) < 1e-13
+    F = np.random.default_rng(8).standard_normal((n, 3))
+    f_ref = o.spread(F)
+    g.ibm_spread(F)
+    for c, fr in zip("uvw", f_ref):
+        got = g.get(c) - cfg["init"][c]
+        assert np.abs(got - fr).max() <= 1e-12 * np.abs(fr).max(), c
+        assert np.array_equal(got != 0.0, fr != 0.0) or np.abs(got[fr == 0.0]).max() < 1e-13
+    g.close()
+
+
+def test_ibm_empty_and_single_marker(fs):
+    cfg = _cfg_periodic(16, 16, 16, max_markers=4)
+    g = fs.Grid(cfg)
+    g.set_markers(np.zeros((0, 3)))
+    assert g.cell_list()["nseg"] == 0
+    xyz = np.array([[1.0, 2.0, 3.0]])
+    g.set_markers(xyz)
+    from oracle import Oracle
+    o = Oracle(cfg); o.set_markers(xyz)
+    a, b = g.cell_list(), o.cell_list()
+    for k in ("base", "perm", "keys", "seg_start"):
+        assert np.array_equal(a[k], b[k]), k
+    with pytest.raises(fs.FsError):
+        g.set_markers(np.zeros((5, 3)))          # > max_markers
+    g.close()
+
+
+# ------------------------------------------------------------------------------------ full steps
+def _compare_state(g, o, tol, fields="uvwp"):
+    errs = {}
+    for c in fields:
+        errs[c] = relerr(g.get(c), o.get(c))
+    # w of 2-D flows is identically zero in the oracle: relerr is then absolute
+    bad = {c: e for c, e in errs.items() if not e < tol}
+    assert not bad, errs
+    return errs
+
+
+def _run_pair(fs, cfg, steps, tol=TOL64, iters_pm=1):
+    o = _oracle(cfg)
+    g = fs.from_workload(cfg)
+    io = o.step(steps)
+    ig = g.step(steps, per_step=True)
+    assert ig["nan_flag"] == 0 and ig["converged"] == 1
+    for a, b in zip(ig["iters_per_step"], io["iters_per_step"]):
+        assert abs(a - b) <= iters_pm, (ig["iters_per_step"], io["iters_per_step"])
+    errs = _compare_state(g, o, tol)
+    assert ig["step"] == io["step"] == steps
+    return g, o, ig, io, errs
+
+
+def test_c1_taylor_green_10_steps(fs):
+    cfg = W.taylor_green()
+    g, o, ig, io, _ = _run_pair(fs, cfg, 10)
+    assert ig["max_abs_div"] < 1e-12
+    # the same closed form that pins the oracle (tests/golden/taylor_green_pins.txt, AB2 a10)
+    assert abs(np.abs(g.get("u")).max() / np.abs(cfg["init"]["u"]).max() - 0.9998006613990811) < 1e-11
+    g.close()
+
+
+def test_c2_channel_reduced_20_steps(fs):
+    cfg = W.channel(n=48)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 20)
+    g.close()
+
+
+def test_c3_sphere_reduced_20_steps(fs):
+    cfg = W.sphere(scale=4, n_markers=400)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 20)
+    np.testing.assert_allclose(ig["body_force"], io["body_force"], rtol=1e-9, atol=1e-12)
+    a, b = g.cell_list(), o.cell_list()
+    for k in ("base", "perm", "keys", "seg_start"):
+        assert np.array_equal(a[k], b[k]), k
+    assert relerr(g.get("marker_f"), o.markers()[2]) < 1e-9
+    g.close()
+
+
+def test_c4_cylinder_fsi_reduced_50_steps(fs):
+    cfg = W.cylinder_fsi(scale=4, per_ring=40)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 50)
+    np.testing.assert_allclose(ig["body_disp"], io["body_disp"], rtol=1e-9, atol=1e-15)
+    np.testing.assert_allclose(ig["body_vel"], io["body_vel"], rtol=1e-9, atol=1e-15)
+    np.testing.assert_allclose(ig["body_force"], io["body_force"], rtol=1e-9, atol=1e-12)
+    # the moving body's cell list is rebuilt every step: still bit-exact at the end
+    o.step(0)
+    a, b = g.cell_list(), o.cell_list()
+    assert relerr(g.get("marker_x"), o.markers()[0]) < 1e-14
+    g.close()
+
+
+def test_c5_hit_64_fp64_10_steps(fs):
+    cfg = W.hit(n=64)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 10)
+    g.close()
+
+
+def test_c5_hit_64_fp32_5_steps(fs):
+    cfg = W.hit(n=64)
+    o = _oracle(cfg)
+    io = o.step(5)
+    g = fs.from_workload(cfg, dtype="f32")
+    ig = g.step(5, per_step=True)
+    assert ig["nan_flag"] == 0
+    errs = {c: relerr(g.get(c), o.get(c)) for c in "uvwp"}
+    assert all(e < TOL32 for e in errs.values()), errs
+    g.close()
+
+
+def test_graph_and_stream_modes_agree_bitwise(fs):
+    cfg = W.sphere(scale=4, n_markers=300)
+    g1 = fs.from_workload(cfg, exec_mode="graph")
+    g2 = fs.from_workload(cfg, exec_mode="stream")
+    i1 = g1.step(5, per_step=True); i2 = g2.step(5, per_step=True)
+    assert i1["iters_per_step"] == i2["iters_per_step"]
+    for c in "uvwp":
+        assert np.array_equal(g1.get(c), g2.get(c)), c
+    g1.close(); g2.close()
+
+
+def test_p16_restart_is_bit_exact(fs):
+    cfg = W.cylinder_fsi(scale=4, per_ring=40)
+    g = fs.from_workload(cfg)
+    g.step(10)
+    ref = {c: g.get(c) for c in "uvwp"}
+    ref_body = g.body_state()
+    a = fs.from_workload(cfg)
+    a.step(5)
+    state = {c: a.get(c) for c in ("u", "v", "w", "p", "hu", "hv", "hw")}
+    mx, mu = a.get("marker_x"), a.get("marker_u")
+    disp, vel, _ = a.body_state()
+    b = fs.Grid(dict(cfg))
+    for c, v in state.items():
+        b.set(c, v)
+    b.set_markers(mx, mu, cfg["markers"][2])
+    b.set_body(*cfg["body"])
+    b.set_body_state(disp, vel)
+    b.set_history(1, 5)
+    b.step(5)
+    for c in "uvwp":
+        assert np.array_equal(b.get(c), ref[c]), c
+    assert np.array_equal(b.body_state()[0], ref_body[0])
+    g.close(); a.close(); b.close()
+
+
+def test_async_steps_equal_sync_steps(fs):
+    cfg = W.taylor_green()
+    g1 = fs.from_workload(cfg); g2 = fs.from_workload(cfg)
+    g1.step(6)
+    g2.step(3, sync=False); g2.step(3, sync=False)
+    for c in "uvwp":
+        assert np.array_equal(g1.get(c), g2.get(c))
+    assert g1.launch_count() == g2.launch_count() > 0
+    g1.close(); g2.close()
+
+
+def test_device_pointer_io_and_dtype_conversion(fs):
+    import torch
+    cfg = W.taylor_green()
+    g = fs.from_workload(cfg, dtype="f32")
+    u64 = torch.from_numpy(cfg["init"]["u"]).cuda()
+    g.set("u", u64)                                   # fp64 device -> fp32 grid
+    out = torch.empty_like(u64)
+    g.get("u", out=out)
+    assert torch.allclose(out, u64, atol=1e-7)
+    host32 = g.get("u", dtype="f32")
+    assert host32.dtype == np.float32 and np.abs(host32 - cfg["init"]["u"]).max() < 1e-7
+    g.close()
+
+
+def test_invalid_arguments(fs):
+    cfg = W.taylor_green()
+    bad = dict(cfg, nx=1)
+    with pytest.raises(fs.FsError):
+        fs.Grid(bad)
+    bad = dict(cfg, precond="gmg", nz=30, lz=cfg["lz"])        # anisotropic spacing -> unsupported
+    with pytest.raises(fs.FsError) as e:
+        fs.Grid(bad)
+    assert e.value.status == 6
+    ch = W.channel(n=16); ch["max_markers"] = 4
+    g = fs.Grid(ch)
+    with pytest.raises(fs.FsError) as e:
+        g.set_markers(np.array([[1.0, 0.0, 1.0]]))               # markers on a y-stretched grid
+    assert e.value.status == 6
+    g.close()
