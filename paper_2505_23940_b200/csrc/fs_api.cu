@@ -671,13 +671,13 @@ fs_status fs_gmg_vcycle(fs_grid* g, const double* r, double* z) {
   fs_status st;
   if (g->f64) {
     st = copy_in<double>(g, g->cd.r, g->nP, r, FS_F64, 0); if (st != FS_OK) return st;
-    g->fixed_launches += launch_vcycle<double>(g->cd, g->md, g->cd.r, g->cd.z, L);
+    g->fixed_launches += launch_vcycle<double>(g->cd, g->md, g->cd.r, g->cd.z, L, nullptr, 1.0);
     launch_scale<double>(g->cd.z, 1.0 / g->hy, (long long)g->nP, g->stream);   // A = h (-L)  =>  M^-1 r = V(r) / h
     CK(cudaGetLastError());
     st = copy_out<double>(g, g->cd.z, g->nP, z, FS_F64, 0); if (st != FS_OK) return st;
   } else {
     st = copy_in<float>(g, g->cf.r, g->nP, r, FS_F64, 0); if (st != FS_OK) return st;
-    g->fixed_launches += launch_vcycle<float>(g->cf, g->mf, g->cf.r, g->cf.z, L);
+    g->fixed_launches += launch_vcycle<float>(g->cf, g->mf, g->cf.r, g->cf.z, L, nullptr, 1.0f);
     launch_scale<float>(g->cf.z, 1.0 / g->hy, (long long)g->nP, g->stream);
     CK(cudaGetLastError());
     st = copy_out<float>(g, g->cf.z, g->nP, z, FS_F64, 0); if (st != FS_OK) return st;

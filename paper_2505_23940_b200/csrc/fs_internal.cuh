@@ -111,7 +111,12 @@ template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, const Launch& L);
 template <class T> int launch_pcg_finish(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_true_residual(const Ctx<T>& c, const Launch& L);
-template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L);
+// dot_fused != nullptr asks for rho_cur = rhs . (zs out) from the last kernel; *dot_fused says whether it was done
+template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs);
+template <class T> int launch_mg_down(const Ctx<T>& c, const T* g, T* e, T* gc, int nx, int ny, int nz, double h, double omega,
+                                      const char* name, const Launch& L);
+template <class T> int launch_mg_up(const Ctx<T>& c, const T* ein, const T* ec, const T* g, T* eo, int nx, int ny, int nz, double h,
+                                    double omega, bool dot, T zs, const char* name, const Launch& L);
 
 template <class T> int launch_ibm_index(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
 template <class T> int launch_ibm_interpolate(const Ctx<T>& c, const IbmCtx& ib, const T* u, const T* v, const T* w, double* out, const Launch& L);

@@ -68,7 +68,7 @@ template <class T> __global__ void __launch_bounds__(256) k_mg_prolong(const int
 }
 
 // Recursion unrolled on the host: emits the kernels of one V-cycle for rhs -> out (out = V(rhs)).
-template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L) {
+template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs) {
   int n = 0;
   const int* done = &c.S->done;
   const T* gl[kMaxLevels]; T* el[kMaxLevels]; T* tl[kMaxLevels]; T* cur[kMaxLevels];
@@ -76,6 +76,39 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     gl[l] = l == 0 ? rhs : (const T*)mg.lev[l].g;
     el[l] = l == 0 ? out : (T*)mg.lev[l].e;
     tl[l] = (T*)mg.lev[l].t;
+  }
+  const bool want_dot = dot_fused != nullptr;
+  if (dot_fused) *dot_fused = false;
+  // Fast path, V(2,2) with at least two levels: two fused kernels per level (fs_kernels_mgf.cu).
+  if (mg.nu1 == 2 && mg.nu2 == 2 && mg.nlev >= 2) {
+    const int last = mg.nlev - 1;
+    for (int l = 0; l < last; ++l) {
+      const MgLevel& V = mg.lev[l];
+      n += launch_mg_down<T>(c, gl[l], tl[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, V.h, mg.omega, l == 0 ? "mg_down_l0" : "mg_coarse", L);
+    }
+    {
+      const MgLevel& V = mg.lev[last];
+      const long long N = (long long)V.nx * V.ny * V.nz;
+      const T ih2 = T(1.0 / (V.h * V.h)), cw = T(mg.omega * V.h * V.h / 6.0);
+      const int pre = mg.coarse_sweeps;
+      if (pre <= 0) { FS_LAUNCH(L, "mg_coarse", 1.0 * sizeof(T) * N, cudaMemsetAsync(el[last], 0, sizeof(T) * (size_t)N, L.s)); ++n; }
+      else {
+        T* a = ((pre - 1) % 2 == 0) ? el[last] : tl[last];
+        T* b = ((pre - 1) % 2 == 0) ? tl[last] : el[last];
+        FS_LAUNCH(L, "mg_coarse", 2.0 * sizeof(T) * N, k_mg_first<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[last], a, cw, N)); ++n;
+        for (int it = 1; it < pre; ++it) {
+          FS_LAUNCH(L, "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[last], a, b, V.nx, V.ny, V.nz, ih2, cw)); ++n;
+          T* t = a; a = b; b = t;
+        }
+      }
+    }
+    for (int l = last - 1; l >= 0; --l) {
+      const MgLevel& V = mg.lev[l];
+      const bool dot = want_dot && l == 0;
+      n += launch_mg_up<T>(c, tl[l], el[l + 1], gl[l], el[l], V.nx, V.ny, V.nz, V.h, mg.omega, dot, zs, l == 0 ? "mg_up_l0" : "mg_coarse", L);
+      if (dot) *dot_fused = true;
+    }
+    return n;
   }
   // downward leg
   for (int l = 0; l < mg.nlev; ++l) {
@@ -122,7 +155,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
   return n;
 }
 
-template int launch_vcycle<float>(const Ctx<float>&, const MgCtx<float>&, const float*, float*, const Launch&);
-template int launch_vcycle<double>(const Ctx<double>&, const MgCtx<double>&, const double*, double*, const Launch&);
+template int launch_vcycle<float>(const Ctx<float>&, const MgCtx<float>&, const float*, float*, const Launch&, bool*, float);
+template int launch_vcycle<double>(const Ctx<double>&, const MgCtx<double>&, const double*, double*, const Launch&, bool*, double);
 
 }  // namespace fs

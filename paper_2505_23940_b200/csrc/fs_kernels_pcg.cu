@@ -185,8 +185,9 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
   T zs = T(1);
   if (c.precond == FS_PC_GMG) {
     zs = T(1.0 / c.hy);
-    n += launch_vcycle<T>(c, mg, c.r, c.z, L);
-    FS_LAUNCH(L, "pcg_dot_rz", 2.0 * sizeof(T) * N, k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n;
+    bool fused = false;
+    n += launch_vcycle<T>(c, mg, c.r, c.z, L, &fused, zs);
+    if (!fused) { FS_LAUNCH(L, "pcg_dot_rz", 2.0 * sizeof(T) * N, k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n; }
   }
   FS_LAUNCH(L, "pcg_dir", 3.0 * sizeof(T) * N, k_pcg_dir<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n;
   FS_LAUNCH(L, "pcg_apply_dot", 2.0 * sizeof(T) * N, k_pcg_apply<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz)); ++n;
