@@ -76,114 +76,172 @@ template <class T> __device__ __forceinline__ T boundary_normal(const Ctx<T>& c,
 // ---------------------------------------------------------------------------------------------------
 // S1: H^n = -div(u u) + nu lap(u) + g (central / central, Eq. 4) and the explicit
 // predictor u~ = u^n + dt (a0 H^n + a1 H^{n-1}); prescribed boundary-normal faces get their O1 values.
-// One thread per cell of the extended box (nxu x nyv x nzw); it owns the three faces u,v,w(i,j,k).
+//
+// 2.5-D halo-tiled streaming kernel: a CTA owns a 30 x 10 column of cells of the extended box
+// (nxu x nyv x nzw) plus a one-cell halo (32 x 12 threads, one thread per extended-tile cell) and marches
+// in z.  Every plane of u, v, w is read once per CTA through the boundary-aware accessor (S0 folded into
+// the tile load: wrap / ghost reflection are resolved when the value enters shared memory), kept in a
+// four-slot ring of shared-memory planes (planes k-1, k, k+1 are live, the fourth slot takes the prefetch
+// without a second barrier) and in a register queue for the thread's own column.  One __syncthreads per
+// plane; H^{n-1} is read and H^n, u~ are written straight from / to global memory, coalesced.
 // ---------------------------------------------------------------------------------------------------
-template <class T> __global__ void __launch_bounds__(256) k_momentum(const Ctx<T> c) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
-  if (i >= c.nxu || j >= c.nyv || k >= c.nzw) return;
+constexpr int kMomTX = 32, kMomTY = 12;
+
+template <class T> struct ColRef { size_t off, pl; T A, B; };   // value = A f[off + pl kz] + B  (x, y ghosts resolved)
+
+template <class T, int C> __device__ __forceinline__ ColRef<T> col_setup(const Ctx<T>& c, int i, int j) {
+  T A = T(1), B = T(0);
+  if (!c.bx) i = wrapi(i, c.nx);
+  else if (C != 0) {
+    int face = -1;
+    if (i < 0) { face = 0; i = -1 - i; } else if (i >= c.nx) { face = 1; i = 2 * c.nx - 1 - i; }
+    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
+  } else i = min(max(i, 0), c.nx);
+  if (!c.by) j = wrapi(j, c.ny);
+  else if (C != 1) {
+    int face = -1;
+    if (j < 0) { face = 2; j = -1 - j; } else if (j >= c.ny) { face = 3; j = 2 * c.ny - 1 - j; }
+    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
+  } else j = min(max(j, 0), c.ny);
+  const int ex = C == 0 ? c.nxu : c.nx, ey = C == 1 ? c.nyv : c.ny;
+  ColRef<T> r;
+  r.off = (size_t)i + (size_t)ex * (size_t)j; r.pl = (size_t)ex * ey; r.A = A; r.B = B;
+  return r;
+}
+// plane kk in [-1, nzw] of component C for this thread's column
+template <class T, int C> __device__ __forceinline__ T col_load(const Ctx<T>& c, const T* __restrict__ f, const ColRef<T>& r, int kk) {
+  T A = r.A, B = r.B;
+  if (!c.bz) kk = wrapi(kk, c.nz);
+  else if (C != 2) {
+    int face = -1;
+    if (kk < 0) { face = 4; kk = -1 - kk; } else if (kk >= c.nz) { face = 5; kk = 2 * c.nz - 1 - kk; }
+    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
+  } else kk = min(max(kk, 0), c.nz);
+  return A * f[r.off + r.pl * (size_t)kk] + B;
+}
+
+template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momentum(const Ctx<T> c, int kz) {
+  __shared__ T SU[4][kMomTY][kMomTX], SV[4][kMomTY][kMomTX], SW[4][kMomTY][kMomTX];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int iu = blockIdx.x * (kMomTX - 2) + tx - 1, ju = blockIdx.y * (kMomTY - 2) + ty - 1;   // may be -1 or past the box
+  const int i = min(iu, c.nxu), j = min(ju, c.nyv);
+  const bool own = tx >= 1 && tx <= kMomTX - 2 && ty >= 1 && ty <= kMomTY - 2 && iu < c.nxu && ju < c.nyv;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nzw);
   const bool ab2 = c.time_scheme == FS_TIME_AB2 && c.S->have_hist;
   const T a0 = ab2 ? T(1.5) : T(1), a1 = ab2 ? T(-0.5) : T(0);
   const T dt = T(c.dt), nu = T(c.nu);
   const T* __restrict__ U = c.u; const T* __restrict__ V = c.v; const T* __restrict__ W = c.w;
-#define U_(a, b, cc) ldv<T, 0>(c, U, a, b, cc)
-#define V_(a, b, cc) ldv<T, 1>(c, V, a, b, cc)
-#define W_(a, b, cc) ldv<T, 2>(c, W, a, b, cc)
-  // ---- u face ----
-  if (j < c.ny && k < c.nz) {
-    const size_t q = (size_t)i + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k);
-    if (c.bx && (i == 0 || i == c.nx)) {
-      const int side = i == 0 ? 0 : 1;
-      const size_t qi = side ? q - 1 : q + 1;
-      c.us[q] = boundary_normal<T>(c, U, 0, side, j, k, q, qi, 0);
-      c.hu[q] = T(0);
-    } else {
-      const T uc = U[q];
-      const T uE = U_(i + 1, j, k), uW = U_(i - 1, j, k), uN = U_(i, j + 1, k), uS = U_(i, j - 1, k);
-      const T uT = U_(i, j, k + 1), uB = U_(i, j, k - 1);
-      const T ue = T(0.5) * (uc + uE), uw = T(0.5) * (uW + uc);
-      const T cx = (ue * ue - uw * uw) * c.ihx;
-      const T vn = T(0.5) * (V_(i - 1, j + 1, k) + V_(i, j + 1, k)), un = c.wyl[j + 1] * uc + c.wyh[j + 1] * uN;
-      const T vs = T(0.5) * (V_(i - 1, j, k) + V_(i, j, k)),         us = c.wyl[j] * uS + c.wyh[j] * uc;
-      const T cy = (vn * un - vs * us) * c.idy[j + 1];
-      const T wt = T(0.5) * (W_(i - 1, j, k + 1) + W_(i, j, k + 1)), ut = T(0.5) * (uc + uT);
-      const T wb = T(0.5) * (W_(i - 1, j, k) + W_(i, j, k)),         ub = T(0.5) * (uB + uc);
-      const T cz = (wt * ut - wb * ub) * c.ihz;
-      const T dxx = (uE - T(2) * uc + uW) * c.ihx2;
-      const T dyy = ((uN - uc) * c.idyc[j + 1] - (uc - uS) * c.idyc[j]) * c.idy[j + 1];
-      const T dzz = (uT - T(2) * uc + uB) * c.ihz2;
-      const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[0]);
-      c.us[q] = uc + dt * (a0 * H + a1 * c.hu[q]);
-      c.hu[q] = H;
+  const ColRef<T> ru = col_setup<T, 0>(c, i, j), rv = col_setup<T, 1>(c, i, j), rw = col_setup<T, 2>(c, i, j);
+  // y metrics of this row (j clamped into the tables; unused rows never store)
+  const int jc = min(max(j, 0), c.ny - 1);
+  const T wyl0 = c.wyl[jc], wyh0 = c.wyh[jc], wyl1 = c.wyl[jc + 1], wyh1 = c.wyh[jc + 1];
+  const T idyj = c.idy[jc + 1], idyjm = c.idy[jc], idyc0 = c.idyc[jc], idyc1 = c.idyc[jc + 1];
+  // register queue of the own column: B = k-1, c = k, T = k+1
+  T uB = col_load<T, 0>(c, U, ru, k0 - 1), vB = col_load<T, 1>(c, V, rv, k0 - 1), wB = col_load<T, 2>(c, W, rw, k0 - 1);
+  T uc = col_load<T, 0>(c, U, ru, k0), vc = col_load<T, 1>(c, V, rv, k0), wc = col_load<T, 2>(c, W, rw, k0);
+  T un = col_load<T, 0>(c, U, ru, k0 + 1), vn = col_load<T, 1>(c, V, rv, k0 + 1), wn = col_load<T, 2>(c, W, rw, k0 + 1);
+  SU[(k0 - 1) & 3][ty][tx] = uB; SV[(k0 - 1) & 3][ty][tx] = vB; SW[(k0 - 1) & 3][ty][tx] = wB;
+  SU[k0 & 3][ty][tx] = uc; SV[k0 & 3][ty][tx] = vc; SW[k0 & 3][ty][tx] = wc;
+  const int txm = max(tx - 1, 0), txp = min(tx + 1, kMomTX - 1), tym = max(ty - 1, 0), typ = min(ty + 1, kMomTY - 1);
+  for (int k = k0; k < k1; ++k) {
+    const T uT = un, vT = vn, wT = wn;
+    const int s0 = (k - 1) & 3, s1 = k & 3, s2 = (k + 1) & 3;
+    SU[s2][ty][tx] = uT; SV[s2][ty][tx] = vT; SW[s2][ty][tx] = wT;
+    if (k + 1 < k1) { un = col_load<T, 0>(c, U, ru, k + 2); vn = col_load<T, 1>(c, V, rv, k + 2); wn = col_load<T, 2>(c, W, rw, k + 2); }
+    __syncthreads();
+    if (own) {
+      // ---- u face ----
+      if (j < c.ny && k < c.nz) {
+        const size_t q = (size_t)i + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k);
+        if (c.bx && (i == 0 || i == c.nx)) {
+          const int side = i == 0 ? 0 : 1;
+          const size_t qi = side ? q - 1 : q + 1;
+          c.us[q] = boundary_normal<T>(c, U, 0, side, j, k, q, qi, 0);
+          c.hu[q] = T(0);
+        } else {
+          const T uE = SU[s1][ty][txp], uW = SU[s1][ty][txm], uN = SU[s1][typ][tx], uS = SU[s1][tym][tx];
+          const T ue = T(0.5) * (uc + uE), uw = T(0.5) * (uW + uc);
+          const T cx = (ue * ue - uw * uw) * c.ihx;
+          const T vnn = T(0.5) * (SV[s1][typ][txm] + SV[s1][typ][tx]), unn = wyl1 * uc + wyh1 * uN;
+          const T vss = T(0.5) * (SV[s1][ty][txm] + vc),                uss = wyl0 * uS + wyh0 * uc;
+          const T cy = (vnn * unn - vss * uss) * idyj;
+          const T wt = T(0.5) * (SW[s2][ty][txm] + wT), ut = T(0.5) * (uc + uT);
+          const T wb = T(0.5) * (SW[s1][ty][txm] + wc), ub = T(0.5) * (uB + uc);
+          const T cz = (wt * ut - wb * ub) * c.ihz;
+          const T dxx = (uE - T(2) * uc + uW) * c.ihx2;
+          const T dyy = ((uN - uc) * idyc1 - (uc - uS) * idyc0) * idyj;
+          const T dzz = (uT - T(2) * uc + uB) * c.ihz2;
+          const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[0]);
+          c.us[q] = uc + dt * (a0 * H + a1 * c.hu[q]);
+          c.hu[q] = H;
+        }
+      }
+      // ---- v face (control volume between y_c(j-1) and y_c(j)) ----
+      if (i < c.nx && k < c.nz) {
+        const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.nyv * k);
+        if (c.by && (j == 0 || j == c.ny)) {
+          const int side = j == 0 ? 0 : 1;
+          const size_t qi = side ? q - c.nx : q + c.nx;
+          c.vs[q] = boundary_normal<T>(c, V, 1, side, i, k, q, qi, side ? c.ny - 1 : 0);
+          c.hv[q] = T(0);
+        } else {
+          const T vE = SV[s1][ty][txp], vW = SV[s1][ty][txm], vN = SV[s1][typ][tx], vS = SV[s1][tym][tx];
+          const T wl = wyl0, wh = wyh0;
+          const T ue = wl * SU[s1][tym][txp] + wh * SU[s1][ty][txp], ve = T(0.5) * (vc + vE);
+          const T uw = wl * SU[s1][tym][tx] + wh * uc,               vw = T(0.5) * (vW + vc);
+          const T cx = (ue * ve - uw * vw) * c.ihx;
+          const T vnn = T(0.5) * (vc + vN), vss = T(0.5) * (vS + vc);
+          const T cy = (vnn * vnn - vss * vss) * idyc0;
+          const T wt = wl * SW[s2][tym][tx] + wh * wT, vt = T(0.5) * (vc + vT);
+          const T wb = wl * SW[s1][tym][tx] + wh * wc, vb = T(0.5) * (vB + vc);
+          const T cz = (wt * vt - wb * vb) * c.ihz;
+          const T dxx = (vE - T(2) * vc + vW) * c.ihx2;
+          const T dyy = ((vN - vc) * idyj - (vc - vS) * idyjm) * idyc0;
+          const T dzz = (vT - T(2) * vc + vB) * c.ihz2;
+          const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[1]);
+          c.vs[q] = vc + dt * (a0 * H + a1 * c.hv[q]);
+          c.hv[q] = H;
+        }
+      }
+      // ---- w face ----
+      if (i < c.nx && j < c.ny) {
+        const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k);
+        if (c.bz && (k == 0 || k == c.nz)) {
+          const int side = k == 0 ? 0 : 1;
+          const size_t pl = (size_t)c.nx * c.ny;
+          const size_t qi = side ? q - pl : q + pl;
+          c.ws[q] = boundary_normal<T>(c, W, 2, side, i, j, q, qi, 0);
+          c.hw[q] = T(0);
+        } else {
+          const T wE = SW[s1][ty][txp], wW = SW[s1][ty][txm], wN = SW[s1][typ][tx], wS = SW[s1][tym][tx];
+          const T ue = T(0.5) * (SU[s0][ty][txp] + SU[s1][ty][txp]), we = T(0.5) * (wc + wE);
+          const T uw = T(0.5) * (uB + uc),                           ww = T(0.5) * (wW + wc);
+          const T cx = (ue * we - uw * ww) * c.ihx;
+          const T vnn = T(0.5) * (SV[s0][typ][tx] + SV[s1][typ][tx]), wnn = wyl1 * wc + wyh1 * wN;
+          const T vss = T(0.5) * (vB + vc),                           wss = wyl0 * wS + wyh0 * wc;
+          const T cy = (vnn * wnn - vss * wss) * idyj;
+          const T wt = T(0.5) * (wc + wT), wb = T(0.5) * (wB + wc);
+          const T cz = (wt * wt - wb * wb) * c.ihz;
+          const T dxx = (wE - T(2) * wc + wW) * c.ihx2;
+          const T dyy = ((wN - wc) * idyc1 - (wc - wS) * idyc0) * idyj;
+          const T dzz = (wT - T(2) * wc + wB) * c.ihz2;
+          const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[2]);
+          c.ws[q] = wc + dt * (a0 * H + a1 * c.hw[q]);
+          c.hw[q] = H;
+        }
+      }
     }
+    uB = uc; uc = uT; vB = vc; vc = vT; wB = wc; wc = wT;
   }
-  // ---- v face (control volume between y_c(j-1) and y_c(j)) ----
-  if (i < c.nx && k < c.nz) {
-    const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.nyv * k);
-    if (c.by && (j == 0 || j == c.ny)) {
-      const int side = j == 0 ? 0 : 1;
-      const size_t qi = side ? q - c.nx : q + c.nx;
-      c.vs[q] = boundary_normal<T>(c, V, 1, side, i, k, q, qi, side ? c.ny - 1 : 0);
-      c.hv[q] = T(0);
-    } else {
-      const T vc = V[q];
-      const T vE = V_(i + 1, j, k), vW = V_(i - 1, j, k), vN = V_(i, j + 1, k), vS = V_(i, j - 1, k);
-      const T vT = V_(i, j, k + 1), vB = V_(i, j, k - 1);
-      const T wl = c.wyl[j], wh = c.wyh[j];
-      const T ue = wl * U_(i + 1, j - 1, k) + wh * U_(i + 1, j, k), ve = T(0.5) * (vc + vE);
-      const T uw = wl * U_(i, j - 1, k) + wh * U_(i, j, k),         vw = T(0.5) * (vW + vc);
-      const T cx = (ue * ve - uw * vw) * c.ihx;
-      const T vn = T(0.5) * (vc + vN), vs = T(0.5) * (vS + vc);
-      const T cy = (vn * vn - vs * vs) * c.idyc[j];
-      const T wt = wl * W_(i, j - 1, k + 1) + wh * W_(i, j, k + 1), vt = T(0.5) * (vc + vT);
-      const T wb = wl * W_(i, j - 1, k) + wh * W_(i, j, k),         vb = T(0.5) * (vB + vc);
-      const T cz = (wt * vt - wb * vb) * c.ihz;
-      const T dxx = (vE - T(2) * vc + vW) * c.ihx2;
-      const T dyy = ((vN - vc) * c.idy[j + 1] - (vc - vS) * c.idy[j]) * c.idyc[j];
-      const T dzz = (vT - T(2) * vc + vB) * c.ihz2;
-      const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[1]);
-      c.vs[q] = vc + dt * (a0 * H + a1 * c.hv[q]);
-      c.hv[q] = H;
-    }
-  }
-  // ---- w face ----
-  if (i < c.nx && j < c.ny) {
-    const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k);
-    if (c.bz && (k == 0 || k == c.nz)) {
-      const int side = k == 0 ? 0 : 1;
-      const size_t pl = (size_t)c.nx * c.ny;
-      const size_t qi = side ? q - pl : q + pl;
-      c.ws[q] = boundary_normal<T>(c, W, 2, side, i, j, q, qi, 0);
-      c.hw[q] = T(0);
-    } else {
-      const T wc = W[q];
-      const T wE = W_(i + 1, j, k), wW = W_(i - 1, j, k), wN = W_(i, j + 1, k), wS = W_(i, j - 1, k);
-      const T wT = W_(i, j, k + 1), wB = W_(i, j, k - 1);
-      const T ue = T(0.5) * (U_(i + 1, j, k - 1) + U_(i + 1, j, k)), we = T(0.5) * (wc + wE);
-      const T uw = T(0.5) * (U_(i, j, k - 1) + U_(i, j, k)),         ww = T(0.5) * (wW + wc);
-      const T cx = (ue * we - uw * ww) * c.ihx;
-      const T vn = T(0.5) * (V_(i, j + 1, k - 1) + V_(i, j + 1, k)), wn = c.wyl[j + 1] * wc + c.wyh[j + 1] * wN;
-      const T vs = T(0.5) * (V_(i, j, k - 1) + V_(i, j, k)),         ws = c.wyl[j] * wS + c.wyh[j] * wc;
-      const T cy = (vn * wn - vs * ws) * c.idy[j + 1];
-      const T wt = T(0.5) * (wc + wT), wb = T(0.5) * (wB + wc);
-      const T cz = (wt * wt - wb * wb) * c.ihz;
-      const T dxx = (wE - T(2) * wc + wW) * c.ihx2;
-      const T dyy = ((wN - wc) * c.idyc[j + 1] - (wc - wS) * c.idyc[j]) * c.idy[j + 1];
-      const T dzz = (wT - T(2) * wc + wB) * c.ihz2;
-      const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[2]);
-      c.ws[q] = wc + dt * (a0 * H + a1 * c.hw[q]);
-      c.hw[q] = H;
-    }
-  }
-#undef U_
-#undef V_
-#undef W_
 }
 
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
-  dim3 b(32, 4, 2), g((c.nxu + 31) / 32, (c.nyv + 3) / 4, (c.nzw + 1) / 2);
-  FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T><<<g, b, 0, L.s>>>(c));
+  const int bxn = (c.nxu + kMomTX - 3) / (kMomTX - 2), byn = (c.nyv + kMomTY - 3) / (kMomTY - 2);
+  // z chunks: >= 4 waves of CTAs (5 CTAs of 384 threads per SM) while chunks stay >= 16 planes
+  int kz = c.nzw;
+  while (kz > 16 && (long long)bxn * byn * ((c.nzw + kz - 1) / kz) < 4LL * 148 * 5) kz = (kz + 1) / 2;
+  dim3 b(kMomTX, kMomTY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
+  FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T><<<g, b, 0, L.s>>>(c, kz));
   return 1;
 }
 
