@@ -96,6 +96,7 @@ fs_status validate(const fs_params* p) {
   for (int d = 0; d < 3; ++d)
     if ((p->bc[2 * d] == FS_BC_PERIODIC) != (p->bc[2 * d + 1] == FS_BC_PERIODIC)) return FS_ERR_INVALID_ARG;
   if ((long long)p->nx * p->ny * p->nz > (1LL << 31) - 1) return FS_ERR_UNSUPPORTED;   // int32 cell keys
+  if ((long long)((p->nx + 29) / 30) * ((p->ny + 3) / 4) > kMaxPartials) return FS_ERR_UNSUPPORTED;   // one reduction partial per xy tile
   if (p->yf) for (int j = 0; j < p->ny; ++j) if (!(p->yf[j + 1] > p->yf[j])) return FS_ERR_INVALID_ARG;
   if ((int)p->precond < 0 || (int)p->precond > 2 || (int)p->delta < 0 || (int)p->delta > 1) return FS_ERR_INVALID_ARG;
   if (p->precond == FS_PC_GMG) {
@@ -132,7 +133,7 @@ template <class T> size_t carve(fs_grid* g, char* base) {
   c.u = b.take<T>(g->nU); c.v = b.take<T>(g->nV); c.w = b.take<T>(g->nW);
   c.us = b.take<T>(g->nU); c.vs = b.take<T>(g->nV); c.ws = b.take<T>(g->nW);
   c.hu = b.take<T>(g->nU); c.hv = b.take<T>(g->nV); c.hw = b.take<T>(g->nW);
-  c.p = b.take<T>(g->nP); c.r = b.take<T>(g->nP); c.d = b.take<T>(g->nP); c.q = b.take<T>(g->nP); c.bh = b.take<T>(g->nP);
+  c.p = b.take<T>(g->nP); c.r = b.take<T>(g->nP); c.d = b.take<T>(g->nP); c.d2 = b.take<T>(g->nP); c.q = b.take<T>(g->nP); c.bh = b.take<T>(g->nP);
   c.z = nullptr;
   mg.nlev = 0;
   if (P.precond == FS_PC_GMG) {

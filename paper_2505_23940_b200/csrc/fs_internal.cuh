@@ -11,7 +11,7 @@
 namespace fs {
 
 constexpr int kMaxLevels = 12;
-constexpr int kMaxPartials = 16384;   // partial sums per reduction slot (>= blocks of any reducing kernel)
+constexpr int kMaxPartials = 32768;   // partial sums per reduction slot (>= blocks of any reducing kernel)
 constexpr int kRedSlots = 4;          // values reduced at once by one kernel
 
 // Scalars that live in device memory so that a captured step never needs the host.
@@ -24,6 +24,7 @@ struct Scalars {
   double rmean;         // fp32 only: mean of the recurrence residual, removed with one iteration of lag (null-space deflation)
   double sum_dy;         // sum over all cells of dy_j
   int iter, done, converged, first;
+  int dsel, pad2;        // which of the two direction buffers holds the current d (k_pcg_dirapply)
   int max_iter, pad0;
   double rtol;
   // step control
@@ -59,7 +60,7 @@ template <class T> struct Ctx {
   const double* dy64;  // [ny] fp64 cell heights (reductions, flux areas)
   // fields
   T *u, *v, *w, *p, *us, *vs, *ws, *hu, *hv, *hw;
-  T *r, *d, *q, *z, *bh;
+  T *r, *d, *d2, *q, *z, *bh;
   Scalars* S;
   double* partials;     // [kRedSlots][kMaxPartials]
 };

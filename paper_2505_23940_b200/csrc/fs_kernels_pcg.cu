@@ -72,7 +72,7 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_init(const Ctx<T
     if (threadIdx.x == 0 && threadIdx.y == 0) {
       Scalars* S = c.S;
       S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
-      S->iter = 0; S->first = 1;
+      S->iter = 0; S->first = 1; S->dsel = 0;
       S->rmean = v[3] / ((double)c.nx * c.ny * c.nz);
       const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
       S->converged = conv; S->done = conv || S->max_iter <= 0;
@@ -81,41 +81,88 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_init(const Ctx<T
   }
 }
 
-// ---- K4: d = z + beta d  (z from the point preconditioner, or the V-cycle output scaled by zs) -----
-template <class T> __global__ void __launch_bounds__(256) k_pcg_dir(const Ctx<T> c, T zs) {
+// ---- K4 + K1 fused: d' = z + beta d, q = A d', d'.q -------------------------------------------------------
+// 2.5-D streaming kernel (one thread per cell of a 32 x 16 extended tile, 30 x 14 results, z march with a
+// register queue for the z neighbours and a double-buffered shared-memory plane for the x / y neighbours).
+// d' is computed on the halo as well (from z and d there), so the separate direction pass and its 3 words
+// per cell disappear: the pair moves 4 words (z, d in; d', q out) instead of 3 + 2.  d' goes to the OTHER
+// direction buffer (a neighbouring CTA may still need the old d on its halo); Scalars::dsel says which of
+// the two buffers holds the current direction and is toggled by k_pcg_update.
+// PC: 0 none (z = r), 1 Jacobi (z = r / diag A), 2 GMG (z = zs * V-cycle output).
+constexpr int kDaTX = 32, kDaTY = 16;
+
+template <class T, int PC> __global__ void __launch_bounds__(kDaTX * kDaTY, 2) k_pcg_dirapply(const Ctx<T> c, T zs, int kz) {
+  __shared__ T D[2][kDaTY][kDaTX];
+  __shared__ double sh[32]; __shared__ int flag;
   const Scalars* S = c.S;
   if (S->done) return;
   const bool first = S->first != 0;
   const T beta = first ? T(0) : T(S->rho_cur / S->rho_prev);
-  const long long N = (long long)c.nx * c.ny * c.nz;
-  const bool gmg = c.precond == FS_PC_GMG;
-  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+  const T* __restrict__ dold = S->dsel ? c.d2 : c.d;
+  T* __restrict__ dnew = S->dsel ? c.d : c.d2;
+  const T* __restrict__ zsrc = PC == 2 ? c.z : c.r;
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int iu = blockIdx.x * (kDaTX - 2) + tx - 1, ju = blockIdx.y * (kDaTY - 2) + ty - 1;
+  // source cell of this thread: wrapped (periodic) or clamped (bounded: zero difference = dropped Neumann flux)
+  const int i = c.bx ? min(max(iu, 0), c.nx - 1) : wrapi(iu, c.nx);
+  const int j = c.by ? min(max(ju, 0), c.ny - 1) : wrapi(ju, c.ny);
+  const bool own = tx >= 1 && tx <= kDaTX - 2 && ty >= 1 && ty <= kDaTY - 2 && iu < c.nx && ju < c.ny;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  const size_t pl = (size_t)c.nx * c.ny, oc = (size_t)i + (size_t)c.nx * j;
+  const T cyl = c.cyl[j], cyh = c.cyh[j], idy = c.idy[j + 1], ndy = -c.dy[j + 1];
+  // Jacobi diagonal pieces (same association as diag_A)
+  const T dxy = T((c.bx && i == 0 ? 0 : 1) + (c.bx && i == c.nx - 1 ? 0 : 1)) * c.ihx2;
+  const T dyy = (cyh + cyl) * idy;
+  auto plane_src = [&](int k) { return c.bz ? min(max(k, 0), c.nz - 1) : wrapi(k, c.nz); };
+  auto dir_at = [&](int k) {              // d' at (i, j, plane_src(k))
+    const int ks = plane_src(k);
+    const size_t o = oc + pl * ks;
     T z;
-    if (gmg) z = c.z[q] * zs;
-    else {
-      const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
-      z = precond_point<T>(c, c.r[q], i, j, k);
+    if (PC == 2) z = zsrc[o] * zs;
+    else if (PC == 1) {
+      const T dzz = T((c.bz && ks == 0 ? 0 : 1) + (c.bz && ks == c.nz - 1 ? 0 : 1)) * c.ihz2;
+      z = zsrc[o] / ((dxy + dyy + dzz) * c.dy[j + 1]);
+    } else z = zsrc[o];
+    return first ? z : z + beta * dold[o];
+  };
+  const int txm = max(tx - 1, 0), txp = min(tx + 1, kDaTX - 1), tym = max(ty - 1, 0), typ = min(ty + 1, kDaTY - 1);
+  T dB = dir_at(k0 - 1), dC = dir_at(k0), dT = dir_at(k0 + 1);
+  D[k0 & 1][ty][tx] = dC;
+  __syncthreads();
+  double v[1] = {0.0};
+  for (int k = k0; k < k1; ++k) {
+    T dN = T(0);
+    if (k + 1 < k1) dN = dir_at(k + 2);   // in flight during the stencil
+    const int s = k & 1;
+    const T xw = D[s][ty][txm], xe = D[s][ty][txp], xs = D[s][tym][tx], xn = D[s][typ][tx];
+    T acc = (xe - dC) * c.ihx2 - (dC - xw) * c.ihx2;
+    const T fy = (xn - dC) * cyh - (dC - xs) * cyl;
+    acc += fy * idy;
+    acc += (dT - dC) * c.ihz2 - (dC - dB) * c.ihz2;
+    const T Ax = acc * ndy;
+    if (own) {
+      const size_t o = oc + pl * k;
+      dnew[o] = dC; c.q[o] = Ax;
+      v[0] += (double)dC * (double)Ax;
     }
-    c.d[q] = first ? z : z + beta * c.d[q];
+    D[s ^ 1][ty][tx] = dT;
+    __syncthreads();
+    dB = dC; dC = dT; dT = dN;
+  }
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (tx == 0 && ty == 0) c.S->dq = v[0];
   }
 }
 
-// ---- K1: q = A d fused with d.q ------------------------------------------------------------------------
-template <class T> __global__ void __launch_bounds__(256) k_pcg_apply(const Ctx<T> c, int kz) {
-  __shared__ double sh[32]; __shared__ int flag;
-  if (c.S->done) return;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
-  double v[1] = {0.0};
-  if (i < c.nx && j < c.ny) {
-    march_A<T>(c, c.d, i, j, k0, k1, [&](int k, size_t q, T xc, T Ax) {
-      c.q[q] = Ax;
-      v[0] += (double)xc * (double)Ax;
-    });
-  }
-  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
-    if (threadIdx.x == 0 && threadIdx.y == 0) c.S->dq = v[0];
-  }
+struct DaGeom { dim3 grid; int kz; };
+static DaGeom da_geom(int nx, int ny, int nz) {
+  const int bxn = (nx + kDaTX - 3) / (kDaTX - 2), byn = (ny + kDaTY - 3) / (kDaTY - 2);
+  // z chunks: about 4 waves of 2 CTAs per SM, chunks of at least 16 planes (two halo planes per chunk)
+  int kz = nz;
+  while (kz > 16 && (long long)bxn * byn * ((nz + kz - 1) / kz) < 4LL * 296) kz = (kz + 1) / 2;
+  while ((long long)bxn * byn * ((nz + kz - 1) / kz) > kMaxPartials && kz < nz) kz *= 2;
+  DaGeom g; g.kz = kz; g.grid = dim3(bxn, byn, (nz + kz - 1) / kz);
+  return g;
 }
 
 // ---- K2: x += alpha d, r -= alpha q fused with ||r||^2 and r.z; loop control -------------------------
@@ -131,9 +178,10 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_update(const Ctx
   const long long N = (long long)c.nx * c.ny * c.nz;
   const bool gmg = c.precond == FS_PC_GMG;
   const T rm = sizeof(T) == 4 ? T(S->rmean) : T(0);
+  const T* __restrict__ dcur = S->dsel ? c.d : c.d2;     // written by k_pcg_dirapply of this iteration
   double v[3] = {0.0, 0.0, 0.0};
   for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
-    c.p[q] += alpha * c.d[q];
+    c.p[q] += alpha * dcur[q];
     T r = c.r[q] - alpha * c.q[q];
     if (sizeof(T) == 4) r -= rm;
     c.r[q] = r;
@@ -146,7 +194,7 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_update(const Ctx
   if (grid_sum<3>(v, c.partials, &S->ticket[0], sh, &flag)) {
     if (threadIdx.x == 0) {
       S->rr = v[0]; S->rmean = v[2] / (double)N;
-      S->iter += 1; S->first = 0;
+      S->iter += 1; S->first = 0; S->dsel ^= 1;
       S->rho_prev = S->rho_cur;
       if (!gmg) S->rho_cur = v[1];
       const int conv = sqrt(v[0]) <= S->rtol * sqrt(S->bnorm2);
@@ -180,7 +228,6 @@ template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L) {
 
 template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;
-  ColGeom g = col_geom(c.nx, c.ny, c.nz);
   int n = 0;
   T zs = T(1);
   if (c.precond == FS_PC_GMG) {
@@ -189,8 +236,14 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
     n += launch_vcycle<T>(c, mg, c.r, c.z, L, &fused, zs);
     if (!fused) { FS_LAUNCH(L, "pcg_dot_rz", 2.0 * sizeof(T) * N, k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n; }
   }
-  FS_LAUNCH(L, "pcg_dir", 3.0 * sizeof(T) * N, k_pcg_dir<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n;
-  FS_LAUNCH(L, "pcg_apply_dot", 2.0 * sizeof(T) * N, k_pcg_apply<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz)); ++n;
+  {
+    const DaGeom G = da_geom(c.nx, c.ny, c.nz);
+    const dim3 blk(kDaTX, kDaTY);
+    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    ++n;
+  }
   FS_LAUNCH(L, "pcg_update_norm", 6.0 * sizeof(T) * N, k_pcg_update<T><<<flat_blocks(N), 256, 0, L.s>>>(c, L)); ++n;
   return n;
 }

@@ -142,8 +142,11 @@ def test_poisson_zero_rhs_and_max_iter(fs):
     g.close()
 
 
-def test_gmg_vcycle_elementwise(fs):
-    cfg = _cfg_periodic(48, 32, 40, precond="gmg")
+@pytest.mark.parametrize("dims", [(48, 32, 40), (136, 56, 72), (8, 8, 8), (64, 64, 64)])
+def test_gmg_vcycle_elementwise(fs, dims):
+    # several xy tiles of the fused kernels (60 x 12 cells), ragged tile tails, several z chunks, and a
+    # box smaller than one tile (8^3: the tile wraps around the periodic box more than once)
+    cfg = _cfg_periodic(*dims, precond="gmg")
     rng = np.random.default_rng(2)
     r = rng.standard_normal(W.shapes(cfg)["p"])
     z_ref = _oracle(cfg).vcycle(r)
