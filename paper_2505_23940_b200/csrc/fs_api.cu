@@ -95,7 +95,7 @@ fs_status validate(const fs_params* p) {
   for (int f = 0; f < 6; ++f) if ((int)p->bc[f] < 0 || (int)p->bc[f] > 4) return FS_ERR_INVALID_ARG;
   for (int d = 0; d < 3; ++d)
     if ((p->bc[2 * d] == FS_BC_PERIODIC) != (p->bc[2 * d + 1] == FS_BC_PERIODIC)) return FS_ERR_INVALID_ARG;
-  if ((long long)p->nx * p->ny * p->nz > (1LL << 31) - 1) return FS_ERR_UNSUPPORTED;   // int32 cell keys
+  if ((long long)(p->nx + 1) * (p->ny + 1) * (p->nz + 1) > (1LL << 31) - 1) return FS_ERR_UNSUPPORTED;   // int32 cell keys, 32-bit field offsets
   if ((long long)((p->nx + 29) / 30) * ((p->ny + 3) / 4) > kMaxPartials) return FS_ERR_UNSUPPORTED;   // one reduction partial per xy tile
   if (p->yf) for (int j = 0; j < p->ny; ++j) if (!(p->yf[j + 1] > p->yf[j])) return FS_ERR_INVALID_ARG;
   if ((int)p->precond < 0 || (int)p->precond > 2 || (int)p->delta < 0 || (int)p->delta > 1) return FS_ERR_INVALID_ARG;

@@ -126,6 +126,16 @@ template <class T> int launch_ibm_spread(const Ctx<T>& c, const IbmCtx& ib, cons
 
 // ---- device helpers ---------------------------------------------------------------------------------
 #ifdef __CUDACC__
+// two x-adjacent cells handled by one thread (16-byte accesses for fp64, 8-byte for fp32)
+template <class T> struct V2T;
+template <> struct V2T<double> { using type = double2; };
+template <> struct V2T<float> { using type = float2; };
+template <class T> struct V16T;
+template <> struct V16T<double> { using type = double2; };
+template <> struct V16T<float> { using type = float4; };
+template <class T, class V> __device__ __forceinline__ V ldv2(const T* p) { return *reinterpret_cast<const V*>(p); }
+template <class T, class V> __device__ __forceinline__ void stv2(T* p, const V& v) { *reinterpret_cast<V*>(p) = v; }
+
 __device__ __forceinline__ int wrapi(int i, int n) { i %= n; return i < 0 ? i + n : i; }
 
 __device__ __forceinline__ double warp_sum(double v) {

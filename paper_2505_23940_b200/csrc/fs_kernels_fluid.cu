@@ -87,7 +87,7 @@ template <class T> __device__ __forceinline__ T boundary_normal(const Ctx<T>& c,
 // ---------------------------------------------------------------------------------------------------
 constexpr int kMomTX = 32, kMomTY = 12;
 
-template <class T> struct ColRef { size_t off, pl; T A, B; };   // value = A f[off + pl kz] + B  (x, y ghosts resolved)
+template <class T> struct ColRef { unsigned off, pl; T A, B; };   // 32-bit element offsets: every field has < 2^32 entries (validated)   // value = A f[off + pl kz] + B  (x, y ghosts resolved)
 
 template <class T, int C> __device__ __forceinline__ ColRef<T> col_setup(const Ctx<T>& c, int i, int j) {
   T A = T(1), B = T(0);
@@ -105,7 +105,7 @@ template <class T, int C> __device__ __forceinline__ ColRef<T> col_setup(const C
   } else j = min(max(j, 0), c.ny);
   const int ex = C == 0 ? c.nxu : c.nx, ey = C == 1 ? c.nyv : c.ny;
   ColRef<T> r;
-  r.off = (size_t)i + (size_t)ex * (size_t)j; r.pl = (size_t)ex * ey; r.A = A; r.B = B;
+  r.off = (unsigned)i + (unsigned)ex * (unsigned)j; r.pl = (unsigned)ex * (unsigned)ey; r.A = A; r.B = B;
   return r;
 }
 // plane kk in [-1, nzw] of component C for this thread's column
@@ -117,7 +117,7 @@ template <class T, int C> __device__ __forceinline__ T col_load(const Ctx<T>& c,
     if (kk < 0) { face = 4; kk = -1 - kk; } else if (kk >= c.nz) { face = 5; kk = 2 * c.nz - 1 - kk; }
     if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
   } else kk = min(max(kk, 0), c.nz);
-  return A * f[r.off + r.pl * (size_t)kk] + B;
+  return A * f[r.off + r.pl * (unsigned)kk] + B;
 }
 
 template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momentum(const Ctx<T> c, int kz) {
@@ -132,10 +132,14 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
   const T dt = T(c.dt), nu = T(c.nu);
   const T* __restrict__ U = c.u; const T* __restrict__ V = c.v; const T* __restrict__ W = c.w;
   const ColRef<T> ru = col_setup<T, 0>(c, i, j), rv = col_setup<T, 1>(c, i, j), rw = col_setup<T, 2>(c, i, j);
-  // y metrics of this row (j clamped into the tables; unused rows never store)
-  const int jc = min(max(j, 0), c.ny - 1);
-  const T wyl0 = c.wyl[jc], wyh0 = c.wyh[jc], wyl1 = c.wyl[jc + 1], wyh1 = c.wyh[jc + 1];
-  const T idyj = c.idy[jc + 1], idyjm = c.idy[jc], idyc0 = c.idyc[jc], idyc1 = c.idyc[jc + 1];
+  // y metrics of the tile rows, in shared memory (j clamped into the tables; unused rows never store)
+  __shared__ T MY[8][kMomTY];
+  if (tx < 8) {
+    const int jc = min(max(j, 0), c.ny - 1);
+    const T* tab = tx == 0 ? c.wyl + jc : tx == 1 ? c.wyh + jc : tx == 2 ? c.wyl + jc + 1 : tx == 3 ? c.wyh + jc + 1
+                 : tx == 4 ? c.idy + jc + 1 : tx == 5 ? c.idy + jc : tx == 6 ? c.idyc + jc : c.idyc + jc + 1;
+    MY[tx][ty] = *tab;
+  }
   // register queue of the own column: B = k-1, c = k, T = k+1
   T uB = col_load<T, 0>(c, U, ru, k0 - 1), vB = col_load<T, 1>(c, V, rv, k0 - 1), wB = col_load<T, 2>(c, W, rw, k0 - 1);
   T uc = col_load<T, 0>(c, U, ru, k0), vc = col_load<T, 1>(c, V, rv, k0), wc = col_load<T, 2>(c, W, rw, k0);
@@ -143,16 +147,32 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
   SU[(k0 - 1) & 3][ty][tx] = uB; SV[(k0 - 1) & 3][ty][tx] = vB; SW[(k0 - 1) & 3][ty][tx] = wB;
   SU[k0 & 3][ty][tx] = uc; SV[k0 & 3][ty][tx] = vc; SW[k0 & 3][ty][tx] = wc;
   const int txm = max(tx - 1, 0), txp = min(tx + 1, kMomTX - 1), tym = max(ty - 1, 0), typ = min(ty + 1, kMomTY - 1);
+  // H^{n-1} of the own faces, prefetched one plane ahead (zero where the face does not exist)
+  const bool hasu = own && j < c.ny, hasv = own && i < c.nx, hasw = own && i < c.nx && j < c.ny;
+  const unsigned qu0 = (unsigned)i + (unsigned)c.nxu * (unsigned)j, plu = (unsigned)c.nxu * (unsigned)c.ny;
+  const unsigned qv0 = (unsigned)i + (unsigned)c.nx * (unsigned)j, plv = (unsigned)c.nx * (unsigned)c.nyv;
+  const unsigned qw0 = qv0, plw = (unsigned)c.nx * (unsigned)c.ny;
+  T hun = (hasu && k0 < c.nz) ? c.hu[qu0 + plu * k0] : T(0);
+  T hvn = (hasv && k0 < c.nz) ? c.hv[qv0 + plv * k0] : T(0);
+  T hwn = hasw ? c.hw[qw0 + plw * k0] : T(0);
   for (int k = k0; k < k1; ++k) {
     const T uT = un, vT = vn, wT = wn;
+    const T huo = hun, hvo = hvn, hwo = hwn;
+    if (k + 1 < k1) {
+      hun = (hasu && k + 1 < c.nz) ? c.hu[qu0 + plu * (k + 1)] : T(0);
+      hvn = (hasv && k + 1 < c.nz) ? c.hv[qv0 + plv * (k + 1)] : T(0);
+      hwn = hasw ? c.hw[qw0 + plw * (k + 1)] : T(0);
+    }
     const int s0 = (k - 1) & 3, s1 = k & 3, s2 = (k + 1) & 3;
     SU[s2][ty][tx] = uT; SV[s2][ty][tx] = vT; SW[s2][ty][tx] = wT;
     if (k + 1 < k1) { un = col_load<T, 0>(c, U, ru, k + 2); vn = col_load<T, 1>(c, V, rv, k + 2); wn = col_load<T, 2>(c, W, rw, k + 2); }
     __syncthreads();
     if (own) {
+      const T wyl0 = MY[0][ty], wyh0 = MY[1][ty], wyl1 = MY[2][ty], wyh1 = MY[3][ty];
+      const T idyj = MY[4][ty], idyjm = MY[5][ty], idyc0 = MY[6][ty], idyc1 = MY[7][ty];
       // ---- u face ----
       if (j < c.ny && k < c.nz) {
-        const size_t q = (size_t)i + (size_t)c.nxu * ((size_t)j + (size_t)c.ny * k);
+        const size_t q = qu0 + plu * (unsigned)k;
         if (c.bx && (i == 0 || i == c.nx)) {
           const int side = i == 0 ? 0 : 1;
           const size_t qi = side ? q - 1 : q + 1;
@@ -172,13 +192,13 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
           const T dyy = ((uN - uc) * idyc1 - (uc - uS) * idyc0) * idyj;
           const T dzz = (uT - T(2) * uc + uB) * c.ihz2;
           const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[0]);
-          c.us[q] = uc + dt * (a0 * H + a1 * c.hu[q]);
+          c.us[q] = uc + dt * (a0 * H + a1 * huo);
           c.hu[q] = H;
         }
       }
       // ---- v face (control volume between y_c(j-1) and y_c(j)) ----
       if (i < c.nx && k < c.nz) {
-        const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.nyv * k);
+        const size_t q = qv0 + plv * (unsigned)k;
         if (c.by && (j == 0 || j == c.ny)) {
           const int side = j == 0 ? 0 : 1;
           const size_t qi = side ? q - c.nx : q + c.nx;
@@ -199,13 +219,13 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
           const T dyy = ((vN - vc) * idyj - (vc - vS) * idyjm) * idyc0;
           const T dzz = (vT - T(2) * vc + vB) * c.ihz2;
           const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[1]);
-          c.vs[q] = vc + dt * (a0 * H + a1 * c.hv[q]);
+          c.vs[q] = vc + dt * (a0 * H + a1 * hvo);
           c.hv[q] = H;
         }
       }
       // ---- w face ----
       if (i < c.nx && j < c.ny) {
-        const size_t q = (size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k);
+        const size_t q = qw0 + plw * (unsigned)k;
         if (c.bz && (k == 0 || k == c.nz)) {
           const int side = k == 0 ? 0 : 1;
           const size_t pl = (size_t)c.nx * c.ny;
@@ -226,7 +246,7 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
           const T dyy = ((wN - wc) * idyc1 - (wc - wS) * idyc0) * idyj;
           const T dzz = (wT - T(2) * wc + wB) * c.ihz2;
           const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[2]);
-          c.ws[q] = wc + dt * (a0 * H + a1 * c.hw[q]);
+          c.ws[q] = wc + dt * (a0 * H + a1 * hwo);
           c.hw[q] = H;
         }
       }

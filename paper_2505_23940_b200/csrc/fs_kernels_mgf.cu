@@ -14,9 +14,6 @@
 
 namespace fs {
 
-template <class T> struct V2T;
-template <> struct V2T<double> { using type = double2; };
-template <> struct V2T<float> { using type = float2; };
 
 constexpr int kMgTY = 16;                 // rows of the extended tile
 constexpr int kMgIX = 60, kMgIY = kMgTY - 4;
@@ -42,8 +39,6 @@ static MgGeom mg_geom(int nx, int ny, int nz) {
 // even chunk boundaries
 __device__ __forceinline__ int chunk_lo(int c, int nchunks, int nz) { return 2 * (int)(((long long)c * (nz / 2)) / nchunks); }
 
-template <class T, class V> __device__ __forceinline__ V ldv2(const T* p) { return *reinterpret_cast<const V*>(p); }
-template <class T, class V> __device__ __forceinline__ void stv2(T* p, const V& v) { *reinterpret_cast<V*>(p) = v; }
 
 constexpr int kMgPL = kMgTY * 32;         // pairs per shared-memory plane
 

@@ -165,28 +165,163 @@ static DaGeom da_geom(int nx, int ny, int nz) {
   return g;
 }
 
+// Same operation, two x-adjacent cells per thread (nx even): 16-byte (fp64) / 8-byte (fp32) accesses, half
+// the index arithmetic per cell, 64 x 16 extended tile -> 60 x 14 results, z loop unrolled by renaming.
+constexpr int kDa2IX = 60, kDa2IY = kDaTY - 2, kDa2PL = kDaTY * 32;
+
+template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pcg_dirapply2(const Ctx<T> c, T zs, int kz) {
+  using V = typename V2T<T>::type;
+  __shared__ V D[2 * kDa2PL];
+  __shared__ double sh[32]; __shared__ int flag;
+  const Scalars* S = c.S;
+  if (S->done) return;
+  const bool first = S->first != 0;
+  const T beta = first ? T(0) : T(S->rho_cur / S->rho_prev);
+  const T* __restrict__ dold = S->dsel ? c.d2 : c.d;
+  T* __restrict__ dnew = S->dsel ? c.d : c.d2;
+  const T* __restrict__ zsrc = PC == 2 ? c.z : c.r;
+  const int lane = threadIdx.x, ty = threadIdx.y;
+  const int gx = blockIdx.x * kDa2IX - 2 + 2 * lane, gy = blockIdx.y * kDa2IY - 1 + ty;
+  const int sx = c.bx ? min(max(gx, 0), c.nx - 2) : wrapi(gx, c.nx);
+  const int sy = c.by ? min(max(gy, 0), c.ny - 1) : wrapi(gy, c.ny);
+  const bool fixl = c.bx && gx < 0, fixr = c.bx && gx >= c.nx;       // clamped halo pairs: both cells = the boundary cell
+  const bool own = lane >= 1 && lane <= 30 && ty >= 1 && ty <= kDaTY - 2 && gx < c.nx && gy < c.ny;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  const unsigned pl = (unsigned)c.nx * c.ny, row = (unsigned)sx + (unsigned)c.nx * sy;
+  const T cyl = c.cyl[sy], cyh = c.cyh[sy], idy = c.idy[sy + 1], ndy = -c.dy[sy + 1];
+  const T ihx2 = c.ihx2, ihz2 = c.ihz2;
+  T dgx = T(0), dgy = T(0);                // Jacobi: x + y parts of diag A / dy for the two cells
+  if (PC == 1) {
+    const T dyy = (cyh + cyl) * idy;
+    dgx = T((c.bx && sx == 0 ? 0 : 1) + 1) * ihx2 + dyy;
+    dgy = T(1 + (c.bx && sx + 1 == c.nx - 1 ? 0 : 1)) * ihx2 + dyy;
+  }
+  const int own_o = ty * 32 + lane;
+  const int oS = (ty > 0 ? ty - 1 : 0) * 32 + lane, oN = (ty < kDaTY - 1 ? ty + 1 : ty) * 32 + lane;
+  const int oW = ty * 32 + (lane > 0 ? lane - 1 : 0), oE = ty * 32 + (lane < 31 ? lane + 1 : 31);
+  V rz, rd;                                 // raw z and old d of the plane in flight
+  int ksrc = 0;
+  auto fetch = [&](int k) {
+    ksrc = c.bz ? min(max(k, 0), c.nz - 1) : (k < 0 ? k + c.nz : (k >= c.nz ? k - c.nz : k));
+    const unsigned o = row + pl * (unsigned)ksrc;
+    rz = ldv2<T, V>(zsrc + o);
+    if (!first) rd = ldv2<T, V>(dold + o);
+  };
+  auto make = [&]() {                       // d' of the fetched plane
+    V z;
+    if (PC == 2) { z.x = rz.x * zs; z.y = rz.y * zs; }
+    else if (PC == 1) {
+      const T dzz = T((c.bz && ksrc == 0 ? 0 : 1) + (c.bz && ksrc == c.nz - 1 ? 0 : 1)) * ihz2;
+      z.x = rz.x / ((dgx + dzz) * c.dy[sy + 1]); z.y = rz.y / ((dgy + dzz) * c.dy[sy + 1]);
+    } else z = rz;
+    V d = z;
+    if (!first) { d.x = z.x + beta * rd.x; d.y = z.y + beta * rd.y; }
+    if (fixl) d.y = d.x;
+    if (fixr) d.x = d.y;
+    return d;
+  };
+  rd.x = rd.y = T(0);
+  V d0, d1, d2;
+  fetch(k0 - 1); d0 = make();
+  fetch(k0); d1 = make();
+  int b = 0;
+  D[own_o] = d1;
+  fetch(k0 + 1);
+  __syncthreads();
+  double dot = 0.0;
+  // dB, dC = d'(k-1), d'(k); dT receives d'(k+1)
+  auto step = [&](int k, const V& dB, const V& dC, V& dT) {
+    dT = make();
+    if (k + 1 < k1) fetch(k + 2);
+    const V* P = D + b;
+    const V Sv = P[oS], Nv = P[oN];
+    const T xw = P[oW].y, xe = P[oE].x;
+    T ax = (dC.y - dC.x) * ihx2 - (dC.x - xw) * ihx2;
+    T ay = (xe - dC.y) * ihx2 - (dC.y - dC.x) * ihx2;
+    ax += ((Nv.x - dC.x) * cyh - (dC.x - Sv.x) * cyl) * idy;
+    ay += ((Nv.y - dC.y) * cyh - (dC.y - Sv.y) * cyl) * idy;
+    ax += (dT.x - dC.x) * ihz2 - (dC.x - dB.x) * ihz2;
+    ay += (dT.y - dC.y) * ihz2 - (dC.y - dB.y) * ihz2;
+    V q; q.x = ax * ndy; q.y = ay * ndy;
+    if (own) {
+      const unsigned o = row + pl * (unsigned)k;
+      stv2<T, V>(dnew + o, dC); stv2<T, V>(c.q + o, q);
+      dot += (double)(dC.x * q.x + dC.y * q.y);
+    }
+    b = kDa2PL - b;
+    D[b + own_o] = dT;
+    __syncthreads();
+  };
+  int k = k0;
+  for (;;) {
+    step(k, d0, d1, d2); if (++k >= k1) break;
+    step(k, d1, d2, d0); if (++k >= k1) break;
+    step(k, d2, d0, d1); if (++k >= k1) break;
+  }
+  double v[1] = {dot};
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (lane == 0 && ty == 0) c.S->dq = v[0];
+  }
+}
+
+static DaGeom da2_geom(int nx, int ny, int nz) {
+  const int bxn = (nx + kDa2IX - 1) / kDa2IX, byn = (ny + kDa2IY - 1) / kDa2IY;
+  int kz = nz;
+  while (kz > 16 && (long long)bxn * byn * ((nz + kz - 1) / kz) < 4LL * 296) kz = (kz + 1) / 2;
+  DaGeom g; g.kz = kz; g.grid = dim3(bxn, byn, (nz + kz - 1) / kz);
+  return g;
+}
+
 // ---- K2: x += alpha d, r -= alpha q fused with ||r||^2 and r.z; loop control -------------------------
 // fp32 only: rounding makes sum(q) != 0, so r slowly acquires a component along the null space of A
 // (constants) that CG can never remove; once it dominates r the fp32 stencil differences lose all
 // accuracy and the iteration diverges.  The mean of r measured by the previous pass is subtracted here
 // (one iteration of lag; exactly zero in exact arithmetic, where sum(r) = 0).  fp64 follows O7 literally.
-template <class T> __global__ void __launch_bounds__(256) k_pcg_update(const Ctx<T> c, Launch L) {
+template <class T, bool GMG> __global__ void __launch_bounds__(256) k_pcg_update(const Ctx<T> c, Launch L) {
   __shared__ double sh[3 * 32]; __shared__ int flag;
   Scalars* S = c.S;
   if (S->done) return;
   const T alpha = T(S->rho_cur / S->dq);
   const long long N = (long long)c.nx * c.ny * c.nz;
-  const bool gmg = c.precond == FS_PC_GMG;
   const T rm = sizeof(T) == 4 ? T(S->rmean) : T(0);
   const T* __restrict__ dcur = S->dsel ? c.d : c.d2;     // written by k_pcg_dirapply of this iteration
   double v[3] = {0.0, 0.0, 0.0};
-  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
-    c.p[q] += alpha * dcur[q];
-    T r = c.r[q] - alpha * c.q[q];
-    if (sizeof(T) == 4) r -= rm;
-    c.r[q] = r;
-    v[0] += (double)r * (double)r; v[2] += (double)r;
-    if (!gmg) {
+  if (GMG) {
+    // 16-byte accesses; per-vector partial sums in T, accumulated in fp64 (fp32: one conversion per 4 cells)
+    constexpr int VW = 16 / sizeof(T);
+    using V = typename V16T<T>::type;
+    const long long NV = N / VW;
+    const V* __restrict__ dv = reinterpret_cast<const V*>(dcur); const V* __restrict__ qv = reinterpret_cast<const V*>(c.q);
+    V* __restrict__ pv = reinterpret_cast<V*>(c.p); V* __restrict__ rv = reinterpret_cast<V*>(c.r);
+    for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < NV; q += (long long)gridDim.x * blockDim.x) {
+      V p = pv[q], r = rv[q]; const V d = dv[q], qq = qv[q];
+      T* pe = reinterpret_cast<T*>(&p); T* re = reinterpret_cast<T*>(&r);
+      const T* de = reinterpret_cast<const T*>(&d); const T* qe = reinterpret_cast<const T*>(&qq);
+      T s2 = T(0), s1 = T(0);
+#pragma unroll
+      for (int a = 0; a < VW; ++a) {
+        pe[a] += alpha * de[a];
+        T t = re[a] - alpha * qe[a];
+        if (sizeof(T) == 4) t -= rm;
+        re[a] = t; s2 += t * t; s1 += t;
+      }
+      pv[q] = p; rv[q] = r;
+      v[0] += (double)s2; v[2] += (double)s1;
+    }
+    for (long long q = NV * VW + blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+      c.p[q] += alpha * dcur[q];
+      T r = c.r[q] - alpha * c.q[q];
+      if (sizeof(T) == 4) r -= rm;
+      c.r[q] = r;
+      v[0] += (double)r * (double)r; v[2] += (double)r;
+    }
+  } else {
+    for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+      c.p[q] += alpha * dcur[q];
+      T r = c.r[q] - alpha * c.q[q];
+      if (sizeof(T) == 4) r -= rm;
+      c.r[q] = r;
+      v[0] += (double)r * (double)r; v[2] += (double)r;
       const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
       v[1] += (double)r * (double)precond_point<T>(c, r, i, j, k);
     }
@@ -196,7 +331,7 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_update(const Ctx
       S->rr = v[0]; S->rmean = v[2] / (double)N;
       S->iter += 1; S->first = 0; S->dsel ^= 1;
       S->rho_prev = S->rho_cur;
-      if (!gmg) S->rho_cur = v[1];
+      if (!GMG) S->rho_cur = v[1];
       const int conv = sqrt(v[0]) <= S->rtol * sqrt(S->bnorm2);
       S->converged = conv;
       S->done = conv || S->iter >= S->max_iter;
@@ -236,7 +371,14 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
     n += launch_vcycle<T>(c, mg, c.r, c.z, L, &fused, zs);
     if (!fused) { FS_LAUNCH(L, "pcg_dot_rz", 2.0 * sizeof(T) * N, k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n; }
   }
-  {
+  if (c.nx % 2 == 0) {
+    const DaGeom G = da2_geom(c.nx, c.ny, c.nz);
+    const dim3 blk(32, kDaTY);
+    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply2<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply2<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply2<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    ++n;
+  } else {
     const DaGeom G = da_geom(c.nx, c.ny, c.nz);
     const dim3 blk(kDaTX, kDaTY);
     if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
@@ -244,7 +386,9 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
     else FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
     ++n;
   }
-  FS_LAUNCH(L, "pcg_update_norm", 6.0 * sizeof(T) * N, k_pcg_update<T><<<flat_blocks(N), 256, 0, L.s>>>(c, L)); ++n;
+  if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_update_norm", 6.0 * sizeof(T) * N, k_pcg_update<T, true><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
+  else FS_LAUNCH(L, "pcg_update_norm", 6.0 * sizeof(T) * N, k_pcg_update<T, false><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
+  ++n;
   return n;
 }
 
