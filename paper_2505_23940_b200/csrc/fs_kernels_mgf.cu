@@ -4,26 +4,29 @@
 // prolong+correct 2.125); the two kernels here move 2.125 + 3.125:
 //   k_mg_down : g -> e = two damped-Jacobi sweeps from a zero guess, gc = R (g - (-L) e)
 //   k_mg_up   : e, ec, g -> e' = two sweeps applied to (e + P ec)   [level 0: also r . z for PCG]
-// Both are 2.5-D streaming kernels: a CTA owns an xy tile and marches in z.  A thread owns two x-adjacent
-// cells (16-byte loads for fp64, 8 for fp32), keeps the z neighbours of every pipeline stage in a register
-// queue, gets the x and y neighbours
-// through a double-buffered shared-memory plane (a warp is one row of the tile); one __syncthreads per plane.  Each later stage is valid on
-// a tile one cell smaller per side (overlapped tiling: 64 x TY extended tile -> 60 x (TY-4) results); the
-// halo re-reads hit L2.  All grids are periodic (GMG is only offered for triply periodic boxes).
+// Both are 2.5-D streaming kernels: a CTA owns an xy tile and marches in z.  A thread owns a 2 x 2 patch of
+// cells (two x-adjacent pairs: 16-byte global accesses for fp64, 8 for fp32; the patch is exactly one coarse
+// cell, so restriction and prolongation need no exchange), keeps the z neighbours of every pipeline stage
+// in a register queue that rotates by renaming (z loop unrolled), and exchanges only the patch edges through
+// double-buffered shared-memory planes (separate planes for the even and the odd x column, so that every
+// shared access is a compact row: the kernels are bound by shared-memory wavefronts, not by HBM, if the
+// patch is smaller -- profiles/).  One __syncthreads per plane.  Each later stage is valid on a tile one
+// cell smaller per side (overlapped tiling: 64 x 2TR extended tile -> 60 x (2TR-4) results); the halo
+// re-reads hit L2.  All grids are periodic (GMG is only offered for triply periodic boxes).
+#include <cstdlib>
 #include "fs_internal.cuh"
 
 namespace fs {
 
-
-constexpr int kMgTY = 16;                 // rows of the extended tile
-constexpr int kMgIX = 60, kMgIY = kMgTY - 4;
+constexpr int kMgIX = 60;                 // result columns per tile (extended tile: 64 = 32 lanes x 2)
+template <int TR> struct MgTile { static constexpr int ROWS = 2 * TR, IY = 2 * TR - 4, PL = 2 * TR * 32; };
 
 __device__ __forceinline__ int modp(int a, int n) { a %= n; return a < 0 ? a + n : a; }
 
 struct MgGeom { dim3 grid; int zchunks; };
-static MgGeom mg_geom(int nx, int ny, int nz) {
-  const int bxn = (nx + kMgIX - 1) / kMgIX, byn = (ny + kMgIY - 1) / kMgIY;
-  const long long slots = 2LL * 148;      // two CTAs of 512 threads per SM
+static MgGeom mg_geom(int nx, int ny, int nz, int iy, int slots_per_sm) {
+  const int bxn = (nx + kMgIX - 1) / kMgIX, byn = (ny + iy - 1) / iy;
+  const long long slots = 148LL * slots_per_sm;
   int best = 1; double best_cost = 1e300;
   for (int zc = 1; zc <= 64 && nz / zc >= 8; ++zc) {
     const long long blocks = (long long)bxn * byn * zc;
@@ -39,85 +42,94 @@ static MgGeom mg_geom(int nx, int ny, int nz) {
 // even chunk boundaries
 __device__ __forceinline__ int chunk_lo(int c, int nchunks, int nz) { return 2 * (int)(((long long)c * (nz / 2)) / nchunks); }
 
+// A thread's 2 x 2 patch at one plane: lo = pair of row 2 ty, hi = pair of row 2 ty + 1.
+template <class T> struct Quad { typename V2T<T>::type lo, hi; };
 
-constexpr int kMgPL = kMgTY * 32;         // pairs per shared-memory plane
-
-// Shared-memory positions of a thread: own pair, the rows below / above, the pairs left / right (clamped at
-// the tile edge: edge results are never used).
-struct MgPos { int own, s, n, w, e; };
-__device__ __forceinline__ MgPos mg_pos(int lane, int ty) {
+// Shared-memory offsets of a thread (elements of T inside one plane of ROWS x 32).
+struct MgPos { int own0, s, n, w0, e0; };
+template <int TR> __device__ __forceinline__ MgPos mg_pos(int lane, int ty) {
+  const int r0 = 2 * ty, rs = r0 > 0 ? r0 - 1 : 0, rn = r0 + 2 < 2 * TR ? r0 + 2 : r0 + 1;
   MgPos p;
-  p.own = ty * 32 + lane;
-  p.s = (ty > 0 ? ty - 1 : 0) * 32 + lane;
-  p.n = (ty < kMgTY - 1 ? ty + 1 : ty) * 32 + lane;
-  p.w = ty * 32 + (lane > 0 ? lane - 1 : 0);
-  p.e = ty * 32 + (lane < 31 ? lane + 1 : 31);
+  p.own0 = r0 * 32 + lane; p.s = rs * 32 + lane; p.n = rn * 32 + lane;
+  p.w0 = r0 * 32 + (lane > 0 ? lane - 1 : 0); p.e0 = r0 * 32 + (lane < 31 ? lane + 1 : 31);
   return p;
 }
-// sum of the six neighbours of both cells of the pair c held at plane buffer P (the pair's own plane);
-// zm / zp = the pairs below / above (register queue).
-template <class T, class V> __device__ __forceinline__ V nb6(const V* __restrict__ P, const MgPos& q, const V& c, const V& zm, const V& zp) {
-  const V S = P[q.s], N = P[q.n];
-  const T left = P[q.w].y, right = P[q.e].x;
-  V r;
-  r.x = ((left + c.y) + (S.x + N.x)) + (zm.x + zp.x);
-  r.y = ((c.x + right) + (S.y + N.y)) + (zm.y + zp.y);
+// Sum of the six neighbours of the four cells of patch c, whose plane is in the shared planes X (even
+// columns) / Y (odd columns); zm / zp = the patches below / above (register queue).
+template <class T> __device__ __forceinline__ Quad<T> nbq(const T* __restrict__ X, const T* __restrict__ Y, const MgPos& q,
+                                                         const Quad<T>& c, const Quad<T>& zm, const Quad<T>& zp) {
+  const T sx = X[q.s], sy = Y[q.s], nx_ = X[q.n], ny_ = Y[q.n];
+  const T w0 = Y[q.w0], e0 = X[q.e0], w1 = Y[q.w0 + 32], e1 = X[q.e0 + 32];
+  Quad<T> r;
+  r.lo.x = ((w0 + c.lo.y) + (sx + c.hi.x)) + (zm.lo.x + zp.lo.x);
+  r.lo.y = ((c.lo.x + e0) + (sy + c.hi.y)) + (zm.lo.y + zp.lo.y);
+  r.hi.x = ((w1 + c.hi.y) + (c.lo.x + nx_)) + (zm.hi.x + zp.hi.x);
+  r.hi.y = ((c.hi.x + e1) + (c.lo.y + ny_)) + (zm.hi.y + zp.hi.y);
   return r;
+}
+template <class T> __device__ __forceinline__ void stq(T* __restrict__ X, T* __restrict__ Y, const MgPos& q, const Quad<T>& c) {
+  X[q.own0] = c.lo.x; Y[q.own0] = c.lo.y; X[q.own0 + 32] = c.hi.x; Y[q.own0 + 32] = c.hi.y;
 }
 
 // ---- downward leg: e = S^2(0; g), gc = R (g - (-L) e) -----------------------------------------------------
 // Two damped-Jacobi sweeps from a zero guess collapse to e = cg g + cn nb(g) with cg = 2 cw - 6 cw^2 / h^2,
 // cn = cw^2 / h^2  (first sweep: cw g; second: cw g + cw (g - (6 cw g - cw nb) / h^2)).
-// The z loop is unrolled three times so that the register queues rotate by renaming.
-template <class T> __global__ void __launch_bounds__(32 * kMgTY, 2)
+template <class T, int TR> __global__ void __launch_bounds__(32 * TR, (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1))
 k_mg_down(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__ eo, T* __restrict__ gc,
           int nx, int ny, int nz, T cg, T cn, T ih2) {
   using V = typename V2T<T>::type;
+  constexpr int PL = MgTile<TR>::PL;
   if (done && *done) return;
-  __shared__ V G[2 * kMgPL];
-  __shared__ V E[2 * kMgPL];
-  __shared__ T R[2 * kMgPL];
+  extern __shared__ __align__(16) unsigned char mg_smem[];
+  T* GX = reinterpret_cast<T*>(mg_smem); T* GY = GX + 2 * PL; T* EX = GY + 2 * PL; T* EY = EX + 2 * PL;
   const int lane = threadIdx.x, ty = threadIdx.y;
-  const int gx = blockIdx.x * kMgIX - 2 + 2 * lane, gy = blockIdx.y * kMgIY - 2 + ty;
-  const unsigned pl = (unsigned)nx * ny, row = (unsigned)modp(gx, nx) + (unsigned)nx * modp(gy, ny);
-  const bool interior = lane >= 1 && lane <= 30 && ty >= 2 && ty < kMgTY - 2 && gx < nx && gy < ny;
-  const bool comb = interior && ((ty & 1) == 0);
+  const int gx = blockIdx.x * kMgIX - 2 + 2 * lane, gy = blockIdx.y * MgTile<TR>::IY - 2 + 2 * ty;
+  const unsigned pl = (unsigned)nx * ny, gxw = (unsigned)modp(gx, nx);
+  const unsigned row0 = gxw + (unsigned)nx * modp(gy, ny), row1 = gxw + (unsigned)nx * modp(gy + 1, ny);
+  const bool interior = lane >= 1 && lane <= 30 && ty >= 1 && ty <= TR - 2 && gx < nx && gy < ny;
   const int z0 = chunk_lo(blockIdx.z, gridDim.z, nz), z1 = chunk_lo(blockIdx.z + 1, gridDim.z, nz);
   const int tend = z1 + 1;
-  const MgPos q = mg_pos(lane, ty);
+  const MgPos q = mg_pos<TR>(lane, ty);
   const unsigned cpl = (unsigned)(nx >> 1) * (ny >> 1), crow = (unsigned)(gx >> 1) + (unsigned)(nx >> 1) * (gy >> 1);
   const T m6 = T(-6) * ih2;
   T acc = T(0);
   int zl = modp(z0 - 2, nz);              // plane of the load in flight
-  int b = 0;                              // buffer of plane t (toggles); plane t-1 lives in kMgPL - b
-  V nxt = ldv2<T, V>(g + (row + pl * zl));
+  int b = 0;                              // buffer of plane t (toggles); plane t-1 lives in PL - b
+  Quad<T> nxt;
+  nxt.lo = ldv2<T, V>(g + (row0 + pl * zl)); nxt.hi = ldv2<T, V>(g + (row1 + pl * zl));
   // one plane: gA, gB = g(t-2), g(t-1); gC receives g(t).  eA, eB = e(t-3), e(t-2); eC receives e(t-1).
-  auto step = [&](int t, const V& gA, const V& gB, V& gC, const V& eA, const V& eB, V& eC) {
+  auto step = [&](int t, const Quad<T>& gA, const Quad<T>& gB, Quad<T>& gC, const Quad<T>& eA, const Quad<T>& eB, Quad<T>& eC) {
     gC = nxt;
-    if (t < tend) { zl = zl + 1 == nz ? 0 : zl + 1; nxt = ldv2<T, V>(g + (row + pl * zl)); }
-    const int pb = kMgPL - b;
+    if (t < tend) {
+      zl = zl + 1 == nz ? 0 : zl + 1;
+      nxt.lo = ldv2<T, V>(g + (row0 + pl * zl)); nxt.hi = ldv2<T, V>(g + (row1 + pl * zl));
+    }
+    const int pb = PL - b;
     if (t >= z0) {            // e(t-1)
-      const V nb = nb6<T, V>(G + pb, q, gB, gA, gC);
-      eC.x = cg * gB.x + cn * nb.x; eC.y = cg * gB.y + cn * nb.y;
+      const Quad<T> nb = nbq<T>(GX + pb, GY + pb, q, gB, gA, gC);
+      eC.lo.x = cg * gB.lo.x + cn * nb.lo.x; eC.lo.y = cg * gB.lo.y + cn * nb.lo.y;
+      eC.hi.x = cg * gB.hi.x + cn * nb.hi.x; eC.hi.y = cg * gB.hi.y + cn * nb.hi.y;
     }
-    if (t >= z0 + 2) {        // residual at plane t-2, its x-pair sum, store of e(t-2)
-      const V nb = nb6<T, V>(E + b, q, eB, eA, eC);
-      const T rx = (gA.x + m6 * eB.x) + ih2 * nb.x;
-      const T ry = (gA.y + m6 * eB.y) + ih2 * nb.y;
-      R[b + q.own] = rx + ry;
-      if (interior) stv2<T, V>(eo + (row + pl * (unsigned)(t - 2)), eB);
+    if (t >= z0 + 2) {        // residual at plane t-2 summed over the patch, store of e(t-2)
+      const Quad<T> nb = nbq<T>(EX + b, EY + b, q, eB, eA, eC);
+      const T r0 = ((gA.lo.x + m6 * eB.lo.x) + ih2 * nb.lo.x) + ((gA.lo.y + m6 * eB.lo.y) + ih2 * nb.lo.y);
+      const T r1 = ((gA.hi.x + m6 * eB.hi.x) + ih2 * nb.hi.x) + ((gA.hi.y + m6 * eB.hi.y) + ih2 * nb.hi.y);
+      acc += r0 + r1;
+      if (interior) {
+        const unsigned o = pl * (unsigned)(t - 2);
+        stv2<T, V>(eo + (row0 + o), eB.lo); stv2<T, V>(eo + (row1 + o), eB.hi);
+        if ((t - z0) & 1) gc[crow + cpl * (unsigned)((t - 2) >> 1)] = T(0.125) * acc;
+      }
+      if ((t - z0) & 1) acc = T(0);
     }
-    G[b + q.own] = gC;
-    if (t >= z0) E[pb + q.own] = eC;
+    stq<T>(GX + b, GY + b, q, gC);
+    if (t >= z0) stq<T>(EX + pb, EY + pb, q, eC);
     __syncthreads();
-    if (t >= z0 + 2 && comb) {
-      acc += R[b + q.own] + R[b + q.own + 32];
-      if ((t - z0) & 1) { gc[crow + cpl * (unsigned)((t - 2) >> 1)] = T(0.125) * acc; acc = T(0); }
-    }
     b = pb;
   };
-  const V zero = {T(0), T(0)};
-  V g0 = zero, g1 = zero, g2 = zero, e0 = zero, e1 = zero, e2 = zero;
+  Quad<T> g0, g1, g2, e0, e1, e2;
+  g0.lo.x = g0.lo.y = g0.hi.x = g0.hi.y = T(0);
+  g1 = g0; g2 = g0; e0 = g0; e1 = g0; e2 = g0;
   int t = z0 - 2;
   for (;;) {
     step(t, g0, g1, g2, e0, e1, e2); if (++t > tend) break;
@@ -128,63 +140,75 @@ k_mg_down(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__
 
 // ---- upward leg: e' = S^2(e + P ec; g); DOT (level 0 inside PCG): rho = r . (zs e') ---------------------
 // One sweep: e + cw (g - (6 e - nb) / h^2) = ce e + cw g + cn nb with ce = 1 - 6 cw / h^2, cn = cw / h^2.
-template <class T, bool DOT> __global__ void __launch_bounds__(32 * kMgTY, 2)
+template <class T> __device__ __forceinline__ Quad<T> sweepq(const Quad<T>& e, const Quad<T>& nb, const Quad<T>& g, T ce, T cw, T cn) {
+  Quad<T> o;
+  o.lo.x = (ce * e.lo.x + cw * g.lo.x) + cn * nb.lo.x; o.lo.y = (ce * e.lo.y + cw * g.lo.y) + cn * nb.lo.y;
+  o.hi.x = (ce * e.hi.x + cw * g.hi.x) + cn * nb.hi.x; o.hi.y = (ce * e.hi.y + cw * g.hi.y) + cn * nb.hi.y;
+  return o;
+}
+
+template <class T, int TR, bool DOT> __global__ void __launch_bounds__(32 * TR, (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1))
 k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __restrict__ ec, const T* __restrict__ g,
         T* __restrict__ eo, int nx, int ny, int nz, T ce, T cw, T cn, T zs, Scalars* S_, double* partials) {
   using V = typename V2T<T>::type;
+  constexpr int PL = MgTile<TR>::PL;
   if (done && *done) return;
-  __shared__ V A[2 * kMgPL];
-  __shared__ V B[2 * kMgPL];
+  extern __shared__ __align__(16) unsigned char mg_smem[];
+  T* AX = reinterpret_cast<T*>(mg_smem); T* AY = AX + 2 * PL; T* BX = AY + 2 * PL; T* BY = BX + 2 * PL;
   __shared__ double sh[32]; __shared__ int flag;
   const int lane = threadIdx.x, ty = threadIdx.y;
-  const int gx = blockIdx.x * kMgIX - 2 + 2 * lane, gy = blockIdx.y * kMgIY - 2 + ty;
+  const int gx = blockIdx.x * kMgIX - 2 + 2 * lane, gy = blockIdx.y * MgTile<TR>::IY - 2 + 2 * ty;
   const int gxw = modp(gx, nx), gyw = modp(gy, ny);
-  const unsigned pl = (unsigned)nx * ny, row = (unsigned)gxw + (unsigned)nx * gyw;
-  const bool interior = lane >= 1 && lane <= 30 && ty >= 2 && ty < kMgTY - 2 && gx < nx && gy < ny;
+  const unsigned pl = (unsigned)nx * ny;
+  const unsigned row0 = (unsigned)gxw + (unsigned)nx * gyw, row1 = (unsigned)gxw + (unsigned)nx * modp(gy + 1, ny);
+  const bool interior = lane >= 1 && lane <= 30 && ty >= 1 && ty <= TR - 2 && gx < nx && gy < ny;
   const int z0 = chunk_lo(blockIdx.z, gridDim.z, nz), z1 = chunk_lo(blockIdx.z + 1, gridDim.z, nz);
   const int tend = z1 + 1;
-  const MgPos q = mg_pos(lane, ty);
+  const MgPos q = mg_pos<TR>(lane, ty);
   const unsigned cpl = (unsigned)(nx >> 1) * (ny >> 1), crow = (unsigned)(gxw >> 1) + (unsigned)(nx >> 1) * (gyw >> 1);
   double dot = 0.0;
   int zl = modp(z0 - 2, nz);              // plane of the e / ec load in flight; the g load in flight is one plane behind
   int b = 0;
-  V nxa = ldv2<T, V>(ein + (row + pl * zl));
+  Quad<T> nxa, nxg;
+  nxa.lo = ldv2<T, V>(ein + (row0 + pl * zl)); nxa.hi = ldv2<T, V>(ein + (row1 + pl * zl));
   T nxc = ec[crow + cpl * (unsigned)(zl >> 1)];
-  const V zero = {T(0), T(0)};
-  V nxg = zero;
+  nxg.lo.x = nxg.lo.y = nxg.hi.x = nxg.hi.y = T(0);
   // aA, aB = (e + P ec)(t-2), (t-1); aC receives plane t.  bA, bB = first post-sweep at t-3, t-2; bC receives t-1.
   // gA = g(t-2); gB receives g(t-1).
-  auto step = [&](int t, const V& aA, const V& aB, V& aC, const V& bA, const V& bB, V& bC, const V& gA, V& gB) {
-    aC.x = nxa.x + nxc; aC.y = nxa.y + nxc;
+  auto step = [&](int t, const Quad<T>& aA, const Quad<T>& aB, Quad<T>& aC, const Quad<T>& bA, const Quad<T>& bB, Quad<T>& bC,
+                  const Quad<T>& gA, Quad<T>& gB) {
+    aC.lo.x = nxa.lo.x + nxc; aC.lo.y = nxa.lo.y + nxc; aC.hi.x = nxa.hi.x + nxc; aC.hi.y = nxa.hi.y + nxc;
     gB = nxg;
     if (t < tend) {
-      nxg = ldv2<T, V>(g + (row + pl * zl));           // plane t
+      const unsigned og = pl * zl;                     // plane t
+      nxg.lo = ldv2<T, V>(g + (row0 + og)); nxg.hi = ldv2<T, V>(g + (row1 + og));
       zl = zl + 1 == nz ? 0 : zl + 1;
-      nxa = ldv2<T, V>(ein + (row + pl * zl));         // plane t+1
+      const unsigned oa = pl * zl;                     // plane t+1
+      nxa.lo = ldv2<T, V>(ein + (row0 + oa)); nxa.hi = ldv2<T, V>(ein + (row1 + oa));
       nxc = ec[crow + cpl * (unsigned)(zl >> 1)];
     }
-    const int pb = kMgPL - b;
+    const int pb = PL - b;
     if (t >= z0) {            // first post-sweep at plane t-1
-      const V nb = nb6<T, V>(A + pb, q, aB, aA, aC);
-      bC.x = (ce * aB.x + cw * gB.x) + cn * nb.x;
-      bC.y = (ce * aB.y + cw * gB.y) + cn * nb.y;
+      const Quad<T> nb = nbq<T>(AX + pb, AY + pb, q, aB, aA, aC);
+      bC = sweepq<T>(aB, nb, gB, ce, cw, cn);
     }
     if (t >= z0 + 2) {        // second post-sweep at plane t-2
-      const V nb = nb6<T, V>(B + b, q, bB, bA, bC);
-      V o;
-      o.x = (ce * bB.x + cw * gA.x) + cn * nb.x;
-      o.y = (ce * bB.y + cw * gA.y) + cn * nb.y;
+      const Quad<T> nb = nbq<T>(BX + b, BY + b, q, bB, bA, bC);
+      const Quad<T> o = sweepq<T>(bB, nb, gA, ce, cw, cn);
       if (interior) {
-        stv2<T, V>(eo + (row + pl * (unsigned)(t - 2)), o);
-        if (DOT) dot += (double)gA.x * (double)(o.x * zs) + (double)gA.y * (double)(o.y * zs);
+        const unsigned oo = pl * (unsigned)(t - 2);
+        stv2<T, V>(eo + (row0 + oo), o.lo); stv2<T, V>(eo + (row1 + oo), o.hi);
+        if (DOT) dot += (double)(((gA.lo.x * o.lo.x + gA.lo.y * o.lo.y) + (gA.hi.x * o.hi.x + gA.hi.y * o.hi.y)) * zs);
       }
     }
-    A[b + q.own] = aC;
-    if (t >= z0) B[pb + q.own] = bC;
+    stq<T>(AX + b, AY + b, q, aC);
+    if (t >= z0) stq<T>(BX + pb, BY + pb, q, bC);
     __syncthreads();
     b = pb;
   };
-  V a0 = zero, a1 = zero, a2 = zero, b0 = zero, b1 = zero, b2 = zero, g0 = zero, g1 = zero;
+  Quad<T> a0, a1, a2, b0, b1, b2, g0, g1;
+  a0.lo.x = a0.lo.y = a0.hi.x = a0.hi.y = T(0);
+  a1 = a0; a2 = a0; b0 = a0; b1 = a0; b2 = a0; g0 = a0; g1 = a0;
   int t = z0 - 2;
   for (;;) {
     step(t, a0, a1, a2, b0, b1, b2, g0, g1); if (++t > tend) break;
@@ -202,23 +226,52 @@ k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __rest
   }
 }
 
+// Tile height: TR thread rows (2 TR cell rows).  fp64 patches need ~128 registers per thread.
+static int mg_tr() {
+  static int tr = 0;
+  if (!tr) { const char* e = getenv("FS_MG_TR"); tr = (e && atoi(e) == 16) ? 16 : 8; }
+  return tr;
+}
+template <class T, int TR> static int slots_per_sm() { return (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1); }
+template <class K> static void allow_smem(K kernel, size_t bytes) {
+  cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+template <class T, int TR> static void down_tr(const Ctx<T>& c, const T* g, T* e, T* gc, int nx, int ny, int nz, T cg, T cn, T ih2, cudaStream_t s) {
+  const MgGeom G = mg_geom(nx, ny, nz, MgTile<TR>::IY, slots_per_sm<T, TR>());
+  const size_t smem = 8 * (size_t)MgTile<TR>::PL * sizeof(T);
+  static bool once = false;
+  if (!once) { allow_smem(k_mg_down<T, TR>, smem); once = true; }
+  k_mg_down<T, TR><<<G.grid, dim3(32, TR), smem, s>>>(&c.S->done, g, e, gc, nx, ny, nz, cg, cn, ih2);
+}
+template <class T, int TR, bool DOT> static void up_tr(const Ctx<T>& c, const T* ein, const T* ec, const T* g, T* eo, int nx, int ny, int nz,
+                                                       T ce, T cw, T cn, T zs, cudaStream_t s) {
+  const MgGeom G = mg_geom(nx, ny, nz, MgTile<TR>::IY, slots_per_sm<T, TR>());
+  const size_t smem = 8 * (size_t)MgTile<TR>::PL * sizeof(T);
+  static bool once = false;
+  if (!once) { allow_smem(k_mg_up<T, TR, DOT>, smem); once = true; }
+  k_mg_up<T, TR, DOT><<<G.grid, dim3(32, TR), smem, s>>>(&c.S->done, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, c.S, c.partials);
+}
+
 template <class T> int launch_mg_down(const Ctx<T>& c, const T* g, T* e, T* gc, int nx, int ny, int nz, double h, double omega,
                                       const char* name, const Launch& L) {
-  const MgGeom G = mg_geom(nx, ny, nz);
   const double N = (double)nx * ny * nz;
   const double ih2 = 1.0 / (h * h), cw = omega * h * h / 6.0;
-  FS_LAUNCH(L, name, 2.125 * sizeof(T) * N,
-            k_mg_down<T><<<G.grid, dim3(32, kMgTY), 0, L.s>>>(&c.S->done, g, e, gc, nx, ny, nz, T(2.0 * cw - 6.0 * cw * cw * ih2), T(cw * cw * ih2), T(ih2)));
+  const T cg = T(2.0 * cw - 6.0 * cw * cw * ih2), cn = T(cw * cw * ih2);
+  if (mg_tr() == 16) FS_LAUNCH(L, name, 2.125 * sizeof(T) * N, down_tr<T, 16>(c, g, e, gc, nx, ny, nz, cg, cn, T(ih2), L.s));
+  else FS_LAUNCH(L, name, 2.125 * sizeof(T) * N, down_tr<T, 8>(c, g, e, gc, nx, ny, nz, cg, cn, T(ih2), L.s));
   return 1;
 }
 template <class T> int launch_mg_up(const Ctx<T>& c, const T* ein, const T* ec, const T* g, T* eo, int nx, int ny, int nz, double h,
                                     double omega, bool dot, T zs, const char* name, const Launch& L) {
-  const MgGeom G = mg_geom(nx, ny, nz);
   const double N = (double)nx * ny * nz;
   const double ih2d = 1.0 / (h * h), cwd = omega * h * h / 6.0;
   const T ce = T(1.0 - 6.0 * cwd * ih2d), cw = T(cwd), cn = T(cwd * ih2d);
-  if (dot) FS_LAUNCH(L, name, 3.125 * sizeof(T) * N, k_mg_up<T, true><<<G.grid, dim3(32, kMgTY), 0, L.s>>>(&c.S->done, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, c.S, c.partials));
-  else FS_LAUNCH(L, name, 3.125 * sizeof(T) * N, k_mg_up<T, false><<<G.grid, dim3(32, kMgTY), 0, L.s>>>(&c.S->done, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, c.S, c.partials));
+  const bool big = mg_tr() == 16;
+  FS_LAUNCH(L, name, 3.125 * sizeof(T) * N, {
+    if (big) { if (dot) up_tr<T, 16, true>(c, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 16, false>(c, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
+    else { if (dot) up_tr<T, 8, true>(c, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 8, false>(c, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
+  });
   return 1;
 }
 
