@@ -77,15 +77,15 @@ template <class T> __device__ __forceinline__ T boundary_normal(const Ctx<T>& c,
 // S1: H^n = -div(u u) + nu lap(u) + g (central / central, Eq. 4) and the explicit
 // predictor u~ = u^n + dt (a0 H^n + a1 H^{n-1}); prescribed boundary-normal faces get their O1 values.
 //
-// 2.5-D halo-tiled streaming kernel: a CTA owns a 30 x 10 column of cells of the extended box
-// (nxu x nyv x nzw) plus a one-cell halo (32 x 12 threads, one thread per extended-tile cell) and marches
+// 2.5-D halo-tiled streaming kernel: a CTA owns a 30 x 8 column of cells of the extended box
+// (nxu x nyv x nzw) plus a one-cell halo (32 x 10 threads, one thread per extended-tile cell) and marches
 // in z.  Every plane of u, v, w is read once per CTA through the boundary-aware accessor (S0 folded into
 // the tile load: wrap / ghost reflection are resolved when the value enters shared memory), kept in a
 // four-slot ring of shared-memory planes (planes k-1, k, k+1 are live, the fourth slot takes the prefetch
 // without a second barrier) and in a register queue for the thread's own column.  One __syncthreads per
 // plane; H^{n-1} is read and H^n, u~ are written straight from / to global memory, coalesced.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kMomTX = 32, kMomTY = 12;
+constexpr int kMomTX = 32, kMomTY = 10;
 
 template <class T> struct ColRef { unsigned off, pl; T A, B; };   // 32-bit element offsets: every field has < 2^32 entries (validated)   // value = A f[off + pl kz] + B  (x, y ghosts resolved)
 
@@ -108,16 +108,26 @@ template <class T, int C> __device__ __forceinline__ ColRef<T> col_setup(const C
   r.off = (unsigned)i + (unsigned)ex * (unsigned)j; r.pl = (unsigned)ex * (unsigned)ey; r.A = A; r.B = B;
   return r;
 }
-// plane kk in [-1, nzw] of component C for this thread's column
-template <class T, int C> __device__ __forceinline__ T col_load(const Ctx<T>& c, const T* __restrict__ f, const ColRef<T>& r, int kk) {
+// plane kk in [-1, nzw] of component C for this thread's column: the raw load and, separately, the ghost
+// fix-up (so that the load can stay in flight for a whole plane before its value is touched)
+template <class T, int C> __device__ __forceinline__ int col_plane(const Ctx<T>& c, int kk) {
+  if (!c.bz) return kk < 0 ? kk + c.nz : (kk >= c.nz ? kk - c.nz : kk);
+  if (C != 2) return kk < 0 ? -1 - kk : (kk >= c.nz ? 2 * c.nz - 1 - kk : kk);
+  return min(max(kk, 0), c.nz);
+}
+template <class T, int C> __device__ __forceinline__ T col_raw(const Ctx<T>& c, const T* __restrict__ f, const ColRef<T>& r, int kk) {
+  return f[r.off + r.pl * (unsigned)col_plane<T, C>(c, kk)];
+}
+template <class T, int C> __device__ __forceinline__ T col_fix(const Ctx<T>& c, const ColRef<T>& r, int kk, T raw) {
   T A = r.A, B = r.B;
-  if (!c.bz) kk = wrapi(kk, c.nz);
-  else if (C != 2) {
-    int face = -1;
-    if (kk < 0) { face = 4; kk = -1 - kk; } else if (kk >= c.nz) { face = 5; kk = 2 * c.nz - 1 - kk; }
+  if (c.bz && C != 2) {
+    const int face = kk < 0 ? 4 : (kk >= c.nz ? 5 : -1);
     if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
-  } else kk = min(max(kk, 0), c.nz);
-  return A * f[r.off + r.pl * (unsigned)kk] + B;
+  }
+  return A * raw + B;
+}
+template <class T, int C> __device__ __forceinline__ T col_load(const Ctx<T>& c, const T* __restrict__ f, const ColRef<T>& r, int kk) {
+  return col_fix<T, C>(c, r, kk, col_raw<T, C>(c, f, r, kk));
 }
 
 template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momentum(const Ctx<T> c, int kz) {
@@ -143,7 +153,7 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
   // register queue of the own column: B = k-1, c = k, T = k+1
   T uB = col_load<T, 0>(c, U, ru, k0 - 1), vB = col_load<T, 1>(c, V, rv, k0 - 1), wB = col_load<T, 2>(c, W, rw, k0 - 1);
   T uc = col_load<T, 0>(c, U, ru, k0), vc = col_load<T, 1>(c, V, rv, k0), wc = col_load<T, 2>(c, W, rw, k0);
-  T un = col_load<T, 0>(c, U, ru, k0 + 1), vn = col_load<T, 1>(c, V, rv, k0 + 1), wn = col_load<T, 2>(c, W, rw, k0 + 1);
+  T un = col_raw<T, 0>(c, U, ru, k0 + 1), vn = col_raw<T, 1>(c, V, rv, k0 + 1), wn = col_raw<T, 2>(c, W, rw, k0 + 1);   // raw, in flight
   SU[(k0 - 1) & 3][ty][tx] = uB; SV[(k0 - 1) & 3][ty][tx] = vB; SW[(k0 - 1) & 3][ty][tx] = wB;
   SU[k0 & 3][ty][tx] = uc; SV[k0 & 3][ty][tx] = vc; SW[k0 & 3][ty][tx] = wc;
   const int txm = max(tx - 1, 0), txp = min(tx + 1, kMomTX - 1), tym = max(ty - 1, 0), typ = min(ty + 1, kMomTY - 1);
@@ -156,7 +166,7 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
   T hvn = (hasv && k0 < c.nz) ? c.hv[qv0 + plv * k0] : T(0);
   T hwn = hasw ? c.hw[qw0 + plw * k0] : T(0);
   for (int k = k0; k < k1; ++k) {
-    const T uT = un, vT = vn, wT = wn;
+    const T uT = col_fix<T, 0>(c, ru, k + 1, un), vT = col_fix<T, 1>(c, rv, k + 1, vn), wT = col_fix<T, 2>(c, rw, k + 1, wn);
     const T huo = hun, hvo = hvn, hwo = hwn;
     if (k + 1 < k1) {
       hun = (hasu && k + 1 < c.nz) ? c.hu[qu0 + plu * (k + 1)] : T(0);
@@ -165,7 +175,7 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
     }
     const int s0 = (k - 1) & 3, s1 = k & 3, s2 = (k + 1) & 3;
     SU[s2][ty][tx] = uT; SV[s2][ty][tx] = vT; SW[s2][ty][tx] = wT;
-    if (k + 1 < k1) { un = col_load<T, 0>(c, U, ru, k + 2); vn = col_load<T, 1>(c, V, rv, k + 2); wn = col_load<T, 2>(c, W, rw, k + 2); }
+    if (k + 1 < k1) { un = col_raw<T, 0>(c, U, ru, k + 2); vn = col_raw<T, 1>(c, V, rv, k + 2); wn = col_raw<T, 2>(c, W, rw, k + 2); }
     __syncthreads();
     if (own) {
       const T wyl0 = MY[0][ty], wyh0 = MY[1][ty], wyl1 = MY[2][ty], wyh1 = MY[3][ty];
@@ -257,9 +267,9 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
 
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
   const int bxn = (c.nxu + kMomTX - 3) / (kMomTX - 2), byn = (c.nyv + kMomTY - 3) / (kMomTY - 2);
-  // z chunks: >= 4 waves of CTAs (5 CTAs of 384 threads per SM) while chunks stay >= 16 planes
+  // z chunks: >= 4 waves of CTAs (2 CTAs of 320 threads per SM) while chunks stay >= 16 planes
   int kz = c.nzw;
-  while (kz > 16 && (long long)bxn * byn * ((c.nzw + kz - 1) / kz) < 4LL * 148 * 5) kz = (kz + 1) / 2;
+  while (kz > 16 && (long long)bxn * byn * ((c.nzw + kz - 1) / kz) < 4LL * 148 * 2) kz = (kz + 1) / 2;
   dim3 b(kMomTX, kMomTY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
   FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T><<<g, b, 0, L.s>>>(c, kz));
   return 1;

@@ -67,6 +67,95 @@ template <class T> __global__ void __launch_bounds__(256) k_mg_prolong(const int
   }
 }
 
+// ---- tail of the V-cycle in ONE CTA ------------------------------------------------------------------
+// Levels of at most kTailCells cells (16^3) and everything below them fit in shared memory together: one
+// launch runs their downward legs, the coarsest-level sweeps and their upward legs, instead of ~20 launches
+// that each do microseconds of work.  Same operations, in the same order, as the per-level kernels above.
+constexpr int kTailCells = 4096;
+struct MgTail { int nlev; int nx[kMaxLevels], ny[kMaxLevels], nz[kMaxLevels]; double h[kMaxLevels]; };
+
+template <class T> __device__ __forceinline__ T tail_neg_lap(const T* e, int q, int nx, int ny, int nz, T ih2) {
+  const int i = q % nx, t = q / nx, j = t % ny, k = t / ny;
+  const int ip = i + 1 == nx ? 0 : i + 1, im = i == 0 ? nx - 1 : i - 1;
+  const int jp = j + 1 == ny ? 0 : j + 1, jm = j == 0 ? ny - 1 : j - 1;
+  const int kp = k + 1 == nz ? 0 : k + 1, km = k == 0 ? nz - 1 : k - 1;
+  const int row = nx * (j + ny * k);
+  const T nb = e[row + ip] + e[row + im] + e[i + nx * (jp + ny * k)] + e[i + nx * (jm + ny * k)] + e[i + nx * (j + ny * kp)] + e[i + nx * (j + ny * km)];
+  return (T(6) * e[q] - nb) * ih2;
+}
+
+template <class T> __global__ void __launch_bounds__(1024) k_mg_tail(const int* __restrict__ done, const T* __restrict__ g_in, T* __restrict__ e_out,
+                                                                      MgTail a, int nu1, int nu2, int ncoarse, double omega) {
+  if (done && *done) return;
+  extern __shared__ __align__(16) unsigned char tail_smem[];
+  T* base = reinterpret_cast<T*>(tail_smem);
+  T* G[kMaxLevels]; T* E[kMaxLevels]; T* Tm[kMaxLevels]; T* cur[kMaxLevels];
+  int N[kMaxLevels];
+  {
+    T* p = base;
+    for (int l = 0; l < a.nlev; ++l) { N[l] = a.nx[l] * a.ny[l] * a.nz[l]; G[l] = p; p += N[l]; E[l] = p; p += N[l]; Tm[l] = p; p += N[l]; }
+  }
+  const int tid = threadIdx.x, nth = blockDim.x;
+  for (int q = tid; q < N[0]; q += nth) G[0][q] = g_in[q];
+  __syncthreads();
+  const int last = a.nlev - 1;
+  // sweeps from a zero guess: returns the buffer that holds the iterate (nullptr = still zero)
+  auto smooth0 = [&](int l, int n) -> T* {
+    if (n <= 0) return nullptr;
+    const T ih2 = T(1.0 / (a.h[l] * a.h[l])), cw = T(omega * a.h[l] * a.h[l] / 6.0);
+    T* x = E[l]; T* y = Tm[l];
+    for (int q = tid; q < N[l]; q += nth) x[q] = cw * G[l][q];
+    __syncthreads();
+    for (int it = 1; it < n; ++it) {
+      for (int q = tid; q < N[l]; q += nth) y[q] = x[q] + cw * (G[l][q] - tail_neg_lap<T>(x, q, a.nx[l], a.ny[l], a.nz[l], ih2));
+      __syncthreads();
+      T* t = x; x = y; y = t;
+    }
+    return x;
+  };
+  auto smooth = [&](int l, T* x, int n) -> T* {
+    const T ih2 = T(1.0 / (a.h[l] * a.h[l])), cw = T(omega * a.h[l] * a.h[l] / 6.0);
+    T* y = x == E[l] ? Tm[l] : E[l];
+    for (int it = 0; it < n; ++it) {
+      for (int q = tid; q < N[l]; q += nth) y[q] = x[q] + cw * (G[l][q] - tail_neg_lap<T>(x, q, a.nx[l], a.ny[l], a.nz[l], ih2));
+      __syncthreads();
+      T* t = x; x = y; y = t;
+    }
+    return x;
+  };
+  for (int l = 0; l < last; ++l) {        // downward legs
+    cur[l] = smooth0(l, nu1);
+    const int nx = a.nx[l], ny = a.ny[l], nz = a.nz[l], cx = nx / 2, cy = ny / 2;
+    const T ih2 = T(1.0 / (a.h[l] * a.h[l]));
+    for (int q = tid; q < N[l + 1]; q += nth) {
+      const int i = q % cx, t = q / cx, j = t % cy, k = t / cy;
+      T s = T(0);
+      for (int dk = 0; dk < 2; ++dk) for (int dj = 0; dj < 2; ++dj) for (int di = 0; di < 2; ++di) {
+        const int fq = (2 * i + di) + nx * ((2 * j + dj) + ny * (2 * k + dk));
+        s += cur[l] ? G[l][fq] - tail_neg_lap<T>(cur[l], fq, nx, ny, nz, ih2) : G[l][fq];
+      }
+      G[l + 1][q] = T(0.125) * s;
+    }
+    __syncthreads();
+  }
+  cur[last] = smooth0(last, ncoarse);
+  if (!cur[last]) { for (int q = tid; q < N[last]; q += nth) E[last][q] = T(0); __syncthreads(); cur[last] = E[last]; }
+  for (int l = last - 1; l >= 0; --l) {   // upward legs
+    const int nx = a.nx[l], ny = a.ny[l], cx = nx / 2, cy = ny / 2;
+    T* x = cur[l] ? cur[l] : E[l];
+    const T* ec = cur[l + 1];
+    const bool add = cur[l] != nullptr;
+    for (int q = tid; q < N[l]; q += nth) {
+      const int i = q % nx, t = q / nx, j = t % ny, k = t / ny;
+      const T cv = ec[(i >> 1) + cx * ((j >> 1) + cy * (k >> 1))];
+      x[q] = add ? x[q] + cv : cv;
+    }
+    __syncthreads();
+    cur[l] = smooth(l, x, nu2);
+  }
+  for (int q = tid; q < N[0]; q += nth) e_out[q] = cur[0][q];
+}
+
 // Recursion unrolled on the host: emits the kernels of one V-cycle for rhs -> out (out = V(rhs)).
 template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs) {
   int n = 0;
@@ -82,11 +171,29 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
   // Fast path, V(2,2) with at least two levels: two fused kernels per level (fs_kernels_mgf.cu).
   if (mg.nu1 == 2 && mg.nu2 == 2 && mg.nlev >= 2) {
     const int last = mg.nlev - 1;
-    for (int l = 0; l < last; ++l) {
+    // tail levels (small enough to live in one CTA's shared memory together): from level lt down
+    int lt = last;
+    while (lt > 1 && (long long)mg.lev[lt - 1].nx * mg.lev[lt - 1].ny * mg.lev[lt - 1].nz <= kTailCells) --lt;
+    const bool tail_ok = (long long)mg.lev[lt].nx * mg.lev[lt].ny * mg.lev[lt].nz <= kTailCells;
+    if (!tail_ok) lt = mg.nlev;          // no tail: the coarsest level is too big (cannot happen with >= 4-cell coarse boxes, kept for safety)
+    const int top = tail_ok ? lt : last; // levels 0..top-1 run the fused per-level kernels
+    for (int l = 0; l < top; ++l) {
       const MgLevel& V = mg.lev[l];
       n += launch_mg_down<T>(c, gl[l], tl[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, V.h, mg.omega, l == 0 ? "mg_down_l0" : "mg_coarse", L);
     }
-    {
+    if (tail_ok) {
+      MgTail a; a.nlev = mg.nlev - lt;
+      size_t cells = 0;
+      for (int l = lt; l < mg.nlev; ++l) {
+        a.nx[l - lt] = mg.lev[l].nx; a.ny[l - lt] = mg.lev[l].ny; a.nz[l - lt] = mg.lev[l].nz; a.h[l - lt] = mg.lev[l].h;
+        cells += (size_t)mg.lev[l].nx * mg.lev[l].ny * mg.lev[l].nz;
+      }
+      const size_t smem = 3 * cells * sizeof(T);
+      static bool once = false;
+      if (!once) { cudaFuncSetAttribute(k_mg_tail<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * (kTailCells + kTailCells / 7 + 8) * sizeof(T))); once = true; }
+      FS_LAUNCH(L, "mg_coarse", 2.0 * sizeof(T) * mg.lev[lt].nx * mg.lev[lt].ny * mg.lev[lt].nz,
+                k_mg_tail<T><<<1, 1024, smem, L.s>>>(done, gl[lt], el[lt], a, mg.nu1, mg.nu2, mg.coarse_sweeps, mg.omega)); ++n;
+    } else {
       const MgLevel& V = mg.lev[last];
       const long long N = (long long)V.nx * V.ny * V.nz;
       const T ih2 = T(1.0 / (V.h * V.h)), cw = T(mg.omega * V.h * V.h / 6.0);
@@ -102,7 +209,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
         }
       }
     }
-    for (int l = last - 1; l >= 0; --l) {
+    for (int l = top - 1; l >= 0; --l) {
       const MgLevel& V = mg.lev[l];
       const bool dot = want_dot && l == 0;
       n += launch_mg_up<T>(c, tl[l], el[l + 1], gl[l], el[l], V.nx, V.ny, V.nz, V.h, mg.omega, dot, zs, l == 0 ? "mg_up_l0" : "mg_coarse", L);
