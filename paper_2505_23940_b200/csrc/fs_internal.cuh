@@ -24,7 +24,9 @@ struct Scalars {
   double rmean;         // fp32 only: mean of the recurrence residual, removed with one iteration of lag (null-space deflation)
   double sum_dy;         // sum over all cells of dy_j
   int iter, done, converged, first;
-  int dsel, pad2;        // which of the two direction buffers holds the current d (k_pcg_dirapply)
+  int dsel, pending;     // pending: the x += alpha_prev d of the last k_pcg_update has not been applied yet
+  double alpha_prev, sum_p, sum_d;   // deferred x update (k_pcg_dirapply / k_pflush)
+  int pad2_unused, pad3_unused; //       // which of the two direction buffers holds the current d (k_pcg_dirapply)
   int max_iter, pad0;
   double rtol;
   // step control

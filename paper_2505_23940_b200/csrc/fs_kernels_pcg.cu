@@ -72,7 +72,7 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_init(const Ctx<T
     if (threadIdx.x == 0 && threadIdx.y == 0) {
       Scalars* S = c.S;
       S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
-      S->iter = 0; S->first = 1; S->dsel = 0;
+      S->iter = 0; S->first = 1; S->dsel = 0; S->pending = 0;
       S->rmean = v[3] / ((double)c.nx * c.ny * c.nz);
       const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
       S->converged = conv; S->done = conv || S->max_iter <= 0;
@@ -93,7 +93,7 @@ constexpr int kDaTX = 32, kDaTY = 16;
 
 template <class T, int PC> __global__ void __launch_bounds__(kDaTX * kDaTY, 2) k_pcg_dirapply(const Ctx<T> c, T zs, int kz) {
   __shared__ T D[2][kDaTY][kDaTX];
-  __shared__ double sh[32]; __shared__ int flag;
+  __shared__ double sh[3 * 32]; __shared__ int flag;
   const Scalars* S = c.S;
   if (S->done) return;
   const bool first = S->first != 0;
@@ -114,16 +114,30 @@ template <class T, int PC> __global__ void __launch_bounds__(kDaTX * kDaTY, 2) k
   const T dxy = T((c.bx && i == 0 ? 0 : 1) + (c.bx && i == c.nx - 1 ? 0 : 1)) * c.ihx2;
   const T dyy = (cyh + cyl) * idy;
   auto plane_src = [&](int k) { return c.bz ? min(max(k, 0), c.nz - 1) : wrapi(k, c.nz); };
+  // Deferred x update (the x += alpha d of the PREVIOUS iteration rides on this kernel's read of the old d):
+  // applied to the own cells when their d' is formed; sums of x and d' (volume weighted) for the final mean.
+  const bool pend = S->pending != 0;
+  const T alpha_p = pend ? T(S->alpha_prev) : T(0);
+  double sp = 0.0, sd = 0.0;
   auto dir_at = [&](int k) {              // d' at (i, j, plane_src(k))
     const int ks = plane_src(k);
     const size_t o = oc + pl * ks;
+    const bool upd = own && k >= k0 && k < k1;
+    T pv = T(0);
+    if (upd) pv = c.p[o];
     T z;
     if (PC == 2) z = zsrc[o] * zs;
     else if (PC == 1) {
       const T dzz = T((c.bz && ks == 0 ? 0 : 1) + (c.bz && ks == c.nz - 1 ? 0 : 1)) * c.ihz2;
       z = zsrc[o] / ((dxy + dyy + dzz) * c.dy[j + 1]);
     } else z = zsrc[o];
-    return first ? z : z + beta * dold[o];
+    const T dol = first ? T(0) : dold[o];
+    const T dn = first ? z : z + beta * dol;
+    if (upd) {
+      if (pend) { pv += alpha_p * dol; c.p[o] = pv; }
+      sp += (double)pv; sd += (double)dn;
+    }
+    return dn;
   };
   const int txm = max(tx - 1, 0), txp = min(tx + 1, kDaTX - 1), tym = max(ty - 1, 0), typ = min(ty + 1, kDaTY - 1);
   T dB = dir_at(k0 - 1), dC = dir_at(k0), dT = dir_at(k0 + 1);
@@ -149,8 +163,10 @@ template <class T, int PC> __global__ void __launch_bounds__(kDaTX * kDaTY, 2) k
     __syncthreads();
     dB = dC; dC = dT; dT = dN;
   }
-  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
-    if (tx == 0 && ty == 0) c.S->dq = v[0];
+  const double wy = c.dy64[j];
+  double v3[3] = {v[0], sp * wy, sd * wy};
+  if (grid_sum<3>(v3, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (tx == 0 && ty == 0) { c.S->dq = v3[0]; c.S->sum_p = v3[1]; c.S->sum_d = v3[2]; }
   }
 }
 
@@ -172,7 +188,7 @@ constexpr int kDa2IX = 60, kDa2IY = kDaTY - 2, kDa2PL = kDaTY * 32;
 template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pcg_dirapply2(const Ctx<T> c, T zs, int kz) {
   using V = typename V2T<T>::type;
   __shared__ V D[2 * kDa2PL];
-  __shared__ double sh[32]; __shared__ int flag;
+  __shared__ double sh[3 * 32]; __shared__ int flag;
   const Scalars* S = c.S;
   if (S->done) return;
   const bool first = S->first != 0;
@@ -199,13 +215,19 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
   const int own_o = ty * 32 + lane;
   const int oS = (ty > 0 ? ty - 1 : 0) * 32 + lane, oN = (ty < kDaTY - 1 ? ty + 1 : ty) * 32 + lane;
   const int oW = ty * 32 + (lane > 0 ? lane - 1 : 0), oE = ty * 32 + (lane < 31 ? lane + 1 : 31);
-  V rz, rd;                                 // raw z and old d of the plane in flight
-  int ksrc = 0;
+  // Deferred x update: see k_pcg_dirapply.
+  const bool pend = S->pending != 0;
+  const T alpha_p = pend ? T(S->alpha_prev) : T(0);
+  double sp = 0.0, sd = 0.0;
+  V rz, rd, rp;                             // raw z, old d and x of the plane in flight
+  int ksrc = 0; bool upd = false;
   auto fetch = [&](int k) {
     ksrc = c.bz ? min(max(k, 0), c.nz - 1) : (k < 0 ? k + c.nz : (k >= c.nz ? k - c.nz : k));
     const unsigned o = row + pl * (unsigned)ksrc;
     rz = ldv2<T, V>(zsrc + o);
     if (!first) rd = ldv2<T, V>(dold + o);
+    upd = own && k >= k0 && k < k1;
+    if (upd) rp = ldv2<T, V>(c.p + o);
   };
   auto make = [&]() {                       // d' of the fetched plane
     V z;
@@ -216,11 +238,15 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
     } else z = rz;
     V d = z;
     if (!first) { d.x = z.x + beta * rd.x; d.y = z.y + beta * rd.y; }
+    if (upd) {                              // own cells: never a clamped halo pair
+      if (pend) { rp.x += alpha_p * rd.x; rp.y += alpha_p * rd.y; stv2<T, V>(c.p + (row + pl * (unsigned)ksrc), rp); }
+      sp += (double)(rp.x + rp.y); sd += (double)(d.x + d.y);
+    }
     if (fixl) d.y = d.x;
     if (fixr) d.x = d.y;
     return d;
   };
-  rd.x = rd.y = T(0);
+  rd.x = rd.y = T(0); rp = rd;
   V d0, d1, d2;
   fetch(k0 - 1); d0 = make();
   fetch(k0); d1 = make();
@@ -258,14 +284,168 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
     step(k, d1, d2, d0); if (++k >= k1) break;
     step(k, d2, d0, d1); if (++k >= k1) break;
   }
-  double v[1] = {dot};
-  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
-    if (lane == 0 && ty == 0) c.S->dq = v[0];
+  const double wy = c.dy64[sy];
+  double v[3] = {dot, sp * wy, sd * wy};
+  if (grid_sum<3>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (lane == 0 && ty == 0) { c.S->dq = v[0]; c.S->sum_p = v[1]; c.S->sum_d = v[2]; }
   }
 }
 
 static DaGeom da2_geom(int nx, int ny, int nz) {
   const int bxn = (nx + kDa2IX - 1) / kDa2IX, byn = (ny + kDa2IY - 1) / kDa2IY;
+  int kz = nz;
+  while (kz > 16 && (long long)bxn * byn * ((nz + kz - 1) / kz) < 4LL * 296) kz = (kz + 1) / 2;
+  DaGeom g; g.kz = kz; g.grid = dim3(bxn, byn, (nz + kz - 1) / kz);
+  return g;
+}
+
+// Same operation, one 16-byte vector of x-adjacent cells per thread (fp32: VX = 4 cells; in fp64 the pair
+// kernel above is the faster of the two and is the one used; nx a
+// multiple of VX): vector global accesses, the index arithmetic shared by VX cells, a 32 VX x 16 extended
+// tile -> 30 VX x 14 results (lanes 0 and 31 are halo), z loop unrolled by renaming.
+template <class T> struct Vec16 {
+  static constexpr int VX = 16 / sizeof(T);
+  T a[VX];
+};
+template <class T> __device__ __forceinline__ Vec16<T> ld16(const T* p) {
+  Vec16<T> v; *reinterpret_cast<typename V16T<T>::type*>(v.a) = *reinterpret_cast<const typename V16T<T>::type*>(p); return v;
+}
+template <class T> __device__ __forceinline__ void st16(T* p, const Vec16<T>& v) {
+  *reinterpret_cast<typename V16T<T>::type*>(p) = *reinterpret_cast<const typename V16T<T>::type*>(v.a);
+}
+constexpr int kDaVIY = kDaTY - 2;
+
+template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pcg_dirapplyv(const Ctx<T> c, T zs, int kz) {
+  constexpr int VX = Vec16<T>::VX;
+  constexpr int ROWE = 32 * VX;             // cells per shared-memory row
+  constexpr int PLN = kDaTY * ROWE;
+  using W = Vec16<T>;
+  __shared__ __align__(16) T D[2 * PLN];
+  __shared__ double sh[3 * 32]; __shared__ int flag;
+  const Scalars* S = c.S;
+  if (S->done) return;
+  const bool first = S->first != 0;
+  const T beta = first ? T(0) : T(S->rho_cur / S->rho_prev);
+  const T* __restrict__ dold = S->dsel ? c.d2 : c.d;
+  T* __restrict__ dnew = S->dsel ? c.d : c.d2;
+  const T* __restrict__ zsrc = PC == 2 ? c.z : c.r;
+  const int lane = threadIdx.x, ty = threadIdx.y;
+  const int gx = (blockIdx.x * 30 - 1 + lane) * VX, gy = blockIdx.y * kDaVIY - 1 + ty;
+  const int sx = c.bx ? min(max(gx, 0), c.nx - VX) : wrapi(gx, c.nx);
+  const int sy = c.by ? min(max(gy, 0), c.ny - 1) : wrapi(gy, c.ny);
+  const bool fixl = c.bx && gx < 0, fixr = c.bx && gx >= c.nx;       // clamped halo vectors: every cell = the boundary cell
+  const bool own = lane >= 1 && lane <= 30 && ty >= 1 && ty <= kDaTY - 2 && gx < c.nx && gy < c.ny;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  const unsigned pl = (unsigned)c.nx * c.ny, row = (unsigned)sx + (unsigned)c.nx * sy;
+  const T cyl = c.cyl[sy], cyh = c.cyh[sy], idy = c.idy[sy + 1], dyj = c.dy[sy + 1], ndy = -dyj;
+  const T ihx2 = c.ihx2, ihz2 = c.ihz2;
+  T dg[VX];                                 // Jacobi: x + y parts of diag A / dy per cell
+#pragma unroll
+  for (int a = 0; a < VX; ++a) {
+    const int i = sx + a;
+    dg[a] = PC == 1 ? T((c.bx && i == 0 ? 0 : 1) + (c.bx && i == c.nx - 1 ? 0 : 1)) * ihx2 + (cyh + cyl) * idy : T(0);
+  }
+  const int o_own = ty * ROWE + lane * VX;
+  const int o_s = (ty > 0 ? ty - 1 : 0) * ROWE + lane * VX, o_n = (ty < kDaTY - 1 ? ty + 1 : ty) * ROWE + lane * VX;
+  const int o_w = ty * ROWE + (lane > 0 ? lane * VX - 1 : 0), o_e = ty * ROWE + (lane < 31 ? lane * VX + VX : 32 * VX - 1);
+  // Deferred x update: see k_pcg_dirapply.
+  const bool pend = S->pending != 0;
+  const T alpha_p = pend ? T(S->alpha_prev) : T(0);
+  double sp = 0.0, sd = 0.0;
+  W rz, rd, rp;                             // raw z, old d and x of the plane in flight
+#pragma unroll
+  for (int a = 0; a < VX; ++a) { rd.a[a] = T(0); rp.a[a] = T(0); }
+  int ksrc = 0; bool upd = false;
+  auto fetch = [&](int k) {
+    ksrc = c.bz ? min(max(k, 0), c.nz - 1) : (k < 0 ? k + c.nz : (k >= c.nz ? k - c.nz : k));
+    const unsigned o = row + pl * (unsigned)ksrc;
+    rz = ld16<T>(zsrc + o);
+    if (!first) rd = ld16<T>(dold + o);
+    upd = own && k >= k0 && k < k1;
+    if (upd) rp = ld16<T>(c.p + o);
+  };
+  auto make = [&]() {                       // d' of the fetched plane
+    W d;
+    T dzz = T(0);
+    if (PC == 1) dzz = T((c.bz && ksrc == 0 ? 0 : 1) + (c.bz && ksrc == c.nz - 1 ? 0 : 1)) * ihz2;
+#pragma unroll
+    for (int a = 0; a < VX; ++a) {
+      T z;
+      if (PC == 2) z = rz.a[a] * zs;
+      else if (PC == 1) z = rz.a[a] / ((dg[a] + dzz) * dyj);
+      else z = rz.a[a];
+      d.a[a] = first ? z : z + beta * rd.a[a];
+    }
+    if (upd) {                              // own cells: never a clamped halo vector
+      T s1 = T(0), s2 = T(0);
+#pragma unroll
+      for (int a = 0; a < VX; ++a) { if (pend) rp.a[a] += alpha_p * rd.a[a]; s1 += rp.a[a]; s2 += d.a[a]; }
+      if (pend) st16<T>(c.p + (row + pl * (unsigned)ksrc), rp);
+      sp += (double)s1; sd += (double)s2;
+    }
+    if (fixl) {
+#pragma unroll
+      for (int a = 1; a < VX; ++a) d.a[a] = d.a[0];
+    }
+    if (fixr) {
+#pragma unroll
+      for (int a = 0; a < VX - 1; ++a) d.a[a] = d.a[VX - 1];
+    }
+    return d;
+  };
+  W d0, d1, d2;
+  fetch(k0 - 1); d0 = make();
+  fetch(k0); d1 = make();
+  int b = 0;
+  st16<T>(D + o_own, d1);
+  fetch(k0 + 1);
+  __syncthreads();
+  double dot = 0.0;
+  // dB, dC = d'(k-1), d'(k); dT receives d'(k+1)
+  auto step = [&](int k, const W& dB, const W& dC, W& dT) {
+    dT = make();
+    if (k + 1 < k1) fetch(k + 2);
+    const T* P = D + b;
+    const W Sv = ld16<T>(P + o_s), Nv = ld16<T>(P + o_n);
+    const T xw0 = P[o_w], xeL = P[o_e];
+    W q;
+    T sdot = T(0);
+#pragma unroll
+    for (int a = 0; a < VX; ++a) {
+      const T xc = dC.a[a];
+      const T xw = a > 0 ? dC.a[a > 0 ? a - 1 : 0] : xw0;
+      const T xe = a < VX - 1 ? dC.a[a < VX - 1 ? a + 1 : a] : xeL;
+      T acc = (xe - xc) * ihx2 - (xc - xw) * ihx2;
+      acc += ((Nv.a[a] - xc) * cyh - (xc - Sv.a[a]) * cyl) * idy;
+      acc += (dT.a[a] - xc) * ihz2 - (xc - dB.a[a]) * ihz2;
+      q.a[a] = acc * ndy;
+      sdot += xc * q.a[a];
+    }
+    if (own) {
+      const unsigned o = row + pl * (unsigned)k;
+      st16<T>(dnew + o, dC); st16<T>(c.q + o, q);
+      dot += (double)sdot;
+    }
+    b = PLN - b;
+    st16<T>(D + b + o_own, dT);
+    __syncthreads();
+  };
+  int k = k0;
+  for (;;) {
+    step(k, d0, d1, d2); if (++k >= k1) break;
+    step(k, d1, d2, d0); if (++k >= k1) break;
+    step(k, d2, d0, d1); if (++k >= k1) break;
+  }
+  const double wy = c.dy64[sy];
+  double v[3] = {dot, sp * wy, sd * wy};
+  if (grid_sum<3>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (lane == 0 && ty == 0) { c.S->dq = v[0]; c.S->sum_p = v[1]; c.S->sum_d = v[2]; }
+  }
+}
+
+template <class T> static DaGeom dav_geom(int nx, int ny, int nz) {
+  const int ix = 30 * Vec16<T>::VX;
+  const int bxn = (nx + ix - 1) / ix, byn = (ny + kDaVIY - 1) / kDaVIY;
   int kz = nz;
   while (kz > 16 && (long long)bxn * byn * ((nz + kz - 1) / kz) < 4LL * 296) kz = (kz + 1) / 2;
   DaGeom g; g.kz = kz; g.grid = dim3(bxn, byn, (nz + kz - 1) / kz);
@@ -281,35 +461,33 @@ template <class T, bool GMG> __global__ void __launch_bounds__(256) k_pcg_update
   __shared__ double sh[3 * 32]; __shared__ int flag;
   Scalars* S = c.S;
   if (S->done) return;
-  const T alpha = T(S->rho_cur / S->dq);
+  const double alpha_d = S->rho_cur / S->dq;
+  const T alpha = T(alpha_d);
   const long long N = (long long)c.nx * c.ny * c.nz;
   const T rm = sizeof(T) == 4 ? T(S->rmean) : T(0);
-  const T* __restrict__ dcur = S->dsel ? c.d : c.d2;     // written by k_pcg_dirapply of this iteration
   double v[3] = {0.0, 0.0, 0.0};
   if (GMG) {
     // 16-byte accesses; per-vector partial sums in T, accumulated in fp64 (fp32: one conversion per 4 cells)
     constexpr int VW = 16 / sizeof(T);
     using V = typename V16T<T>::type;
     const long long NV = N / VW;
-    const V* __restrict__ dv = reinterpret_cast<const V*>(dcur); const V* __restrict__ qv = reinterpret_cast<const V*>(c.q);
-    V* __restrict__ pv = reinterpret_cast<V*>(c.p); V* __restrict__ rv = reinterpret_cast<V*>(c.r);
+    const V* __restrict__ qv = reinterpret_cast<const V*>(c.q);
+    V* __restrict__ rv = reinterpret_cast<V*>(c.r);
     for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < NV; q += (long long)gridDim.x * blockDim.x) {
-      V p = pv[q], r = rv[q]; const V d = dv[q], qq = qv[q];
-      T* pe = reinterpret_cast<T*>(&p); T* re = reinterpret_cast<T*>(&r);
-      const T* de = reinterpret_cast<const T*>(&d); const T* qe = reinterpret_cast<const T*>(&qq);
+      V r = rv[q]; const V qq = qv[q];
+      T* re = reinterpret_cast<T*>(&r);
+      const T* qe = reinterpret_cast<const T*>(&qq);
       T s2 = T(0), s1 = T(0);
 #pragma unroll
       for (int a = 0; a < VW; ++a) {
-        pe[a] += alpha * de[a];
         T t = re[a] - alpha * qe[a];
         if (sizeof(T) == 4) t -= rm;
         re[a] = t; s2 += t * t; s1 += t;
       }
-      pv[q] = p; rv[q] = r;
+      rv[q] = r;
       v[0] += (double)s2; v[2] += (double)s1;
     }
     for (long long q = NV * VW + blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
-      c.p[q] += alpha * dcur[q];
       T r = c.r[q] - alpha * c.q[q];
       if (sizeof(T) == 4) r -= rm;
       c.r[q] = r;
@@ -317,7 +495,6 @@ template <class T, bool GMG> __global__ void __launch_bounds__(256) k_pcg_update
     }
   } else {
     for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
-      c.p[q] += alpha * dcur[q];
       T r = c.r[q] - alpha * c.q[q];
       if (sizeof(T) == 4) r -= rm;
       c.r[q] = r;
@@ -330,6 +507,7 @@ template <class T, bool GMG> __global__ void __launch_bounds__(256) k_pcg_update
     if (threadIdx.x == 0) {
       S->rr = v[0]; S->rmean = v[2] / (double)N;
       S->iter += 1; S->first = 0; S->dsel ^= 1;
+      S->alpha_prev = alpha_d; S->pending = 1;       // x += alpha d is applied by the next k_pcg_dirapply or by k_pflush
       S->rho_prev = S->rho_cur;
       if (!GMG) S->rho_cur = v[1];
       const int conv = sqrt(v[0]) <= S->rtol * sqrt(S->bnorm2);
@@ -371,30 +549,63 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
     n += launch_vcycle<T>(c, mg, c.r, c.z, L, &fused, zs);
     if (!fused) { FS_LAUNCH(L, "pcg_dot_rz", 2.0 * sizeof(T) * N, k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n; }
   }
-  if (c.nx % 2 == 0) {
+  if (sizeof(T) == 8 && c.nx % 2 == 0) {
     const DaGeom G = da2_geom(c.nx, c.ny, c.nz);
     const dim3 blk(32, kDaTY);
-    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply2<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply2<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply2<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    ++n;
+  } else if (sizeof(T) == 4 && c.nx % 4 == 0) {
+    const DaGeom G = dav_geom<T>(c.nx, c.ny, c.nz);
+    const dim3 blk(32, kDaTY);
+    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
     ++n;
   } else {
     const DaGeom G = da_geom(c.nx, c.ny, c.nz);
     const dim3 blk(kDaTX, kDaTY);
-    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else FS_LAUNCH(L, "pcg_dir_apply_dot", 4.0 * sizeof(T) * N, k_pcg_dirapply<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
     ++n;
   }
-  if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_update_norm", 6.0 * sizeof(T) * N, k_pcg_update<T, true><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
-  else FS_LAUNCH(L, "pcg_update_norm", 6.0 * sizeof(T) * N, k_pcg_update<T, false><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
+  if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_update_norm", 3.0 * sizeof(T) * N, k_pcg_update<T, true><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
+  else FS_LAUNCH(L, "pcg_update_norm", 3.0 * sizeof(T) * N, k_pcg_update<T, false><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
   ++n;
   return n;
 }
 
-// ---- after the loop: zero-mean pressure (volume-weighted), SURVEY O6 ---------------------------------
+// ---- after the loop: last deferred x update and zero-mean pressure (volume-weighted), SURVEY O6 -------
+// With at least one iteration the mean of the final x follows from the sums k_pcg_dirapply left behind
+// (sum x dV before the last update, sum d dV), so one pass does x += alpha d - mean.  With no iteration
+// (converged at the start) the plain mean + shift kernels run instead; each kernel checks which case holds.
+template <class T> __global__ void __launch_bounds__(256) k_pflush(const Ctx<T> c) {
+  const Scalars* S = c.S;
+  if (!S->pending) return;
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  const double al = S->alpha_prev;
+  const T alpha = T(al), m = T((S->sum_p + al * S->sum_d) / S->sum_dy);
+  const T* __restrict__ dcur = S->dsel ? c.d2 : c.d;     // the direction of the last iteration
+  constexpr int VW = 16 / sizeof(T);
+  using V = typename V16T<T>::type;
+  const long long NV = N / VW;
+  const V* __restrict__ dv = reinterpret_cast<const V*>(dcur);
+  V* __restrict__ pv = reinterpret_cast<V*>(c.p);
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < NV; q += (long long)gridDim.x * blockDim.x) {
+    V p = pv[q]; const V d = dv[q];
+    T* pe = reinterpret_cast<T*>(&p); const T* de = reinterpret_cast<const T*>(&d);
+#pragma unroll
+    for (int a = 0; a < VW; ++a) pe[a] = (pe[a] + alpha * de[a]) - m;
+    pv[q] = p;
+  }
+  for (long long q = NV * VW + blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x)
+    c.p[q] = (c.p[q] + alpha * dcur[q]) - m;
+}
 template <class T> __global__ void __launch_bounds__(256) k_pmean(const Ctx<T> c) {
   __shared__ double sh[32]; __shared__ int flag;
+  if (c.S->pending) return;
   const long long N = (long long)c.nx * c.ny * c.nz;
   double v[1] = {0.0};
   for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
@@ -406,15 +617,19 @@ template <class T> __global__ void __launch_bounds__(256) k_pmean(const Ctx<T> c
   }
 }
 template <class T> __global__ void __launch_bounds__(256) k_pshift(const Ctx<T> c) {
+  if (c.S->pending) return;
   const long long N = (long long)c.nx * c.ny * c.nz;
   const T m = T(c.S->pmean);
   for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) c.p[q] -= m;
 }
+template <class T> __global__ void k_pflush_done(const Ctx<T> c) { c.S->pending = 0; }
 template <class T> int launch_pcg_finish(const Ctx<T>& c, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;
-  FS_LAUNCH(L, "p_mean", 1.0 * sizeof(T) * N, k_pmean<T><<<flat_blocks(N), 256, 0, L.s>>>(c));
-  FS_LAUNCH(L, "p_shift", 2.0 * sizeof(T) * N, k_pshift<T><<<flat_blocks(N), 256, 0, L.s>>>(c));
-  return 2;
+  FS_LAUNCH(L, "p_mean", 0.0, k_pmean<T><<<flat_blocks(N), 256, 0, L.s>>>(c));
+  FS_LAUNCH(L, "p_shift", 0.0, k_pshift<T><<<flat_blocks(N), 256, 0, L.s>>>(c));
+  FS_LAUNCH(L, "p_flush_mean", 3.0 * sizeof(T) * N, k_pflush<T><<<flat_blocks(N), 256, 0, L.s>>>(c));
+  FS_LAUNCH(L, "p_flush_mean", 0.0, k_pflush_done<T><<<1, 1, 0, L.s>>>(c));
+  return 4;
 }
 
 // ---- true residual ||bhat - A p||^2 (fs_poisson_solve; fs_step gets it from the projection) ---------
