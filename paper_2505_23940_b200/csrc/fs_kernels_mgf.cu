@@ -93,16 +93,18 @@ k_mg_down(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__
   const unsigned cpl = (unsigned)(nx >> 1) * (ny >> 1), crow = (unsigned)(gx >> 1) + (unsigned)(nx >> 1) * (gy >> 1);
   const T m6 = T(-6) * ih2;
   T acc = T(0);
-  int zl = modp(z0 - 2, nz);              // plane of the load in flight
+  int zl = modp(z0 - 2, nz);              // plane of the youngest load in flight
   int b = 0;                              // buffer of plane t (toggles); plane t-1 lives in PL - b
-  Quad<T> nxt;
+  Quad<T> nxt, nx2;                       // loads in flight: planes t and t+1 (two planes of latency cover)
   nxt.lo = ldv2<T, V>(g + (row0 + pl * zl)); nxt.hi = ldv2<T, V>(g + (row1 + pl * zl));
+  zl = zl + 1 == nz ? 0 : zl + 1;
+  nx2.lo = ldv2<T, V>(g + (row0 + pl * zl)); nx2.hi = ldv2<T, V>(g + (row1 + pl * zl));
   // one plane: gA, gB = g(t-2), g(t-1); gC receives g(t).  eA, eB = e(t-3), e(t-2); eC receives e(t-1).
   auto step = [&](int t, const Quad<T>& gA, const Quad<T>& gB, Quad<T>& gC, const Quad<T>& eA, const Quad<T>& eB, Quad<T>& eC) {
-    gC = nxt;
-    if (t < tend) {
+    gC = nxt; nxt = nx2;
+    if (t + 1 < tend) {
       zl = zl + 1 == nz ? 0 : zl + 1;
-      nxt.lo = ldv2<T, V>(g + (row0 + pl * zl)); nxt.hi = ldv2<T, V>(g + (row1 + pl * zl));
+      nx2.lo = ldv2<T, V>(g + (row0 + pl * zl)); nx2.hi = ldv2<T, V>(g + (row1 + pl * zl));
     }
     const int pb = PL - b;
     if (t >= z0) {            // e(t-1)
