@@ -96,6 +96,33 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(x, dist, device):
+    """Timing rule of the contract: a multi-rank number is the MAX over ranks (replicas run independently,
+    the job is as slow as its slowest rank).  dist is None for a single process."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def ncu_traffic(dtype, label):
+    """DRAM bytes per launch of the kernel behind a profile label, from the committed ncu --set full summary
+    (profiles/r1_traffic.csv: dtype,label,kernel,grid,dram_read_bytes,dram_write_bytes).  None if absent."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 6 and f[0] == dtype and f[1] == label:
+            try:
+                return float(f[4]) + float(f[5])
+            except ValueError:
+                return None
+    return None
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -191,10 +218,7 @@ def run_ours(a):
     info = g.step(0)
     launches = g.launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
-    if dist is not None:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, dev)
     value = world * cells * a.steps / (ms * 1e-3) / 1e6
     iters_total = None
 
@@ -223,10 +247,7 @@ def run_ours(a):
             e2e_step()
         barrier()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, dist, dev)
         e2e = {"value": world * cells * ke / dt / 1e6, "unit": UNIT,
                "h2d_bytes_per_step": 3 * cells * wbytes, "d2h_bytes_per_step": 4 * cells * wbytes,
                "steps": ke, "ms_per_step": 1e3 * dt / ke,
@@ -247,13 +268,20 @@ def run_ours(a):
         top = max(prof.items(), key=lambda kv: kv[1]["ms"])
         ach = top[1]["bytes"] / (top[1]["ms"] * 1e-3) / 1e9
         step_bytes = sum(v["bytes"] for v in prof.values()) / ksteps
+        step_s = ms / a.steps * 1e-3
+        # SURVEY 8(d) model of the UNFUSED formulation: 25 + 29.4 N_it words per cell-step (GMG-PCG)
+        nit = sum(v["launches"] for k, v in prof.items() if k == "pcg_update_norm") / ksteps
+        unfused_bytes = (25.0 + 29.4 * nit) * wbytes * cells
         roof = {"bound": "hbm", "kernel": top[0], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "peak_source": peak_src,
+                "traffic": ncu_traffic(a.dtype, top[0]), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": top[1]["bytes"] / top[1]["launches"],
                 "avg_launch_ms": top[1]["ms"] / top[1]["launches"], "share_of_step": top[1]["ms"] / tot,
-                "step": {"algorithmic_bytes": step_bytes, "achieved": step_bytes / (ms / a.steps * 1e-3) / 1e9,
-                         "frac": step_bytes / (ms / a.steps * 1e-3) / 1e9 / peak,
-                         "note": "sum of per-kernel algorithmic bytes of one step / graph-replay step time"}}
+                "step": {"algorithmic_bytes": step_bytes, "achieved": step_bytes / step_s / 1e9,
+                         "frac": step_bytes / step_s / 1e9 / peak,
+                         "note": "sum of per-kernel algorithmic bytes (fused kernels: DESIGN.md 7) of one step / graph-replay step time"},
+                "step_unfused_model": {"algorithmic_bytes": unfused_bytes, "achieved": unfused_bytes / step_s / 1e9,
+                                       "frac": unfused_bytes / step_s / 1e9 / peak, "pcg_iters_per_step": nit,
+                                       "note": "SURVEY 8(d): (25 + 29.4 N_it) words per cell-step, every pass a separate kernel"}}
     if dist is not None:
         dist.barrier()
 
