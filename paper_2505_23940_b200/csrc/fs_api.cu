@@ -255,7 +255,7 @@ template <class T> int enqueue_pre(fs_grid* g, const Launch& L, bool poisson) {
     n += launch_flux_correction<T>(c, L);
     n += launch_div_rhs<T>(c, L);
   }
-  n += launch_pcg_init<T>(c, L);
+  n += launch_pcg_init<T>(c, L, poisson);
   return n;
 }
 template <class T> int enqueue_body(fs_grid* g, const Launch& L) { return launch_pcg_body<T>(ctx<T>(g), mgc<T>(g), L); }

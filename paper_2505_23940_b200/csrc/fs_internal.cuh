@@ -110,7 +110,7 @@ template <class T> int launch_step_end(const Ctx<T>& c, const IbmCtx& ib, const 
 template <class TS, class TD> void launch_convert(const TS* src, TD* dst, long long n, cudaStream_t s);
 template <class T> void launch_scale(T* x, double a, long long n, cudaStream_t s);
 
-template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L);
+template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L, bool need_bhat);
 template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, const Launch& L);
 template <class T> int launch_pcg_finish(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_true_residual(const Ctx<T>& c, const Launch& L);
@@ -137,6 +137,18 @@ template <> struct V16T<double> { using type = double2; };
 template <> struct V16T<float> { using type = float4; };
 template <class T, class V> __device__ __forceinline__ V ldv2(const T* p) { return *reinterpret_cast<const V*>(p); }
 template <class T, class V> __device__ __forceinline__ void stv2(T* p, const V& v) { *reinterpret_cast<V*>(p) = v; }
+
+// one 16-byte vector of x-adjacent cells as an array (2 fp64 / 4 fp32 cells)
+template <class T> struct Vec16 {
+  static constexpr int VX = 16 / sizeof(T);
+  alignas(16) T a[VX];
+};
+template <class T> __device__ __forceinline__ Vec16<T> ld16(const T* p) {
+  Vec16<T> v; *reinterpret_cast<typename V16T<T>::type*>(v.a) = *reinterpret_cast<const typename V16T<T>::type*>(p); return v;
+}
+template <class T> __device__ __forceinline__ void st16(T* p, const Vec16<T>& v) {
+  *reinterpret_cast<typename V16T<T>::type*>(p) = *reinterpret_cast<const typename V16T<T>::type*>(v.a);
+}
 
 __device__ __forceinline__ int wrapi(int i, int n) { i %= n; return i < 0 ? i + n : i; }
 

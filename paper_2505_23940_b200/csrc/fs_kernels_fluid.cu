@@ -488,6 +488,114 @@ template <class T> __global__ void __launch_bounds__(256) k_project(const Ctx<T>
   }
 }
 
+// Same pass for grids that are periodic in x with nx a multiple of the vector width: 2.5-D streaming kernel,
+// one 16-byte vector of cells per thread, 32 VX x TY extended tile -> 30 VX x (TY - 2) results, z march.  A thread
+// projects its own u, v, w faces of plane k (p of the west / south neighbours through a shared plane, p of
+// the plane below from a register) and publishes the projected u, v in shared memory; the divergence of
+// plane k-1 is formed one plane later from the east / north neighbours' projected faces of that plane and
+// the w faces of planes k-1 and k.  Raw loads stay in flight for two planes.
+// rows of the extended tile: 12 in fp32 (80 registers), 8 in fp64 (114 registers, no spills)
+template <class T> struct PjTile { static constexpr int TY = sizeof(T) == 4 ? 12 : 8; };
+
+template <class T> __global__ void __launch_bounds__(32 * PjTile<T>::TY, 2) k_projectv(const Ctx<T> c, int kz) {
+  constexpr int kPjTY = PjTile<T>::TY;
+  constexpr int VX = Vec16<T>::VX, ROWE = 32 * VX, PLN = kPjTY * ROWE;
+  using W = Vec16<T>;
+  __shared__ __align__(16) T SP[2 * PLN], SU[2 * PLN], SV[2 * PLN];
+  __shared__ double sh[32]; __shared__ int flag;
+  const int lane = threadIdx.x, ty = threadIdx.y;
+  const int gx = (blockIdx.x * 30 - 1 + lane) * VX, gy = blockIdx.y * (kPjTY - 2) - 1 + ty;
+  const int sx = wrapi(gx, c.nx);
+  const int syc = c.by ? min(max(gy, 0), c.ny - 1) : wrapi(gy, c.ny);      // row of cell-shaped arrays
+  const int syv = c.by ? min(max(gy, 0), c.ny) : wrapi(gy, c.ny);          // row of v
+  const bool own = lane >= 1 && lane <= 30 && ty >= 1 && ty <= kPjTY - 2 && gx < c.nx && gy < c.nyv;
+  const bool rowc = gy < c.ny;                                            // the row has cells / u / w faces
+  const bool vbnd = c.by && (gy <= 0 || gy >= c.ny);                       // v face on a wall: not projected
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nzw);
+  const unsigned plc = (unsigned)c.nx * c.ny, plv = (unsigned)c.nx * c.nyv;
+  const unsigned rowc_o = (unsigned)sx + (unsigned)c.nx * syc, rowv_o = (unsigned)sx + (unsigned)c.nx * syv;
+  const T dtr = T(c.dt / c.rho), ihx = c.ihx, ihz = c.ihz;
+  const T idycj = c.idyc[syv], idyj = c.idy[syc + 1];
+  const double sc = c.rho / c.dt, mc = c.S->mean_coef, dyj = c.dy64[syc];
+  const int o_own = ty * ROWE + lane * VX;
+  const int o_s = (ty > 0 ? ty - 1 : 0) * ROWE + lane * VX, o_n = (ty < kPjTY - 1 ? ty + 1 : ty) * ROWE + lane * VX;
+  const int o_w = ty * ROWE + (lane > 0 ? lane * VX - 1 : 0), o_e = ty * ROWE + (lane < 31 ? lane * VX + VX : 32 * VX - 1);
+  auto kcell = [&](int k) { return c.bz ? min(max(k, 0), c.nz - 1) : (k < 0 ? k + c.nz : (k >= c.nz ? k - c.nz : k)); };
+  auto kwf = [&](int k) { return c.bz ? min(max(k, 0), c.nz) : (k < 0 ? k + c.nz : (k >= c.nz ? k - c.nz : k)); };
+  struct Raw { W p, us, vs, ws; };
+  auto fetch = [&](int k, Raw& r) {
+    const unsigned kc = (unsigned)kcell(k);
+    r.p = ld16<T>(c.p + (rowc_o + plc * kc));
+    r.us = ld16<T>(c.us + (rowc_o + plc * kc));
+    r.vs = ld16<T>(c.vs + (rowv_o + plv * kc));
+    r.ws = ld16<T>(c.ws + (rowc_o + plc * (unsigned)kwf(k)));
+  };
+  Raw r0, r1;
+  W pB = ld16<T>(c.p + (rowc_o + plc * (unsigned)kcell(k0 - 1)));
+  fetch(k0, r0);
+  fetch(k0 + 1, r1);
+  W wnP;                                    // projected w faces of plane k-1
+#pragma unroll
+  for (int a = 0; a < VX; ++a) wnP.a[a] = T(0);
+  double ss = 0.0, md = 0.0; int nan = 0;
+  int b = 0;
+  // one plane; r holds its raw loads and is refilled with plane k+2 at the end (the two Raw buffers alternate)
+  auto body = [&](int k, Raw& r) {
+    st16<T>(SP + b + o_own, r.p);
+    __syncthreads();
+    const W pS = ld16<T>(SP + b + o_s);
+    const T pW0 = SP[b + o_w];
+    const bool wbnd = c.bz && (k == 0 || k >= c.nz);
+    W un, vn, wn;
+#pragma unroll
+    for (int a = 0; a < VX; ++a) {
+      const T pc = r.p.a[a], pw = a > 0 ? r.p.a[a > 0 ? a - 1 : 0] : pW0;
+      un.a[a] = r.us.a[a] - dtr * ((pc - pw) * ihx);
+      vn.a[a] = vbnd ? r.vs.a[a] : r.vs.a[a] - dtr * ((pc - pS.a[a]) * idycj);
+      wn.a[a] = wbnd ? r.ws.a[a] : r.ws.a[a] - dtr * ((pc - pB.a[a]) * ihz);
+    }
+    if (own && k < k1) {
+      if (rowc && k < c.nz) st16<T>(c.u + (rowc_o + plc * (unsigned)k), un);
+      if (k < c.nz) st16<T>(c.v + (rowv_o + plv * (unsigned)k), vn);
+      if (rowc) st16<T>(c.w + (rowc_o + plc * (unsigned)k), wn);
+    }
+    // divergence of plane k-1 (its projected u, v faces were published one iteration ago)
+    if (k > k0 && own && rowc && k - 1 < c.nz) {
+      const int pb = PLN - b;
+      const W vN = ld16<T>(SV + pb + o_n), vO = ld16<T>(SV + pb + o_own), uO = ld16<T>(SU + pb + o_own);
+      const T uE0 = SU[pb + o_e];
+#pragma unroll
+      for (int a = 0; a < VX; ++a) {
+        const T ue = a < VX - 1 ? uO.a[a < VX - 1 ? a + 1 : a] : uE0;
+        const T div = (ue - uO.a[a]) * ihx + (vN.a[a] - vO.a[a]) * idyj + (wn.a[a] - wnP.a[a]) * ihz;
+        const double ad = fabs((double)div);
+        if (ad != ad) nan = 1;
+        md = fmax(md, ad);
+        const double e = -dyj * sc * (double)div - mc * dyj;
+        ss += e * e;
+      }
+    }
+    st16<T>(SU + b + o_own, un); st16<T>(SV + b + o_own, vn);
+    wnP = wn; pB = r.p;
+    if (k + 2 <= k1) fetch(k + 2, r);
+    b = PLN - b;
+  };
+  for (int k = k0;;) {
+    body(k, r0); if (++k > k1) break;
+    body(k, r1); if (++k > k1) break;
+  }
+  md = warp_max(md);
+  nan = __any_sync(0xffffffffu, nan);
+  if (lane == 0) {
+    if (md > 0.0) atomicMax((unsigned long long*)&c.S->max_div, (unsigned long long)__double_as_longlong(md));
+    if (nan) atomicOr(&c.S->nan_flag, 1);
+  }
+  double v[1] = {ss};
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (lane == 0 && ty == 0) c.S->true_rr = v[0];
+  }
+}
+
 struct ColGeom { dim3 grid, block; int kz; };
 ColGeom col_geom(int nx, int ny, int nz);
 ColGeom col_geom(int nx, int ny, int nz) {
@@ -505,6 +613,14 @@ ColGeom col_geom(int nx, int ny, int nz) {
 }
 
 template <class T> int launch_project(const Ctx<T>& c, const Launch& L) {
+  if (!c.bx && c.nx % Vec16<T>::VX == 0) {
+    const int bxn = (c.nx + 30 * Vec16<T>::VX - 1) / (30 * Vec16<T>::VX), byn = (c.nyv + PjTile<T>::TY - 3) / (PjTile<T>::TY - 2);
+    int kz = c.nzw;
+    while (kz > 16 && (long long)bxn * byn * ((c.nzw + kz - 1) / kz) < 4LL * 296) kz = (kz + 1) / 2;
+    FS_LAUNCH(L, "project", 7.0 * sizeof(T) * c.nx * c.ny * c.nz,
+              k_projectv<T><<<dim3(bxn, byn, (c.nzw + kz - 1) / kz), dim3(32, PjTile<T>::TY), 0, L.s>>>(c, kz));
+    return 1;
+  }
   ColGeom g = col_geom(c.nxu, c.nyv, c.nzw);
   FS_LAUNCH(L, "project", 7.0 * sizeof(T) * c.nx * c.ny * c.nz, k_project<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz));
   return 1;

@@ -303,16 +303,6 @@ static DaGeom da2_geom(int nx, int ny, int nz) {
 // kernel above is the faster of the two and is the one used; nx a
 // multiple of VX): vector global accesses, the index arithmetic shared by VX cells, a 32 VX x 16 extended
 // tile -> 30 VX x 14 results (lanes 0 and 31 are halo), z loop unrolled by renaming.
-template <class T> struct Vec16 {
-  static constexpr int VX = 16 / sizeof(T);
-  T a[VX];
-};
-template <class T> __device__ __forceinline__ Vec16<T> ld16(const T* p) {
-  Vec16<T> v; *reinterpret_cast<typename V16T<T>::type*>(v.a) = *reinterpret_cast<const typename V16T<T>::type*>(p); return v;
-}
-template <class T> __device__ __forceinline__ void st16(T* p, const Vec16<T>& v) {
-  *reinterpret_cast<typename V16T<T>::type*>(p) = *reinterpret_cast<const typename V16T<T>::type*>(v.a);
-}
 constexpr int kDaVIY = kDaTY - 2;
 
 template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pcg_dirapplyv(const Ctx<T> c, T zs, int kz) {
@@ -452,6 +442,112 @@ template <class T> static DaGeom dav_geom(int nx, int ny, int nz) {
   return g;
 }
 
+// Same start, streaming form of k_pcg_dirapplyv (one 16-byte vector of cells per thread, A applied to x0
+// through a shared plane and a register queue); bhat is only stored when the caller needs it later (WBH:
+// fs_poisson_solve's true residual; fs_step gets that from the projection).
+template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pcg_initv(const Ctx<T> c, int kz, Launch L) {
+  constexpr int VX = Vec16<T>::VX;
+  constexpr int ROWE = 32 * VX;
+  constexpr int PLN = kDaTY * ROWE;
+  using W = Vec16<T>;
+  __shared__ __align__(16) T D[2 * PLN];
+  __shared__ double sh[4 * 32]; __shared__ int flag;
+  const int lane = threadIdx.x, ty = threadIdx.y;
+  const int gx = (blockIdx.x * 30 - 1 + lane) * VX, gy = blockIdx.y * kDaVIY - 1 + ty;
+  const int sx = c.bx ? min(max(gx, 0), c.nx - VX) : wrapi(gx, c.nx);
+  const int sy = c.by ? min(max(gy, 0), c.ny - 1) : wrapi(gy, c.ny);
+  const bool fixl = c.bx && gx < 0, fixr = c.bx && gx >= c.nx;
+  const bool own = lane >= 1 && lane <= 30 && ty >= 1 && ty <= kDaTY - 2 && gx < c.nx && gy < c.ny;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  const unsigned pl = (unsigned)c.nx * c.ny, row = (unsigned)sx + (unsigned)c.nx * sy;
+  const T cyl = c.cyl[sy], cyh = c.cyh[sy], idy = c.idy[sy + 1], dyj = c.dy[sy + 1], ndy = -dyj;
+  const T ihx2 = c.ihx2, ihz2 = c.ihz2;
+  const T shift = T(c.S->mean_coef) * dyj;
+  T dg[VX];
+#pragma unroll
+  for (int a = 0; a < VX; ++a) {
+    const int i = sx + a;
+    dg[a] = PC == 1 ? T((c.bx && i == 0 ? 0 : 1) + (c.bx && i == c.nx - 1 ? 0 : 1)) * ihx2 + (cyh + cyl) * idy : T(0);
+  }
+  const int o_own = ty * ROWE + lane * VX;
+  const int o_s = (ty > 0 ? ty - 1 : 0) * ROWE + lane * VX, o_n = (ty < kDaTY - 1 ? ty + 1 : ty) * ROWE + lane * VX;
+  const int o_w = ty * ROWE + (lane > 0 ? lane * VX - 1 : 0), o_e = ty * ROWE + (lane < 31 ? lane * VX + VX : 32 * VX - 1);
+  auto fetch = [&](int k) {
+    const int ks = c.bz ? min(max(k, 0), c.nz - 1) : (k < 0 ? k + c.nz : (k >= c.nz ? k - c.nz : k));
+    W d = ld16<T>(c.p + (row + pl * (unsigned)ks));
+    if (fixl) {
+#pragma unroll
+      for (int a = 1; a < VX; ++a) d.a[a] = d.a[0];
+    }
+    if (fixr) {
+#pragma unroll
+      for (int a = 0; a < VX - 1; ++a) d.a[a] = d.a[VX - 1];
+    }
+    return d;
+  };
+  W d0 = fetch(k0 - 1), d1 = fetch(k0), d2, nx1 = fetch(k0 + 1);
+  W rb;                                     // raw right-hand side of the plane about to be processed
+#pragma unroll
+  for (int a = 0; a < VX; ++a) rb.a[a] = T(0);
+  if (own) rb = ld16<T>(c.r + (row + pl * (unsigned)k0));
+  int b = 0;
+  st16<T>(D + o_own, d1);
+  __syncthreads();
+  double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
+  auto step = [&](int k, const W& dB, const W& dC, W& dT) {
+    dT = nx1;
+    if (k + 1 < k1) nx1 = fetch(k + 2);
+    const W rcur = rb;
+    if (own && k + 1 < k1) rb = ld16<T>(c.r + (row + pl * (unsigned)(k + 1)));
+    const T* P = D + b;
+    const W Sv = ld16<T>(P + o_s), Nv = ld16<T>(P + o_n);
+    const T xw0 = P[o_w], xeL = P[o_e];
+    if (own) {
+      const T dzz = PC == 1 ? T((c.bz && k == 0 ? 0 : 1) + (c.bz && k == c.nz - 1 ? 0 : 1)) * ihz2 : T(0);
+      W r, bh;
+      T s0 = T(0), s1 = T(0), s2 = T(0), s3 = T(0);
+#pragma unroll
+      for (int a = 0; a < VX; ++a) {
+        const T xc = dC.a[a];
+        const T xw = a > 0 ? dC.a[a > 0 ? a - 1 : 0] : xw0;
+        const T xe = a < VX - 1 ? dC.a[a < VX - 1 ? a + 1 : a] : xeL;
+        T acc = (xe - xc) * ihx2 - (xc - xw) * ihx2;
+        acc += ((Nv.a[a] - xc) * cyh - (xc - Sv.a[a]) * cyl) * idy;
+        acc += (dT.a[a] - xc) * ihz2 - (xc - dB.a[a]) * ihz2;
+        bh.a[a] = rcur.a[a] - shift;
+        r.a[a] = bh.a[a] - acc * ndy;
+        const T z = PC == 1 ? r.a[a] / ((dg[a] + dzz) * dyj) : r.a[a];
+        s0 += bh.a[a] * bh.a[a]; s1 += r.a[a] * r.a[a]; s2 += r.a[a] * z; s3 += r.a[a];
+      }
+      const unsigned o = row + pl * (unsigned)k;
+      st16<T>(c.r + o, r);
+      if (WBH) st16<T>(c.bh + o, bh);
+      v0 += (double)s0; v1 += (double)s1; v2 += (double)s2; v3 += (double)s3;
+    }
+    b = PLN - b;
+    st16<T>(D + b + o_own, dT);
+    __syncthreads();
+  };
+  int k = k0;
+  for (;;) {
+    step(k, d0, d1, d2); if (++k >= k1) break;
+    step(k, d1, d2, d0); if (++k >= k1) break;
+    step(k, d2, d0, d1); if (++k >= k1) break;
+  }
+  double v[4] = {v0, v1, v2, v3};
+  if (grid_sum<4>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (lane == 0 && ty == 0) {
+      Scalars* S = c.S;
+      S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
+      S->iter = 0; S->first = 1; S->dsel = 0; S->pending = 0;
+      S->rmean = v[3] / ((double)c.nx * c.ny * c.nz);
+      const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
+      S->converged = conv; S->done = conv || S->max_iter <= 0;
+      if (L.use_cond) cudaGraphSetConditional(L.cond, S->done ? 0u : 1u);
+    }
+  }
+}
+
 // ---- K2: x += alpha d, r -= alpha q fused with ||r||^2 and r.z; loop control -------------------------
 // fp32 only: rounding makes sum(q) != 0, so r slowly acquires a component along the null space of A
 // (constants) that CG can never remove; once it dominates r the fp32 stencil differences lose all
@@ -531,11 +627,22 @@ template <class T> __global__ void __launch_bounds__(256) k_dot_rz(const Ctx<T> 
   }
 }
 
-template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L) {
-  ColGeom g = col_geom(c.nx, c.ny, c.nz);
+template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L, bool need_bhat) {
   int n = 0;
-  if (!c.warm_start) { FS_LAUNCH(L, "memset_p", 1.0 * sizeof(T) * c.nx * c.ny * c.nz, cudaMemsetAsync(c.p, 0, sizeof(T) * (size_t)c.nx * c.ny * c.nz, L.s)); ++n; }
-  FS_LAUNCH(L, "pcg_init", 4.0 * sizeof(T) * c.nx * c.ny * c.nz, k_pcg_init<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz, L));
+  const double N = (double)c.nx * c.ny * c.nz;
+  if (!c.warm_start) { FS_LAUNCH(L, "memset_p", 1.0 * sizeof(T) * N, cudaMemsetAsync(c.p, 0, sizeof(T) * (size_t)c.nx * c.ny * c.nz, L.s)); ++n; }
+  if (c.nx % Vec16<T>::VX == 0) {
+    const DaGeom G = dav_geom<T>(c.nx, c.ny, c.nz);
+    const dim3 blk(32, kDaTY);
+    const bool jac = c.precond == FS_PC_JACOBI;
+    FS_LAUNCH(L, "pcg_init", (need_bhat ? 4.0 : 3.0) * sizeof(T) * N, {
+      if (jac) { if (need_bhat) k_pcg_initv<T, 1, true><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); else k_pcg_initv<T, 1, false><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); }
+      else { if (need_bhat) k_pcg_initv<T, 0, true><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); else k_pcg_initv<T, 0, false><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); }
+    });
+    return n + 1;
+  }
+  ColGeom g = col_geom(c.nx, c.ny, c.nz);
+  FS_LAUNCH(L, "pcg_init", 4.0 * sizeof(T) * N, k_pcg_init<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz, L));
   return n + 1;
 }
 
@@ -655,7 +762,7 @@ template <class T> int launch_true_residual(const Ctx<T>& c, const Launch& L) {
 }
 
 #define INST(T)                                                                   \
-  template int launch_pcg_init<T>(const Ctx<T>&, const Launch&);                  \
+  template int launch_pcg_init<T>(const Ctx<T>&, const Launch&, bool);                  \
   template int launch_pcg_body<T>(const Ctx<T>&, const MgCtx<T>&, const Launch&); \
   template int launch_pcg_finish<T>(const Ctx<T>&, const Launch&);                \
   template int launch_true_residual<T>(const Ctx<T>&, const Launch&);
