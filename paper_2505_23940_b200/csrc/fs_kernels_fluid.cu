@@ -385,10 +385,66 @@ template <class T> __global__ void __launch_bounds__(256) k_div_rhs(const Ctx<T>
     }
   }
 }
+// Same pass for grids periodic in x with nx a multiple of the vector width: one 16-byte vector of cells per
+// thread, 32 x 8 threads per CTA marching a z chunk (the top w face of one plane is the bottom of the next),
+// no integer division.
+template <class T> __global__ void __launch_bounds__(256) k_div_rhsv(const Ctx<T> c, int kz) {
+  constexpr int VX = Vec16<T>::VX;
+  using W = Vec16<T>;
+  __shared__ double sh[32]; __shared__ int flag;
+  const int gx = (blockIdx.x * 32 + threadIdx.x) * VX, gy = blockIdx.y * 8 + threadIdx.y;
+  const bool valid = gx < c.nx && gy < c.ny;
+  const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  double sum = 0.0;
+  if (valid) {
+    const int jp = c.by ? gy + 1 : (gy + 1 == c.ny ? 0 : gy + 1);
+    const int xe = gx + VX == c.nx ? 0 : gx + VX;
+    const unsigned plc = (unsigned)c.nx * c.ny, plv = (unsigned)c.nx * c.nyv;
+    const unsigned oc = (unsigned)gx + (unsigned)c.nx * gy, oe = (unsigned)xe + (unsigned)c.nx * gy;
+    const unsigned ov = (unsigned)gx + (unsigned)c.nx * gy, ovp = (unsigned)gx + (unsigned)c.nx * jp;
+    const T ihx = c.ihx, ihz = c.ihz, idy = c.idy[gy + 1], sc = T(c.rho / c.dt), mdy = -c.dy[gy + 1];
+    W wb = ld16<T>(c.ws + (oc + plc * (unsigned)k0));
+#pragma unroll 2
+    for (int k = k0; k < k1; ++k) {
+      const int kp = c.bz ? k + 1 : (k + 1 == c.nz ? 0 : k + 1);
+      const W u = ld16<T>(c.us + (oc + plc * (unsigned)k));
+      const T uE = c.us[oe + plc * (unsigned)k];
+      const W vs = ld16<T>(c.vs + (ov + plv * (unsigned)k)), vn = ld16<T>(c.vs + (ovp + plv * (unsigned)k));
+      const W wt = ld16<T>(c.ws + (oc + plc * (unsigned)kp));
+      W r;
+      T s = T(0);
+#pragma unroll
+      for (int a = 0; a < VX; ++a) {
+        const T ue = a < VX - 1 ? u.a[a < VX - 1 ? a + 1 : a] : uE;
+        const T div = (ue - u.a[a]) * ihx + (vn.a[a] - vs.a[a]) * idy + (wt.a[a] - wb.a[a]) * ihz;
+        r.a[a] = mdy * (div * sc);
+        s += r.a[a];
+      }
+      st16<T>(c.r + (oc + plc * (unsigned)k), r);
+      sum += (double)s;
+      wb = wt;
+    }
+  }
+  double v[1] = {sum};
+  if (grid_sum<1>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0 && threadIdx.y == 0) {
+      c.S->mean_coef = v[0] / c.S->sum_dy;
+      c.S->max_div = 0.0; c.S->nan_flag = 0; c.S->true_rr = 0.0;
+    }
+  }
+}
 static inline int flat_blocks(long long n) { long long b = (n + 255) / 256; return (int)(b < kFlatBlocks ? (b < 1 ? 1 : b) : kFlatBlocks); }
 
 template <class T> int launch_div_rhs(const Ctx<T>& c, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;
+  if (!c.bx && c.nx % Vec16<T>::VX == 0) {
+    const int bxn = (c.nx + 32 * Vec16<T>::VX - 1) / (32 * Vec16<T>::VX), byn = (c.ny + 7) / 8;
+    int kz = c.nz;
+    while (kz > 16 && (long long)bxn * byn * ((c.nz + kz - 1) / kz) < 8LL * 148 * 8) kz = (kz + 1) / 2;
+    while ((long long)bxn * byn * ((c.nz + kz - 1) / kz) > kMaxPartials) kz *= 2;
+    FS_LAUNCH(L, "div_rhs", 4.0 * sizeof(T) * N, k_div_rhsv<T><<<dim3(bxn, byn, (c.nz + kz - 1) / kz), dim3(32, 8), 0, L.s>>>(c, kz));
+    return 1;
+  }
   FS_LAUNCH(L, "div_rhs", 4.0 * sizeof(T) * N, k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, nullptr));
   return 1;
 }
