@@ -134,10 +134,11 @@ template <class T> size_t carve(fs_grid* g, char* base) {
   c.us = b.take<T>(g->nU); c.vs = b.take<T>(g->nV); c.ws = b.take<T>(g->nW);
   c.hu = b.take<T>(g->nU); c.hv = b.take<T>(g->nV); c.hw = b.take<T>(g->nW);
   c.p = b.take<T>(g->nP); c.r = b.take<T>(g->nP); c.d = b.take<T>(g->nP); c.d2 = b.take<T>(g->nP); c.q = b.take<T>(g->nP); c.bh = b.take<T>(g->nP);
-  c.z = nullptr;
+  c.z = nullptr; c.r2 = nullptr;
   mg.nlev = 0;
   if (P.precond == FS_PC_GMG) {
     c.z = b.take<T>(g->nP);
+    if (P.mg_nu1 == 2 && P.mg_nu2 == 2) c.r2 = b.take<T>(g->nP);   // second residual buffer of the fused update (k_mg_down<UPD>)
     mg.nlev = mg_levels(P.nx, P.ny, P.nz);
     mg.nu1 = P.mg_nu1; mg.nu2 = P.mg_nu2; mg.coarse_sweeps = P.mg_coarse_sweeps; mg.omega = P.mg_omega;
     int nx = P.nx, nyy = P.ny, nz = P.nz; double h = g->hx;

@@ -24,6 +24,7 @@ struct Scalars {
   double rmean;         // fp32 only: mean of the recurrence residual, removed with one iteration of lag (null-space deflation)
   double sum_dy;         // sum over all cells of dy_j
   int iter, done, converged, first;
+  int rsel, need_update; // rsel: which residual buffer (r / r2) is current; need_update: K2 of the last iteration still to do (k_mg_down<UPD>)
   int dsel, pending;     // pending: the x += alpha_prev d of the last k_pcg_update has not been applied yet
   double alpha_prev, sum_p, sum_d;   // deferred x update (k_pcg_dirapply / k_pflush)
   int pad2_unused, pad3_unused; //       // which of the two direction buffers holds the current d (k_pcg_dirapply)
@@ -62,7 +63,7 @@ template <class T> struct Ctx {
   const double* dy64;  // [ny] fp64 cell heights (reductions, flux areas)
   // fields
   T *u, *v, *w, *p, *us, *vs, *ws, *hu, *hv, *hw;
-  T *r, *d, *d2, *q, *z, *bh;
+  T *r, *r2, *d, *d2, *q, *z, *bh;   // r2: second residual buffer (GMG fused update), else nullptr
   Scalars* S;
   double* partials;     // [kRedSlots][kMaxPartials]
 };
@@ -115,11 +116,14 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
 template <class T> int launch_pcg_finish(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_true_residual(const Ctx<T>& c, const Launch& L);
 // dot_fused != nullptr asks for rho_cur = rhs . (zs out) from the last kernel; *dot_fused says whether it was done
-template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs);
+// upd_fused != nullptr additionally asks the level-0 down kernel to perform the residual update of the previous
+// PCG iteration (fs_kernels_mgf.cu k_mg_down<UPD>); *upd_fused says whether it was done
+template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs,
+                                     bool* upd_fused = nullptr);
 template <class T> int launch_mg_down(const Ctx<T>& c, const T* g, T* e, T* gc, int nx, int ny, int nz, double h, double omega,
-                                      const char* name, const Launch& L);
+                                      const char* name, const Launch& L, bool upd = false, T* g2 = nullptr, const T* q = nullptr);
 template <class T> int launch_mg_up(const Ctx<T>& c, const T* ein, const T* ec, const T* g, T* eo, int nx, int ny, int nz, double h,
-                                    double omega, bool dot, T zs, const char* name, const Launch& L);
+                                    double omega, bool dot, T zs, const char* name, const Launch& L, const T* g2 = nullptr);
 
 template <class T> int launch_ibm_index(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
 template <class T> int launch_ibm_interpolate(const Ctx<T>& c, const IbmCtx& ib, const T* u, const T* v, const T* w, double* out, const Launch& L);

@@ -157,7 +157,7 @@ template <class T> __global__ void __launch_bounds__(1024) k_mg_tail(const int* 
 }
 
 // Recursion unrolled on the host: emits the kernels of one V-cycle for rhs -> out (out = V(rhs)).
-template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs) {
+template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs, bool* upd_fused) {
   int n = 0;
   const int* done = &c.S->done;
   const T* gl[kMaxLevels]; T* el[kMaxLevels]; T* tl[kMaxLevels]; T* cur[kMaxLevels];
@@ -168,6 +168,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
   }
   const bool want_dot = dot_fused != nullptr;
   if (dot_fused) *dot_fused = false;
+  if (upd_fused) *upd_fused = false;
   // Fast path, V(2,2) with at least two levels: two fused kernels per level (fs_kernels_mgf.cu).
   if (mg.nu1 == 2 && mg.nu2 == 2 && mg.nlev >= 2) {
     const int last = mg.nlev - 1;
@@ -179,8 +180,12 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     const int top = tail_ok ? lt : last; // levels 0..top-1 run the fused per-level kernels
     for (int l = 0; l < top; ++l) {
       const MgLevel& V = mg.lev[l];
-      n += launch_mg_down<T>(c, gl[l], tl[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, V.h, mg.omega, l == 0 ? "mg_down_l0" : "mg_coarse", L);
+      const bool upd = l == 0 && upd_fused != nullptr && want_dot && c.r2 != nullptr && rhs == c.r;
+      n += launch_mg_down<T>(c, gl[l], tl[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, V.h, mg.omega, l == 0 ? "mg_down_l0" : "mg_coarse", L,
+                             upd, upd ? c.r2 : nullptr, upd ? c.q : nullptr);
+      if (upd) *upd_fused = true;
     }
+    const bool r_pingpong = upd_fused && *upd_fused;
     if (tail_ok) {
       MgTail a; a.nlev = mg.nlev - lt;
       size_t cells = 0;
@@ -212,7 +217,8 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     for (int l = top - 1; l >= 0; --l) {
       const MgLevel& V = mg.lev[l];
       const bool dot = want_dot && l == 0;
-      n += launch_mg_up<T>(c, tl[l], el[l + 1], gl[l], el[l], V.nx, V.ny, V.nz, V.h, mg.omega, dot, zs, l == 0 ? "mg_up_l0" : "mg_coarse", L);
+      n += launch_mg_up<T>(c, tl[l], el[l + 1], gl[l], el[l], V.nx, V.ny, V.nz, V.h, mg.omega, dot, zs, l == 0 ? "mg_up_l0" : "mg_coarse", L,
+                           (l == 0 && r_pingpong) ? c.r2 : nullptr);
       if (dot) *dot_fused = true;
     }
     return n;
@@ -262,7 +268,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
   return n;
 }
 
-template int launch_vcycle<float>(const Ctx<float>&, const MgCtx<float>&, const float*, float*, const Launch&, bool*, float);
-template int launch_vcycle<double>(const Ctx<double>&, const MgCtx<double>&, const double*, double*, const Launch&, bool*, double);
+template int launch_vcycle<float>(const Ctx<float>&, const MgCtx<float>&, const float*, float*, const Launch&, bool*, float, bool*);
+template int launch_vcycle<double>(const Ctx<double>&, const MgCtx<double>&, const double*, double*, const Launch&, bool*, double, bool*);
 
 }  // namespace fs

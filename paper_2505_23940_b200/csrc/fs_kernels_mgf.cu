@@ -74,14 +74,29 @@ template <class T> __device__ __forceinline__ void stq(T* __restrict__ X, T* __r
 // ---- downward leg: e = S^2(0; g), gc = R (g - (-L) e) -----------------------------------------------------
 // Two damped-Jacobi sweeps from a zero guess collapse to e = cg g + cn nb(g) with cg = 2 cw - 6 cw^2 / h^2,
 // cn = cw^2 / h^2  (first sweep: cw g; second: cw g + cw (g - (6 cw g - cw nb) / h^2)).
-template <class T, int TR> __global__ void __launch_bounds__(32 * TR, (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1))
-k_mg_down(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__ eo, T* __restrict__ gc,
-          int nx, int ny, int nz, T cg, T cn, T ih2) {
+//
+// UPD (level 0 inside PCG): the kernel also performs K2 of the PREVIOUS iteration on the fly, g = r - alpha q
+// (halo included, so q is read with the same halo as r), stores the new r for the tile interior into the
+// OTHER residual buffer (neighbouring CTAs still read the old one on their halos; Scalars::rsel says which
+// buffer is current), and its last CTA does the loop control that k_pcg_update does in the unfused path:
+// ||r||^2, iteration count, convergence flag, graph WHILE condition.  The separate update pass (3 words per
+// cell) disappears; when the flag says "done" the remaining kernels of the iteration exit at once.
+template <class T, int TR, bool UPD> __global__ void __launch_bounds__(32 * TR, (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1))
+k_mg_down(const int* __restrict__ done, const T* __restrict__ g_a, T* __restrict__ g_b, const T* __restrict__ qv,
+          T* __restrict__ eo, T* __restrict__ gc, int nx, int ny, int nz, T cg, T cn, T ih2, Scalars* S_, double* partials, Launch L) {
   using V = typename V2T<T>::type;
   constexpr int PL = MgTile<TR>::PL;
   if (done && *done) return;
   extern __shared__ __align__(16) unsigned char mg_smem[];
   T* GX = reinterpret_cast<T*>(mg_smem); T* GY = GX + 2 * PL; T* EX = GY + 2 * PL; T* EY = EX + 2 * PL;
+  __shared__ double sh[2 * 32]; __shared__ int flag;
+  const T* __restrict__ g = g_a; T* __restrict__ rout = nullptr;
+  bool upd = false; T alpha = T(0), rm = T(0);
+  if (UPD) {
+    if (S_->rsel) { g = g_b; rout = const_cast<T*>(g_a); } else { g = g_a; rout = g_b; }
+    upd = S_->need_update != 0;
+    if (upd) { alpha = T(S_->rho_cur / S_->dq); rm = sizeof(T) == 4 ? T(S_->rmean) : T(0); }
+  }
   const int lane = threadIdx.x, ty = threadIdx.y;
   const int gx = blockIdx.x * kMgIX - 2 + 2 * lane, gy = blockIdx.y * MgTile<TR>::IY - 2 + 2 * ty;
   const unsigned pl = (unsigned)nx * ny, gxw = (unsigned)modp(gx, nx);
@@ -93,18 +108,30 @@ k_mg_down(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__
   const unsigned cpl = (unsigned)(nx >> 1) * (ny >> 1), crow = (unsigned)(gx >> 1) + (unsigned)(nx >> 1) * (gy >> 1);
   const T m6 = T(-6) * ih2;
   T acc = T(0);
+  double s2 = 0.0, s1 = 0.0;
   int zl = modp(z0 - 2, nz);              // plane of the youngest load in flight
   int b = 0;                              // buffer of plane t (toggles); plane t-1 lives in PL - b
-  Quad<T> nxt, nx2;                       // loads in flight: planes t and t+1 (two planes of latency cover)
-  nxt.lo = ldv2<T, V>(g + (row0 + pl * zl)); nxt.hi = ldv2<T, V>(g + (row1 + pl * zl));
+  Quad<T> nxt, nx2, qn1, qn2;             // loads in flight: planes t and t+1 (two planes of latency cover)
+  qn1.lo.x = qn1.lo.y = qn1.hi.x = qn1.hi.y = T(0); qn2 = qn1;
+  auto fetch = [&](Quad<T>& gq, Quad<T>& qq) {
+    const unsigned o = pl * zl;
+    gq.lo = ldv2<T, V>(g + (row0 + o)); gq.hi = ldv2<T, V>(g + (row1 + o));
+    if (UPD && upd) { qq.lo = ldv2<T, V>(qv + (row0 + o)); qq.hi = ldv2<T, V>(qv + (row1 + o)); }
+  };
+  fetch(nxt, qn1);
   zl = zl + 1 == nz ? 0 : zl + 1;
-  nx2.lo = ldv2<T, V>(g + (row0 + pl * zl)); nx2.hi = ldv2<T, V>(g + (row1 + pl * zl));
+  fetch(nx2, qn2);
   // one plane: gA, gB = g(t-2), g(t-1); gC receives g(t).  eA, eB = e(t-3), e(t-2); eC receives e(t-1).
   auto step = [&](int t, const Quad<T>& gA, const Quad<T>& gB, Quad<T>& gC, const Quad<T>& eA, const Quad<T>& eB, Quad<T>& eC) {
-    gC = nxt; nxt = nx2;
+    gC = nxt;
+    if (UPD && upd) {
+      gC.lo.x = (gC.lo.x - alpha * qn1.lo.x) - rm; gC.lo.y = (gC.lo.y - alpha * qn1.lo.y) - rm;
+      gC.hi.x = (gC.hi.x - alpha * qn1.hi.x) - rm; gC.hi.y = (gC.hi.y - alpha * qn1.hi.y) - rm;
+    }
+    nxt = nx2; if (UPD) qn1 = qn2;
     if (t + 1 < tend) {
       zl = zl + 1 == nz ? 0 : zl + 1;
-      nx2.lo = ldv2<T, V>(g + (row0 + pl * zl)); nx2.hi = ldv2<T, V>(g + (row1 + pl * zl));
+      fetch(nx2, qn2);
     }
     const int pb = PL - b;
     if (t >= z0) {            // e(t-1)
@@ -121,6 +148,11 @@ k_mg_down(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__
         const unsigned o = pl * (unsigned)(t - 2);
         stv2<T, V>(eo + (row0 + o), eB.lo); stv2<T, V>(eo + (row1 + o), eB.hi);
         if ((t - z0) & 1) gc[crow + cpl * (unsigned)((t - 2) >> 1)] = T(0.125) * acc;
+        if (UPD && upd) {
+          stv2<T, V>(rout + (row0 + o), gA.lo); stv2<T, V>(rout + (row1 + o), gA.hi);
+          s2 += (double)((gA.lo.x * gA.lo.x + gA.lo.y * gA.lo.y) + (gA.hi.x * gA.hi.x + gA.hi.y * gA.hi.y));
+          s1 += (double)((gA.lo.x + gA.lo.y) + (gA.hi.x + gA.hi.y));
+        }
       }
       if ((t - z0) & 1) acc = T(0);
     }
@@ -138,6 +170,23 @@ k_mg_down(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__
     step(t, g1, g2, g0, e1, e2, e0); if (++t > tend) break;
     step(t, g2, g0, g1, e2, e0, e1); if (++t > tend) break;
   }
+  if (UPD && upd) {           // what the last CTA of k_pcg_update does in the unfused path
+    double v[2] = {s2, s1};
+    if (grid_sum<2>(v, partials, &S_->ticket[0], sh, &flag)) {
+      if (threadIdx.x == 0 && threadIdx.y == 0) {
+        Scalars* S = S_;
+        const double N = (double)nx * ny * nz;
+        S->rr = v[0]; S->rmean = v[1] / N;
+        S->alpha_prev = S->rho_cur / S->dq; S->pending = 1;
+        S->iter += 1; S->first = 0; S->dsel ^= 1; S->rsel ^= 1; S->need_update = 0;
+        S->rho_prev = S->rho_cur;
+        const int conv = sqrt(v[0]) <= S->rtol * sqrt(S->bnorm2);
+        S->converged = conv;
+        S->done = conv || S->iter >= S->max_iter;
+        if (L.use_cond) cudaGraphSetConditional(L.cond, S->done ? 0u : 1u);
+      }
+    }
+  }
 }
 
 // ---- upward leg: e' = S^2(e + P ec; g); DOT (level 0 inside PCG): rho = r . (zs e') ---------------------
@@ -150,11 +199,12 @@ template <class T> __device__ __forceinline__ Quad<T> sweepq(const Quad<T>& e, c
 }
 
 template <class T, int TR, bool DOT> __global__ void __launch_bounds__(32 * TR, (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1))
-k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __restrict__ ec, const T* __restrict__ g,
-        T* __restrict__ eo, int nx, int ny, int nz, T ce, T cw, T cn, T zs, Scalars* S_, double* partials) {
+k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __restrict__ ec, const T* __restrict__ g_a,
+        const T* __restrict__ g_b, T* __restrict__ eo, int nx, int ny, int nz, T ce, T cw, T cn, T zs, Scalars* S_, double* partials) {
   using V = typename V2T<T>::type;
   constexpr int PL = MgTile<TR>::PL;
   if (done && *done) return;
+  const T* __restrict__ g = (g_b && S_->rsel) ? g_b : g_a;      // current residual buffer (k_mg_down<UPD> toggles rsel)
   extern __shared__ __align__(16) unsigned char mg_smem[];
   T* AX = reinterpret_cast<T*>(mg_smem); T* AY = AX + 2 * PL; T* BX = AY + 2 * PL; T* BY = BX + 2 * PL;
   __shared__ double sh[32]; __shared__ int flag;
@@ -239,47 +289,53 @@ template <class K> static void allow_smem(K kernel, size_t bytes) {
   cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-template <class T, int TR> static void down_tr(const Ctx<T>& c, const T* g, T* e, T* gc, int nx, int ny, int nz, T cg, T cn, T ih2, cudaStream_t s) {
+template <class T, int TR, bool UPD> static void down_tr(const Ctx<T>& c, const T* g, T* g2, const T* q, T* e, T* gc, int nx, int ny, int nz,
+                                                         T cg, T cn, T ih2, const Launch& L) {
   const MgGeom G = mg_geom(nx, ny, nz, MgTile<TR>::IY, slots_per_sm<T, TR>());
   const size_t smem = 8 * (size_t)MgTile<TR>::PL * sizeof(T);
   static bool once = false;
-  if (!once) { allow_smem(k_mg_down<T, TR>, smem); once = true; }
-  k_mg_down<T, TR><<<G.grid, dim3(32, TR), smem, s>>>(&c.S->done, g, e, gc, nx, ny, nz, cg, cn, ih2);
+  if (!once) { allow_smem(k_mg_down<T, TR, UPD>, smem); once = true; }
+  k_mg_down<T, TR, UPD><<<G.grid, dim3(32, TR), smem, L.s>>>(&c.S->done, g, g2, q, e, gc, nx, ny, nz, cg, cn, ih2, c.S, c.partials, L);
 }
-template <class T, int TR, bool DOT> static void up_tr(const Ctx<T>& c, const T* ein, const T* ec, const T* g, T* eo, int nx, int ny, int nz,
+template <class T, int TR, bool DOT> static void up_tr(const Ctx<T>& c, const T* ein, const T* ec, const T* g, const T* g2, T* eo, int nx, int ny, int nz,
                                                        T ce, T cw, T cn, T zs, cudaStream_t s) {
   const MgGeom G = mg_geom(nx, ny, nz, MgTile<TR>::IY, slots_per_sm<T, TR>());
   const size_t smem = 8 * (size_t)MgTile<TR>::PL * sizeof(T);
   static bool once = false;
   if (!once) { allow_smem(k_mg_up<T, TR, DOT>, smem); once = true; }
-  k_mg_up<T, TR, DOT><<<G.grid, dim3(32, TR), smem, s>>>(&c.S->done, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, c.S, c.partials);
+  k_mg_up<T, TR, DOT><<<G.grid, dim3(32, TR), smem, s>>>(&c.S->done, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, c.S, c.partials);
 }
 
+// upd: level 0 inside PCG with the residual update of the previous iteration fused in (g2 = the other residual
+// buffer, q = A d); the launch then moves 4.125 words per cell (r, q in; r, e, gc out)
 template <class T> int launch_mg_down(const Ctx<T>& c, const T* g, T* e, T* gc, int nx, int ny, int nz, double h, double omega,
-                                      const char* name, const Launch& L) {
+                                      const char* name, const Launch& L, bool upd, T* g2, const T* q) {
   const double N = (double)nx * ny * nz;
   const double ih2 = 1.0 / (h * h), cw = omega * h * h / 6.0;
   const T cg = T(2.0 * cw - 6.0 * cw * cw * ih2), cn = T(cw * cw * ih2);
-  if (mg_tr() == 16) FS_LAUNCH(L, name, 2.125 * sizeof(T) * N, down_tr<T, 16>(c, g, e, gc, nx, ny, nz, cg, cn, T(ih2), L.s));
-  else FS_LAUNCH(L, name, 2.125 * sizeof(T) * N, down_tr<T, 8>(c, g, e, gc, nx, ny, nz, cg, cn, T(ih2), L.s));
+  const bool big = mg_tr() == 16;
+  FS_LAUNCH(L, name, (upd ? 4.125 : 2.125) * sizeof(T) * N, {
+    if (upd) { if (big) down_tr<T, 16, true>(c, g, g2, q, e, gc, nx, ny, nz, cg, cn, T(ih2), L); else down_tr<T, 8, true>(c, g, g2, q, e, gc, nx, ny, nz, cg, cn, T(ih2), L); }
+    else { if (big) down_tr<T, 16, false>(c, g, nullptr, nullptr, e, gc, nx, ny, nz, cg, cn, T(ih2), L); else down_tr<T, 8, false>(c, g, nullptr, nullptr, e, gc, nx, ny, nz, cg, cn, T(ih2), L); }
+  });
   return 1;
 }
 template <class T> int launch_mg_up(const Ctx<T>& c, const T* ein, const T* ec, const T* g, T* eo, int nx, int ny, int nz, double h,
-                                    double omega, bool dot, T zs, const char* name, const Launch& L) {
+                                    double omega, bool dot, T zs, const char* name, const Launch& L, const T* g2) {
   const double N = (double)nx * ny * nz;
   const double ih2d = 1.0 / (h * h), cwd = omega * h * h / 6.0;
   const T ce = T(1.0 - 6.0 * cwd * ih2d), cw = T(cwd), cn = T(cwd * ih2d);
   const bool big = mg_tr() == 16;
   FS_LAUNCH(L, name, 3.125 * sizeof(T) * N, {
-    if (big) { if (dot) up_tr<T, 16, true>(c, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 16, false>(c, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
-    else { if (dot) up_tr<T, 8, true>(c, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 8, false>(c, ein, ec, g, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
+    if (big) { if (dot) up_tr<T, 16, true>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 16, false>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
+    else { if (dot) up_tr<T, 8, true>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 8, false>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
   });
   return 1;
 }
 
 #define INST(T)                                                                                                              \
-  template int launch_mg_down<T>(const Ctx<T>&, const T*, T*, T*, int, int, int, double, double, const char*, const Launch&); \
-  template int launch_mg_up<T>(const Ctx<T>&, const T*, const T*, const T*, T*, int, int, int, double, double, bool, T, const char*, const Launch&);
+  template int launch_mg_down<T>(const Ctx<T>&, const T*, T*, T*, int, int, int, double, double, const char*, const Launch&, bool, T*, const T*); \
+  template int launch_mg_up<T>(const Ctx<T>&, const T*, const T*, const T*, T*, int, int, int, double, double, bool, T, const char*, const Launch&, const T*);
 INST(float)
 INST(double)
 

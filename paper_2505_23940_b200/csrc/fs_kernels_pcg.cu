@@ -72,7 +72,7 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_init(const Ctx<T
     if (threadIdx.x == 0 && threadIdx.y == 0) {
       Scalars* S = c.S;
       S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
-      S->iter = 0; S->first = 1; S->dsel = 0; S->pending = 0;
+      S->iter = 0; S->first = 1; S->dsel = 0; S->pending = 0; S->rsel = 0; S->need_update = 0;
       S->rmean = v[3] / ((double)c.nx * c.ny * c.nz);
       const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
       S->converged = conv; S->done = conv || S->max_iter <= 0;
@@ -166,7 +166,7 @@ template <class T, int PC> __global__ void __launch_bounds__(kDaTX * kDaTY, 2) k
   const double wy = c.dy64[j];
   double v3[3] = {v[0], sp * wy, sd * wy};
   if (grid_sum<3>(v3, c.partials, &c.S->ticket[0], sh, &flag)) {
-    if (tx == 0 && ty == 0) { c.S->dq = v3[0]; c.S->sum_p = v3[1]; c.S->sum_d = v3[2]; }
+    if (tx == 0 && ty == 0) { c.S->dq = v3[0]; c.S->sum_p = v3[1]; c.S->sum_d = v3[2]; c.S->need_update = 1; }
   }
 }
 
@@ -287,7 +287,7 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
   const double wy = c.dy64[sy];
   double v[3] = {dot, sp * wy, sd * wy};
   if (grid_sum<3>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
-    if (lane == 0 && ty == 0) { c.S->dq = v[0]; c.S->sum_p = v[1]; c.S->sum_d = v[2]; }
+    if (lane == 0 && ty == 0) { c.S->dq = v[0]; c.S->sum_p = v[1]; c.S->sum_d = v[2]; c.S->need_update = 1; }
   }
 }
 
@@ -429,7 +429,7 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
   const double wy = c.dy64[sy];
   double v[3] = {dot, sp * wy, sd * wy};
   if (grid_sum<3>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
-    if (lane == 0 && ty == 0) { c.S->dq = v[0]; c.S->sum_p = v[1]; c.S->sum_d = v[2]; }
+    if (lane == 0 && ty == 0) { c.S->dq = v[0]; c.S->sum_p = v[1]; c.S->sum_d = v[2]; c.S->need_update = 1; }
   }
 }
 
@@ -539,7 +539,7 @@ template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaT
     if (lane == 0 && ty == 0) {
       Scalars* S = c.S;
       S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
-      S->iter = 0; S->first = 1; S->dsel = 0; S->pending = 0;
+      S->iter = 0; S->first = 1; S->dsel = 0; S->pending = 0; S->rsel = 0; S->need_update = 0;
       S->rmean = v[3] / ((double)c.nx * c.ny * c.nz);
       const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
       S->converged = conv; S->done = conv || S->max_iter <= 0;
@@ -649,11 +649,12 @@ template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L, bool ne
 template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;
   int n = 0;
+  bool upd_fused = false;                  // K2 done by the level-0 down kernel of the NEXT iteration (k_mg_down<UPD>)
   T zs = T(1);
   if (c.precond == FS_PC_GMG) {
     zs = T(1.0 / c.hy);
     bool fused = false;
-    n += launch_vcycle<T>(c, mg, c.r, c.z, L, &fused, zs);
+    n += launch_vcycle<T>(c, mg, c.r, c.z, L, &fused, zs, &upd_fused);
     if (!fused) { FS_LAUNCH(L, "pcg_dot_rz", 2.0 * sizeof(T) * N, k_dot_rz<T><<<flat_blocks(N), 256, 0, L.s>>>(c, zs)); ++n; }
   }
   if (sizeof(T) == 8 && c.nx % 2 == 0) {
@@ -678,6 +679,7 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
     else FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
     ++n;
   }
+  if (upd_fused) return n;
   if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_update_norm", 3.0 * sizeof(T) * N, k_pcg_update<T, true><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
   else FS_LAUNCH(L, "pcg_update_norm", 3.0 * sizeof(T) * N, k_pcg_update<T, false><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
   ++n;
