@@ -291,9 +291,9 @@ def run_ours(a):
     # ---- CPU oracle on a bounded sample (rank 0, N=1 only) ----
     cpu = None
     if not a.no_cpu and rank == 0 and world == 1:
-        v, dt, _ = oracle_sample(a.ref_n, 3)
+        v, dt, _ = oracle_sample(a.ref_n, 6)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": "c5 HIT replica %d^3, 3 steps, %.1f s (single-threaded fp64 C++ oracle)" % (a.ref_n, dt)}
+               "sample": "c5 HIT replica %d^3, 6 steps, %.1f s (single-threaded fp64 C++ oracle)" % (a.ref_n, dt)}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,

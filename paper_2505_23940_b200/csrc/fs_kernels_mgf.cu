@@ -13,7 +13,6 @@
 // patch is smaller -- profiles/).  One __syncthreads per plane.  Each later stage is valid on a tile one
 // cell smaller per side (overlapped tiling: 64 x 2TR extended tile -> 60 x (2TR-4) results); the halo
 // re-reads hit L2.  All grids are periodic (GMG is only offered for triply periodic boxes).
-#include <cstdlib>
 #include "fs_internal.cuh"
 
 namespace fs {
@@ -278,12 +277,8 @@ k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __rest
   }
 }
 
-// Tile height: TR thread rows (2 TR cell rows).  fp64 patches need ~128 registers per thread.
-static int mg_tr() {
-  static int tr = 0;
-  if (!tr) { const char* e = getenv("FS_MG_TR"); tr = (e && atoi(e) == 16) ? 16 : 8; }
-  return tr;
-}
+// Tile height: TR thread rows (2 TR cell rows; 16 on big levels: fewer halo rows per result, 8 below: more CTAs).
+static int mg_tr(int ny) { return ny >= 256 ? 16 : 8; }
 template <class T, int TR> static int slots_per_sm() { return (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1); }
 template <class K> static void allow_smem(K kernel, size_t bytes) {
   cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -313,7 +308,7 @@ template <class T> int launch_mg_down(const Ctx<T>& c, const T* g, T* e, T* gc, 
   const double N = (double)nx * ny * nz;
   const double ih2 = 1.0 / (h * h), cw = omega * h * h / 6.0;
   const T cg = T(2.0 * cw - 6.0 * cw * cw * ih2), cn = T(cw * cw * ih2);
-  const bool big = mg_tr() == 16;
+  const bool big = mg_tr(ny) == 16;
   FS_LAUNCH(L, name, (upd ? 4.125 : 2.125) * sizeof(T) * N, {
     if (upd) { if (big) down_tr<T, 16, true>(c, g, g2, q, e, gc, nx, ny, nz, cg, cn, T(ih2), L); else down_tr<T, 8, true>(c, g, g2, q, e, gc, nx, ny, nz, cg, cn, T(ih2), L); }
     else { if (big) down_tr<T, 16, false>(c, g, nullptr, nullptr, e, gc, nx, ny, nz, cg, cn, T(ih2), L); else down_tr<T, 8, false>(c, g, nullptr, nullptr, e, gc, nx, ny, nz, cg, cn, T(ih2), L); }
@@ -325,7 +320,7 @@ template <class T> int launch_mg_up(const Ctx<T>& c, const T* ein, const T* ec, 
   const double N = (double)nx * ny * nz;
   const double ih2d = 1.0 / (h * h), cwd = omega * h * h / 6.0;
   const T ce = T(1.0 - 6.0 * cwd * ih2d), cw = T(cwd), cn = T(cwd * ih2d);
-  const bool big = mg_tr() == 16;
+  const bool big = mg_tr(ny) == 16;
   FS_LAUNCH(L, name, 3.125 * sizeof(T) * N, {
     if (big) { if (dot) up_tr<T, 16, true>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 16, false>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
     else { if (dot) up_tr<T, 8, true>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 8, false>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
