@@ -278,7 +278,7 @@ k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __rest
 }
 
 // Tile height: TR thread rows (2 TR cell rows; 16 on big levels: fewer halo rows per result, 8 below: more CTAs).
-static int mg_tr(int ny) { return ny >= 256 ? 16 : 8; }
+static int mg_tr(int ny) { return ny >= 384 ? 16 : 8; }
 template <class T, int TR> static int slots_per_sm() { return (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1); }
 template <class K> static void allow_smem(K kernel, size_t bytes) {
   cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
