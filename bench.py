@@ -41,6 +41,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--n", type=int, default=512, help="cells per direction of the HIT box (c5: 512)")
+    ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5"],
+                    help="c5 (default) is the metric's configuration; c1-c4 are the small, L2-resident parity configs "
+                         "(launch/latency bound: reported for context in profiles/, fp64 only)")
     ap.add_argument("--ref-n", type=int, default=128, help="replica size the CPU oracle is timed on")
     ap.add_argument("--exec", dest="exec_mode", default="graph", choices=["graph", "stream"],
                     help="graph: one CUDA-graph replay per step (default); stream: same kernels launched directly (for ncu)")
@@ -186,9 +189,12 @@ def run_ours(a):
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
     n = a.n
-    cells = n ** 3
     wbytes = 8 if a.dtype == "f64" else 4
-    cfg = W.hit(n=n, dtype=a.dtype, device=dev, exec_mode=a.exec_mode)   # seeded IC, built with torch FFT on the device
+    if a.workload == "c5":
+        cfg = W.hit(n=n, dtype=a.dtype, device=dev, exec_mode=a.exec_mode)   # seeded IC, built with torch FFT on the device
+    else:
+        cfg = W.make(a.workload, dtype=a.dtype, exec_mode=a.exec_mode)
+    cells = cfg["nx"] * cfg["ny"] * cfg["nz"]
     g = fs.from_workload(cfg, device=dev)
     cfg["init"] = None
     torch.cuda.empty_cache()
@@ -274,7 +280,7 @@ def run_ours(a):
         step_s = ms / a.steps * 1e-3
         # SURVEY 8(d) model of the UNFUSED formulation: 25 + 29.4 N_it words per cell-step (GMG-PCG)
         nit = sum(v["launches"] for k, v in prof.items() if k == "pcg_dir_apply_dot") / ksteps
-        unfused_bytes = (25.0 + 29.4 * nit) * wbytes * cells
+        unfused_bytes = (25.0 + (29.4 if cfg["precond"] == "gmg" else 11.0) * nit) * wbytes * cells
         roof = {"bound": "hbm", "kernel": top[0], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": ncu_traffic(a.dtype, top[0]), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": top[1]["bytes"] / top[1]["launches"],
@@ -299,9 +305,10 @@ def run_ours(a):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
                 "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": a.dtype, "data": "synthetic",
-                "config": {"workload": "c5 decaying HIT %d^3 triply periodic, AB2, GMG-PCG rtol 1e-8 (BASELINE.json configs[4])" % n,
+                "config": {"workload": ("c5 decaying HIT %d^3 triply periodic, AB2, GMG-PCG rtol 1e-8 (BASELINE.json configs[4])" % n) if a.workload == "c5"
+                           else "%s %dx%dx%d (BASELINE.json configs[%d]; small L2-resident case, context only)" % (cfg["name"], cfg["nx"], cfg["ny"], cfg["nz"], int(a.workload[1]) - 1),
                            "cells": cells, "parallelism": "replicas x%d (no sharding)" % world,
-                           "l2": "inputs larger than L2 (each field %.0f MB vs 126 MB L2)" % (cells * wbytes / 1e6),
+                           "l2": ("inputs larger than L2 (each field %.0f MB vs 126 MB L2)" if cells * wbytes > 126e6 else "fields of %.0f MB: L2 resident, no flush (context run)") % (cells * wbytes / 1e6),
                            "pcg_iters_last_step": info["pcg_iters"], "rel_residual": info["rel_residual"],
                            "true_rel_residual": info["true_rel_residual"], "max_abs_div": info["max_abs_div"],
                            "converged": info["converged"], "nan_flag": info["nan_flag"],
