@@ -28,7 +28,7 @@ class _Params(C.Structure):
                 ("time_scheme", C.c_int),
                 ("precond", C.c_int), ("rtol", C.c_double), ("max_iter", C.c_int), ("warm_start", C.c_int),
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
-                ("delta", C.c_int), ("seed", C.c_uint64), ("inflow_noise", C.c_double)]
+                ("delta", C.c_int), ("seed", C.c_uint64), ("inflow_noise", C.c_double), ("convection", C.c_int)]
 
 
 class _Info(C.Structure):
@@ -116,6 +116,7 @@ class Oracle:
         P.time_scheme = TIME[cfg["time_scheme"]]
         P.precond = PC[cfg["precond"]]
         P.delta = DELTA[cfg["delta"]]
+        P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
         self.h = L.orc_create(C.byref(P))
         if not self.h:
             raise ValueError("oracle: invalid parameters")

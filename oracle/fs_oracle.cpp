@@ -89,6 +89,13 @@ static inline double interpY(const orc_sim* s, double a, double b, int jf) {
 
 // ---- O2: momentum right-hand side H = -C + nu*Lap(u) + g -----------------------------------
 // (Eq. 4: divergence form; central convection and diffusion, L100)
+// Convection variant of L100 / Table 1 (L444-447), "first-order upwind" (reading N3-1): in every
+// convective flux a*phi the advecting face velocity a keeps its central / linear interpolation and the
+// transported value phi is the one on the upwind side of the face, phi = a > 0 ? phi_minus : phi_plus
+// (ghost values come from the same boundary accessors as in the central scheme).
+static inline double TR(const orc_sim* s, double a, double minus, double plus, double central) {
+  return s->P.convection == ORC_CONV_UPWIND ? (a > 0.0 ? minus : plus) : central;
+}
 static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& ww,
                      double nu, const double g[3], vec& HU, vec& HV, vec& HW) {
   const int nx = s->nx, ny = s->ny, nz = s->nz;
@@ -98,12 +105,12 @@ static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& 
   for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = s->bx; i < nx; ++i) {
     double uc = U_(i, j, k);
     double ue = 0.5 * (uc + U_(i + 1, j, k)), uw = 0.5 * (U_(i - 1, j, k) + uc);
-    double cx = (ue * ue - uw * uw) / hx;
-    double vn = 0.5 * (V_(i - 1, j + 1, k) + V_(i, j + 1, k)), un = interpY(s, uc, U_(i, j + 1, k), j + 1);
-    double vs = 0.5 * (V_(i - 1, j, k) + V_(i, j, k)),         us = interpY(s, U_(i, j - 1, k), uc, j);
+    double cx = (ue * TR(s, ue, uc, U_(i + 1, j, k), ue) - uw * TR(s, uw, U_(i - 1, j, k), uc, uw)) / hx;
+    double vn = 0.5 * (V_(i - 1, j + 1, k) + V_(i, j + 1, k)), un = TR(s, vn, uc, U_(i, j + 1, k), interpY(s, uc, U_(i, j + 1, k), j + 1));
+    double vs = 0.5 * (V_(i - 1, j, k) + V_(i, j, k)),         us = TR(s, vs, U_(i, j - 1, k), uc, interpY(s, U_(i, j - 1, k), uc, j));
     double cy = (vn * un - vs * us) / s->dy[j];
-    double wt = 0.5 * (W_(i - 1, j, k + 1) + W_(i, j, k + 1)), ut = 0.5 * (uc + U_(i, j, k + 1));
-    double wb = 0.5 * (W_(i - 1, j, k) + W_(i, j, k)),         ub = 0.5 * (U_(i, j, k - 1) + uc);
+    double wt = 0.5 * (W_(i - 1, j, k + 1) + W_(i, j, k + 1)), ut = TR(s, wt, uc, U_(i, j, k + 1), 0.5 * (uc + U_(i, j, k + 1)));
+    double wb = 0.5 * (W_(i - 1, j, k) + W_(i, j, k)),         ub = TR(s, wb, U_(i, j, k - 1), uc, 0.5 * (U_(i, j, k - 1) + uc));
     double cz = (wt * ut - wb * ub) / hz;
     double dxx = (U_(i + 1, j, k) - 2.0 * uc + U_(i - 1, j, k)) / (hx * hx);
     double dyy = ((U_(i, j + 1, k) - uc) / DYC(s, j + 1) - (uc - U_(i, j - 1, k)) / DYC(s, j)) / s->dy[j];
@@ -113,13 +120,13 @@ static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& 
   // v faces (control volume between y_c(j-1) and y_c(j), height DYC(j))
   for (int k = 0; k < nz; ++k) for (int j = s->by; j < ny; ++j) for (int i = 0; i < nx; ++i) {
     double vc = V_(i, j, k);
-    double ue = interpY(s, U_(i + 1, j - 1, k), U_(i + 1, j, k), j), ve = 0.5 * (vc + V_(i + 1, j, k));
-    double uw = interpY(s, U_(i, j - 1, k), U_(i, j, k), j),         vw = 0.5 * (V_(i - 1, j, k) + vc);
+    double ue = interpY(s, U_(i + 1, j - 1, k), U_(i + 1, j, k), j), ve = TR(s, ue, vc, V_(i + 1, j, k), 0.5 * (vc + V_(i + 1, j, k)));
+    double uw = interpY(s, U_(i, j - 1, k), U_(i, j, k), j),         vw = TR(s, uw, V_(i - 1, j, k), vc, 0.5 * (V_(i - 1, j, k) + vc));
     double cx = (ue * ve - uw * vw) / hx;
     double vn = 0.5 * (vc + V_(i, j + 1, k)), vs = 0.5 * (V_(i, j - 1, k) + vc);
-    double cy = (vn * vn - vs * vs) / DYC(s, j);
-    double wt = interpY(s, W_(i, j - 1, k + 1), W_(i, j, k + 1), j), vt = 0.5 * (vc + V_(i, j, k + 1));
-    double wb = interpY(s, W_(i, j - 1, k), W_(i, j, k), j),         vb = 0.5 * (V_(i, j, k - 1) + vc);
+    double cy = (vn * TR(s, vn, vc, V_(i, j + 1, k), vn) - vs * TR(s, vs, V_(i, j - 1, k), vc, vs)) / DYC(s, j);
+    double wt = interpY(s, W_(i, j - 1, k + 1), W_(i, j, k + 1), j), vt = TR(s, wt, vc, V_(i, j, k + 1), 0.5 * (vc + V_(i, j, k + 1)));
+    double wb = interpY(s, W_(i, j - 1, k), W_(i, j, k), j),         vb = TR(s, wb, V_(i, j, k - 1), vc, 0.5 * (V_(i, j, k - 1) + vc));
     double cz = (wt * vt - wb * vb) / hz;
     double dxx = (V_(i + 1, j, k) - 2.0 * vc + V_(i - 1, j, k)) / (hx * hx);
     double dyy = ((V_(i, j + 1, k) - vc) / DY(s, j) - (vc - V_(i, j - 1, k)) / DY(s, j - 1)) / DYC(s, j);
@@ -129,14 +136,14 @@ static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& 
   // w faces
   for (int k = s->bz; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
     double wc = W_(i, j, k);
-    double ue = 0.5 * (U_(i + 1, j, k - 1) + U_(i + 1, j, k)), we = 0.5 * (wc + W_(i + 1, j, k));
-    double uw = 0.5 * (U_(i, j, k - 1) + U_(i, j, k)),         wwst = 0.5 * (W_(i - 1, j, k) + wc);
+    double ue = 0.5 * (U_(i + 1, j, k - 1) + U_(i + 1, j, k)), we = TR(s, ue, wc, W_(i + 1, j, k), 0.5 * (wc + W_(i + 1, j, k)));
+    double uw = 0.5 * (U_(i, j, k - 1) + U_(i, j, k)),         wwst = TR(s, uw, W_(i - 1, j, k), wc, 0.5 * (W_(i - 1, j, k) + wc));
     double cx = (ue * we - uw * wwst) / hx;
-    double vn = 0.5 * (V_(i, j + 1, k - 1) + V_(i, j + 1, k)), wn = interpY(s, wc, W_(i, j + 1, k), j + 1);
-    double vs = 0.5 * (V_(i, j, k - 1) + V_(i, j, k)),         ws = interpY(s, W_(i, j - 1, k), wc, j);
+    double vn = 0.5 * (V_(i, j + 1, k - 1) + V_(i, j + 1, k)), wn = TR(s, vn, wc, W_(i, j + 1, k), interpY(s, wc, W_(i, j + 1, k), j + 1));
+    double vs = 0.5 * (V_(i, j, k - 1) + V_(i, j, k)),         ws = TR(s, vs, W_(i, j - 1, k), wc, interpY(s, W_(i, j - 1, k), wc, j));
     double cy = (vn * wn - vs * ws) / s->dy[j];
     double wt = 0.5 * (wc + W_(i, j, k + 1)), wb = 0.5 * (W_(i, j, k - 1) + wc);
-    double cz = (wt * wt - wb * wb) / hz;
+    double cz = (wt * TR(s, wt, wc, W_(i, j, k + 1), wt) - wb * TR(s, wb, W_(i, j, k - 1), wc, wb)) / hz;
     double dxx = (W_(i + 1, j, k) - 2.0 * wc + W_(i - 1, j, k)) / (hx * hx);
     double dyy = ((W_(i, j + 1, k) - wc) / DYC(s, j + 1) - (wc - W_(i, j - 1, k)) / DYC(s, j)) / s->dy[j];
     double dzz = (W_(i, j, k + 1) - 2.0 * wc + W_(i, j, k - 1)) / (hz * hz);

@@ -26,6 +26,7 @@ enum { ORC_BC_PERIODIC = 0, ORC_BC_NOSLIP = 1, ORC_BC_SLIP = 2, ORC_BC_INFLOW = 
 enum { ORC_TIME_EULER = 0, ORC_TIME_AB2 = 1 };
 enum { ORC_PC_NONE = 0, ORC_PC_JACOBI = 1, ORC_PC_GMG = 2 };
 enum { ORC_DELTA_ROMA3 = 0, ORC_DELTA_PESKIN4 = 1 };
+enum { ORC_CONV_CENTRAL = 0, ORC_CONV_UPWIND = 1 };   /* 2nd-order central or 1st-order upwind convection */
 enum { ORC_U = 0, ORC_V, ORC_W, ORC_P, ORC_HU, ORC_HV, ORC_HW, ORC_DIV };
 
 typedef struct {
@@ -40,6 +41,7 @@ typedef struct {
   int mg_nu1, mg_nu2, mg_coarse_sweeps; double mg_omega;
   int delta;
   uint64_t seed; double inflow_noise;
+  int convection;            /* ORC_CONV_* */
 } orc_params;
 
 typedef struct {
