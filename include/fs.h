@@ -55,6 +55,9 @@ typedef enum { FS_DELTA_ROMA3 = 0, FS_DELTA_PESKIN4 = 1 } fs_delta;        /* Eq
 typedef enum { FS_EXEC_GRAPH = 0,   /* one CUDA-graph replay per step, PCG loop = conditional WHILE node */
                FS_EXEC_STREAM = 1   /* same kernels launched directly; host polls the PCG flag (debug) */
              } fs_exec;
+typedef enum { FS_CONV_CENTRAL = 0,  /* 2nd-order central convective fluxes (the default of every config) */
+               FS_CONV_UPWIND = 1    /* 1st-order upwind: transported value from the upwind side of each face (L100, Table 1) */
+             } fs_conv;
 typedef enum { FS_U = 0, FS_V, FS_W, FS_P, FS_HU, FS_HV, FS_HW, FS_DIV,
                FS_MARKER_X,      /* n*3 fp64 positions */
                FS_MARKER_U,      /* n*3 fp64 target velocities U^b */
@@ -80,6 +83,7 @@ typedef struct {
   fs_delta delta; int max_markers;
   uint64_t seed; double inflow_noise;
   fs_exec exec_mode;
+  fs_conv convection;          /* convective flux scheme of the momentum RHS */
 } fs_params;
 
 typedef struct {

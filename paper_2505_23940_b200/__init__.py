@@ -47,7 +47,7 @@ class fs_params(C.Structure):
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
                 ("delta", C.c_int), ("max_markers", C.c_int),
                 ("seed", C.c_uint64), ("inflow_noise", C.c_double),
-                ("exec_mode", C.c_int)]
+                ("exec_mode", C.c_int), ("convection", C.c_int)]
 
 
 class fs_step_info(C.Structure):
@@ -149,6 +149,7 @@ def make_params(cfg):
     P.precond = PC[cfg["precond"]]
     P.delta = DELTA[cfg["delta"]]
     P.exec_mode = EXEC[cfg.get("exec_mode", "graph")]
+    P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
     return P, keep
 
 

@@ -98,6 +98,7 @@ fs_status validate(const fs_params* p) {
   if ((long long)(p->nx + 1) * (p->ny + 1) * (p->nz + 1) > (1LL << 31) - 1) return FS_ERR_UNSUPPORTED;   // int32 cell keys, 32-bit field offsets
   if ((long long)((p->nx + 29) / 30) * ((p->ny + 3) / 4) > kMaxPartials) return FS_ERR_UNSUPPORTED;   // one reduction partial per xy tile
   if (p->yf) for (int j = 0; j < p->ny; ++j) if (!(p->yf[j + 1] > p->yf[j])) return FS_ERR_INVALID_ARG;
+  if ((int)p->convection < 0 || (int)p->convection > 1) return FS_ERR_INVALID_ARG;
   if ((int)p->precond < 0 || (int)p->precond > 2 || (int)p->delta < 0 || (int)p->delta > 1) return FS_ERR_INVALID_ARG;
   if (p->precond == FS_PC_GMG) {
     const double hx = p->lx / p->nx, hy = p->ly / p->ny, hz = p->lz / p->nz;
@@ -221,7 +222,7 @@ template <class T> fs_status upload_metrics(fs_grid* g) {
   c.ihx = (T)(1.0 / g->hx); c.ihz = (T)(1.0 / g->hz);
   c.ihx2 = (T)(1.0 / (g->hx * g->hx)); c.ihz2 = (T)(1.0 / (g->hz * g->hz));
   c.time_scheme = (int)P.time_scheme; c.precond = (int)P.precond; c.warm_start = P.warm_start; c.delta = (int)P.delta;
-  c.uniform_y = g->uniform_y; c.seed = P.seed; c.inflow_noise = P.inflow_noise;
+  c.uniform_y = g->uniform_y; c.convection = (int)P.convection; c.seed = P.seed; c.inflow_noise = P.inflow_noise;
   return FS_OK;
 }
 

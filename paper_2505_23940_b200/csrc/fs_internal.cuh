@@ -50,7 +50,7 @@ template <class T> struct Ctx {
   double hx, hy, hz, dt, rho, nu, g[3];
   double x0, y0, z0;
   T ihx, ihz, ihx2, ihz2;
-  int time_scheme, precond, warm_start, delta, uniform_y;
+  int time_scheme, precond, warm_start, delta, uniform_y, convection;
   uint64_t seed; double inflow_noise;
   // y metrics (device arrays of T unless noted)
   const T* dy;     // [ny+2]: dy[j+1] = DY(j), j in [-1, ny] (mirrored ghost at walls, wrapped if periodic)

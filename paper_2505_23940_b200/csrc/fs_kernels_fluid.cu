@@ -87,6 +87,12 @@ template <class T> __device__ __forceinline__ T boundary_normal(const Ctx<T>& c,
 // ---------------------------------------------------------------------------------------------------
 constexpr int kMomTX = 32, kMomTY = 10;
 
+// transported face value of a convective flux a * phi: central interpolation, or (first-order upwind, PAPER.md L100;
+// DESIGN.md reading N3-1) the value on the upwind side of the face
+template <class T> __device__ __forceinline__ T transported(bool upwind, T a, T minus, T plus, T central) {
+  return upwind ? (a > T(0) ? minus : plus) : central;
+}
+
 template <class T> struct ColRef { unsigned off, pl; T A, B; };   // 32-bit element offsets: every field has < 2^32 entries (validated)   // value = A f[off + pl kz] + B  (x, y ghosts resolved)
 
 template <class T, int C> __device__ __forceinline__ ColRef<T> col_setup(const Ctx<T>& c, int i, int j) {
@@ -130,7 +136,7 @@ template <class T, int C> __device__ __forceinline__ T col_load(const Ctx<T>& c,
   return col_fix<T, C>(c, r, kk, col_raw<T, C>(c, f, r, kk));
 }
 
-template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momentum(const Ctx<T> c, int kz) {
+template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momentum(const Ctx<T> c, int kz) {
   __shared__ T SU[4][kMomTY][kMomTX], SV[4][kMomTY][kMomTX], SW[4][kMomTY][kMomTX];
   const int tx = threadIdx.x, ty = threadIdx.y;
   const int iu = blockIdx.x * (kMomTX - 2) + tx - 1, ju = blockIdx.y * (kMomTY - 2) + ty - 1;   // may be -1 or past the box
@@ -140,6 +146,7 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
   const bool ab2 = c.time_scheme == FS_TIME_AB2 && c.S->have_hist;
   const T a0 = ab2 ? T(1.5) : T(1), a1 = ab2 ? T(-0.5) : T(0);
   const T dt = T(c.dt), nu = T(c.nu);
+  constexpr bool upw = UPW;                // convective scheme: compile-time, so the central path carries no selects
   const T* __restrict__ U = c.u; const T* __restrict__ V = c.v; const T* __restrict__ W = c.w;
   const ColRef<T> ru = col_setup<T, 0>(c, i, j), rv = col_setup<T, 1>(c, i, j), rw = col_setup<T, 2>(c, i, j);
   // y metrics of the tile rows, in shared memory (j clamped into the tables; unused rows never store)
@@ -191,12 +198,12 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
         } else {
           const T uE = SU[s1][ty][txp], uW = SU[s1][ty][txm], uN = SU[s1][typ][tx], uS = SU[s1][tym][tx];
           const T ue = T(0.5) * (uc + uE), uw = T(0.5) * (uW + uc);
-          const T cx = (ue * ue - uw * uw) * c.ihx;
-          const T vnn = T(0.5) * (SV[s1][typ][txm] + SV[s1][typ][tx]), unn = wyl1 * uc + wyh1 * uN;
-          const T vss = T(0.5) * (SV[s1][ty][txm] + vc),                uss = wyl0 * uS + wyh0 * uc;
+          const T cx = (ue * transported<T>(upw, ue, uc, uE, ue) - uw * transported<T>(upw, uw, uW, uc, uw)) * c.ihx;
+          const T vnn = T(0.5) * (SV[s1][typ][txm] + SV[s1][typ][tx]), unn = transported<T>(upw, vnn, uc, uN, wyl1 * uc + wyh1 * uN);
+          const T vss = T(0.5) * (SV[s1][ty][txm] + vc),                uss = transported<T>(upw, vss, uS, uc, wyl0 * uS + wyh0 * uc);
           const T cy = (vnn * unn - vss * uss) * idyj;
-          const T wt = T(0.5) * (SW[s2][ty][txm] + wT), ut = T(0.5) * (uc + uT);
-          const T wb = T(0.5) * (SW[s1][ty][txm] + wc), ub = T(0.5) * (uB + uc);
+          const T wt = T(0.5) * (SW[s2][ty][txm] + wT), ut = transported<T>(upw, wt, uc, uT, T(0.5) * (uc + uT));
+          const T wb = T(0.5) * (SW[s1][ty][txm] + wc), ub = transported<T>(upw, wb, uB, uc, T(0.5) * (uB + uc));
           const T cz = (wt * ut - wb * ub) * c.ihz;
           const T dxx = (uE - T(2) * uc + uW) * c.ihx2;
           const T dyy = ((uN - uc) * idyc1 - (uc - uS) * idyc0) * idyj;
@@ -217,13 +224,13 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
         } else {
           const T vE = SV[s1][ty][txp], vW = SV[s1][ty][txm], vN = SV[s1][typ][tx], vS = SV[s1][tym][tx];
           const T wl = wyl0, wh = wyh0;
-          const T ue = wl * SU[s1][tym][txp] + wh * SU[s1][ty][txp], ve = T(0.5) * (vc + vE);
-          const T uw = wl * SU[s1][tym][tx] + wh * uc,               vw = T(0.5) * (vW + vc);
+          const T ue = wl * SU[s1][tym][txp] + wh * SU[s1][ty][txp], ve = transported<T>(upw, ue, vc, vE, T(0.5) * (vc + vE));
+          const T uw = wl * SU[s1][tym][tx] + wh * uc,               vw = transported<T>(upw, uw, vW, vc, T(0.5) * (vW + vc));
           const T cx = (ue * ve - uw * vw) * c.ihx;
           const T vnn = T(0.5) * (vc + vN), vss = T(0.5) * (vS + vc);
-          const T cy = (vnn * vnn - vss * vss) * idyc0;
-          const T wt = wl * SW[s2][tym][tx] + wh * wT, vt = T(0.5) * (vc + vT);
-          const T wb = wl * SW[s1][tym][tx] + wh * wc, vb = T(0.5) * (vB + vc);
+          const T cy = (vnn * transported<T>(upw, vnn, vc, vN, vnn) - vss * transported<T>(upw, vss, vS, vc, vss)) * idyc0;
+          const T wt = wl * SW[s2][tym][tx] + wh * wT, vt = transported<T>(upw, wt, vc, vT, T(0.5) * (vc + vT));
+          const T wb = wl * SW[s1][tym][tx] + wh * wc, vb = transported<T>(upw, wb, vB, vc, T(0.5) * (vB + vc));
           const T cz = (wt * vt - wb * vb) * c.ihz;
           const T dxx = (vE - T(2) * vc + vW) * c.ihx2;
           const T dyy = ((vN - vc) * idyj - (vc - vS) * idyjm) * idyc0;
@@ -244,14 +251,14 @@ template <class T> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momen
           c.hw[q] = T(0);
         } else {
           const T wE = SW[s1][ty][txp], wW = SW[s1][ty][txm], wN = SW[s1][typ][tx], wS = SW[s1][tym][tx];
-          const T ue = T(0.5) * (SU[s0][ty][txp] + SU[s1][ty][txp]), we = T(0.5) * (wc + wE);
-          const T uw = T(0.5) * (uB + uc),                           ww = T(0.5) * (wW + wc);
+          const T ue = T(0.5) * (SU[s0][ty][txp] + SU[s1][ty][txp]), we = transported<T>(upw, ue, wc, wE, T(0.5) * (wc + wE));
+          const T uw = T(0.5) * (uB + uc),                           ww = transported<T>(upw, uw, wW, wc, T(0.5) * (wW + wc));
           const T cx = (ue * we - uw * ww) * c.ihx;
-          const T vnn = T(0.5) * (SV[s0][typ][tx] + SV[s1][typ][tx]), wnn = wyl1 * wc + wyh1 * wN;
-          const T vss = T(0.5) * (vB + vc),                           wss = wyl0 * wS + wyh0 * wc;
+          const T vnn = T(0.5) * (SV[s0][typ][tx] + SV[s1][typ][tx]), wnn = transported<T>(upw, vnn, wc, wN, wyl1 * wc + wyh1 * wN);
+          const T vss = T(0.5) * (vB + vc),                           wss = transported<T>(upw, vss, wS, wc, wyl0 * wS + wyh0 * wc);
           const T cy = (vnn * wnn - vss * wss) * idyj;
           const T wt = T(0.5) * (wc + wT), wb = T(0.5) * (wB + wc);
-          const T cz = (wt * wt - wb * wb) * c.ihz;
+          const T cz = (wt * transported<T>(upw, wt, wc, wT, wt) - wb * transported<T>(upw, wb, wB, wc, wb)) * c.ihz;
           const T dxx = (wE - T(2) * wc + wW) * c.ihx2;
           const T dyy = ((wN - wc) * idyc1 - (wc - wS) * idyc0) * idyj;
           const T dzz = (wT - T(2) * wc + wB) * c.ihz2;
@@ -271,7 +278,8 @@ template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
   int kz = c.nzw;
   while (kz > 16 && (long long)bxn * byn * ((c.nzw + kz - 1) / kz) < 4LL * 148 * 2) kz = (kz + 1) / 2;
   dim3 b(kMomTX, kMomTY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
-  FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T><<<g, b, 0, L.s>>>(c, kz));
+  if (c.convection == FS_CONV_UPWIND) FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, true><<<g, b, 0, L.s>>>(c, kz));
+  else FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, false><<<g, b, 0, L.s>>>(c, kz));
   return 1;
 }
 

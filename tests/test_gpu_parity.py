@@ -99,6 +99,29 @@ def test_momentum_rhs_elementwise(fs, kind):
     g.close()
 
 
+@pytest.mark.parametrize("kind", ["periodic", "channel", "open"])
+def test_momentum_rhs_upwind_elementwise(fs, kind):
+    # NEXT-3: first-order upwind convective fluxes (random fields: both signs of every advecting velocity)
+    cfg = {"periodic": _cfg_periodic(72, 38, 21, convection="upwind"), "channel": _cfg_channel(40, 50, 19, convection="upwind"),
+           "open": _cfg_open(70, 27, 22, inflow_noise=0.05, seed=3, convection="upwind")}[kind]
+    cfg["init"] = _rand_fields(cfg, 12)
+    ref = _oracle(cfg).momentum_rhs()
+    g = fs.from_workload(cfg)
+    got = g.momentum_rhs()
+    for c, a, b in zip("uvw", got, ref):
+        assert relerr(a, b) < 1e-12, (kind, c, relerr(a, b))
+    g.close()
+
+
+def test_upwind_full_steps_match_oracle(fs):
+    cfg = W.taylor_green(n=24, convection="upwind")
+    g, o, ig, io, _ = _run_pair(fs, cfg, 6)
+    g.close()
+    cfg = W.channel(n=24, convection="upwind", steps=4)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 4)
+    g.close()
+
+
 # ------------------------------------------------------------------------------------ S6/S7 Poisson
 @pytest.mark.parametrize("kind,pc", [("periodic", "none"), ("periodic", "jacobi"), ("periodic", "gmg"),
                                      ("channel", "jacobi"), ("open", "jacobi"), ("open", "none")])
