@@ -331,6 +331,21 @@ def test_c4_cylinder_fsi_reduced_50_steps(fs):
     g.close()
 
 
+def test_two_dof_rigid_body_fsi_reduced(fs):
+    # SURVEY 8(f) NEXT-2, first item: the 2-DOF (in-line + transverse) oscillator of Eq. 12,
+    # with damping, weak coupling; the body moves in x and y and its cell list is rebuilt every step
+    cfg = W.cylinder_fsi(scale=4, per_ring=40)
+    m, _, k, _ = cfg["body"]
+    cfg["body"] = (m, 0.3, k, 3)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 30)
+    assert abs(io["body_disp"][0]) > 0 and abs(io["body_disp"][1]) > 0 and io["body_disp"][2] == 0
+    np.testing.assert_allclose(ig["body_disp"], io["body_disp"], rtol=1e-9, atol=1e-15)
+    np.testing.assert_allclose(ig["body_vel"], io["body_vel"], rtol=1e-9, atol=1e-15)
+    np.testing.assert_allclose(ig["body_force"], io["body_force"], rtol=1e-9, atol=1e-12)
+    assert relerr(g.get("marker_x"), o.markers()[0]) < 1e-14
+    g.close()
+
+
 def test_c5_hit_64_fp64_10_steps(fs):
     cfg = W.hit(n=64)
     g, o, ig, io, _ = _run_pair(fs, cfg, 10)
