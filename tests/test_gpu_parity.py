@@ -203,6 +203,34 @@ def test_gmg_vcycle_elementwise(fs, dims):
     g.close()
 
 
+@pytest.mark.parametrize("nu", [(1, 1, 16), (3, 2, 8), (0, 2, 4), (2, 2, 0)])
+def test_gmg_vcycle_other_smoothing_counts(fs, nu):
+    # V(nu1, nu2) other than the fused V(2,2) fast path: the generic per-sweep kernels (fs_kernels_mg.cu), incl. nu1 = 0
+    # (no pre-smoothing: restriction of the bare right-hand side) and no coarsest-level sweeps
+    cfg = _cfg_periodic(48, 32, 40, precond="gmg", mg_nu1=nu[0], mg_nu2=nu[1], mg_coarse_sweeps=nu[2])
+    rng = np.random.default_rng(3)
+    r = rng.standard_normal(W.shapes(cfg)["p"])
+    z_ref = _oracle(cfg).vcycle(r)
+    g = fs.Grid(cfg)
+    z = g.gmg_vcycle(r)
+    assert relerr(z, z_ref) < 1e-12, (nu, relerr(z, z_ref))
+    g.close()
+
+
+def test_gmg_pcg_with_v11_cycle_matches_oracle(fs):
+    # PCG around the generic V-cycle: separate r.z and update kernels (no fused update, no second residual buffer)
+    h = 2 * math.pi / 48
+    cfg = _cfg_periodic(48, 32, 40, precond="gmg", rtol=1e-10, warm_start=0, mg_nu1=1, mg_nu2=1)
+    cfg.update(lx=48 * h, ly=32 * h, lz=40 * h)
+    rhs = np.random.default_rng(5).standard_normal(W.shapes(cfg)["p"])
+    p_ref, iref = _oracle(cfg).poisson_solve(rhs)
+    g = fs.Grid(cfg)
+    p, info = g.poisson_solve(rhs)
+    assert info["converged"] == 1 and abs(info["iters"] - iref["pcg_iters"]) <= 1, (info, iref)
+    assert relerr(p, p_ref) < TOL64
+    g.close()
+
+
 # ------------------------------------------------------------------------------------ S2-S5 IBM
 def _markers(cfg, n, seed, spread_cells=6.0):
     rng = np.random.default_rng(seed)
