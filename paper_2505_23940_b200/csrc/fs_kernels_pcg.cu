@@ -207,10 +207,16 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
   const T cyl = c.cyl[sy], cyh = c.cyh[sy], idy = c.idy[sy + 1], ndy = -c.dy[sy + 1];
   const T ihx2 = c.ihx2, ihz2 = c.ihz2;
   T dgx = T(0), dgy = T(0);                // Jacobi: x + y parts of diag A / dy for the two cells
+  T ivx_i = T(0), ivx_b = T(0), ivy_i = T(0), ivy_b = T(0);
   if (PC == 1) {
     const T dyy = (cyh + cyl) * idy;
     dgx = T((c.bx && sx == 0 ? 0 : 1) + 1) * ihx2 + dyy;
     dgy = T(1 + (c.bx && sx + 1 == c.nx - 1 ? 0 : 1)) * ihx2 + dyy;
+    // reciprocal diagonals for the two kinds of plane (one or two z neighbours): one division per thread instead
+    // of one per cell and plane; z = r * (1 / diag) differs from the oracle's r / diag by at most one rounding
+    const T dyj_ = c.dy[sy + 1];
+    ivx_i = T(1) / ((dgx + T(2) * ihz2) * dyj_); ivx_b = T(1) / ((dgx + T(1) * ihz2) * dyj_);
+    ivy_i = T(1) / ((dgy + T(2) * ihz2) * dyj_); ivy_b = T(1) / ((dgy + T(1) * ihz2) * dyj_);
   }
   const int own_o = ty * 32 + lane;
   const int oS = (ty > 0 ? ty - 1 : 0) * 32 + lane, oN = (ty < kDaTY - 1 ? ty + 1 : ty) * 32 + lane;
@@ -233,8 +239,8 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
     V z;
     if (PC == 2) { z.x = rz.x * zs; z.y = rz.y * zs; }
     else if (PC == 1) {
-      const T dzz = T((c.bz && ksrc == 0 ? 0 : 1) + (c.bz && ksrc == c.nz - 1 ? 0 : 1)) * ihz2;
-      z.x = rz.x / ((dgx + dzz) * c.dy[sy + 1]); z.y = rz.y / ((dgy + dzz) * c.dy[sy + 1]);
+      const bool zb = c.bz && (ksrc == 0 || ksrc == c.nz - 1);
+      z.x = rz.x * (zb ? ivx_b : ivx_i); z.y = rz.y * (zb ? ivy_b : ivy_i);
     } else z = rz;
     V d = z;
     if (!first) { d.x = z.x + beta * rd.x; d.y = z.y + beta * rd.y; }
@@ -329,11 +335,14 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
   const unsigned pl = (unsigned)c.nx * c.ny, row = (unsigned)sx + (unsigned)c.nx * sy;
   const T cyl = c.cyl[sy], cyh = c.cyh[sy], idy = c.idy[sy + 1], dyj = c.dy[sy + 1], ndy = -dyj;
   const T ihx2 = c.ihx2, ihz2 = c.ihz2;
-  T dg[VX];                                 // Jacobi: x + y parts of diag A / dy per cell
+  T dg[VX], ivi[VX], ivb[VX];               // Jacobi: x + y parts of diag A / dy per cell, reciprocal diagonals
 #pragma unroll
   for (int a = 0; a < VX; ++a) {
     const int i = sx + a;
     dg[a] = PC == 1 ? T((c.bx && i == 0 ? 0 : 1) + (c.bx && i == c.nx - 1 ? 0 : 1)) * ihx2 + (cyh + cyl) * idy : T(0);
+    // reciprocal diagonals for planes with two / one z neighbours (see k_pcg_dirapply2)
+    ivi[a] = PC == 1 ? T(1) / ((dg[a] + T(2) * ihz2) * dyj) : T(1);
+    ivb[a] = PC == 1 ? T(1) / ((dg[a] + T(1) * ihz2) * dyj) : T(1);
   }
   const int o_own = ty * ROWE + lane * VX;
   const int o_s = (ty > 0 ? ty - 1 : 0) * ROWE + lane * VX, o_n = (ty < kDaTY - 1 ? ty + 1 : ty) * ROWE + lane * VX;
@@ -356,13 +365,12 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
   };
   auto make = [&]() {                       // d' of the fetched plane
     W d;
-    T dzz = T(0);
-    if (PC == 1) dzz = T((c.bz && ksrc == 0 ? 0 : 1) + (c.bz && ksrc == c.nz - 1 ? 0 : 1)) * ihz2;
+    const bool zb = PC == 1 && c.bz && (ksrc == 0 || ksrc == c.nz - 1);
 #pragma unroll
     for (int a = 0; a < VX; ++a) {
       T z;
       if (PC == 2) z = rz.a[a] * zs;
-      else if (PC == 1) z = rz.a[a] / ((dg[a] + dzz) * dyj);
+      else if (PC == 1) z = rz.a[a] * (zb ? ivb[a] : ivi[a]);
       else z = rz.a[a];
       d.a[a] = first ? z : z + beta * rd.a[a];
     }
@@ -463,11 +471,14 @@ template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaT
   const T cyl = c.cyl[sy], cyh = c.cyh[sy], idy = c.idy[sy + 1], dyj = c.dy[sy + 1], ndy = -dyj;
   const T ihx2 = c.ihx2, ihz2 = c.ihz2;
   const T shift = T(c.S->mean_coef) * dyj;
-  T dg[VX];
+  T dg[VX], ivi[VX], ivb[VX];
 #pragma unroll
   for (int a = 0; a < VX; ++a) {
     const int i = sx + a;
     dg[a] = PC == 1 ? T((c.bx && i == 0 ? 0 : 1) + (c.bx && i == c.nx - 1 ? 0 : 1)) * ihx2 + (cyh + cyl) * idy : T(0);
+    // reciprocal diagonals for planes with two / one z neighbours (see k_pcg_dirapply2)
+    ivi[a] = PC == 1 ? T(1) / ((dg[a] + T(2) * ihz2) * dyj) : T(1);
+    ivb[a] = PC == 1 ? T(1) / ((dg[a] + T(1) * ihz2) * dyj) : T(1);
   }
   const int o_own = ty * ROWE + lane * VX;
   const int o_s = (ty > 0 ? ty - 1 : 0) * ROWE + lane * VX, o_n = (ty < kDaTY - 1 ? ty + 1 : ty) * ROWE + lane * VX;
@@ -503,7 +514,7 @@ template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaT
     const W Sv = ld16<T>(P + o_s), Nv = ld16<T>(P + o_n);
     const T xw0 = P[o_w], xeL = P[o_e];
     if (own) {
-      const T dzz = PC == 1 ? T((c.bz && k == 0 ? 0 : 1) + (c.bz && k == c.nz - 1 ? 0 : 1)) * ihz2 : T(0);
+      const bool zb = PC == 1 && c.bz && (k == 0 || k == c.nz - 1);
       W r, bh;
       T s0 = T(0), s1 = T(0), s2 = T(0), s3 = T(0);
 #pragma unroll
@@ -516,7 +527,7 @@ template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaT
         acc += (dT.a[a] - xc) * ihz2 - (xc - dB.a[a]) * ihz2;
         bh.a[a] = rcur.a[a] - shift;
         r.a[a] = bh.a[a] - acc * ndy;
-        const T z = PC == 1 ? r.a[a] / ((dg[a] + dzz) * dyj) : r.a[a];
+        const T z = PC == 1 ? r.a[a] * (zb ? ivb[a] : ivi[a]) : r.a[a];
         s0 += bh.a[a] * bh.a[a]; s1 += r.a[a] * r.a[a]; s2 += r.a[a] * z; s3 += r.a[a];
       }
       const unsigned o = row + pl * (unsigned)k;
@@ -632,25 +643,27 @@ template <class T, int PC> __global__ void __launch_bounds__(256) k_pcg_updatev(
   if (gx < c.nx && gy < c.ny) {
     const unsigned pl = (unsigned)c.nx * c.ny, o0 = (unsigned)gx + (unsigned)c.nx * gy;
     const T dyj = c.dy[gy + 1];
-    T dg[VX];
+    T dg[VX], ivi[VX], ivb[VX];
 #pragma unroll
     for (int a = 0; a < VX; ++a) {
       const int i = gx + a;
       dg[a] = PC == 1 ? T((c.bx && i == 0 ? 0 : 1) + (c.bx && i == c.nx - 1 ? 0 : 1)) * c.ihx2 + (c.cyh[gy] + c.cyl[gy]) * c.idy[gy + 1] : T(0);
+      ivi[a] = PC == 1 ? T(1) / ((dg[a] + T(2) * c.ihz2) * dyj) : T(1);
+      ivb[a] = PC == 1 ? T(1) / ((dg[a] + T(1) * c.ihz2) * dyj) : T(1);
     }
 #pragma unroll 2
     for (int k = k0; k < k1; ++k) {
       const unsigned o = o0 + pl * (unsigned)k;
       W r = ld16<T>(c.r + o);
       const W q = ld16<T>(c.q + o);
-      const T dzz = PC == 1 ? T((c.bz && k == 0 ? 0 : 1) + (c.bz && k == c.nz - 1 ? 0 : 1)) * c.ihz2 : T(0);
+      const bool zb = PC == 1 && c.bz && (k == 0 || k == c.nz - 1);
       T s0 = T(0), s1 = T(0), s2 = T(0);
 #pragma unroll
       for (int a = 0; a < VX; ++a) {
         T t = r.a[a] - alpha * q.a[a];
         if (sizeof(T) == 4) t -= rm;
         r.a[a] = t;
-        const T z = PC == 1 ? t / ((dg[a] + dzz) * dyj) : t;
+        const T z = PC == 1 ? t * (zb ? ivb[a] : ivi[a]) : t;
         s0 += t * t; s1 += t * z; s2 += t;
       }
       st16<T>(c.r + o, r);
