@@ -75,6 +75,21 @@ def test_workspace_bytes_and_validation_on_host(fs):
     Pb, keep = fs.make_params(dict(ch, precond="gmg"))
     assert L.fs_workspace_bytes(C.byref(Pb), C.byref(n)) == 6
     assert L.fs_workspace_bytes(None, C.byref(n)) == 1
+    # convection scheme out of range; a grid with more xy tiles than reduction partials; 32-bit field offsets
+    Pb, _ = fs.make_params(cfg); Pb.convection = 2
+    assert L.fs_workspace_bytes(C.byref(Pb), C.byref(n)) == 1
+    Pb, _ = fs.make_params(dict(cfg, nx=4096, ny=1024, nz=2))
+    assert L.fs_workspace_bytes(C.byref(Pb), C.byref(n)) == 6
+    Pb, _ = fs.make_params(dict(cfg, nx=2048, ny=1024, nz=1024))
+    assert L.fs_workspace_bytes(C.byref(Pb), C.byref(n)) == 6
+    # GMG V(2,2) carries the second residual buffer of the fused update; other V(nu1,nu2) do not
+    h = W.hit(n=32, device="cpu"); h["init"] = None
+    n22, n11 = C.c_size_t(0), C.c_size_t(0)
+    Pg, _ = fs.make_params(h)
+    assert L.fs_workspace_bytes(C.byref(Pg), C.byref(n22)) == 0
+    Pg, _ = fs.make_params(dict(h, mg_nu1=1, mg_nu2=1))
+    assert L.fs_workspace_bytes(C.byref(Pg), C.byref(n11)) == 0
+    assert 32 ** 3 * 8 <= n22.value - n11.value <= 32 ** 3 * 8 + 512
     assert L.fs_status_string(6) == b"unsupported configuration"
     # NULL handles never crash
     assert L.fs_grid_destroy(None) == 1 and L.fs_step(None, 1, None) == 1
