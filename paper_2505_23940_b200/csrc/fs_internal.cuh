@@ -100,6 +100,25 @@ struct Launch { cudaStream_t s; cudaGraphConditionalHandle cond; int use_cond; P
     if ((L).prof) prof_end((L).prof, (L).s);                        \
   } while (0)
 
+
+// z chunk length of a streaming kernel: xy tiles x chunks CTAs run in waves of `slots` (CTAs resident on the
+// 148 SMs); every chunk marches its planes plus `halo` redundant ones.  Pick the chunk count that minimises
+// waves x planes per chunk (a half-empty last wave costs as much as a full one), chunks of at least min_kz
+// planes, at most kMaxPartials CTAs (one reduction partial each).
+inline int pick_kz(long long tiles_xy, int nz, long long slots, int halo, int min_kz) {
+  int best = nz; double best_cost = 1e300;
+  for (int zc = 1; zc <= nz; ++zc) {
+    const int kz = (nz + zc - 1) / zc;
+    if (zc > 1 && kz < min_kz) break;
+    if ((nz + kz - 1) / kz != zc) continue;              // same chunk count as a smaller zc: already seen
+    if (tiles_xy * zc > kMaxPartials) break;
+    const long long waves = (tiles_xy * zc + slots - 1) / slots;
+    const double cost = (double)waves * (kz + halo);
+    if (cost < best_cost * 0.999) { best_cost = cost; best = kz; }
+  }
+  return best;
+}
+
 // ---- launchers (one per kernel family; each returns the number of kernels it enqueued) ----------
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_flux_correction(const Ctx<T>& c, const Launch& L);

@@ -275,8 +275,7 @@ template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
   const int bxn = (c.nxu + kMomTX - 3) / (kMomTX - 2), byn = (c.nyv + kMomTY - 3) / (kMomTY - 2);
   // z chunks: >= 4 waves of CTAs (2 CTAs of 320 threads per SM) while chunks stay >= 16 planes
-  int kz = c.nzw;
-  while (kz > 16 && (long long)bxn * byn * ((c.nzw + kz - 1) / kz) < 4LL * 148 * 2) kz = (kz + 1) / 2;
+  const int kz = pick_kz((long long)bxn * byn, c.nzw, 2LL * 148, 2, 16);
   dim3 b(kMomTX, kMomTY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
   if (c.convection == FS_CONV_UPWIND) FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, true><<<g, b, 0, L.s>>>(c, kz));
   else FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, false><<<g, b, 0, L.s>>>(c, kz));
@@ -679,8 +678,7 @@ ColGeom col_geom(int nx, int ny, int nz) {
 template <class T> int launch_project(const Ctx<T>& c, const Launch& L) {
   if (!c.bx && c.nx % Vec16<T>::VX == 0) {
     const int bxn = (c.nx + 30 * Vec16<T>::VX - 1) / (30 * Vec16<T>::VX), byn = (c.nyv + PjTile<T>::TY - 3) / (PjTile<T>::TY - 2);
-    int kz = c.nzw;
-    while (kz > 16 && (long long)bxn * byn * ((c.nzw + kz - 1) / kz) < 4LL * 296) kz = (kz + 1) / 2;
+    const int kz = pick_kz((long long)bxn * byn, c.nzw, 2LL * 148, 1, 16);
     FS_LAUNCH(L, "project", 7.0 * sizeof(T) * c.nx * c.ny * c.nz,
               k_projectv<T><<<dim3(bxn, byn, (c.nzw + kz - 1) / kz), dim3(32, PjTile<T>::TY), 0, L.s>>>(c, kz));
     return 1;

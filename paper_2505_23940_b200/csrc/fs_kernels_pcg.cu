@@ -299,8 +299,7 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
 
 static DaGeom da2_geom(int nx, int ny, int nz) {
   const int bxn = (nx + kDa2IX - 1) / kDa2IX, byn = (ny + kDa2IY - 1) / kDa2IY;
-  int kz = nz;
-  while (kz > 16 && (long long)bxn * byn * ((nz + kz - 1) / kz) < 4LL * 296) kz = (kz + 1) / 2;
+  const int kz = pick_kz((long long)bxn * byn, nz, 2LL * 148, 2, 16);
   DaGeom g; g.kz = kz; g.grid = dim3(bxn, byn, (nz + kz - 1) / kz);
   return g;
 }
@@ -444,8 +443,7 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
 template <class T> static DaGeom dav_geom(int nx, int ny, int nz) {
   const int ix = 30 * Vec16<T>::VX;
   const int bxn = (nx + ix - 1) / ix, byn = (ny + kDaVIY - 1) / kDaVIY;
-  int kz = nz;
-  while (kz > 16 && (long long)bxn * byn * ((nz + kz - 1) / kz) < 4LL * 296) kz = (kz + 1) / 2;
+  const int kz = pick_kz((long long)bxn * byn, nz, 2LL * 148, 2, 16);
   DaGeom g; g.kz = kz; g.grid = dim3(bxn, byn, (nz + kz - 1) / kz);
   return g;
 }
