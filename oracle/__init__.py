@@ -154,6 +154,8 @@ class Oracle:
         d = _f64(dvol).reshape(-1) if dvol is not None else None
         rc = lib().orc_set_markers(self.h, n, _dp(xyz), _dp(v) if v is not None else None,
                                    _dp(d) if d is not None else None)
+        if rc == 2:
+            raise ValueError("oracle: unsupported -- a marker support touches a non-periodic boundary")
         if rc:
             raise ValueError("oracle: set_markers failed")
         self.nl = n
@@ -179,7 +181,9 @@ class Oracle:
     def step(self, nsteps=1):
         info = _Info()
         iters = np.zeros(nsteps, dtype=np.int32)
-        lib().orc_step(self.h, nsteps, C.byref(info), _ip(iters))
+        rc = lib().orc_step(self.h, nsteps, C.byref(info), _ip(iters))
+        if rc == 2:
+            raise ValueError("oracle: unsupported -- a marker support touches a non-periodic boundary")
         d = info_dict(info)
         d["iters_per_step"] = iters.tolist()
         return d
@@ -215,6 +219,12 @@ class Oracle:
     def momentum_rhs(self):
         g = [np.empty(self.shape[c]) for c in "uvw"]
         lib().orc_momentum_rhs(self.h, _dp(g[0]), _dp(g[1]), _dp(g[2])); return g
+
+    def predict(self, stage):
+        """Predicted field without advancing the state: stage 0 after O3, 1 after O4 (IBM), 2 after O5."""
+        g = [np.empty(self.shape[c]) for c in "uvw"]
+        assert lib().orc_predict(self.h, int(stage), _dp(g[0]), _dp(g[1]), _dp(g[2])) == 0
+        return g
 
     def convection(self):
         g = [np.empty(self.shape[c]) for c in "uvw"]

@@ -6,9 +6,12 @@
 // Triple loops, explicit index wrapping, sums in index order, no blocking / fusion / threads.
 // Compile: g++ -O2 -ffp-contract=off (no FMA contraction, so index arithmetic is reproducible).
 //
-// Pins (tests/test_oracle_*.py, -m "not gpu"): P1..P15 of SURVEY.md 8(c).
-// Parity unpinned (readings of formulas the paper does not give):
-//   convective outflow update, outflow flux correction, inflow noise  -- only mass balance is pinned.
+// Pins (tests/test_oracle_*.py, -m "not gpu"): P1..P17 of SURVEY.md 8(c) / DESIGN.md 4 and P18..P23
+// (tests/test_oracle_boundary.py): slip / no-slip / inflow / outflow tangential ghosts, the convective outflow
+// update, the direct-forcing scale of I-3 / I-4, the uniform outflow flux shift, rejection of supports that reach a
+// non-periodic boundary, and the inflow-noise hash (published SplitMix64 vectors + frozen table).
+// Parity unpinned: no function.  The convective-outflow formula, the flux correction and the hash chaining are
+// READINGS of what the paper leaves open: the pins fix what the oracle computes, not the paper's intent.
 #include "fs_oracle.h"
 #include <cmath>
 #include <cstdlib>
@@ -30,6 +33,7 @@ struct orc_sim {
   // markers (always fp64)
   int nl; vec X, Ub, dV, Fl, Ul;       // positions, target vel, volumes, force, interpolated vel
   std::vector<int> base, perm, keys, seg; int nseg;
+  bool oob;                            // a support reached a prescribed face / left a bounded box (unsupported)
   // body (Eq. 12)
   bool has_body; double bm, bc_, bk; int dof; double bdisp[3], bvel[3], bforce[3];
   // GMG levels
@@ -256,6 +260,10 @@ extern "C" void orc_ibm_index(orc_sim* s) {
   for (int l = 0; l < nl; ++l) {
     for (int c = 0; c < 3; ++c) for (int d = 0; d < 3; ++d)
       s->base[((size_t)c * nl + l) * 3 + d] = support_base(s, scaled_coord(s, s->X[3 * l + d], c, d));
+    // a support that reaches a non-periodic boundary is unsupported (the delta-kernel moment
+    // identities P8-P10 do not hold for a truncated support); flagged here, reported by orc_set_markers / orc_step
+    for (int c = 0; c < 3; ++c) for (int d = 0; d < 3; ++d) for (int a = 0; a < support_width(s); ++a)
+      if (node_index(s, s->base[((size_t)c * nl + l) * 3 + d] + a, c, d) < 0) s->oob = true;
     int ic[3];
     for (int d = 0; d < 3; ++d) {
       double t = s->X[3 * l + d] - o[d];
@@ -527,14 +535,16 @@ extern "C" void orc_rk4_body(double m, double c, double k, double F, double dt, 
   *wd = y1 + dt / 6.0 * (k1b + 2.0 * k2b + 2.0 * k3b + k4b);
 }
 
-// ---- one fractional step (O1..O9 in order) -----------------------------------------------------
-static void one_step(orc_sim* s, orc_info* info) {
+// ---- O1..O5: the predicted field ----------------------------------------------------------------
+// upto = 0: after O3 (explicit predictor + prescribed boundary-normal faces), 1: after O4 (IBM direct forcing),
+// 2: after O5 (outflow flux correction).  one_step uses upto = 2; orc_predict exposes the intermediate stages so the
+// tests can pin O1 (convective outflow), I-3/I-4 (forcing scale) and O5 (uniform shift) one by one.
+static void predictor(orc_sim* s, int upto, vec& us, vec& vs, vec& ws, vec& HU, vec& HV, vec& HW) {
   const double dt = s->P.dt, rho = s->P.rho;
-  vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size());
   momentum(s, s->u, s->v, s->w, s->P.nu, s->P.body_force, HU, HV, HW);                 // O1+O2
   double a0 = 1.0, a1 = 0.0;
   if (s->P.time_scheme == ORC_TIME_AB2 && s->have_hist) { a0 = 1.5; a1 = -0.5; }
-  vec us = s->u, vs = s->v, ws = s->w;                                                 // O3
+  us = s->u; vs = s->v; ws = s->w;                                                     // O3
   for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = s->bx; i < s->nx; ++i) {
     size_t q = IU(s, i, j, k); us[q] = s->u[q] + dt * (a0 * HU[q] + a1 * s->hu[q]); }
   for (int k = 0; k < s->nz; ++k) for (int j = s->by; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i) {
@@ -543,6 +553,7 @@ static void one_step(orc_sim* s, orc_info* info) {
     size_t q = IW(s, i, j, k); ws[q] = s->w[q] + dt * (a0 * HW[q] + a1 * s->hw[q]); }
   set_boundary_normal(s, us, vs, ws, s->u, s->v, s->w);
   for (int c = 0; c < 3; ++c) s->bforce[c] = 0.0;
+  if (upto < 1) return;
   if (s->nl > 0) {                                                                     // O4
     orc_ibm_index(s);                                                                  // I-1
     interpolate(s, us, vs, ws, s->Ul);                                                 // I-2
@@ -556,7 +567,15 @@ static void one_step(orc_sim* s, orc_info* info) {
     for (size_t q = 0; q < vs.size(); ++q) vs[q] += dt * fv[q];
     for (size_t q = 0; q < ws.size(); ++q) ws[q] += dt * fw[q];
   }
+  if (upto < 2) return;
   flux_correction(s, us, vs, ws);                                                      // O5
+}
+
+// ---- one fractional step (O1..O9 in order) -----------------------------------------------------
+static void one_step(orc_sim* s, orc_info* info) {
+  const double dt = s->P.dt, rho = s->P.rho;
+  vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size()), us, vs, ws;
+  predictor(s, 2, us, vs, ws, HU, HV, HW);                                             // O1..O5
   vec b(s->p.size());
   divergence(s, us, vs, ws, b);                                                        // O6
   for (size_t q = 0; q < b.size(); ++q) b[q] *= rho / dt;
@@ -615,7 +634,7 @@ extern "C" orc_sim* orc_create(const orc_params* p) {
   s->u.assign((size_t)s->nxu * s->ny * s->nz, 0.0); s->v.assign((size_t)s->nx * s->nyv * s->nz, 0.0);
   s->w.assign((size_t)s->nx * s->ny * s->nzw, 0.0); s->p.assign(N, 0.0); s->divu.assign(N, 0.0);
   s->hu = s->u; s->hv = s->v; s->hw = s->w;
-  s->have_hist = false; s->step = 0; s->nl = 0; s->nseg = 0; s->has_body = false; s->dof = 0;
+  s->have_hist = false; s->step = 0; s->nl = 0; s->nseg = 0; s->has_body = false; s->dof = 0; s->oob = false;
   for (int c = 0; c < 3; ++c) s->bdisp[c] = s->bvel[c] = s->bforce[c] = 0.0;
   return s;
 }
@@ -636,7 +655,9 @@ extern "C" int orc_set_markers(orc_sim* s, int n, const double* xyz, const doubl
   s->Ub.assign((size_t)3 * n, 0.0); if (vel) s->Ub.assign(vel, vel + (size_t)3 * n);
   s->dV.assign(n, s->hx * s->hy * s->hz); if (dvol) s->dV.assign(dvol, dvol + n);
   s->Fl.assign((size_t)3 * n, 0.0); s->Ul.assign((size_t)3 * n, 0.0);
+  s->oob = false;
   orc_ibm_index(s);
+  if (s->oob) { s->nl = 0; s->oob = false; return 2; }   // unsupported: marker support touches a non-periodic boundary
   return 0;
 }
 extern "C" int orc_set_body(orc_sim* s, double m, double c, double k, int dof) {
@@ -647,7 +668,7 @@ extern "C" int orc_step(orc_sim* s, int nsteps, orc_info* last, int* iters) {
   orc_info info; std::memset(&info, 0, sizeof info);
   for (int n = 0; n < nsteps; ++n) { one_step(s, &info); if (iters) iters[n] = info.pcg_iters; }
   if (last) *last = info;
-  return 0;
+  return s->oob ? 2 : 0;                                  // a moving body carried a support into a boundary
 }
 extern "C" int orc_poisson_solve(orc_sim* s, const double* rhs, double* p, orc_info* info) {
   size_t N = s->p.size(); vec b(rhs, rhs + N), x(p, p + N); orc_info I; std::memset(&I, 0, sizeof I);
@@ -669,6 +690,13 @@ extern "C" void orc_momentum_rhs(orc_sim* s, double* hu, double* hv, double* hw)
   vec a(s->u.size()), b(s->v.size()), c(s->w.size());
   momentum(s, s->u, s->v, s->w, s->P.nu, s->P.body_force, a, b, c);
   std::copy(a.begin(), a.end(), hu); std::copy(b.begin(), b.end(), hv); std::copy(c.begin(), c.end(), hw);
+}
+extern "C" int orc_predict(orc_sim* s, int stage, double* us, double* vs, double* ws) {
+  if (stage < 0 || stage > 2) return 1;
+  vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size()), a, b, c;
+  predictor(s, stage, a, b, c, HU, HV, HW);
+  std::copy(a.begin(), a.end(), us); std::copy(b.begin(), b.end(), vs); std::copy(c.begin(), c.end(), ws);
+  return 0;
 }
 extern "C" void orc_convection(orc_sim* s, double* cu, double* cv, double* cw) {
   vec a(s->u.size()), b(s->v.size()), c(s->w.size()); const double g0[3] = {0, 0, 0};

@@ -72,6 +72,10 @@ void orc_divergence(orc_sim*, const double* u, const double* v, const double* w,
 void orc_gradient(orc_sim*, const double* p, double* gu, double* gv, double* gw); /* 0 on boundary faces */
 void orc_momentum_rhs(orc_sim*, double* hu, double* hv, double* hw); /* H^n of current u,v,w */
 void orc_convection(orc_sim*, double* cu, double* cv, double* cw);   /* C only (nu=0, g=0) */
+/* The predicted field of the current state without advancing it: stage 0 = after O3 (predictor + prescribed
+ * boundary-normal faces, incl. the convective-outflow update), 1 = after O4 (IBM direct forcing, u*),
+ * 2 = after O5 (outflow flux correction).  Returns non-zero for an unknown stage. */
+int  orc_predict(orc_sim*, int stage, double* us, double* vs, double* ws);
 void orc_vcycle(orc_sim*, const double* r, double* z);          /* z = M^-1 r, GMG */
 void orc_jacobi_diag(orc_sim*, double* diag);
 /* IBM pieces: arrays sized by the current marker count n */
