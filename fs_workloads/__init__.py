@@ -195,5 +195,39 @@ def hit(n=512, seed=777, dtype="f64", device="cpu", **kw):
     return cfg
 
 
+def hit_box(nx, ny, nz, seed=778, dtype="f64", **kw):
+    """The c5 recipe on a non-cubic triply periodic box with isotropic spacing h = 2 pi / min(nx, ny, nz) (parity
+    cases that need a particular extent, e.g. ny >= 384 for the 32-row V-cycle tiles): random phases, the same
+    spectrum E(k) ~ k^4 exp(-2 (k/4)^2) in physical wavenumbers, exact discrete projection, u_rms = 1.  CPU only."""
+    import torch
+    nref = min(nx, ny, nz)
+    h = 2.0 * math.pi / nref
+    cfg = _base(name="c5_hit_box", nx=nx, ny=ny, nz=nz, lx=nx * h, ly=ny * h, lz=nz * h, nu=1e-3, dt=5e-4, precond="gmg",
+                rtol=1e-8, max_iter=200, steps=10, seed=seed, dtype=dtype)
+    cfg.update(kw)
+    g = torch.Generator(device="cpu")
+    g.manual_seed(seed)
+    kz = (torch.fft.fftfreq(nz, d=1.0 / nz, dtype=torch.float64) * (nref / nz))[:, None, None]
+    ky = (torch.fft.fftfreq(ny, d=1.0 / ny, dtype=torch.float64) * (nref / ny))[None, :, None]
+    kx = (torch.fft.rfftfreq(nx, d=1.0 / nx, dtype=torch.float64) * (nref / nx))[None, None, :]
+    kk = torch.sqrt(kx * kx + ky * ky + kz * kz)
+    amp = torch.where(kk > 0, torch.sqrt(kk ** 4 * torch.exp(-2.0 * (kk / 4.0) ** 2)) / torch.clamp(kk, min=1e-30), torch.zeros_like(kk))
+    spec = []
+    for _ in range(3):
+        f = torch.fft.rfftn(torch.randn((nz, ny, nx), generator=g, dtype=torch.float64))
+        spec.append(f / torch.clamp(f.abs(), min=1e-300) * amp)
+    ks = (kx, ky, kz)
+    Dd = [(torch.exp(1j * k * h) - 1.0) / h for k in ks]
+    Gd = [(1.0 - torch.exp(-1j * k * h)) / h for k in ks]
+    div = Dd[0] * spec[0] + Dd[1] * spec[1] + Dd[2] * spec[2]
+    lap = Dd[0] * Gd[0] + Dd[1] * Gd[1] + Dd[2] * Gd[2]
+    lap = torch.where(lap.abs() > 0, lap, torch.ones_like(lap))
+    phi = div / lap
+    out = [torch.fft.irfftn(spec[d] - Gd[d] * phi, s=(nz, ny, nx)) for d in range(3)]
+    rms = math.sqrt(float(sum((o * o).mean() for o in out)) / 3.0)
+    cfg["init"] = {c: (o / rms).contiguous().numpy() for c, o in zip("uvw", out)}
+    return cfg
+
+
 def make(name, **kw):
     return {"c1": taylor_green, "c2": channel, "c3": sphere, "c4": cylinder_fsi, "c5": hit}[name](**kw)

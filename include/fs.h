@@ -30,8 +30,13 @@
  *    fs_workspace_bytes() bytes (256-byte aligned) and the CUDA stream everything runs on; both
  *    must outlive the fs_grid.  The fs_grid host object (and its CUDA graphs) belongs to the
  *    library and is released by fs_grid_destroy.  All set calls copy; all get calls copy out.
+ *  - Device: a grid lives on the CUDA device that owns its workspace, which must be the caller's current device
+ *    when fs_grid_create is called (the stream belongs to it too).  Every later call makes that device current
+ *    for its duration and restores the caller's, so grids on several GPUs can be driven from one thread.
  *  - Errors: every call returns fs_status; nothing throws or aborts across the ABI; out-parameters
- *    are untouched on failure.
+ *    are untouched on failure.  Two documented exceptions, where the out-parameter IS filled because it
+ *    describes the failure: fs_step(..., last) returning FS_ERR_NOT_CONVERGED / FS_ERR_UNSUPPORTED, and
+ *    fs_poisson_solve(..., info) returning FS_ERR_NOT_CONVERGED.
  */
 #ifndef FS_H
 #define FS_H
@@ -93,15 +98,24 @@ typedef struct {
   double max_abs_div;         /* max |D u^{n+1}| */
   double body_force[3], body_disp[3], body_vel[3];
   long long step;
+  long long unconverged_steps;  /* sticky, since fs_grid_create: steps whose PCG hit max_iter ...            */
+  long long nan_steps;          /* ... and steps whose projected field held a NaN (also seen by async steps) */
 } fs_step_info;
 typedef struct { int iters; int converged; double rel_residual, true_rel_residual; } fs_poisson_info;
 
-/* Bytes of device workspace fs_grid_create needs for these parameters.  HOST pointers. */
+/* Bytes of device workspace fs_grid_create needs for these parameters: the fields of one fractional step (u, v, w,
+ * u*, H^{n-1}, p: Eq. 4-10), the PCG vectors of the Poisson solve (Eq. 7; CG L449), the
+ * GMG levels, and the marker arrays (Eq. 18 notation, L183-185).  HOST pointers.  FS_ERR_INVALID_ARG /
+ * FS_ERR_UNSUPPORTED as for fs_grid_create; *bytes untouched then. */
 fs_status fs_workspace_bytes(const fs_params* params, size_t* bytes);
 
-/* Creates a grid.  params: HOST.  workspace: DEVICE, >= fs_workspace_bytes, 256-byte aligned, owned
- * by the caller, zeroed by this call.  cuda_stream: a cudaStream_t (NULL = legacy default stream).
- * FS_ERR_UNSUPPORTED: GMG on a grid that is not uniform/isotropic/all-periodic. */
+/* Creates a grid: the staggered finite-volume arrangement of PAPER.md L100 (p at cell centres, velocity
+ * components on their faces; uniform, or y-stretched through params->yf) with the boundary types of Table 1
+ * (L429, L454-456).  params: HOST.  workspace: DEVICE memory of the CURRENT device, >= fs_workspace_bytes,
+ * 256-byte aligned, owned by the caller, zeroed by this call.  cuda_stream: a cudaStream_t of the current
+ * device (NULL = legacy default stream).  FS_ERR_INVALID_ARG: bad parameters, misaligned / too small / non-device
+ * workspace or one that belongs to another device.  FS_ERR_UNSUPPORTED: GMG on a grid that is not uniform /
+ * isotropic / all-periodic; more than 2^31 - 1 stored values per field. */
 fs_status fs_grid_create(const fs_params* params, void* workspace, size_t bytes, void* cuda_stream,
                          fs_grid** out);
 fs_status fs_grid_destroy(fs_grid* g);
@@ -109,8 +123,9 @@ fs_status fs_grid_destroy(fs_grid* g);
 /* Number of elements of a field (HOST out pointer). */
 fs_status fs_field_size(fs_grid* g, fs_field f, long long* count);
 
-/* Copy a whole field in / out.  src/dst is a HOST pointer when *_on_device == 0, else a DEVICE
- * pointer.  dtype applies to FS_U..FS_DIV (converted if it differs from the grid's); marker fields
+/* Copy a whole field of the solver state (u, v, w on faces, p at centres; H = the explicit right-hand
+ * side of Eq. 4; the marker arrays of Eq. 18) in / out.  src/dst is a HOST pointer when
+ * *_on_device == 0, else a DEVICE pointer.  dtype applies to FS_U..FS_DIV (converted if it differs from the grid's); marker fields
  * are fp64 / int32 regardless.  Synchronises the stream.  FS_DIV is computed on demand (get only). */
 fs_status fs_fields_set(fs_grid* g, fs_field f, const void* src, fs_dtype dtype, int src_on_device);
 fs_status fs_fields_get(fs_grid* g, fs_field f, void* dst, fs_dtype dtype, int dst_on_device);
@@ -120,8 +135,9 @@ fs_status fs_set_history(fs_grid* g, int have_history, long long step);
 
 /* Lagrangian markers (Eq. 18 notation: X_l, velocity, volume element dV_l; L183-185).  HOST
  * pointers, fp64: xyz n*3, vel n*3 (NULL = 0), dvol n (NULL = hx*hy*hz).  n = 0 removes them.
- * Rebuilds indices and the cell list.  FS_ERR_UNSUPPORTED on a y-stretched grid, n > max_markers
- * is FS_ERR_INVALID_ARG. */
+ * Rebuilds indices and the cell list.  FS_ERR_UNSUPPORTED on a y-stretched grid, and when the delta-function
+ * support of a marker (3 or 4 nodes per direction, Eq. 21-22) reaches a prescribed boundary-normal face or leaves
+ * the box in a non-periodic direction (the grid then keeps no markers); n > max_markers is FS_ERR_INVALID_ARG. */
 fs_status fs_set_ibm_markers(fs_grid* g, int n, const double* xyz, const double* vel, const double* dvol);
 fs_status fs_marker_segments(fs_grid* g, int* nseg);
 
@@ -130,9 +146,13 @@ fs_status fs_marker_segments(fs_grid* g, int* nseg);
 fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask);
 fs_status fs_set_body_state(fs_grid* g, const double* disp3, const double* vel3);   /* HOST */
 
-/* Advance nsteps fractional steps.  last == NULL: fully asynchronous on the grid's stream.
- * last != NULL (HOST): synchronises and reports the final step; FS_ERR_NOT_CONVERGED if that
- * step's PCG hit max_iter. */
+/* Advance nsteps fractional steps: predictor (Eq. 4) -> IBM interpolate / force / spread (Eq. 3b, 5, 3a;
+ * L89-91, L108) -> Poisson (Eq. 7) by PCG (L449, L686) -> projection (Eq. 6/10, L114, L131) -> rigid body
+ * (Eq. 12), one CUDA-graph replay per step.  last == NULL: fully asynchronous on the grid's stream.
+ * last != NULL (HOST): synchronises and fills *last for the final step (also when it returns
+ * FS_ERR_NOT_CONVERGED: that step's PCG hit max_iter; or FS_ERR_UNSUPPORTED: a moving body carried a marker
+ * support into a non-periodic boundary).  unconverged_steps / nan_steps count such steps over ALL steps since the
+ * grid was created, including asynchronous ones. */
 fs_status fs_step(fs_grid* g, int nsteps, fs_step_info* last);
 
 /* Solves lap p = rhs (Eq. 7 form; homogeneous Neumann on bounded faces, zero-mean solution) with
@@ -165,6 +185,12 @@ fs_status fs_profile_reset(fs_grid* g);
 
 /* Number of kernel launches (graph kernel nodes incl. loop-body replays) issued so far. */
 fs_status fs_launch_count(fs_grid* g, long long* launches);
+
+/* Which kernel instantiations this grid has enqueued so far, as one ';'-separated string of names such as
+ * "k_mg_down<f64,TR16,UPD>" (lets a parity test assert that it exercised the instantiation it was written for).
+ * buf: HOST, cap bytes; *needed (HOST, may be NULL) = bytes including the terminator.  buf == NULL && cap == 0
+ * only queries the size; a too small buf is FS_ERR_INVALID_ARG. */
+fs_status fs_kernels_used(fs_grid* g, char* buf, size_t cap, size_t* needed);
 
 const char* fs_status_string(fs_status s);
 

@@ -22,6 +22,7 @@ FS_OK = 0
 STATUS = {0: "FS_OK", 1: "FS_ERR_INVALID_ARG", 2: "FS_ERR_BAD_STATE", 3: "FS_ERR_OOM", 4: "FS_ERR_CUDA",
           5: "FS_ERR_NOT_CONVERGED", 6: "FS_ERR_UNSUPPORTED"}
 FS_ERR_NOT_CONVERGED = 5
+FS_ERR_UNSUPPORTED = 6
 DTYPE = {"f32": 0, "f64": 1}
 BC = {"periodic": 0, "noslip": 1, "slip": 2, "inflow": 3, "outflow": 4}
 TIME = {"euler": 0, "ab2": 1}
@@ -54,7 +55,7 @@ class fs_step_info(C.Structure):
     _fields_ = [("pcg_iters", C.c_int), ("converged", C.c_int), ("nan_flag", C.c_int),
                 ("rel_residual", C.c_double), ("true_rel_residual", C.c_double), ("max_abs_div", C.c_double),
                 ("body_force", C.c_double * 3), ("body_disp", C.c_double * 3), ("body_vel", C.c_double * 3),
-                ("step", C.c_longlong)]
+                ("step", C.c_longlong), ("unconverged_steps", C.c_longlong), ("nan_steps", C.c_longlong)]
 
 
 class fs_poisson_info(C.Structure):
@@ -67,7 +68,7 @@ SYMBOLS = ("fs_workspace_bytes", "fs_grid_create", "fs_grid_destroy", "fs_field_
            "fs_fields_get", "fs_set_history", "fs_set_ibm_markers", "fs_marker_segments", "fs_set_body",
            "fs_set_body_state", "fs_step", "fs_poisson_solve", "fs_ibm_interpolate", "fs_ibm_spread",
            "fs_gmg_vcycle", "fs_momentum_rhs", "fs_profile_step", "fs_profile_count", "fs_profile_entry",
-           "fs_profile_reset", "fs_launch_count", "fs_status_string")
+           "fs_profile_reset", "fs_launch_count", "fs_kernels_used", "fs_status_string")
 
 _lib = None
 
@@ -110,6 +111,7 @@ def lib():
                                        C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.fs_profile_reset.argtypes = [vp]
         L.fs_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.fs_kernels_used.argtypes = [vp, C.c_char_p, C.c_size_t, C.POINTER(C.c_size_t)]
         L.fs_status_string.argtypes = [ip]
         L.fs_status_string.restype = C.c_char_p
         for s in SYMBOLS:
@@ -157,7 +159,7 @@ def _info_dict(i):
     return dict(pcg_iters=i.pcg_iters, converged=i.converged, nan_flag=i.nan_flag,
                 rel_residual=i.rel_residual, true_rel_residual=i.true_rel_residual,
                 max_abs_div=i.max_abs_div, body_force=list(i.body_force), body_disp=list(i.body_disp),
-                body_vel=list(i.body_vel), step=i.step)
+                body_vel=list(i.body_vel), step=i.step, unconverged_steps=i.unconverged_steps, nan_steps=i.nan_steps)
 
 
 class Grid:
@@ -358,6 +360,14 @@ class Grid:
             _check(L.fs_profile_entry(self.h, i, C.byref(name), C.byref(cnt), C.byref(ms), C.byref(by)), "fs_profile_entry")
             out[name.value.decode()] = dict(launches=cnt.value, ms=ms.value, bytes=by.value)
         return out
+
+    def kernels_used(self):
+        """Names of the kernel instantiations this grid has enqueued so far (fs_kernels_used)."""
+        need = C.c_size_t(0)
+        _check(lib().fs_kernels_used(self.h, None, 0, C.byref(need)), "fs_kernels_used")
+        buf = C.create_string_buffer(need.value)
+        _check(lib().fs_kernels_used(self.h, buf, need.value, None), "fs_kernels_used")
+        return [x for x in buf.value.decode().split(";") if x]
 
     def launch_count(self):
         n = C.c_longlong(0)

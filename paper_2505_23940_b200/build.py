@@ -18,6 +18,18 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
 
+def csrc_hash():
+    """sha256 over csrc/*.cu, csrc/*.cuh and include/fs.h (sorted by name): identifies the sources a profile was
+    captured from (bench.py refuses a committed ncu capture whose hash differs from the current sources)."""
+    import hashlib
+    h = hashlib.sha256()
+    files = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh")))
+    for f in files + [os.path.normpath(HEADERS[1])]:
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()
+
+
 def _stale(target, deps):
     if not os.path.exists(target):
         return True

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <string>
 #include <vector>
 
 using namespace fs;
@@ -43,11 +44,18 @@ static void prof_collect(Prof* p) {     // caller has synchronised the stream
   }
   p->recs.clear();
 }
+struct Seen { std::vector<const char*> names; };
+void seen_add(Seen* s, const char* inst) {
+  for (const char* n : s->names) if (n == inst || std::strcmp(n, inst) == 0) return;
+  s->names.push_back(inst);
+}
 }  // namespace fs
 
 struct fs_grid {
   fs_params P;
+  int device = 0;                       // the CUDA device the workspace lives on; every entry point runs on it
   fs::Prof prof; bool profiling = false;
+  fs::Seen seen;
   std::vector<double> yf;
   bool f64 = true;
   int bx = 0, by = 0, bz = 0, nxu = 0, nyv = 0, nzw = 0;
@@ -69,6 +77,18 @@ struct fs_grid {
 };
 
 namespace {
+
+// Every entry point that takes an fs_grid makes the grid's device current for the call and restores the caller's
+// device afterwards, so grids on several GPUs can be driven from one thread (replicas).
+struct DeviceGuard {
+  int prev = -1; bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; prev = -1; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define GUARD(g) DeviceGuard guard_((g)->device); if (!guard_.ok) return FS_ERR_CUDA
 
 struct Bump {
   char* base; size_t off;
@@ -269,14 +289,13 @@ template <class T> int enqueue_post(fs_grid* g, const Launch& L, bool poisson) {
   return n;
 }
 
-template <class T> fs_status build_graph(fs_grid* g, bool poisson, cudaGraphExec_t* out, int* n_fixed, int* n_body) {
+template <class T> fs_status build_graph_impl(fs_grid* g, bool poisson, cudaGraphExec_t* out, int* n_fixed, int* n_body, bool* body_open) {
   cudaStream_t s = g->cap;
   cudaStreamCaptureStatus st; cudaGraph_t graph = nullptr; const cudaGraphNode_t* deps = nullptr; size_t nd = 0;
-  CK(cudaStreamBeginCapture(s, cudaStreamCaptureModeRelaxed));
   CK(cudaStreamGetCaptureInfo_v2(s, &st, nullptr, &graph, &deps, &nd));
   cudaGraphConditionalHandle h;
   CK(cudaGraphConditionalHandleCreate(&h, graph, 0, cudaGraphCondAssignDefault));
-  Launch L{s, h, 1};
+  Launch L{s, h, 1, nullptr, &g->seen};
   const int npre = enqueue_pre<T>(g, L, poisson);
   CK(cudaGetLastError());
   CK(cudaStreamGetCaptureInfo_v2(s, &st, nullptr, &graph, &deps, &nd));
@@ -286,25 +305,43 @@ template <class T> fs_status build_graph(fs_grid* g, bool poisson, cudaGraphExec
   CK(cudaGraphAddNode(&node, graph, deps, nd, &np));
   cudaGraph_t body = np.conditional.phGraph_out[0];
   CK(cudaStreamBeginCaptureToGraph(g->cap2, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
-  Launch Lb{g->cap2, h, 1};
+  *body_open = true;
+  Launch Lb{g->cap2, h, 1, nullptr, &g->seen};
   const int nbody = enqueue_body<T>(g, Lb);
   CK(cudaGetLastError());
   cudaGraph_t tmp = nullptr;
+  *body_open = false;
   CK(cudaStreamEndCapture(g->cap2, &tmp));
   CK(cudaStreamUpdateCaptureDependencies(s, &node, 1, cudaStreamSetCaptureDependencies));
   const int npost = enqueue_post<T>(g, L, poisson);
   CK(cudaGetLastError());
-  CK(cudaStreamEndCapture(s, &graph));
-  if (*out) { cudaGraphExecDestroy(*out); *out = nullptr; }
-  CK(cudaGraphInstantiate(out, graph, 0));
-  CK(cudaGraphDestroy(graph));
   *n_fixed = npre + npost; *n_body = nbody;
   return FS_OK;
 }
 
+// Captures pre-loop kernels, the conditional WHILE node with the PCG body, and the post-loop kernels into one
+// graph.  Whatever fails in between, both capture streams are taken out of capture mode and the partial graph
+// is destroyed before the error is returned, so a later call starts from a clean state.
+template <class T> fs_status build_graph(fs_grid* g, bool poisson, cudaGraphExec_t* out, int* n_fixed, int* n_body) {
+  CK(cudaStreamBeginCapture(g->cap, cudaStreamCaptureModeRelaxed));
+  bool body_open = false;
+  fs_status st = build_graph_impl<T>(g, poisson, out, n_fixed, n_body, &body_open);
+  cudaGraph_t graph = nullptr, tmp = nullptr;
+  if (body_open) cudaStreamEndCapture(g->cap2, &tmp);           // the body graph is owned by the conditional node
+  const cudaError_t ec = cudaStreamEndCapture(g->cap, &graph);
+  if (st == FS_OK && ec != cudaSuccess) { std::fprintf(stderr, "libfs: graph capture failed: %s\n", cudaGetErrorString(ec)); st = FS_ERR_CUDA; }
+  if (st == FS_OK) {
+    if (*out) { cudaGraphExecDestroy(*out); *out = nullptr; }
+    if (cudaGraphInstantiate(out, graph, 0) != cudaSuccess) { *out = nullptr; st = FS_ERR_CUDA; }
+  }
+  if (graph) cudaGraphDestroy(graph);
+  if (st != FS_OK) cudaGetLastError();                          // clear the sticky-free error state of the failed capture
+  return st;
+}
+
 // FS_EXEC_STREAM: same kernels, launched directly; the host polls the done flag between chunks.
 template <class T> fs_status run_stream(fs_grid* g, bool poisson, int* n_fixed, int* n_body) {
-  Launch L{g->stream, 0, 0, g->profiling ? &g->prof : nullptr};
+  Launch L{g->stream, 0, 0, g->profiling ? &g->prof : nullptr, &g->seen};
   const int npre = enqueue_pre<T>(g, L, poisson);
   int nbody = 0;
   for (;;) {
@@ -405,7 +442,7 @@ template <class T> fs_status fields_io(fs_grid* g, fs_field f, void* buf, fs_dty
   }
   if (f == FS_DIV) {
     Ctx<T>& c = ctx<T>(g);
-    Launch L{g->stream, 0, 0};
+    Launch L{g->stream, 0, 0, nullptr, &g->seen};
     launch_divergence<T>(c, c.u, c.v, c.w, c.q, L);
     CK(cudaGetLastError());
   }
@@ -421,7 +458,7 @@ template <class T> fs_status poisson_impl(fs_grid* g, const void* rhs, void* p_i
   st = copy_in<T>(g, c.p, N, p_inout, dtype, on_device); if (st != FS_OK) return st;
   st = run_once<T>(g, true); if (st != FS_OK) return st;
   Scalars hs; st = read_scalars(g, &hs); if (st != FS_OK) return st;
-  g->body_iters_poisson += hs.iter;
+  g->body_iters_poisson += hs.body_runs;
   st = copy_out<T>(g, c.p, N, p_inout, dtype, on_device); if (st != FS_OK) return st;
   CK(cudaMemcpyAsync(c.p, c.us, N * sizeof(T), cudaMemcpyDeviceToDevice, g->stream));
   CK(cudaStreamSynchronize(g->stream));
@@ -470,6 +507,23 @@ fs_status fs_grid_create(const fs_params* params, void* workspace, size_t bytes,
   g->stream = (cudaStream_t)cuda_stream; g->ws = (char*)workspace; g->ws_bytes = bytes;
   if (g->f64) carve<double>(g, g->ws); else carve<float>(g, g->ws);
   auto fail = [&](fs_status s) { fs_grid_destroy(g); return s; };
+  // the grid lives on the device that owns the workspace; that device must be the caller's current one (the
+  // stream handle belongs to it too) and stays the grid's device for every later call, whatever is current then
+  if (cudaGetDevice(&g->device) != cudaSuccess) { delete g; return FS_ERR_CUDA; }
+  {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, workspace) != cudaSuccess) { cudaGetLastError(); delete g; return FS_ERR_INVALID_ARG; }
+    if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) { delete g; return FS_ERR_INVALID_ARG; }
+    if (pa.type == cudaMemoryTypeDevice && pa.device != g->device) { delete g; return FS_ERR_INVALID_ARG; }
+  }
+  if (g->P.precond == FS_PC_GMG) {
+    const cudaError_t e1 = g->f64 ? mg_configure_device<double>() : mg_configure_device<float>();
+    const cudaError_t e2 = g->f64 ? mgf_configure_device<double>() : mgf_configure_device<float>();
+    if (e1 != cudaSuccess || e2 != cudaSuccess) {
+      std::fprintf(stderr, "libfs: cudaFuncSetAttribute(max dynamic shared memory) failed: %s\n", cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+      delete g; return FS_ERR_CUDA;
+    }
+  }
   if (cudaStreamCreateWithFlags(&g->cap, cudaStreamNonBlocking) != cudaSuccess) return fail(FS_ERR_CUDA);
   if (cudaStreamCreateWithFlags(&g->cap2, cudaStreamNonBlocking) != cudaSuccess) return fail(FS_ERR_CUDA);
   if (cudaMemsetAsync(g->ws, 0, need, g->stream) != cudaSuccess) return fail(FS_ERR_CUDA);
@@ -482,6 +536,7 @@ fs_status fs_grid_create(const fs_params* params, void* workspace, size_t bytes,
 
 fs_status fs_grid_destroy(fs_grid* g) {
   if (!g) return FS_ERR_INVALID_ARG;
+  DeviceGuard guard_(g->device);
   if (g->stream || g->cap) cudaStreamSynchronize(g->stream);
   if (g->step_exec) cudaGraphExecDestroy(g->step_exec);
   if (g->poisson_exec) cudaGraphExecDestroy(g->poisson_exec);
@@ -511,6 +566,7 @@ fs_status fs_field_size(fs_grid* g, fs_field f, long long* count) {
 
 fs_status fs_fields_set(fs_grid* g, fs_field f, const void* src, fs_dtype dtype, int src_on_device) {
   if (!g || !src) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   if (f <= FS_DIV) return g->f64 ? fields_io<double>(g, f, const_cast<void*>(src), dtype, src_on_device, true)
                                  : fields_io<float>(g, f, const_cast<void*>(src), dtype, src_on_device, true);
   const cudaMemcpyKind kind = src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
@@ -527,6 +583,7 @@ fs_status fs_fields_set(fs_grid* g, fs_field f, const void* src, fs_dtype dtype,
 
 fs_status fs_fields_get(fs_grid* g, fs_field f, void* dst, fs_dtype dtype, int dst_on_device) {
   if (!g || !dst) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   if (f <= FS_DIV) return g->f64 ? fields_io<double>(g, f, dst, dtype, dst_on_device, false)
                                  : fields_io<float>(g, f, dst, dtype, dst_on_device, false);
   const cudaMemcpyKind kind = dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
@@ -556,6 +613,7 @@ fs_status fs_fields_get(fs_grid* g, fs_field f, void* dst, fs_dtype dtype, int d
 
 fs_status fs_set_history(fs_grid* g, int have_history, long long step) {
   if (!g) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   const int hh = have_history != 0;
   CK(cudaMemcpyAsync(&g->S->have_hist, &hh, sizeof(int), cudaMemcpyHostToDevice, g->stream));
   CK(cudaMemcpyAsync(&g->S->step, &step, sizeof(long long), cudaMemcpyHostToDevice, g->stream));
@@ -565,6 +623,7 @@ fs_status fs_set_history(fs_grid* g, int have_history, long long step) {
 
 fs_status fs_set_ibm_markers(fs_grid* g, int n, const double* xyz, const double* vel, const double* dvol) {
   if (!g || n < 0 || (n > 0 && !xyz)) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   if (n > g->P.max_markers) return FS_ERR_INVALID_ARG;
   if (n > 0 && !g->uniform_y) return FS_ERR_UNSUPPORTED;
   IbmCtx& ib = g->ib;
@@ -584,16 +643,27 @@ fs_status fs_set_ibm_markers(fs_grid* g, int n, const double* xyz, const double*
   CK(cudaMemcpyAsync(ib.dV, dv.data(), (size_t)n * sizeof(double), cudaMemcpyHostToDevice, g->stream));
   CK(cudaMemsetAsync(ib.Fl, 0, 3 * (size_t)n * sizeof(double), g->stream));
   CK(cudaMemsetAsync(ib.Ul, 0, 3 * (size_t)n * sizeof(double), g->stream));
-  Launch L{g->stream, 0, 0};
+  CK(cudaMemsetAsync(&g->S->ibm_oob, 0, sizeof(int), g->stream));
+  Launch L{g->stream, 0, 0, nullptr, &g->seen};
   g->fixed_launches += g->f64 ? launch_ibm_index<double>(g->cd, ib, L) : launch_ibm_index<float>(g->cf, ib, L);
   CK(cudaGetLastError());
+  int oob = 0;
+  CK(cudaMemcpyAsync(&oob, &g->S->ibm_oob, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
   CK(cudaStreamSynchronize(g->stream));
+  if (oob) {                        // a support reaches a non-periodic boundary: refused, the grid keeps no markers
+    const int zero = 0;
+    ib.n = 0; g->nl = 0;
+    CK(cudaMemcpyAsync(&g->S->ibm_oob, &zero, sizeof(int), cudaMemcpyHostToDevice, g->stream));
+    CK(cudaStreamSynchronize(g->stream));
+    return FS_ERR_UNSUPPORTED;
+  }
   g->indexed = true;
   return FS_OK;
 }
 
 fs_status fs_marker_segments(fs_grid* g, int* nseg) {
   if (!g || !nseg) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   if (g->ib.n == 0) { *nseg = 0; return FS_OK; }
   int v = 0;
   CK(cudaMemcpyAsync(&v, &g->S->nseg, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
@@ -604,6 +674,7 @@ fs_status fs_marker_segments(fs_grid* g, int* nseg) {
 
 fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask) {
   if (!g || !(m > 0)) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   g->ib.has_body = 1; g->ib.bm = m; g->ib.bc = c; g->ib.bk = k; g->ib.dof = dof_mask;
   invalidate(g);
   return FS_OK;
@@ -611,6 +682,7 @@ fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask) {
 
 fs_status fs_set_body_state(fs_grid* g, const double* disp3, const double* vel3) {
   if (!g || !disp3 || !vel3) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   CK(cudaMemcpyAsync(g->S->body_disp, disp3, 3 * sizeof(double), cudaMemcpyHostToDevice, g->stream));
   CK(cudaMemcpyAsync(g->S->body_vel, vel3, 3 * sizeof(double), cudaMemcpyHostToDevice, g->stream));
   CK(cudaStreamSynchronize(g->stream));
@@ -619,6 +691,7 @@ fs_status fs_set_body_state(fs_grid* g, const double* disp3, const double* vel3)
 
 fs_status fs_step(fs_grid* g, int nsteps, fs_step_info* last) {
   if (!g || nsteps < 0) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   for (int s = 0; s < nsteps; ++s) {
     fs_status st = g->f64 ? run_once<double>(g, false) : run_once<float>(g, false);
     if (st != FS_OK) return st;
@@ -632,19 +705,23 @@ fs_status fs_step(fs_grid* g, int nsteps, fs_step_info* last) {
   I.max_abs_div = hs.max_div;
   for (int a = 0; a < 3; ++a) { I.body_force[a] = hs.body_force[a]; I.body_disp[a] = hs.body_disp[a]; I.body_vel[a] = hs.body_vel[a]; }
   I.step = hs.step;
-  *last = I;
+  I.unconverged_steps = hs.unconverged_steps; I.nan_steps = hs.nan_steps;
+  *last = I;                        // valid for FS_OK, FS_ERR_NOT_CONVERGED and FS_ERR_UNSUPPORTED (fs.h)
+  if (hs.ibm_oob) return FS_ERR_UNSUPPORTED;
   return (nsteps > 0 && !hs.converged) ? FS_ERR_NOT_CONVERGED : FS_OK;
 }
 
 fs_status fs_poisson_solve(fs_grid* g, const void* rhs, void* p_inout, fs_dtype dtype, int on_device, fs_poisson_info* info) {
   if (!g || !rhs || !p_inout) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   return g->f64 ? poisson_impl<double>(g, rhs, p_inout, dtype, on_device, info) : poisson_impl<float>(g, rhs, p_inout, dtype, on_device, info);
 }
 
 fs_status fs_ibm_interpolate(fs_grid* g, double* out) {
   if (!g || !out) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   if (g->ib.n == 0) return FS_ERR_BAD_STATE;
-  Launch L{g->stream, 0, 0};
+  Launch L{g->stream, 0, 0, nullptr, &g->seen};
   if (g->f64) g->fixed_launches += launch_ibm_interpolate<double>(g->cd, g->ib, g->cd.u, g->cd.v, g->cd.w, g->ib.Ul, L);
   else g->fixed_launches += launch_ibm_interpolate<float>(g->cf, g->ib, g->cf.u, g->cf.v, g->cf.w, g->ib.Ul, L);
   CK(cudaGetLastError());
@@ -655,9 +732,10 @@ fs_status fs_ibm_interpolate(fs_grid* g, double* out) {
 
 fs_status fs_ibm_spread(fs_grid* g, const double* F) {
   if (!g || !F) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   if (g->ib.n == 0) return FS_ERR_BAD_STATE;
   CK(cudaMemcpyAsync(g->ib.Fl, F, 3 * (size_t)g->ib.n * sizeof(double), cudaMemcpyHostToDevice, g->stream));
-  Launch L{g->stream, 0, 0};
+  Launch L{g->stream, 0, 0, nullptr, &g->seen};
   if (g->f64) g->fixed_launches += launch_ibm_spread<double>(g->cd, g->ib, g->ib.Fl, g->cd.u, g->cd.v, g->cd.w, 1.0, L);
   else g->fixed_launches += launch_ibm_spread<float>(g->cf, g->ib, g->ib.Fl, g->cf.u, g->cf.v, g->cf.w, 1.0, L);
   CK(cudaGetLastError());
@@ -667,10 +745,11 @@ fs_status fs_ibm_spread(fs_grid* g, const double* F) {
 
 fs_status fs_gmg_vcycle(fs_grid* g, const double* r, double* z) {
   if (!g || !r || !z) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   if (g->P.precond != FS_PC_GMG) return FS_ERR_BAD_STATE;
   const int zero = 0;
   CK(cudaMemcpyAsync(&g->S->done, &zero, sizeof(int), cudaMemcpyHostToDevice, g->stream));
-  Launch L{g->stream, 0, 0};
+  Launch L{g->stream, 0, 0, nullptr, &g->seen};
   fs_status st;
   if (g->f64) {
     st = copy_in<double>(g, g->cd.r, g->nP, r, FS_F64, 0); if (st != FS_OK) return st;
@@ -690,7 +769,8 @@ fs_status fs_gmg_vcycle(fs_grid* g, const double* r, double* z) {
 
 fs_status fs_momentum_rhs(fs_grid* g) {
   if (!g) return FS_ERR_INVALID_ARG;
-  Launch L{g->stream, 0, 0};
+  GUARD(g);
+  Launch L{g->stream, 0, 0, nullptr, &g->seen};
   g->fixed_launches += g->f64 ? launch_momentum<double>(g->cd, L) : launch_momentum<float>(g->cf, L);
   CK(cudaGetLastError());
   CK(cudaStreamSynchronize(g->stream));
@@ -699,6 +779,7 @@ fs_status fs_momentum_rhs(fs_grid* g) {
 
 fs_status fs_profile_step(fs_grid* g, int nsteps) {
   if (!g || nsteps < 0) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   g->profiling = true;
   fs_status st = FS_OK;
   for (int s = 0; s < nsteps && st == FS_OK; ++s) {
@@ -729,10 +810,21 @@ fs_status fs_profile_reset(fs_grid* g) {
   return FS_OK;
 }
 
+fs_status fs_kernels_used(fs_grid* g, char* buf, size_t cap, size_t* needed) {
+  if (!g || (!buf && cap > 0)) return FS_ERR_INVALID_ARG;
+  std::string all;
+  for (const char* n : g->seen.names) { if (!all.empty()) all += ';'; all += n; }
+  if (needed) *needed = all.size() + 1;
+  if (cap < all.size() + 1) return buf ? FS_ERR_INVALID_ARG : FS_OK;
+  std::memcpy(buf, all.c_str(), all.size() + 1);
+  return FS_OK;
+}
+
 fs_status fs_launch_count(fs_grid* g, long long* launches) {
   if (!g || !launches) return FS_ERR_INVALID_ARG;
+  GUARD(g);
   Scalars hs; fs_status st = read_scalars(g, &hs); if (st != FS_OK) return st;
-  *launches = g->fixed_launches + hs.total_iters * (long long)g->step_body + g->body_iters_poisson * (long long)g->poisson_body;
+  *launches = g->fixed_launches + hs.total_body * (long long)g->step_body + g->body_iters_poisson * (long long)g->poisson_body;
   return FS_OK;
 }
 

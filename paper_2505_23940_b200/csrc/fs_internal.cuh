@@ -27,13 +27,15 @@ struct Scalars {
   int rsel, need_update; // rsel: which residual buffer (r / r2) is current; need_update: K2 of the last iteration still to do (k_mg_down<UPD>)
   int dsel, pending;     // pending: the x += alpha_prev d of the last k_pcg_update has not been applied yet
   double alpha_prev, sum_p, sum_d;   // deferred x update (k_pcg_dirapply / k_pflush)
-  int pad2_unused, pad3_unused; //       // which of the two direction buffers holds the current d (k_pcg_dirapply)
+  int body_runs;         // replays of the PCG loop body in the current solve (counted by the direction kernel)
+  int ibm_oob;           // sticky: a marker support reached a non-periodic boundary (unsupported)
   int max_iter, pad0;
   double rtol;
   // step control
   long long step; int have_hist; int nan_flag;
   double max_div, true_rr;
-  long long total_iters;
+  long long total_iters, total_body;          // PCG iterations / loop-body replays of all steps so far
+  long long unconverged_steps, nan_steps;     // sticky: steps whose PCG hit max_iter / whose projected field held a NaN
   // open-boundary flux correction (O5)
   double flux_phi, flux_aout;
   // IBM
@@ -92,13 +94,21 @@ struct IbmCtx {
 struct Prof;
 void prof_begin(Prof* p, const char* name, double bytes, cudaStream_t s);
 void prof_end(Prof* p, cudaStream_t s);
-struct Launch { cudaStream_t s; cudaGraphConditionalHandle cond; int use_cond; Prof* prof; };
-#define FS_LAUNCH(L, name, bytes, ...)                              \
+// Which kernel instantiations a grid has enqueued so far (always on; host side, recorded at launch / capture time):
+// lets a parity test assert that it exercised the template instantiation it was written for (fs_kernels_used).
+struct Seen;
+void seen_add(Seen* s, const char* inst);
+struct Launch { cudaStream_t s; cudaGraphConditionalHandle cond; int use_cond; Prof* prof; Seen* seen; };
+// name: profile label (what the pass is); inst: the kernel instantiation that runs it
+#define FS_LAUNCHI(L, name, inst, bytes, ...)                       \
   do {                                                              \
+    if ((L).seen) seen_add((L).seen, inst);                         \
     if ((L).prof) prof_begin((L).prof, name, (double)(bytes), (L).s); \
     __VA_ARGS__;                                                    \
     if ((L).prof) prof_end((L).prof, (L).s);                        \
   } while (0)
+#define FS_LAUNCH(L, name, bytes, ...) FS_LAUNCHI(L, name, name, bytes, __VA_ARGS__)
+template <class T> constexpr const char* tname() { return sizeof(T) == 8 ? "f64" : "f32"; }
 
 
 // z chunk length of a streaming kernel: xy tiles x chunks CTAs run in waves of `slots` (CTAs resident on the
@@ -143,6 +153,11 @@ template <class T> int launch_mg_down(const Ctx<T>& c, const T* g, T* e, T* gc, 
                                       const char* name, const Launch& L, bool upd = false, T* g2 = nullptr, const T* q = nullptr);
 template <class T> int launch_mg_up(const Ctx<T>& c, const T* ein, const T* ec, const T* g, T* eo, int nx, int ny, int nz, double h,
                                     double omega, bool dot, T zs, const char* name, const Launch& L, const T* g2 = nullptr);
+
+// raises the dynamic shared-memory limit of every GMG kernel instantiation of type T on the CURRENT device
+// (cudaFuncSetAttribute is per device: called by fs_grid_create for each grid, not once per process)
+template <class T> cudaError_t mg_configure_device();
+template <class T> cudaError_t mgf_configure_device();
 
 template <class T> int launch_ibm_index(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
 template <class T> int launch_ibm_interpolate(const Ctx<T>& c, const IbmCtx& ib, const T* u, const T* v, const T* w, double* out, const Launch& L);

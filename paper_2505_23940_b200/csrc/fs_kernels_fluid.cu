@@ -6,38 +6,12 @@
 namespace fs {
 
 // ---------------------------------------------------------------------------------------------------
-// Boundary-aware velocity access (S0).
+// Boundary-aware velocity access (S0): see col_setup / col_fix below.
 // Component C at (i,j,k), at most one layer outside the stored range in a direction tangential to C:
 //   periodic      : index wrap
 //   no-slip/inflow: ghost = 2*u_wall - u_interior      slip/outflow: ghost = u_interior
 // Along its own normal a bounded component stores faces 0..n, so no ghost is needed there.
 // ---------------------------------------------------------------------------------------------------
-template <class T, int C> __device__ __forceinline__ T ldv(const Ctx<T>& c, const T* __restrict__ f, int i, int j, int k) {
-  T A = T(1), B = T(0);
-  // x
-  if (!c.bx) { i = i < 0 ? i + c.nx : (i >= c.nx ? i - c.nx : i); }
-  else if (C != 0) {
-    int face = -1;
-    if (i < 0) { face = 0; i = -1 - i; } else if (i >= c.nx) { face = 1; i = 2 * c.nx - 1 - i; }
-    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
-  }
-  // y
-  if (!c.by) { j = j < 0 ? j + c.ny : (j >= c.ny ? j - c.ny : j); }
-  else if (C != 1) {
-    int face = -1;
-    if (j < 0) { face = 2; j = -1 - j; } else if (j >= c.ny) { face = 3; j = 2 * c.ny - 1 - j; }
-    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
-  }
-  // z
-  if (!c.bz) { k = k < 0 ? k + c.nz : (k >= c.nz ? k - c.nz : k); }
-  else if (C != 2) {
-    int face = -1;
-    if (k < 0) { face = 4; k = -1 - k; } else if (k >= c.nz) { face = 5; k = 2 * c.nz - 1 - k; }
-    if (face >= 0 && (c.bc[face] == FS_BC_NOSLIP || c.bc[face] == FS_BC_INFLOW)) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
-  }
-  const int ex = C == 0 ? c.nxu : c.nx, ey = C == 1 ? c.nyv : c.ny;
-  return A * f[(size_t)i + (size_t)ex * ((size_t)j + (size_t)ey * (size_t)k)] + B;
-}
 
 // Counter-based inflow noise (O1): SplitMix64 finaliser chained over (seed, face, step, a, b) and
 // mapped to [0,1) by (x >> 11) * 2^-53.  The oracle implements the same generator independently.
@@ -277,8 +251,8 @@ template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
   // z chunks: >= 4 waves of CTAs (2 CTAs of 320 threads per SM) while chunks stay >= 16 planes
   const int kz = pick_kz((long long)bxn * byn, c.nzw, 2LL * 148, 2, 16);
   dim3 b(kMomTX, kMomTY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
-  if (c.convection == FS_CONV_UPWIND) FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, true><<<g, b, 0, L.s>>>(c, kz));
-  else FS_LAUNCH(L, "momentum_predictor", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, false><<<g, b, 0, L.s>>>(c, kz));
+  if (c.convection == FS_CONV_UPWIND) FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,upwind>" : "k_momentum<f32,upwind>", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, true><<<g, b, 0, L.s>>>(c, kz));
+  else FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,central>" : "k_momentum<f32,central>", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, false><<<g, b, 0, L.s>>>(c, kz));
   return 1;
 }
 
@@ -449,10 +423,10 @@ template <class T> int launch_div_rhs(const Ctx<T>& c, const Launch& L) {
     int kz = c.nz;
     while (kz > 16 && (long long)bxn * byn * ((c.nz + kz - 1) / kz) < 8LL * 148 * 8) kz = (kz + 1) / 2;
     while ((long long)bxn * byn * ((c.nz + kz - 1) / kz) > kMaxPartials) kz *= 2;
-    FS_LAUNCH(L, "div_rhs", 4.0 * sizeof(T) * N, k_div_rhsv<T><<<dim3(bxn, byn, (c.nz + kz - 1) / kz), dim3(32, 8), 0, L.s>>>(c, kz));
+    FS_LAUNCHI(L, "div_rhs", sizeof(T) == 8 ? "k_div_rhsv<f64>" : "k_div_rhsv<f32>", 4.0 * sizeof(T) * N, k_div_rhsv<T><<<dim3(bxn, byn, (c.nz + kz - 1) / kz), dim3(32, 8), 0, L.s>>>(c, kz));
     return 1;
   }
-  FS_LAUNCH(L, "div_rhs", 4.0 * sizeof(T) * N, k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, nullptr));
+  FS_LAUNCHI(L, "div_rhs", sizeof(T) == 8 ? "k_div_rhs<f64>" : "k_div_rhs<f32>", 4.0 * sizeof(T) * N, k_div_rhs<T><<<flat_blocks(N), 256, 0, L.s>>>(c, nullptr));
   return 1;
 }
 template <class T> int launch_rhs_from_b(const Ctx<T>& c, const T* b, const Launch& L) {
@@ -679,12 +653,12 @@ template <class T> int launch_project(const Ctx<T>& c, const Launch& L) {
   if (!c.bx && c.nx % Vec16<T>::VX == 0) {
     const int bxn = (c.nx + 30 * Vec16<T>::VX - 1) / (30 * Vec16<T>::VX), byn = (c.nyv + PjTile<T>::TY - 3) / (PjTile<T>::TY - 2);
     const int kz = pick_kz((long long)bxn * byn, c.nzw, 2LL * 148, 1, 16);
-    FS_LAUNCH(L, "project", 7.0 * sizeof(T) * c.nx * c.ny * c.nz,
+    FS_LAUNCHI(L, "project", sizeof(T) == 8 ? "k_projectv<f64>" : "k_projectv<f32>", 7.0 * sizeof(T) * c.nx * c.ny * c.nz,
               k_projectv<T><<<dim3(bxn, byn, (c.nzw + kz - 1) / kz), dim3(32, PjTile<T>::TY), 0, L.s>>>(c, kz));
     return 1;
   }
   ColGeom g = col_geom(c.nxu, c.nyv, c.nzw);
-  FS_LAUNCH(L, "project", 7.0 * sizeof(T) * c.nx * c.ny * c.nz, k_project<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz));
+  FS_LAUNCHI(L, "project", sizeof(T) == 8 ? "k_project<f64>" : "k_project<f32>", 7.0 * sizeof(T) * c.nx * c.ny * c.nz, k_project<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz));
   return 1;
 }
 
@@ -714,7 +688,8 @@ template <class T> __global__ void k_step_end(const Ctx<T> c, const IbmCtx ib) {
         S->body_disp[a] = w1; S->body_vel[a] = v1;
       }
     }
-    S->have_hist = 1; S->step += 1; S->total_iters += S->iter;
+    S->have_hist = 1; S->step += 1; S->total_iters += S->iter; S->total_body += S->body_runs;
+    S->unconverged_steps += S->converged ? 0 : 1; S->nan_steps += S->nan_flag ? 1 : 0;
   }
   __syncthreads();
   if (ib.has_body) {

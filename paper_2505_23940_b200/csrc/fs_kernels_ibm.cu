@@ -51,6 +51,9 @@ template <class T> __global__ void k_ibm_index(const Ctx<T> c, const IbmCtx ib) 
       if (ib.delta == FS_DELTA_ROMA3) base = (int)floor(__dadd_rn(sc, 0.5)) - 1;
       else base = (int)floor(sc) - 1;
       ib.base[((size_t)comp * ib.n + l) * 3 + d] = base;
+      // a support that reaches a prescribed boundary-normal face or leaves a bounded box is unsupported
+      // (sticky flag; fs_set_ibm_markers / fs_step report FS_ERR_UNSUPPORTED).  node_index keeps memory accesses safe.
+      for (int a = 0; a < ib.sw; ++a) if (node_index<T>(c, base + a, comp, d) < 0) c.S->ibm_oob = 1;
       double* wt = ib.wts + (((size_t)comp * ib.n + l) * 3 + d) * 4;
       for (int a = 0; a < 4; ++a) {
         const double r = __dsub_rn(sc, (double)(base + a));

@@ -156,6 +156,14 @@ template <class T> __global__ void __launch_bounds__(1024) k_mg_tail(const int* 
   for (int q = tid; q < N[0]; q += nth) e_out[q] = cur[0][q];
 }
 
+// k_mg_tail needs up to 3 (4096 + 4096/7 + 8) words of dynamic shared memory (112 KB in fp64): per-device opt-in,
+// applied by fs_grid_create for the device the grid lives on.
+template <class T> cudaError_t mg_configure_device() {
+  return cudaFuncSetAttribute(k_mg_tail<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * (kTailCells + kTailCells / 7 + 8) * sizeof(T)));
+}
+template cudaError_t mg_configure_device<float>();
+template cudaError_t mg_configure_device<double>();
+
 // Recursion unrolled on the host: emits the kernels of one V-cycle for rhs -> out (out = V(rhs)).
 template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs, bool* upd_fused) {
   int n = 0;
@@ -194,8 +202,6 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
         cells += (size_t)mg.lev[l].nx * mg.lev[l].ny * mg.lev[l].nz;
       }
       const size_t smem = 3 * cells * sizeof(T);
-      static bool once = false;
-      if (!once) { cudaFuncSetAttribute(k_mg_tail<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * (kTailCells + kTailCells / 7 + 8) * sizeof(T))); once = true; }
       FS_LAUNCH(L, "mg_coarse", 2.0 * sizeof(T) * mg.lev[lt].nx * mg.lev[lt].ny * mg.lev[lt].nz,
                 k_mg_tail<T><<<1, 1024, smem, L.s>>>(done, gl[lt], el[lt], a, mg.nu1, mg.nu2, mg.coarse_sweeps, mg.omega)); ++n;
     } else {

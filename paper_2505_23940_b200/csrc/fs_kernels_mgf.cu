@@ -280,24 +280,34 @@ k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __rest
 // Tile height: TR thread rows (2 TR cell rows; 16 on big levels: fewer halo rows per result, 8 below: more CTAs).
 static int mg_tr(int ny) { return ny >= 384 ? 16 : 8; }
 template <class T, int TR> static int slots_per_sm() { return (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1); }
-template <class K> static void allow_smem(K kernel, size_t bytes) {
-  cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+template <class K> static cudaError_t allow_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+// Dynamic shared memory of the fused legs exceeds the 48 KB default at TR = 16 in fp64 (64 KB): the opt-in is a
+// per-device function attribute, so it is (re)applied for the current device whenever a grid is created there.
+template <class T, int TR> static cudaError_t configure_tr() {
+  const size_t smem = 8 * (size_t)MgTile<TR>::PL * sizeof(T);
+  cudaError_t e;
+  if ((e = allow_smem(k_mg_down<T, TR, true>, smem)) != cudaSuccess) return e;
+  if ((e = allow_smem(k_mg_down<T, TR, false>, smem)) != cudaSuccess) return e;
+  if ((e = allow_smem(k_mg_up<T, TR, true>, smem)) != cudaSuccess) return e;
+  return allow_smem(k_mg_up<T, TR, false>, smem);
+}
+template <class T> cudaError_t mgf_configure_device() {
+  cudaError_t e = configure_tr<T, 8>();
+  return e != cudaSuccess ? e : configure_tr<T, 16>();
 }
 
 template <class T, int TR, bool UPD> static void down_tr(const Ctx<T>& c, const T* g, T* g2, const T* q, T* e, T* gc, int nx, int ny, int nz,
                                                          T cg, T cn, T ih2, const Launch& L) {
   const MgGeom G = mg_geom(nx, ny, nz, MgTile<TR>::IY, slots_per_sm<T, TR>());
   const size_t smem = 8 * (size_t)MgTile<TR>::PL * sizeof(T);
-  static bool once = false;
-  if (!once) { allow_smem(k_mg_down<T, TR, UPD>, smem); once = true; }
   k_mg_down<T, TR, UPD><<<G.grid, dim3(32, TR), smem, L.s>>>(&c.S->done, g, g2, q, e, gc, nx, ny, nz, cg, cn, ih2, c.S, c.partials, L);
 }
 template <class T, int TR, bool DOT> static void up_tr(const Ctx<T>& c, const T* ein, const T* ec, const T* g, const T* g2, T* eo, int nx, int ny, int nz,
                                                        T ce, T cw, T cn, T zs, cudaStream_t s) {
   const MgGeom G = mg_geom(nx, ny, nz, MgTile<TR>::IY, slots_per_sm<T, TR>());
   const size_t smem = 8 * (size_t)MgTile<TR>::PL * sizeof(T);
-  static bool once = false;
-  if (!once) { allow_smem(k_mg_up<T, TR, DOT>, smem); once = true; }
   k_mg_up<T, TR, DOT><<<G.grid, dim3(32, TR), smem, s>>>(&c.S->done, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, c.S, c.partials);
 }
 
@@ -309,7 +319,9 @@ template <class T> int launch_mg_down(const Ctx<T>& c, const T* g, T* e, T* gc, 
   const double ih2 = 1.0 / (h * h), cw = omega * h * h / 6.0;
   const T cg = T(2.0 * cw - 6.0 * cw * cw * ih2), cn = T(cw * cw * ih2);
   const bool big = mg_tr(ny) == 16;
-  FS_LAUNCH(L, name, (upd ? 4.125 : 2.125) * sizeof(T) * N, {
+  const char* inst = sizeof(T) == 8 ? (big ? (upd ? "k_mg_down<f64,TR16,UPD>" : "k_mg_down<f64,TR16>") : (upd ? "k_mg_down<f64,TR8,UPD>" : "k_mg_down<f64,TR8>"))
+                                    : (big ? (upd ? "k_mg_down<f32,TR16,UPD>" : "k_mg_down<f32,TR16>") : (upd ? "k_mg_down<f32,TR8,UPD>" : "k_mg_down<f32,TR8>"));
+  FS_LAUNCHI(L, name, inst, (upd ? 4.125 : 2.125) * sizeof(T) * N, {
     if (upd) { if (big) down_tr<T, 16, true>(c, g, g2, q, e, gc, nx, ny, nz, cg, cn, T(ih2), L); else down_tr<T, 8, true>(c, g, g2, q, e, gc, nx, ny, nz, cg, cn, T(ih2), L); }
     else { if (big) down_tr<T, 16, false>(c, g, nullptr, nullptr, e, gc, nx, ny, nz, cg, cn, T(ih2), L); else down_tr<T, 8, false>(c, g, nullptr, nullptr, e, gc, nx, ny, nz, cg, cn, T(ih2), L); }
   });
@@ -321,7 +333,9 @@ template <class T> int launch_mg_up(const Ctx<T>& c, const T* ein, const T* ec, 
   const double ih2d = 1.0 / (h * h), cwd = omega * h * h / 6.0;
   const T ce = T(1.0 - 6.0 * cwd * ih2d), cw = T(cwd), cn = T(cwd * ih2d);
   const bool big = mg_tr(ny) == 16;
-  FS_LAUNCH(L, name, 3.125 * sizeof(T) * N, {
+  const char* inst = sizeof(T) == 8 ? (big ? (dot ? "k_mg_up<f64,TR16,DOT>" : "k_mg_up<f64,TR16>") : (dot ? "k_mg_up<f64,TR8,DOT>" : "k_mg_up<f64,TR8>"))
+                                    : (big ? (dot ? "k_mg_up<f32,TR16,DOT>" : "k_mg_up<f32,TR16>") : (dot ? "k_mg_up<f32,TR8,DOT>" : "k_mg_up<f32,TR8>"));
+  FS_LAUNCHI(L, name, inst, 3.125 * sizeof(T) * N, {
     if (big) { if (dot) up_tr<T, 16, true>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 16, false>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
     else { if (dot) up_tr<T, 8, true>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); else up_tr<T, 8, false>(c, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, L.s); }
   });
@@ -333,5 +347,7 @@ template <class T> int launch_mg_up(const Ctx<T>& c, const T* ein, const T* ec, 
   template int launch_mg_up<T>(const Ctx<T>&, const T*, const T*, const T*, T*, int, int, int, double, double, bool, T, const char*, const Launch&, const T*);
 INST(float)
 INST(double)
+template cudaError_t mgf_configure_device<float>();
+template cudaError_t mgf_configure_device<double>();
 
 }  // namespace fs

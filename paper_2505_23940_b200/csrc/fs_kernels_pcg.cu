@@ -72,7 +72,7 @@ template <class T> __global__ void __launch_bounds__(256) k_pcg_init(const Ctx<T
     if (threadIdx.x == 0 && threadIdx.y == 0) {
       Scalars* S = c.S;
       S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
-      S->iter = 0; S->first = 1; S->dsel = 0; S->pending = 0; S->rsel = 0; S->need_update = 0;
+      S->iter = 0; S->body_runs = 0; S->first = 1; S->dsel = 0; S->pending = 0; S->rsel = 0; S->need_update = 0;
       S->rmean = v[3] / ((double)c.nx * c.ny * c.nz);
       const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
       S->converged = conv; S->done = conv || S->max_iter <= 0;
@@ -95,6 +95,7 @@ template <class T, int PC> __global__ void __launch_bounds__(kDaTX * kDaTY, 2) k
   __shared__ T D[2][kDaTY][kDaTX];
   __shared__ double sh[3 * 32]; __shared__ int flag;
   const Scalars* S = c.S;
+  if (blockIdx.x + blockIdx.y + blockIdx.z == 0 && threadIdx.x + threadIdx.y == 0) c.S->body_runs += 1;   // one writer: loop-body replays of this solve
   if (S->done) return;
   const bool first = S->first != 0;
   const T beta = first ? T(0) : T(S->rho_cur / S->rho_prev);
@@ -190,6 +191,7 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
   __shared__ V D[2 * kDa2PL];
   __shared__ double sh[3 * 32]; __shared__ int flag;
   const Scalars* S = c.S;
+  if (blockIdx.x + blockIdx.y + blockIdx.z == 0 && threadIdx.x + threadIdx.y == 0) c.S->body_runs += 1;   // one writer: loop-body replays of this solve
   if (S->done) return;
   const bool first = S->first != 0;
   const T beta = first ? T(0) : T(S->rho_cur / S->rho_prev);
@@ -318,6 +320,7 @@ template <class T, int PC> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pc
   __shared__ __align__(16) T D[2 * PLN];
   __shared__ double sh[3 * 32]; __shared__ int flag;
   const Scalars* S = c.S;
+  if (blockIdx.x + blockIdx.y + blockIdx.z == 0 && threadIdx.x + threadIdx.y == 0) c.S->body_runs += 1;   // one writer: loop-body replays of this solve
   if (S->done) return;
   const bool first = S->first != 0;
   const T beta = first ? T(0) : T(S->rho_cur / S->rho_prev);
@@ -548,7 +551,7 @@ template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaT
     if (lane == 0 && ty == 0) {
       Scalars* S = c.S;
       S->bnorm2 = v[0]; S->rr = v[1]; S->rho_cur = v[2]; S->rho_prev = 1.0; S->dq = 1.0;
-      S->iter = 0; S->first = 1; S->dsel = 0; S->pending = 0; S->rsel = 0; S->need_update = 0;
+      S->iter = 0; S->body_runs = 0; S->first = 1; S->dsel = 0; S->pending = 0; S->rsel = 0; S->need_update = 0;
       S->rmean = v[3] / ((double)c.nx * c.ny * c.nz);
       const int conv = (v[0] == 0.0) || (sqrt(v[1]) <= S->rtol * sqrt(v[0]));
       S->converged = conv; S->done = conv || S->max_iter <= 0;
@@ -705,14 +708,14 @@ template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L, bool ne
     const DaGeom G = dav_geom<T>(c.nx, c.ny, c.nz);
     const dim3 blk(32, kDaTY);
     const bool jac = c.precond == FS_PC_JACOBI;
-    FS_LAUNCH(L, "pcg_init", (need_bhat ? 4.0 : 3.0) * sizeof(T) * N, {
+    FS_LAUNCHI(L, "pcg_init", sizeof(T) == 8 ? "k_pcg_initv<f64>" : "k_pcg_initv<f32>", (need_bhat ? 4.0 : 3.0) * sizeof(T) * N, {
       if (jac) { if (need_bhat) k_pcg_initv<T, 1, true><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); else k_pcg_initv<T, 1, false><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); }
       else { if (need_bhat) k_pcg_initv<T, 0, true><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); else k_pcg_initv<T, 0, false><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); }
     });
     return n + 1;
   }
   ColGeom g = col_geom(c.nx, c.ny, c.nz);
-  FS_LAUNCH(L, "pcg_init", 4.0 * sizeof(T) * N, k_pcg_init<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz, L));
+  FS_LAUNCHI(L, "pcg_init", sizeof(T) == 8 ? "k_pcg_init<f64>" : "k_pcg_init<f32>", 4.0 * sizeof(T) * N, k_pcg_init<T><<<g.grid, g.block, 0, L.s>>>(c, g.kz, L));
   return n + 1;
 }
 
@@ -730,36 +733,36 @@ template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, cons
   if (sizeof(T) == 8 && c.nx % 2 == 0) {
     const DaGeom G = da2_geom(c.nx, c.ny, c.nz);
     const dim3 blk(32, kDaTY);
-    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    if (c.precond == FS_PC_GMG) FS_LAUNCHI(L, "pcg_dir_apply_dot", "k_pcg_dirapply2<f64>", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else if (c.precond == FS_PC_JACOBI) FS_LAUNCHI(L, "pcg_dir_apply_dot", "k_pcg_dirapply2<f64>", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else FS_LAUNCHI(L, "pcg_dir_apply_dot", "k_pcg_dirapply2<f64>", 6.0 * sizeof(T) * N, k_pcg_dirapply2<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
     ++n;
   } else if (sizeof(T) == 4 && c.nx % 4 == 0) {
     const DaGeom G = dav_geom<T>(c.nx, c.ny, c.nz);
     const dim3 blk(32, kDaTY);
-    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    if (c.precond == FS_PC_GMG) FS_LAUNCHI(L, "pcg_dir_apply_dot", "k_pcg_dirapplyv<f32>", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else if (c.precond == FS_PC_JACOBI) FS_LAUNCHI(L, "pcg_dir_apply_dot", "k_pcg_dirapplyv<f32>", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else FS_LAUNCHI(L, "pcg_dir_apply_dot", "k_pcg_dirapplyv<f32>", 6.0 * sizeof(T) * N, k_pcg_dirapplyv<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
     ++n;
   } else {
     const DaGeom G = da_geom(c.nx, c.ny, c.nz);
     const dim3 blk(kDaTX, kDaTY);
-    if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
-    else FS_LAUNCH(L, "pcg_dir_apply_dot", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    if (c.precond == FS_PC_GMG) FS_LAUNCHI(L, "pcg_dir_apply_dot", sizeof(T) == 8 ? "k_pcg_dirapply<f64>" : "k_pcg_dirapply<f32>", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 2><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else if (c.precond == FS_PC_JACOBI) FS_LAUNCHI(L, "pcg_dir_apply_dot", sizeof(T) == 8 ? "k_pcg_dirapply<f64>" : "k_pcg_dirapply<f32>", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 1><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
+    else FS_LAUNCHI(L, "pcg_dir_apply_dot", sizeof(T) == 8 ? "k_pcg_dirapply<f64>" : "k_pcg_dirapply<f32>", 6.0 * sizeof(T) * N, k_pcg_dirapply<T, 0><<<G.grid, blk, 0, L.s>>>(c, zs, G.kz));
     ++n;
   }
   if (upd_fused) return n;
-  if (c.precond == FS_PC_GMG) FS_LAUNCH(L, "pcg_update_norm", 3.0 * sizeof(T) * N, k_pcg_update<T, true><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
+  if (c.precond == FS_PC_GMG) FS_LAUNCHI(L, "pcg_update_norm", sizeof(T) == 8 ? "k_pcg_update<f64,GMG>" : "k_pcg_update<f32,GMG>", 3.0 * sizeof(T) * N, k_pcg_update<T, true><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
   else if (c.nx % Vec16<T>::VX == 0) {
     const int bxn = (c.nx + 32 * Vec16<T>::VX - 1) / (32 * Vec16<T>::VX), byn = (c.ny + 7) / 8;
     int kz = c.nz;
     while (kz > 4 && (long long)bxn * byn * ((c.nz + kz - 1) / kz) < 8LL * 148) kz = (kz + 1) / 2;
     while ((long long)bxn * byn * ((c.nz + kz - 1) / kz) > kMaxPartials) kz *= 2;
     const dim3 grid(bxn, byn, (c.nz + kz - 1) / kz), blk(32, 8);
-    if (c.precond == FS_PC_JACOBI) FS_LAUNCH(L, "pcg_update_norm", 3.0 * sizeof(T) * N, k_pcg_updatev<T, 1><<<grid, blk, 0, L.s>>>(c, kz, L));
-    else FS_LAUNCH(L, "pcg_update_norm", 3.0 * sizeof(T) * N, k_pcg_updatev<T, 0><<<grid, blk, 0, L.s>>>(c, kz, L));
-  } else FS_LAUNCH(L, "pcg_update_norm", 3.0 * sizeof(T) * N, k_pcg_update<T, false><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
+    if (c.precond == FS_PC_JACOBI) FS_LAUNCHI(L, "pcg_update_norm", sizeof(T) == 8 ? "k_pcg_updatev<f64>" : "k_pcg_updatev<f32>", 3.0 * sizeof(T) * N, k_pcg_updatev<T, 1><<<grid, blk, 0, L.s>>>(c, kz, L));
+    else FS_LAUNCHI(L, "pcg_update_norm", sizeof(T) == 8 ? "k_pcg_updatev<f64>" : "k_pcg_updatev<f32>", 3.0 * sizeof(T) * N, k_pcg_updatev<T, 0><<<grid, blk, 0, L.s>>>(c, kz, L));
+  } else FS_LAUNCHI(L, "pcg_update_norm", sizeof(T) == 8 ? "k_pcg_update<f64>" : "k_pcg_update<f32>", 3.0 * sizeof(T) * N, k_pcg_update<T, false><<<flat_blocks(N), 256, 0, L.s>>>(c, L));
   ++n;
   return n;
 }

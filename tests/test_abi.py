@@ -93,6 +93,7 @@ def test_workspace_bytes_and_validation_on_host(fs):
     assert L.fs_status_string(6) == b"unsupported configuration"
     # NULL handles never crash
     assert L.fs_grid_destroy(None) == 1 and L.fs_step(None, 1, None) == 1
+    assert L.fs_kernels_used(None, None, 0, None) == 1
 
 
 def test_product_never_imports_oracle():

@@ -9,6 +9,7 @@ The oracle cannot run 512^3 in test time, so (task statement, parity at full siz
     128^3 replica (the V-cycle makes them h-independent, pin P14), divergence-free projected field, zero-mean p.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -86,13 +87,83 @@ def test_c5_512_fp64_sampled_momentum_projection_and_solver_properties(fs):
     g.close()
 
 
-def test_c5_512_fp32_solver_properties(fs):
-    cfg = W.hit(n=N, dtype="f32", device="cuda:0")
+def test_c5_512_fp32_fields_within_1e4_of_fp64_after_5_steps(fs):
+    # north_star: fp32 fields within 1e-4 over 5 steps.  At 512^3 the fp64 reference is the fp64 CUDA path, itself
+    # compared with the oracle at this size (tests/test_gpu_zz_fullsize_oracle.py and the golden pins below).
+    cfg = W.hit(n=N, device="cuda:0")
+    g64 = fs.from_workload(cfg, device="cuda:0")
+    g32 = fs.from_workload(cfg, device="cuda:0", dtype="f32")
+    cfg["init"] = None
+    i64 = g64.step(5, per_step=True)
+    i32 = g32.step(5, per_step=True)
+    assert i32["nan_flag"] == 0 and i32["converged"] == 1 and i32["unconverged_steps"] == 0, i32
+    assert all(abs(a - b) <= 1 for a, b in zip(i32["iters_per_step"], i64["iters_per_step"])), (i32["iters_per_step"], i64["iters_per_step"])
+    assert i32["rel_residual"] <= 1e-8                                     # recurrence residual (reading A14)
+    assert i32["true_rel_residual"] < 1e-4, i32                            # reported: the fp32 true residual stalls near 1e-6
+    used = g32.kernels_used()
+    for k in ("k_mg_down<f32,TR16,UPD>", "k_mg_up<f32,TR16,DOT>", "k_pcg_dirapplyv<f32>", "k_projectv<f32>"):
+        assert k in used, (k, used)
+    errs = {}
+    for c in "uvwp":
+        ref = g64.get(c)
+        errs[c] = float(np.abs(g32.get(c) - ref).max() / np.abs(ref).max())
+    assert all(e < 1e-4 for e in errs.values()), errs
+    g64.close(); g32.close()
+
+
+# ---- full size AND full step count, on sampled points: golden values written by tests/golden/make_fullsize_pins.py
+#      (a committed script that calls only oracle/; hours of single-threaded oracle time, done once)
+def _pins(case):
+    path = os.path.join(os.path.dirname(__file__), "golden", "fullsize_%s.txt" % case)
+    P = {"ic": {c: [] for c in "uvw"}, "val": {c: [] for c in "uvwp"}, "max": {}}
+    for line in open(path):
+        f = line.split()
+        if not f or f[0].startswith("#"):
+            continue
+        if f[0] == "steps":
+            P["steps"] = int(f[1])
+        elif f[0] == "iters":
+            P["iters"] = [int(x) for x in f[1:]]
+        elif f[0] in ("body_force", "body_disp", "body_vel"):
+            P[f[0]] = [float.fromhex(x) for x in f[1:]]
+        elif f[0] == "max_abs_div":
+            P["max_abs_div"] = float.fromhex(f[1])
+        elif f[0] == "max":
+            P["max"][f[1]] = float.fromhex(f[2])
+        else:
+            P[f[0]][f[1]].append((int(f[2]), float.fromhex(f[3])))
+    return P
+
+
+@pytest.mark.parametrize("case", ["c2", "c3", "c4", "c5"])
+def test_full_size_full_step_count_against_oracle_pins(fs, case):
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_fullsize_pins", os.path.join(os.path.dirname(__file__), "golden", "make_fullsize_pins.py"))
+    mk = importlib.util.module_from_spec(spec); spec.loader.exec_module(mk)
+    P = _pins(case)
+    cfg = W.make(case, device="cuda:0") if case == "c5" else W.make(case)
+    assert P["steps"] == cfg["steps"]
     g = fs.from_workload(cfg, device="cuda:0")
-    info = g.step(2, per_step=True)
-    assert info["nan_flag"] == 0 and info["converged"] == 1, info
-    assert all(5 <= n <= 16 for n in info["iters_per_step"]), info
-    assert info["rel_residual"] <= 1e-8                                     # recurrence residual (reading A14)
-    h = cfg["lx"] / N
-    assert info["max_abs_div"] < 1e-3, info                                 # fp32 rounding of O(1) velocities / h (h = 0.012)
+    sh = g.shape
+    # the stored samples are at the indices the script draws from the config; the initial field must be the one the
+    # oracle started from (c5: built by FFT on the device here, on the CPU there: equal to rounding)
+    for c in "uvw":
+        idx = mk.sample_indices(cfg, c, sh[c])
+        assert [q for q, _ in P["ic"][c]] == idx.tolist()
+        got = g.get(c).reshape(-1)[idx]
+        want = np.array([v for _, v in P["ic"][c]])
+        assert np.abs(got - want).max() < 1e-12 * max(1.0, np.abs(want).max()), (case, c)
+    ig = g.step(P["steps"], per_step=True)
+    assert ig["nan_flag"] == 0 and ig["converged"] == 1 and ig["unconverged_steps"] == 0, ig
+    assert all(abs(a - b) <= 1 for a, b in zip(ig["iters_per_step"], P["iters"])), (ig["iters_per_step"], P["iters"])
+    errs = {}
+    for c in "uvwp":
+        a = g.get(c)
+        idx = np.array([q for q, _ in P["val"][c]])
+        want = np.array([v for _, v in P["val"][c]])
+        errs[c] = float(np.abs(a.reshape(-1)[idx] - want).max() / P["max"][c])
+        assert abs(np.abs(a).max() - P["max"][c]) < 1e-9 * P["max"][c], (case, c)
+    assert all(e < 1e-9 for e in errs.values()), (case, errs)
+    for k in ("body_force", "body_disp", "body_vel"):
+        np.testing.assert_allclose(ig[k], P[k], rtol=1e-9, atol=1e-12)
     g.close()

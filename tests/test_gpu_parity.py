@@ -386,9 +386,46 @@ def test_c5_hit_64_fp32_5_steps(fs):
     io = o.step(5)
     g = fs.from_workload(cfg, dtype="f32")
     ig = g.step(5, per_step=True)
-    assert ig["nan_flag"] == 0
+    assert ig["nan_flag"] == 0 and ig["converged"] == 1 and ig["unconverged_steps"] == 0, ig
+    assert all(abs(a - b) <= 1 for a, b in zip(ig["iters_per_step"], io["iters_per_step"])), (ig["iters_per_step"], io["iters_per_step"])
     errs = {c: relerr(g.get(c), o.get(c)) for c in "uvwp"}
     assert all(e < TOL32 for e in errs.values()), errs
+    g.close()
+
+
+def test_tr16_instantiation_vcycle_and_full_steps_on_64x384x64(fs):
+    # ny >= 384 selects the 32-row tiles (TR = 16) of the fused V-cycle legs -- the instantiation bench.py times at
+    # 512^3 -- on a box the oracle steps in seconds: V-cycle element-wise, 10 fp64 steps (1e-9, iterations +-1) and
+    # 5 fp32 steps (1e-4); each part asserts that it ran the instantiation it is meant for.
+    cfg = W.hit_box(64, 384, 64)
+    r = np.random.default_rng(6).standard_normal(W.shapes(cfg)["p"])
+    o = _oracle(cfg)
+    z_ref = o.vcycle(r)
+    g = fs.from_workload(cfg)
+    z = g.gmg_vcycle(r)
+    assert relerr(z, z_ref) < 1e-12, relerr(z, z_ref)
+    used = g.kernels_used()
+    assert "k_mg_down<f64,TR16>" in used and "k_mg_up<f64,TR16>" in used, used
+    io5 = o.step(5)
+    ref5 = {c: o.get(c) for c in "uvwp"}
+    io10 = o.step(5)
+    ig = g.step(10, per_step=True)
+    assert ig["nan_flag"] == 0 and ig["converged"] == 1
+    want = io5["iters_per_step"] + io10["iters_per_step"]
+    assert all(abs(a - b) <= 1 for a, b in zip(ig["iters_per_step"], want)), (ig["iters_per_step"], want)
+    _compare_state(g, o, TOL64)
+    used = g.kernels_used()
+    for k in ("k_mg_down<f64,TR16,UPD>", "k_mg_up<f64,TR16,DOT>", "k_pcg_dirapply2<f64>", "k_projectv<f64>", "k_div_rhsv<f64>", "k_pcg_initv<f64>"):
+        assert k in used, (k, used)
+    g.close()
+    g = fs.from_workload(cfg, dtype="f32")
+    i32 = g.step(5, per_step=True)
+    assert i32["nan_flag"] == 0 and i32["converged"] == 1
+    assert all(abs(a - b) <= 1 for a, b in zip(i32["iters_per_step"], io5["iters_per_step"])), (i32["iters_per_step"], io5["iters_per_step"])
+    errs = {c: relerr(g.get(c), ref5[c]) for c in "uvwp"}
+    assert all(e < TOL32 for e in errs.values()), errs
+    used = g.kernels_used()
+    assert "k_mg_down<f32,TR16,UPD>" in used and "k_mg_up<f32,TR16,DOT>" in used and "k_pcg_dirapplyv<f32>" in used, used
     g.close()
 
 
@@ -450,6 +487,93 @@ def test_device_pointer_io_and_dtype_conversion(fs):
     assert torch.allclose(out, u64, atol=1e-7)
     host32 = g.get("u", dtype="f32")
     assert host32.dtype == np.float32 and np.abs(host32 - cfg["init"]["u"]).max() < 1e-7
+    g.close()
+
+
+def test_marker_support_touching_a_wall_is_unsupported(fs):
+    # same rule, same threshold as the oracle (pin P22): 1.5 h (Roma) from a non-periodic boundary
+    cfg = _cfg_open(40, 30, 28, max_markers=4)
+    h = 1.0 / 16
+    g = fs.Grid(cfg)
+    mid = np.array([20 * h, 15 * h, 14 * h])
+    ok = np.stack([mid, mid]); ok[0, 0] = 1.5 * h + 1e-9; ok[1, 1] = 30 * h - 1.5 * h - 1e-9
+    g.set_markers(ok)
+    assert g.cell_list()["perm"].size == 2
+    for d, bad in ((0, 1.49 * h), (1, 30 * h - 1.49 * h), (2, 1.2 * h)):
+        x = mid.copy(); x[d] = bad
+        with pytest.raises(fs.FsError) as e:
+            g.set_markers(x[None, :])
+        assert e.value.status == fs.FS_ERR_UNSUPPORTED
+        assert g.cell_list()["nseg"] == 0                         # refused: the grid keeps no markers
+    g.close()
+    # a moving body that carries its markers into the wall: reported by the synchronous fs_step, state info still filled
+    cfg = W.cylinder_fsi(scale=8, per_ring=12, rtol=1e-8)
+    g = fs.from_workload(cfg)
+    g.set_body_state([0.0, 0.0, 0.0], [0.0, 400.0, 0.0])
+    g.step(1)
+    info = fs.fs_step_info()
+    import ctypes as C
+    st = fs.lib().fs_step(g.h, 1, C.byref(info))
+    assert st == fs.FS_ERR_UNSUPPORTED and info.step == 2
+    g.close()
+
+
+def test_step_info_is_filled_when_pcg_does_not_converge_and_sticky_counters_count(fs):
+    import ctypes as C
+    cfg = W.channel(n=24, max_iter=3)
+    g = fs.from_workload(cfg)
+    info = fs.fs_step_info()
+    st = fs.lib().fs_step(g.h, 2, C.byref(info))
+    assert st == fs.FS_ERR_NOT_CONVERGED                           # fs.h: *last is valid for this status
+    assert info.pcg_iters == 3 and info.converged == 0 and info.step == 2 and info.unconverged_steps == 2 and info.nan_steps == 0
+    g.step(3, sync=False)                                           # asynchronous steps are counted too
+    assert g.step(0)["unconverged_steps"] == 5
+    g.close()
+    g = fs.from_workload(W.taylor_green())
+    assert g.step(4)["unconverged_steps"] == 0
+    g.close()
+
+
+def test_two_grids_in_one_process_and_device_guard(fs):
+    # per-device kernel attributes are applied per grid (not once per process), and every entry point runs on the
+    # grid's own device: two GMG grids stepped alternately, on two GPUs when the box has them
+    import torch
+    ndev = torch.cuda.device_count()
+    cfgs = [W.hit(n=32), W.hit(n=32, seed=5)]
+    devs = ["cuda:0", "cuda:%d" % (1 if ndev > 1 else 0)]
+    gs = [fs.from_workload(c, device=d) for c, d in zip(cfgs, devs)]
+    torch.cuda.set_device(0)
+    for _ in range(2):
+        for g in gs:
+            assert g.step(1)["converged"] == 1
+    assert torch.cuda.current_device() == 0                         # the caller's device is restored
+    for g, c in zip(gs, cfgs):
+        o = _oracle(c); o.step(2)
+        _compare_state(g, o, TOL64)
+        g.close()
+    # a workspace that is not device memory is refused
+    import ctypes as C
+    P, keep = fs.make_params(cfgs[0])
+    n = C.c_size_t(0)
+    assert fs.lib().fs_workspace_bytes(C.byref(P), C.byref(n)) == 0
+    host = np.zeros(n.value + 256, dtype=np.uint8)
+    ptr = (host.ctypes.data + 255) & ~255
+    h = C.c_void_p()
+    assert fs.lib().fs_grid_create(C.byref(P), C.c_void_p(ptr), n.value, None, C.byref(h)) == 1
+
+
+def test_launch_count_counts_every_loop_body_replay(fs):
+    # graph mode, 32^3 GMG V(2,2): 9 fixed kernels per step (momentum, div_rhs, pcg_init, 4 x finish, project, step_end)
+    # + 4 per loop-body replay (level-0 down leg, one-CTA tail for 16^3..4^3, level-0 up leg, direction+apply); the
+    # fused residual update makes the body run once more than the solve iterates
+    cfg = W.hit(n=32)
+    g = fs.from_workload(cfg)
+    prev = g.launch_count()
+    for _ in range(4):
+        info = g.step(1)
+        n = g.launch_count()
+        assert n - prev == 9 + 4 * (info["pcg_iters"] + 1), (n - prev, info["pcg_iters"])
+        prev = n
     g.close()
 
 
