@@ -160,6 +160,23 @@ class Oracle:
             raise ValueError("oracle: set_markers failed")
         self.nl = n
 
+    def set_solid_mask(self, eps_cells, uc=None):
+        """eps-mask IBM (reading E1): eps_cells (nz, ny, nx) of 0/1, uc the solid's velocity."""
+        if eps_cells is None:
+            lib().orc_set_solid_mask(self.h, None, None)
+            return
+        e = np.ascontiguousarray(eps_cells, dtype=np.uint8)
+        assert e.shape == self.shape["p"]
+        u = _f64(uc if uc is not None else [0.0, 0.0, 0.0])
+        rc = lib().orc_set_solid_mask(self.h, e.ctypes.data_as(C.POINTER(C.c_ubyte)), _dp(u))
+        if rc:
+            raise ValueError("oracle: set_solid_mask failed")
+
+    def face_masks(self):
+        m = [np.empty(self.shape[c], dtype=np.uint8) for c in "uvw"]
+        lib().orc_get_face_masks(self.h, *[a.ctypes.data_as(C.POINTER(C.c_ubyte)) for a in m])
+        return m
+
     def set_body(self, m, c, k, dof_mask):
         assert lib().orc_set_body(self.h, m, c, k, dof_mask) == 0
 

@@ -38,6 +38,9 @@ struct orc_sim {
   bool has_body; double bm, bc_, bk; int dof; double bdisp[3], bvel[3], bforce[3];
   // GMG levels
   int nlev;
+  // volume-of-solid mask (eps-mask IBM, Eq. 5, 8-9, 18-19, 23; reading E1 in DESIGN.md 3)
+  bool has_mask; double uc[3];         // exact velocity of the immersed solid u_c (Eq. 8); a rigid body overrides it with its velocity
+  std::vector<unsigned char> eps, mu, mv, mw;   // cell mask; per-face class of u, v, w: 0 fluid, 1 solid, 2 IB point
 };
 
 static inline int wrapi(int i, int n) { i %= n; return i < 0 ? i + n : i; }
@@ -535,6 +538,99 @@ extern "C" void orc_rk4_body(double m, double c, double k, double F, double dt, 
   *wd = y1 + dt / 6.0 * (k1b + 2.0 * k2b + 2.0 * k3b + k4b);
 }
 
+// ---- O4': the paper-literal eps-mask direct forcing (NEXT-1) -------------------------
+// Reading E1.  eps is given per pressure cell (1 in solid cells, 0 in fluid cells, L110).  A velocity
+// face belongs to the solid when either of the two cells it separates is solid (its control volume intersects the
+// immersed region, L106); prescribed boundary-normal faces are never forced.  IB points (L74): fluid faces with at
+// least one of their six same-component neighbours in the solid.
+static inline int mask_cell(const orc_sim* s, int i, int j, int k) {
+  const int n[3] = {s->nx, s->ny, s->nz}; const int bd[3] = {s->bx, s->by, s->bz}; int id[3] = {i, j, k};
+  for (int d = 0; d < 3; ++d) { if (bd[d]) { if (id[d] < 0 || id[d] >= n[d]) return 0; } else id[d] = wrapi(id[d], n[d]); }
+  return s->eps[IP(s, id[0], id[1], id[2])] ? 1 : 0;
+}
+static void build_face_masks(orc_sim* s) {
+  const int n[3] = {s->nx, s->ny, s->nz}; const int bd[3] = {s->bx, s->by, s->bz};
+  std::vector<unsigned char>* M[3] = {&s->mu, &s->mv, &s->mw};
+  const size_t sz[3] = {s->u.size(), s->v.size(), s->w.size()};
+  for (int c = 0; c < 3; ++c) {
+    M[c]->assign(sz[c], 0);
+    const int e[3] = {n[0] + (c == 0 ? bd[0] : 0), n[1] + (c == 1 ? bd[1] : 0), n[2] + (c == 2 ? bd[2] : 0)};
+    auto idx = [&](int i, int j, int k) { return (size_t)i + (size_t)e[0] * (j + (size_t)e[1] * k); };
+    auto solid = [&](int i, int j, int k) -> int {            // face (i,j,k) of component c: outside the box / prescribed -> 0
+      int id[3] = {i, j, k};
+      for (int d = 0; d < 3; ++d) {
+        if (!bd[d]) { id[d] = wrapi(id[d], n[d]); continue; }
+        if (d == c) { if (id[d] <= 0 || id[d] >= n[d]) return 0; }
+        else if (id[d] < 0 || id[d] >= n[d]) return 0;
+      }
+      int lo[3] = {id[0], id[1], id[2]}; lo[c] -= 1;
+      return (mask_cell(s, id[0], id[1], id[2]) || mask_cell(s, lo[0], lo[1], lo[2])) ? 1 : 0;
+    };
+    for (int k = 0; k < e[2]; ++k) for (int j = 0; j < e[1]; ++j) for (int i = 0; i < e[0]; ++i) {
+      const int id[3] = {i, j, k};
+      if (bd[c] && (id[c] == 0 || id[c] == n[c])) continue;   // prescribed boundary-normal face
+      if (solid(i, j, k)) { (*M[c])[idx(i, j, k)] = 1; continue; }
+      if (solid(i + 1, j, k) || solid(i - 1, j, k) || solid(i, j + 1, k) || solid(i, j - 1, k) || solid(i, j, k + 1) || solid(i, j, k - 1))
+        (*M[c])[idx(i, j, k)] = 2;
+    }
+  }
+}
+// Eq. 18-19: velocity at the IB points from the structure's markers with the half-distribution normalisation,
+//   u_IB(x) = sum_i (1 / F_Ni) wdot(X_i) delta_h(x - X_i) dV_i,   F_Ni = sum_{x in gamma'} delta_h(x - X_i) dv(x)
+// gamma' = the nodes of marker i's support that are NOT in the solid (Eq. 19 as printed has no dv: it would carry units
+// of 1 / volume); a marker whose support holds no such node contributes nothing.
+static void ib_point_velocity(const orc_sim* s, vec& fu, vec& fv, vec& fw) {
+  const int sw = support_width(s);
+  vec G((size_t)3 * s->nl, 0.0);
+  for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) {
+    const std::vector<unsigned char>& m = c == 0 ? s->mu : c == 1 ? s->mv : s->mw;
+    double FN = 0.0;
+    for (int cc = 0; cc < sw; ++cc) for (int b = 0; b < sw; ++b) for (int a = 0; a < sw; ++a) {
+      double wt; long long q = ibm_node(s, l, c, a, b, cc, &wt);
+      if (q >= 0 && m[(size_t)q] != 1) FN += wt;
+    }
+    G[3 * l + c] = FN > 0.0 ? s->Ub[3 * l + c] / FN : 0.0;
+  }
+  spread(s, G, fu, fv, fw);
+}
+// Eq. 4 + Eq. 5: with f = eps [ -(explicit right-hand side) + (u_s - u^t) / dt ] the predictor becomes
+//   u* = (1 - eps) u~ + eps u_s,   u_s = u_c in the solid (Eq. 23, third branch), u_IB at the IB points (second branch,
+// only when markers carry the structure's velocity).  Returns the force on the body, -rho sum_x f(x) dv (Eq. 20 summed).
+static void mask_forcing(orc_sim* s, vec& us, vec& vs, vec& ws) {
+  const double dt = s->P.dt, rho = s->P.rho, dv = s->hx * s->hy * s->hz;
+  double uc[3]; for (int c = 0; c < 3; ++c) uc[c] = s->has_body ? s->bvel[c] : s->uc[c];
+  vec ib[3];
+  const bool with_ib = s->nl > 0;
+  if (with_ib) {
+    orc_ibm_index(s);
+    ib[0].assign(us.size(), 0.0); ib[1].assign(vs.size(), 0.0); ib[2].assign(ws.size(), 0.0);
+    ib_point_velocity(s, ib[0], ib[1], ib[2]);
+  }
+  vec* F[3] = {&us, &vs, &ws};
+  const std::vector<unsigned char>* M[3] = {&s->mu, &s->mv, &s->mw};
+  for (int c = 0; c < 3; ++c) {
+    double acc = 0.0;
+    for (size_t q = 0; q < F[c]->size(); ++q) {
+      const int m = (*M[c])[q];
+      if (m == 0 || (m == 2 && !with_ib)) continue;
+      const double target = m == 1 ? uc[c] : ib[c][q];
+      acc += (target - (*F[c])[q]) / dt * dv;                 // f dv
+      (*F[c])[q] = target;
+    }
+    s->bforce[c] = -rho * acc;
+  }
+}
+// Eq. 9: the field whose divergence drives the Poisson equation, (1 - eps) u* + eps u_c.
+static void poisson_source_field(const orc_sim* s, vec& us, vec& vs, vec& ws) {
+  double uc[3]; for (int c = 0; c < 3; ++c) uc[c] = s->has_body ? s->bvel[c] : s->uc[c];
+  vec* F[3] = {&us, &vs, &ws};
+  const std::vector<unsigned char>* M[3] = {&s->mu, &s->mv, &s->mw};
+  for (int c = 0; c < 3; ++c) for (size_t q = 0; q < F[c]->size(); ++q) {
+    const double e = (*M[c])[q] == 1 ? 1.0 : 0.0;
+    (*F[c])[q] = (1.0 - e) * (*F[c])[q] + e * uc[c];
+  }
+}
+
 // ---- O1..O5: the predicted field ----------------------------------------------------------------
 // upto = 0: after O3 (explicit predictor + prescribed boundary-normal faces), 1: after O4 (IBM direct forcing),
 // 2: after O5 (outflow flux correction).  one_step uses upto = 2; orc_predict exposes the intermediate stages so the
@@ -554,7 +650,8 @@ static void predictor(orc_sim* s, int upto, vec& us, vec& vs, vec& ws, vec& HU, 
   set_boundary_normal(s, us, vs, ws, s->u, s->v, s->w);
   for (int c = 0; c < 3; ++c) s->bforce[c] = 0.0;
   if (upto < 1) return;
-  if (s->nl > 0) {                                                                     // O4
+  if (s->has_mask) mask_forcing(s, us, vs, ws);                                        // O4' (eps-mask IBM, Eq. 4-5, 18-19, 23)
+  else if (s->nl > 0) {                                                                // O4
     orc_ibm_index(s);                                                                  // I-1
     interpolate(s, us, vs, ws, s->Ul);                                                 // I-2
     for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c)                        // I-3 (Eq. 5 at markers)
@@ -576,6 +673,7 @@ static void one_step(orc_sim* s, orc_info* info) {
   const double dt = s->P.dt, rho = s->P.rho;
   vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size()), us, vs, ws;
   predictor(s, 2, us, vs, ws, HU, HV, HW);                                             // O1..O5
+  if (s->has_mask) poisson_source_field(s, us, vs, ws);                                // Eq. 9 (Eq. 7 when eps = 0, L129)
   vec b(s->p.size());
   divergence(s, us, vs, ws, b);                                                        // O6
   for (size_t q = 0; q < b.size(); ++q) b[q] *= rho / dt;
@@ -635,6 +733,7 @@ extern "C" orc_sim* orc_create(const orc_params* p) {
   s->w.assign((size_t)s->nx * s->ny * s->nzw, 0.0); s->p.assign(N, 0.0); s->divu.assign(N, 0.0);
   s->hu = s->u; s->hv = s->v; s->hw = s->w;
   s->have_hist = false; s->step = 0; s->nl = 0; s->nseg = 0; s->has_body = false; s->dof = 0; s->oob = false;
+  s->has_mask = false; s->uc[0] = s->uc[1] = s->uc[2] = 0.0;
   for (int c = 0; c < 3; ++c) s->bdisp[c] = s->bvel[c] = s->bforce[c] = 0.0;
   return s;
 }
@@ -659,6 +758,18 @@ extern "C" int orc_set_markers(orc_sim* s, int n, const double* xyz, const doubl
   orc_ibm_index(s);
   if (s->oob) { s->nl = 0; s->oob = false; return 2; }   // unsupported: marker support touches a non-periodic boundary
   return 0;
+}
+extern "C" int orc_set_solid_mask(orc_sim* s, const unsigned char* eps_cells, const double* uc) {
+  if (!eps_cells) { s->has_mask = false; return 0; }
+  if (!s->uniform_y) return 1;
+  s->eps.assign(eps_cells, eps_cells + s->p.size());
+  for (int c = 0; c < 3; ++c) s->uc[c] = uc ? uc[c] : 0.0;
+  s->has_mask = true;
+  build_face_masks(s);
+  return 0;
+}
+extern "C" void orc_get_face_masks(orc_sim* s, unsigned char* mu, unsigned char* mv, unsigned char* mw) {
+  std::copy(s->mu.begin(), s->mu.end(), mu); std::copy(s->mv.begin(), s->mv.end(), mv); std::copy(s->mw.begin(), s->mw.end(), mw);
 }
 extern "C" int orc_set_body(orc_sim* s, double m, double c, double k, int dof) {
   if (!(m > 0)) return 1;

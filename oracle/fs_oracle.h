@@ -60,6 +60,11 @@ int  orc_set_field(orc_sim*, int field, const double* src);
 int  orc_get_field(orc_sim*, int field, double* dst);
 int  orc_set_markers(orc_sim*, int n, const double* xyz, const double* vel, const double* dvol);
 int  orc_set_body(orc_sim*, double m, double c, double k, int dof_mask);
+/* eps-mask IBM of the paper (Eq. 5, 8-9, 18-19, 23; reading E1): eps_cells nz*ny*nx bytes (1 = solid cell), uc[3] the exact
+ * solid velocity u_c (NULL = 0).  Switches the IBM from marker forcing to mask forcing; markers, if set, then only carry
+ * the structure velocity to the IB points (Eq. 18-19).  eps_cells == NULL switches back. */
+int  orc_set_solid_mask(orc_sim*, const unsigned char* eps_cells, const double* uc);
+void orc_get_face_masks(orc_sim*, unsigned char* mu, unsigned char* mv, unsigned char* mw);   /* 0 fluid, 1 solid, 2 IB point */
 int  orc_step(orc_sim*, int nsteps, orc_info* last, int* iters_per_step /* nsteps ints or NULL */);
 int  orc_poisson_solve(orc_sim*, const double* rhs, double* p_inout, orc_info* info);
 int  orc_set_history(orc_sim*, int have_history, long long step);   /* restart support */
