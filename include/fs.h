@@ -71,7 +71,9 @@ typedef enum { FS_U = 0, FS_V, FS_W, FS_P, FS_HU, FS_HV, FS_HW, FS_DIV,
                FS_MARKER_PERM,   /* n int32: marker ids sorted by (cell key, id) */
                FS_MARKER_KEYS,   /* n int32: sorted cell keys */
                FS_MARKER_SEG,    /* nseg+1 int32 segment starts (call fs_marker_segments for nseg) */
-               FS_BODY_STATE     /* 9 fp64: displacement[3], velocity[3], force[3] */
+               FS_BODY_STATE,    /* 9 fp64: displacement[3], velocity[3], force[3] */
+               FS_MASK_U, FS_MASK_V, FS_MASK_W   /* uint8 per stored face of u / v / w: 0 fluid, 1 solid, 2 IB point (get only;
+                                                    shapes of FS_U / FS_V / FS_W; eps-mask IBM, fs_set_solid_mask) */
              } fs_field;
 
 typedef struct {
@@ -89,6 +91,7 @@ typedef struct {
   uint64_t seed; double inflow_noise;
   fs_exec exec_mode;
   fs_conv convection;          /* convective flux scheme of the momentum RHS */
+  int solid_mask;              /* != 0: reserve workspace for the eps-mask IBM (fs_set_solid_mask) */
 } fs_params;
 
 typedef struct {
@@ -145,6 +148,20 @@ fs_status fs_marker_segments(fs_grid* g, int* nseg);
  * All markers translate with the body. */
 fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask);
 fs_status fs_set_body_state(fs_grid* g, const double* disp3, const double* vel3);   /* HOST */
+
+/* The paper's own IBM: volume-of-solid function eps (1 in solid cells, 0 in fluid cells,
+ * L110) instead of marker forcing.  eps_cells: HOST, nz*ny*nx bytes; uc: HOST, 3 fp64, the exact velocity u_c of the
+ * immersed solid (Eq. 8; NULL = at rest; a rigid body set with fs_set_body overrides it with its own velocity).
+ *   predictor   u* = (1 - eps) u~ + eps u_s                       (Eq. 4 with the forcing of Eq. 5)
+ *               u_s = u_c on faces of solid cells, u_IB at the IB points (Eq. 23)
+ *   IB points   u_IB = sum_i wdot(X_i) delta_h(x - X_i) dV_i / F_Ni,  F_Ni = sum over the fluid nodes of the support
+ *               of delta_h dv   (Eq. 18-19; only when markers are set: they carry the structure's velocity)
+ *   Poisson     lap p = (rho/dt) div[(1 - eps) u* + eps u_c]      (Eq. 9; = Eq. 7 when eps = 0, L129)
+ *   body force  -rho sum_x f(x) dv,  f = (u* - u~)/dt             (Eq. 20 summed over the body, L193)
+ * A face is solid when either cell it separates is solid; IB points are fluid faces with a solid face among their six
+ * same-component neighbours (L74); prescribed boundary-normal faces are never forced.  eps_cells == NULL returns to
+ * marker forcing.  FS_ERR_BAD_STATE unless params.solid_mask != 0; FS_ERR_UNSUPPORTED on a y-stretched grid. */
+fs_status fs_set_solid_mask(fs_grid* g, const unsigned char* eps_cells, const double* uc);
 
 /* Advance nsteps fractional steps: predictor (Eq. 4) -> IBM interpolate / force / spread (Eq. 3b, 5, 3a;
  * L89-91, L108) -> Poisson (Eq. 7) by PCG (L449, L686) -> projection (Eq. 6/10, L114, L131) -> rigid body

@@ -31,8 +31,9 @@ DELTA = {"roma3": 0, "peskin4": 1}
 EXEC = {"graph": 0, "stream": 1}
 FIELD = {"u": 0, "v": 1, "w": 2, "p": 3, "hu": 4, "hv": 5, "hw": 6, "div": 7,
          "marker_x": 8, "marker_u": 9, "marker_f": 10, "marker_base": 11, "marker_perm": 12,
-         "marker_keys": 13, "marker_seg": 14, "body_state": 15}
+         "marker_keys": 13, "marker_seg": 14, "body_state": 15, "mask_u": 16, "mask_v": 17, "mask_w": 18}
 _INT_FIELDS = ("marker_base", "marker_perm", "marker_keys", "marker_seg")
+_BYTE_FIELDS = {"mask_u": "u", "mask_v": "v", "mask_w": "w"}
 
 
 class fs_params(C.Structure):
@@ -48,7 +49,7 @@ class fs_params(C.Structure):
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
                 ("delta", C.c_int), ("max_markers", C.c_int),
                 ("seed", C.c_uint64), ("inflow_noise", C.c_double),
-                ("exec_mode", C.c_int), ("convection", C.c_int)]
+                ("exec_mode", C.c_int), ("convection", C.c_int), ("solid_mask", C.c_int)]
 
 
 class fs_step_info(C.Structure):
@@ -65,7 +66,7 @@ class fs_poisson_info(C.Structure):
 
 # every symbol include/fs.h declares (tests check the library exports all of them)
 SYMBOLS = ("fs_workspace_bytes", "fs_grid_create", "fs_grid_destroy", "fs_field_size", "fs_fields_set",
-           "fs_fields_get", "fs_set_history", "fs_set_ibm_markers", "fs_marker_segments", "fs_set_body",
+           "fs_fields_get", "fs_set_history", "fs_set_ibm_markers", "fs_marker_segments", "fs_set_body", "fs_set_solid_mask",
            "fs_set_body_state", "fs_step", "fs_poisson_solve", "fs_ibm_interpolate", "fs_ibm_spread",
            "fs_gmg_vcycle", "fs_momentum_rhs", "fs_profile_step", "fs_profile_count", "fs_profile_entry",
            "fs_profile_reset", "fs_launch_count", "fs_kernels_used", "fs_status_string")
@@ -99,6 +100,7 @@ def lib():
         L.fs_marker_segments.argtypes = [vp, C.POINTER(C.c_int)]
         L.fs_set_body.argtypes = [vp, C.c_double, C.c_double, C.c_double, ip]
         L.fs_set_body_state.argtypes = [vp, dp, dp]
+        L.fs_set_solid_mask.argtypes = [vp, C.POINTER(C.c_ubyte), dp]
         L.fs_step.argtypes = [vp, ip, C.POINTER(fs_step_info)]
         L.fs_poisson_solve.argtypes = [vp, vp, vp, ip, ip, C.POINTER(fs_poisson_info)]
         L.fs_ibm_interpolate.argtypes = [vp, dp]
@@ -152,6 +154,7 @@ def make_params(cfg):
     P.delta = DELTA[cfg["delta"]]
     P.exec_mode = EXEC[cfg.get("exec_mode", "graph")]
     P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
+    P.solid_mask = int(cfg.get("solid_mask", 0))
     return P, keep
 
 
@@ -237,6 +240,10 @@ class Grid:
             dt = DTYPE["f64" if out.dtype == torch.float64 else "f32"]
             _check(lib().fs_fields_get(self.h, FIELD[name], C.c_void_p(out.data_ptr()), dt, 1), "fs_fields_get")
             return out
+        if name in _BYTE_FIELDS:
+            a = np.empty(n, dtype=np.uint8)
+            _check(lib().fs_fields_get(self.h, FIELD[name], C.c_void_p(a.ctypes.data), DTYPE[dtype], 0), "fs_fields_get")
+            return a.reshape(self.shape[_BYTE_FIELDS[name]])
         if name in _INT_FIELDS:
             a = np.empty(n, dtype=np.int32)
         else:
@@ -271,6 +278,17 @@ class Grid:
         seg = self.get("marker_seg")
         return dict(base=self.get("marker_base"), perm=self.get("marker_perm"), keys=self.get("marker_keys"),
                     seg_start=seg[:ns.value + 1].copy(), nseg=ns.value)
+
+    def set_solid_mask(self, eps_cells, uc=None):
+        """fs_set_solid_mask: eps_cells (nz, ny, nx) of 0/1 (None: back to marker forcing), uc the solid's velocity."""
+        if eps_cells is None:
+            _check(lib().fs_set_solid_mask(self.h, None, None), "fs_set_solid_mask")
+            return
+        e = np.ascontiguousarray(eps_cells, dtype=np.uint8)
+        assert e.shape == self.shape["p"]
+        u = np.ascontiguousarray(uc if uc is not None else [0.0, 0.0, 0.0], dtype=np.float64)
+        _check(lib().fs_set_solid_mask(self.h, e.ctypes.data_as(C.POINTER(C.c_ubyte)), u.ctypes.data_as(C.POINTER(C.c_double))),
+               "fs_set_solid_mask")
 
     def set_body(self, m, c, k, dof_mask):
         _check(lib().fs_set_body(self.h, m, c, k, dof_mask), "fs_set_body")
@@ -386,4 +404,6 @@ def from_workload(cfg, device="cuda:0", **overrides):
         g.set_markers(*c["markers"])
     if c.get("body") is not None:
         g.set_body(*c["body"])
+    if c.get("mask") is not None:
+        g.set_solid_mask(*c["mask"])
     return g

@@ -179,6 +179,12 @@ template <class T> size_t carve(fs_grid* g, char* base) {
   ib.Fl = b.take<double>(3 * M); ib.Ul = b.take<double>(3 * M); ib.wts = b.take<double>(36 * M);
   ib.base = b.take<int>(9 * M); ib.perm = b.take<int>(M); ib.keys = b.take<int>(M); ib.keys_raw = b.take<int>(M);
   ib.seg = b.take<int>(M + 1); ib.flags = b.take<int>(M);
+  ib.eps = ib.mu = ib.mv = ib.mw = nullptr; ib.ibu = ib.ibv = ib.ibw = nullptr;
+  if (P.solid_mask) {                     // eps-mask IBM: cell mask, face classes, and (with markers) the u_IB scratch fields
+    ib.eps = b.take<unsigned char>(g->nP);
+    ib.mu = b.take<unsigned char>(g->nU); ib.mv = b.take<unsigned char>(g->nV); ib.mw = b.take<unsigned char>(g->nW);
+    if (M > 0) { ib.ibu = b.take<T>(g->nU); ib.ibv = b.take<T>(g->nV); ib.ibw = b.take<T>(g->nW); }
+  }
   return (b.off + 255) & ~size_t(255);
 }
 
@@ -257,6 +263,7 @@ void init_ibm(fs_grid* g) {
   }
   ib.ivol = 1.0 / (g->hx * g->hy * g->hz);
   ib.has_body = 0; ib.dof = 0; ib.bm = 1.0; ib.bc = 0.0; ib.bk = 0.0;
+  ib.has_mask = 0; ib.uc[0] = ib.uc[1] = ib.uc[2] = 0.0;
 }
 
 
@@ -268,7 +275,10 @@ template <class T> int enqueue_pre(fs_grid* g, const Launch& L, bool poisson) {
     n += launch_rhs_from_b<T>(c, c.vs, L);
   } else {
     n += launch_momentum<T>(c, L);
-    if (g->ib.n > 0) {
+    if (g->ib.has_mask) {                 // the paper's eps-mask forcing (markers only carry the structure velocity to the IB points)
+      if (g->ib.n > 0 && (g->ib.has_body || !g->indexed)) n += launch_ibm_index<T>(c, g->ib, L);
+      n += launch_mask_forcing<T>(c, g->ib, L);
+    } else if (g->ib.n > 0) {
       if (g->ib.has_body || !g->indexed) n += launch_ibm_index<T>(c, g->ib, L);
       n += launch_ibm_interpolate<T>(c, g->ib, c.us, c.vs, c.ws, g->ib.Ul, L);
       n += launch_ibm_force<T>(c, g->ib, L);
@@ -559,6 +569,9 @@ fs_status fs_field_size(fs_grid* g, fs_field f, long long* count) {
     case FS_MARKER_PERM: case FS_MARKER_KEYS: *count = n; break;
     case FS_MARKER_SEG: *count = n + 1; break;
     case FS_BODY_STATE: *count = 9; break;
+    case FS_MASK_U: *count = (long long)g->nU; break;
+    case FS_MASK_V: *count = (long long)g->nV; break;
+    case FS_MASK_W: *count = (long long)g->nW; break;
     default: return FS_ERR_INVALID_ARG;
   }
   return FS_OK;
@@ -597,6 +610,11 @@ fs_status fs_fields_get(fs_grid* g, fs_field f, void* dst, fs_dtype dtype, int d
     case FS_MARKER_PERM: src = g->ib.perm; bytes = n * sizeof(int); break;
     case FS_MARKER_KEYS: src = g->ib.keys; bytes = n * sizeof(int); break;
     case FS_MARKER_SEG: src = g->ib.seg; bytes = (n + 1) * sizeof(int); break;
+    case FS_MASK_U: case FS_MASK_V: case FS_MASK_W:
+      if (!g->ib.has_mask) return FS_ERR_BAD_STATE;
+      src = f == FS_MASK_U ? g->ib.mu : (f == FS_MASK_V ? g->ib.mv : g->ib.mw);
+      bytes = f == FS_MASK_U ? g->nU : (f == FS_MASK_V ? g->nV : g->nW);
+      break;
     case FS_BODY_STATE: {
       CK(cudaMemcpyAsync(dst, g->S->body_disp, 3 * sizeof(double), kind, g->stream));
       CK(cudaMemcpyAsync((double*)dst + 3, g->S->body_vel, 3 * sizeof(double), kind, g->stream));
@@ -677,6 +695,24 @@ fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask) {
   GUARD(g);
   g->ib.has_body = 1; g->ib.bm = m; g->ib.bc = c; g->ib.bk = k; g->ib.dof = dof_mask;
   invalidate(g);
+  return FS_OK;
+}
+
+fs_status fs_set_solid_mask(fs_grid* g, const unsigned char* eps_cells, const double* uc) {
+  if (!g) return FS_ERR_INVALID_ARG;
+  GUARD(g);
+  if (!g->P.solid_mask) return FS_ERR_BAD_STATE;
+  if (!g->uniform_y) return FS_ERR_UNSUPPORTED;
+  invalidate(g);
+  IbmCtx& ib = g->ib;
+  if (!eps_cells) { ib.has_mask = 0; return FS_OK; }
+  CK(cudaMemcpyAsync(ib.eps, eps_cells, g->nP, cudaMemcpyHostToDevice, g->stream));
+  for (int a = 0; a < 3; ++a) ib.uc[a] = uc ? uc[a] : 0.0;
+  ib.has_mask = 1;
+  Launch L{g->stream, 0, 0, nullptr, &g->seen};
+  g->fixed_launches += g->f64 ? launch_mask_classify<double>(g->cd, ib, L) : launch_mask_classify<float>(g->cf, ib, L);
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(g->stream));
   return FS_OK;
 }
 

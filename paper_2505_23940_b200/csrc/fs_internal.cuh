@@ -86,6 +86,10 @@ struct IbmCtx {
   int *base, *perm, *keys, *keys_raw, *seg, *flags;
   // body (Eq. 12)
   int has_body, dof; double bm, bc, bk;
+  // eps-mask IBM (Eq. 5, 8-9, 18-19, 23): cell mask, per-face classes (0 fluid, 1 solid, 2 IB point), u_c, scratch for u_IB
+  int has_mask; double uc[3];
+  unsigned char *eps, *mu, *mv, *mw;
+  void *ibu, *ibv, *ibw;       // T*: u_IB spread from the markers (Eq. 18), velocity-shaped
 };
 
 // Per-kernel timing (measurement aid, fs_profile_step): when prof != nullptr every launch is bracketed
@@ -163,6 +167,8 @@ template <class T> int launch_ibm_index(const Ctx<T>& c, const IbmCtx& ib, const
 template <class T> int launch_ibm_interpolate(const Ctx<T>& c, const IbmCtx& ib, const T* u, const T* v, const T* w, double* out, const Launch& L);
 template <class T> int launch_ibm_force(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
 template <class T> int launch_ibm_spread(const Ctx<T>& c, const IbmCtx& ib, const double* F, T* u, T* v, T* w, double scale, const Launch& L);
+template <class T> int launch_mask_classify(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
+template <class T> int launch_mask_forcing(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
 
 // ---- device helpers ---------------------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -268,7 +268,118 @@ template <class T> int launch_ibm_spread(const Ctx<T>& c, const IbmCtx& ib, cons
   return 1;
 }
 
+// =====================================================================================================
+// The paper's eps-mask IBM (NEXT-1; Eq. 5, Eq. 8-9, Eq. 18-19, Eq. 23).
+// =====================================================================================================
+// Face classes from the cell mask: a face is solid (1) when either cell it separates is solid, an IB point (2) when it
+// is fluid and one of its six same-component neighbours is solid (L74); prescribed boundary-normal faces and faces
+// outside a bounded box count as fluid and are never forced.  Integer work: compared bit-exact with the oracle.
+template <class T> __device__ __forceinline__ int mask_cell(const Ctx<T>& c, const unsigned char* __restrict__ eps, int i, int j, int k) {
+  if (c.bx) { if (i < 0 || i >= c.nx) return 0; } else i = wrapi(i, c.nx);
+  if (c.by) { if (j < 0 || j >= c.ny) return 0; } else j = wrapi(j, c.ny);
+  if (c.bz) { if (k < 0 || k >= c.nz) return 0; } else k = wrapi(k, c.nz);
+  return eps[(size_t)i + (size_t)c.nx * ((size_t)j + (size_t)c.ny * k)] ? 1 : 0;
+}
+template <class T> __device__ __forceinline__ int face_solid(const Ctx<T>& c, const unsigned char* __restrict__ eps, int comp, int i, int j, int k) {
+  int id[3] = {i, j, k};
+  const int n[3] = {c.nx, c.ny, c.nz}, bd[3] = {c.bx, c.by, c.bz};
+  for (int d = 0; d < 3; ++d) {
+    if (!bd[d]) { id[d] = wrapi(id[d], n[d]); continue; }
+    if (d == comp) { if (id[d] <= 0 || id[d] >= n[d]) return 0; }
+    else if (id[d] < 0 || id[d] >= n[d]) return 0;
+  }
+  int lo[3] = {id[0], id[1], id[2]}; lo[comp] -= 1;
+  return (mask_cell<T>(c, eps, id[0], id[1], id[2]) || mask_cell<T>(c, eps, lo[0], lo[1], lo[2])) ? 1 : 0;
+}
+template <class T> __global__ void __launch_bounds__(256) k_mask_classify(const Ctx<T> c, const IbmCtx ib) {
+  const long long nU = (long long)c.nxu * c.ny * c.nz, nV = (long long)c.nx * c.nyv * c.nz, nW = (long long)c.nx * c.ny * c.nzw;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < nU + nV + nW; t += (long long)gridDim.x * blockDim.x) {
+    const int comp = t < nU ? 0 : (t < nU + nV ? 1 : 2);
+    const long long q = t - (comp == 0 ? 0 : (comp == 1 ? nU : nU + nV));
+    const int ex = comp == 0 ? c.nxu : c.nx, ey = comp == 1 ? c.nyv : c.ny;
+    const int i = (int)(q % ex), j = (int)((q / ex) % ey), k = (int)(q / ((long long)ex * ey));
+    const int id[3] = {i, j, k}, n[3] = {c.nx, c.ny, c.nz}, bd[3] = {c.bx, c.by, c.bz};
+    unsigned char cls = 0;
+    if (!(bd[comp] && (id[comp] == 0 || id[comp] == n[comp]))) {
+      if (face_solid<T>(c, ib.eps, comp, i, j, k)) cls = 1;
+      else if (face_solid<T>(c, ib.eps, comp, i + 1, j, k) || face_solid<T>(c, ib.eps, comp, i - 1, j, k) ||
+               face_solid<T>(c, ib.eps, comp, i, j + 1, k) || face_solid<T>(c, ib.eps, comp, i, j - 1, k) ||
+               face_solid<T>(c, ib.eps, comp, i, j, k + 1) || face_solid<T>(c, ib.eps, comp, i, j, k - 1)) cls = 2;
+    }
+    (comp == 0 ? ib.mu : (comp == 1 ? ib.mv : ib.mw))[q] = cls;
+  }
+}
+template <class T> int launch_mask_classify(const Ctx<T>& c, const IbmCtx& ib, const Launch& L) {
+  FS_LAUNCH(L, "mask_classify", 0.0, k_mask_classify<T><<<148 * 8, 256, 0, L.s>>>(c, ib));
+  return 1;
+}
+
+// Eq. 19: F_Ni = sum over the support nodes of marker i that are NOT solid of delta_h dv (one thread per marker
+// component); the marker's contribution to Eq. 18 is then spread with the weight wdot_i / F_Ni (stored in Fl).
+template <class T> __global__ void __launch_bounds__(128) k_mask_fn(const Ctx<T> c, const IbmCtx ib) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= 3 * ib.n) return;
+  const int l = t / 3, comp = t - 3 * l;
+  const unsigned char* __restrict__ m = comp == 0 ? ib.mu : (comp == 1 ? ib.mv : ib.mw);
+  const int* base = ib.base + ((size_t)comp * ib.n + l) * 3;
+  const double* wt = ib.wts + ((size_t)comp * ib.n + l) * 12;
+  double FN = 0.0;
+  for (int cc = 0; cc < ib.sw; ++cc) {
+    const int kk = node_index<T>(c, base[2] + cc, comp, 2);
+    for (int b = 0; b < ib.sw; ++b) {
+      const int jj = node_index<T>(c, base[1] + b, comp, 1);
+      for (int a = 0; a < ib.sw; ++a) {
+        const int ii = node_index<T>(c, base[0] + a, comp, 0);
+        if (ii < 0 || jj < 0 || kk < 0) continue;
+        if (m[comp_index<T>(c, comp, ii, jj, kk)] != 1) FN += (wt[a] * wt[4 + b]) * wt[8 + cc];
+      }
+    }
+  }
+  ib.Fl[t] = FN > 0.0 ? ib.Ub[t] / FN : 0.0;
+}
+
+// Eq. 4 + Eq. 5 (u* = (1 - eps) u~ + eps u_s), Eq. 23 (u_s = u_c in the solid, u_IB at the IB points) and the force on the
+// body, -rho sum_x f dv with f = (u* - u~)/dt (Eq. 20 summed).  The forced value is also Eq. 9's field
+// (1 - eps) u* + eps u_c: on a solid face u* = u_c, so the combination returns u_c bit for bit.
+template <class T> __global__ void __launch_bounds__(256) k_mask_apply(const Ctx<T> c, const IbmCtx ib, int with_ib) {
+  __shared__ double sh[3 * 32]; __shared__ int flag;
+  const long long nU = (long long)c.nxu * c.ny * c.nz, nV = (long long)c.nx * c.nyv * c.nz, nW = (long long)c.nx * c.ny * c.nzw;
+  double uc[3];
+  for (int a = 0; a < 3; ++a) uc[a] = ib.has_body ? c.S->body_vel[a] : ib.uc[a];
+  double v[3] = {0.0, 0.0, 0.0};
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < nU + nV + nW; t += (long long)gridDim.x * blockDim.x) {
+    const int comp = t < nU ? 0 : (t < nU + nV ? 1 : 2);
+    const long long q = t - (comp == 0 ? 0 : (comp == 1 ? nU : nU + nV));
+    const int cls = (comp == 0 ? ib.mu : (comp == 1 ? ib.mv : ib.mw))[q];
+    if (cls == 0 || (cls == 2 && !with_ib)) continue;
+    T* f = comp == 0 ? c.us : (comp == 1 ? c.vs : c.ws);
+    const T target = cls == 1 ? T(uc[comp]) : reinterpret_cast<const T*>(comp == 0 ? ib.ibu : (comp == 1 ? ib.ibv : ib.ibw))[q];
+    v[comp] += ((double)target - (double)f[q]) / c.dt;
+    f[q] = target;
+  }
+  if (grid_sum<3>(v, c.partials, &c.S->ticket[0], sh, &flag)) {
+    if (threadIdx.x == 0) for (int a = 0; a < 3; ++a) c.S->body_force[a] = -c.rho * (v[a] * (c.hx * c.hy * c.hz));
+  }
+}
+template <class T> int launch_mask_forcing(const Ctx<T>& c, const IbmCtx& ib, const Launch& L) {
+  int n = 0;
+  const int with_ib = ib.n > 0;
+  if (with_ib) {
+    const size_t nU = (size_t)c.nxu * c.ny * c.nz, nV = (size_t)c.nx * c.nyv * c.nz, nW = (size_t)c.nx * c.ny * c.nzw;
+    FS_LAUNCH(L, "mask_ib_points", 0.0, {
+      k_mask_fn<T><<<(3 * ib.n + 127) / 128, 128, 0, L.s>>>(c, ib);
+      cudaMemsetAsync(ib.ibu, 0, nU * sizeof(T), L.s); cudaMemsetAsync(ib.ibv, 0, nV * sizeof(T), L.s); cudaMemsetAsync(ib.ibw, 0, nW * sizeof(T), L.s);
+    });
+    n += 4;
+    n += launch_ibm_spread<T>(c, ib, ib.Fl, (T*)ib.ibu, (T*)ib.ibv, (T*)ib.ibw, 1.0, L);
+  }
+  FS_LAUNCH(L, "mask_forcing", 0.0, k_mask_apply<T><<<148 * 8, 256, 0, L.s>>>(c, ib, with_ib));
+  return n + 1;
+}
+
 #define INST(T)                                                                                                             \
+  template int launch_mask_classify<T>(const Ctx<T>&, const IbmCtx&, const Launch&);                                        \
+  template int launch_mask_forcing<T>(const Ctx<T>&, const IbmCtx&, const Launch&);                                         \
   template int launch_ibm_index<T>(const Ctx<T>&, const IbmCtx&, const Launch&);                                            \
   template int launch_ibm_interpolate<T>(const Ctx<T>&, const IbmCtx&, const T*, const T*, const T*, double*, const Launch&); \
   template int launch_ibm_force<T>(const Ctx<T>&, const IbmCtx&, const Launch&);                                            \

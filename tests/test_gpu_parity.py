@@ -296,6 +296,83 @@ def test_ibm_empty_and_single_marker(fs):
     g.close()
 
 
+# ------------------------------------------------------------------------------------ NEXT-1: the paper's eps-mask IBM
+def _sphere_mask(cfg, centre, radius):
+    c = W.coords(cfg)
+    d2 = ((c["xc"][None, None, :] - centre[0]) ** 2 + (c["yc"][None, :, None] - centre[1]) ** 2 + (c["zc"][:, None, None] - centre[2]) ** 2)
+    return (d2 < radius ** 2).astype(np.uint8)
+
+
+@pytest.mark.parametrize("kind", ["periodic", "open"])
+def test_mask_face_classes_bit_exact(fs, kind):
+    cfg = _cfg_periodic(26, 19, 14, solid_mask=1) if kind == "periodic" else _cfg_open(30, 21, 17, solid_mask=1)
+    rng = np.random.default_rng(41)
+    eps = (rng.random(W.shapes(cfg)["p"]) < 0.2).astype(np.uint8)
+    eps[:, :3, :4] = 1; eps[-2:, :, -3:] = 1                       # solid cells on the box faces / across the periodic seam
+    from oracle import Oracle
+    o = Oracle(cfg); o.set_solid_mask(eps)
+    g = fs.Grid(cfg); g.set_solid_mask(eps)
+    for name, ref in zip(("mask_u", "mask_v", "mask_w"), o.face_masks()):
+        assert np.array_equal(g.get(name), ref), name
+    g.close()
+    g = fs.Grid(dict(cfg, solid_mask=0))
+    with pytest.raises(fs.FsError) as e:
+        g.set_solid_mask(eps)                                      # workspace was not reserved
+    assert e.value.status == 2
+    g.close()
+
+
+@pytest.mark.parametrize("delta", ["roma3", "peskin4"])
+def test_mask_ibm_full_steps_match_oracle(fs, delta):
+    # sphere-shaped solid in the c3-shaped open box; the markers on its surface carry a rigid rotation to the IB points
+    # (Eq. 18-19), the solid itself translates with u_c (Eq. 23); 6 steps, fields 1e-9, forces, face classes bit-exact
+    cfg = W.sphere(scale=4, n_markers=400, delta=delta, solid_mask=1)
+    X = cfg["markers"][0]
+    ctr = np.array([cfg["lx"] / 4.0, cfg["ly"] / 2.0, cfg["lz"] / 2.0])
+    vel = np.cross(np.array([0.0, 0.0, 0.8]), X - ctr)
+    cfg["markers"] = (X, vel, cfg["markers"][2])
+    cfg["mask"] = (_sphere_mask(cfg, ctr, 0.5), [0.05, -0.02, 0.0])
+    o = _oracle(cfg); o.set_solid_mask(*cfg["mask"])
+    g = fs.from_workload(cfg)
+    for name, ref in zip(("mask_u", "mask_v", "mask_w"), o.face_masks()):
+        assert np.array_equal(g.get(name), ref), name
+    io = o.step(6); ig = g.step(6, per_step=True)
+    assert ig["converged"] == 1 and all(abs(a - b) <= 1 for a, b in zip(ig["iters_per_step"], io["iters_per_step"]))
+    _compare_state(g, o, TOL64)
+    np.testing.assert_allclose(ig["body_force"], io["body_force"], rtol=1e-9, atol=1e-12)
+    assert relerr(g.get("marker_f"), o.markers()[2]) < 1e-12        # wdot_i / F_Ni of Eq. 18-19
+    used = g.kernels_used()
+    assert "mask_forcing" in used and "mask_ib_points" in used and "ibm_spread" in used and "ibm_interpolate" not in used, used
+    g.close()
+
+
+def test_mask_ibm_without_markers_rigid_body_and_fp32(fs):
+    # mask only (IB points not forced), the solid moving with a 2-DOF rigid body (u_c = body velocity); fp64 1e-9, fp32 1e-4
+    cfg = W.cylinder_fsi(scale=8, per_ring=12, solid_mask=1)
+    cfg["markers"] = None; cfg["max_markers"] = 0
+    m, _, k, _ = cfg["body"]
+    cfg["body"] = (m, 0.1, k, 3)
+    c = W.coords(cfg)
+    eps = (((c["xc"][None, None, :] - cfg["lx"] / 3.0) ** 2 + (c["yc"][None, :, None] - cfg["ly"] / 2.0) ** 2) < 0.25).astype(np.uint8)
+    eps = np.broadcast_to(eps, W.shapes(cfg)["p"]).copy()
+    cfg["mask"] = (eps, None)
+    o = _oracle(cfg); o.set_solid_mask(eps)
+    g = fs.from_workload(cfg)
+    io = o.step(8); ig = g.step(8, per_step=True)
+    assert all(abs(a - b) <= 1 for a, b in zip(ig["iters_per_step"], io["iters_per_step"]))
+    _compare_state(g, o, TOL64)
+    for k_ in ("body_force", "body_disp", "body_vel"):
+        np.testing.assert_allclose(ig[k_], io[k_], rtol=1e-9, atol=1e-13)
+    assert abs(io["body_vel"][0]) > 0 and abs(io["body_force"][0]) > 0
+    g.close()
+    o5 = _oracle(cfg); o5.set_solid_mask(eps); o5.step(5)
+    g = fs.from_workload(cfg, dtype="f32")
+    g.step(5)
+    errs = {c_: relerr(g.get(c_), o5.get(c_)) for c_ in "uvwp"}
+    assert all(e < TOL32 for e in errs.values()), errs
+    g.close()
+
+
 # ------------------------------------------------------------------------------------ full steps
 def _compare_state(g, o, tol, fields="uvwp"):
     errs = {}
