@@ -12,7 +12,7 @@ import numpy as np
 from .build import build as _build
 
 BC = {"periodic": 0, "noslip": 1, "slip": 2, "inflow": 3, "outflow": 4}
-TIME = {"euler": 0, "ab2": 1}
+TIME = {"euler": 0, "ab2": 1, "rk3": 2}
 PC = {"none": 0, "jacobi": 1, "gmg": 2}
 DELTA = {"roma3": 0, "peskin4": 1}
 FIELD = {"u": 0, "v": 1, "w": 2, "p": 3, "hu": 4, "hv": 5, "hw": 6, "div": 7}
@@ -28,14 +28,15 @@ class _Params(C.Structure):
                 ("time_scheme", C.c_int),
                 ("precond", C.c_int), ("rtol", C.c_double), ("max_iter", C.c_int), ("warm_start", C.c_int),
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
-                ("delta", C.c_int), ("seed", C.c_uint64), ("inflow_noise", C.c_double), ("convection", C.c_int)]
+                ("delta", C.c_int), ("seed", C.c_uint64), ("inflow_noise", C.c_double), ("convection", C.c_int),
+                ("cfl", C.c_double)]
 
 
 class _Info(C.Structure):
     _fields_ = [("pcg_iters", C.c_int), ("converged", C.c_int), ("nan_flag", C.c_int),
                 ("rel_residual", C.c_double), ("true_rel_residual", C.c_double), ("max_abs_div", C.c_double),
                 ("body_force", C.c_double * 3), ("body_disp", C.c_double * 3), ("body_vel", C.c_double * 3),
-                ("step", C.c_longlong)]
+                ("step", C.c_longlong), ("dt", C.c_double), ("time", C.c_double)]
 
 
 _lib = None
@@ -75,7 +76,7 @@ def info_dict(i):
     return dict(pcg_iters=i.pcg_iters, converged=i.converged, nan_flag=i.nan_flag,
                 rel_residual=i.rel_residual, true_rel_residual=i.true_rel_residual,
                 max_abs_div=i.max_abs_div, body_force=list(i.body_force), body_disp=list(i.body_disp),
-                body_vel=list(i.body_vel), step=i.step)
+                body_vel=list(i.body_vel), step=i.step, dt=i.dt, time=i.time)
 
 
 def delta_phi(kind, r):
@@ -117,6 +118,7 @@ class Oracle:
         P.precond = PC[cfg["precond"]]
         P.delta = DELTA[cfg["delta"]]
         P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
+        P.cfl = float(cfg.get("cfl", 0.0))
         self.h = L.orc_create(C.byref(P))
         if not self.h:
             raise ValueError("oracle: invalid parameters")

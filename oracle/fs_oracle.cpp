@@ -30,6 +30,7 @@ struct orc_sim {
   vec yf, dy, yc;                      // faces (ny+1), cell heights (ny), centres (ny)
   vec u, v, w, p, hu, hv, hw, divu;
   bool have_hist; long long step;
+  double dt, dt_prev, time;            // step size of the current / previous step (CFL-adaptive dt), elapsed time
   // markers (always fp64)
   int nl; vec X, Ub, dV, Fl, Ul;       // positions, target vel, volumes, force, interpolated vel
   std::vector<int> base, perm, keys, seg; int nseg;
@@ -204,7 +205,7 @@ static void set_boundary_normal(const orc_sim* s, vec& us, vec& vs, vec& ws,
         } else {  // convective outflow (reading): d(u)/dt + Uc d(u)/dn = 0, first-order upwind
           double dn = d == 1 ? (side ? s->dy[s->ny - 1] : s->dy[0]) : h[d];
           double grad = side ? (old[q] - old[qi]) / dn : (old[qi] - old[q]) / dn;
-          val = old[q] - Ub * s->P.dt * grad;
+          val = old[q] - Ub * s->dt * grad;
         }
         dst[q] = val;
       }
@@ -597,7 +598,7 @@ static void ib_point_velocity(const orc_sim* s, vec& fu, vec& fv, vec& fw) {
 //   u* = (1 - eps) u~ + eps u_s,   u_s = u_c in the solid (Eq. 23, third branch), u_IB at the IB points (second branch,
 // only when markers carry the structure's velocity).  Returns the force on the body, -rho sum_x f(x) dv (Eq. 20 summed).
 static void mask_forcing(orc_sim* s, vec& us, vec& vs, vec& ws) {
-  const double dt = s->P.dt, rho = s->P.rho, dv = s->hx * s->hy * s->hz;
+  const double dt = s->dt, rho = s->P.rho, dv = s->hx * s->hy * s->hz;
   double uc[3]; for (int c = 0; c < 3; ++c) uc[c] = s->has_body ? s->bvel[c] : s->uc[c];
   vec ib[3];
   const bool with_ib = s->nl > 0;
@@ -636,10 +637,12 @@ static void poisson_source_field(const orc_sim* s, vec& us, vec& vs, vec& ws) {
 // 2: after O5 (outflow flux correction).  one_step uses upto = 2; orc_predict exposes the intermediate stages so the
 // tests can pin O1 (convective outflow), I-3/I-4 (forcing scale) and O5 (uniform shift) one by one.
 static void predictor(orc_sim* s, int upto, vec& us, vec& vs, vec& ws, vec& HU, vec& HV, vec& HW) {
-  const double dt = s->P.dt, rho = s->P.rho;
+  const double dt = s->dt, rho = s->P.rho;
   momentum(s, s->u, s->v, s->w, s->P.nu, s->P.body_force, HU, HV, HW);                 // O1+O2
   double a0 = 1.0, a1 = 0.0;
-  if (s->P.time_scheme == ORC_TIME_AB2 && s->have_hist) { a0 = 1.5; a1 = -0.5; }
+  // AB2 with the step-size ratio r = dt_n / dt_{n-1} (CFL-adaptive dt, L431): a0 = 1 + r/2, a1 = -r/2; r = 1 exactly for
+  // a fixed step, i.e. (3/2, -1/2).  Euler and the stages of the Runge-Kutta scheme use (1, 0) = Eq. 4 as printed.
+  if (s->P.time_scheme == ORC_TIME_AB2 && s->have_hist) { const double r = dt / s->dt_prev; a0 = 1.0 + 0.5 * r; a1 = -0.5 * r; }
   us = s->u; vs = s->v; ws = s->w;                                                     // O3
   for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = s->bx; i < s->nx; ++i) {
     size_t q = IU(s, i, j, k); us[q] = s->u[q] + dt * (a0 * HU[q] + a1 * s->hu[q]); }
@@ -668,10 +671,10 @@ static void predictor(orc_sim* s, int upto, vec& us, vec& vs, vec& ws, vec& HU, 
   flux_correction(s, us, vs, ws);                                                      // O5
 }
 
-// ---- one fractional step (O1..O9 in order) -----------------------------------------------------
-static void one_step(orc_sim* s, orc_info* info) {
-  const double dt = s->P.dt, rho = s->P.rho;
-  vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size()), us, vs, ws;
+// ---- the fluid part of one fractional step (O1..O8) from the current u, v, w, p with step size s->dt ---------------
+static void fluid_substep(orc_sim* s, orc_info* info, vec& HU, vec& HV, vec& HW) {
+  const double dt = s->dt, rho = s->P.rho;
+  vec us, vs, ws;
   predictor(s, 2, us, vs, ws, HU, HV, HW);                                             // O1..O5
   if (s->has_mask) poisson_source_field(s, us, vs, ws);                                // Eq. 9 (Eq. 7 when eps = 0, L129)
   vec b(s->p.size());
@@ -683,6 +686,51 @@ static void one_step(orc_sim* s, orc_info* info) {
   for (size_t q = 0; q < us.size(); ++q) s->u[q] = us[q] - dt / rho * gu[q];
   for (size_t q = 0; q < vs.size(); ++q) s->v[q] = vs[q] - dt / rho * gv[q];
   for (size_t q = 0; q < ws.size(); ++q) s->w[q] = ws[q] - dt / rho * gw[q];
+}
+
+// CFL-adaptive step size ("governed by the CFL condition based on the instantaneous maximum velocity";
+// reading N3-2): dt = min(dt_max, CFL h_min / max(|u|, |v|, |w|)) over all stored faces at time level n, with
+// dt_max = the configured dt and h_min the smallest cell extent.  cfl <= 0: fixed dt.
+static double choose_dt(const orc_sim* s) {
+  if (!(s->P.cfl > 0.0)) return s->P.dt;
+  double umax = 0.0;
+  for (double x : s->u) umax = std::max(umax, std::fabs(x));
+  for (double x : s->v) umax = std::max(umax, std::fabs(x));
+  for (double x : s->w) umax = std::max(umax, std::fabs(x));
+  double hmin = std::min(s->hx, s->hz);
+  for (double d : s->dy) hmin = std::min(hmin, d);
+  if (!(umax > 0.0)) return s->P.dt;
+  return std::min(s->P.dt, s->P.cfl * hmin / umax);
+}
+
+// ---- one fractional step (O1..O9 in order) -----------------------------------------------------
+static void one_step(orc_sim* s, orc_info* info) {
+  s->dt = choose_dt(s);
+  const double dt = s->dt;
+  vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size());
+  if (s->P.time_scheme == ORC_TIME_RK3) {
+    // Explicit Runge-Kutta (L100, L431, Table 1; the paper names no tableau -- reading N3-3): the three-stage
+    // third-order strong-stability-preserving scheme in Shu-Osher form, every stage a complete fractional step
+    // E(u) = P[u + dt H(u) + IBM] (Eq. 4-10 with the Euler coefficients):
+    //   u1 = E(u^n),  u2 = 3/4 u^n + 1/4 E(u1),  u^{n+1} = 1/3 u^n + 2/3 E(u2).
+    // Convex combinations of projected fields stay divergence free.  p is the last stage's pressure (each solve
+    // starts from the previous one), IBM force / body update use the last stage, iterations are summed.
+    const vec u0 = s->u, v0 = s->v, w0 = s->w;
+    const double c0[3] = {0.0, 0.75, 1.0 / 3.0}, c1[3] = {1.0, 0.25, 2.0 / 3.0};
+    int iters = 0, conv = 1;
+    for (int st = 0; st < 3; ++st) {
+      fluid_substep(s, info, HU, HV, HW);
+      iters += info->pcg_iters; conv = conv && info->converged;
+      if (st > 0) {
+        for (size_t q = 0; q < s->u.size(); ++q) s->u[q] = c0[st] * u0[q] + c1[st] * s->u[q];
+        for (size_t q = 0; q < s->v.size(); ++q) s->v[q] = c0[st] * v0[q] + c1[st] * s->v[q];
+        for (size_t q = 0; q < s->w.size(); ++q) s->w[q] = c0[st] * w0[q] + c1[st] * s->w[q];
+      }
+    }
+    info->pcg_iters = iters; info->converged = conv;
+  } else {
+    fluid_substep(s, info, HU, HV, HW);
+  }
   divergence(s, s->u, s->v, s->w, s->divu);
   double md = 0.0; int nan = 0;
   for (size_t q = 0; q < s->divu.size(); ++q) { double a = std::fabs(s->divu[q]); if (a > md) md = a; if (a != a) nan = 1; }
@@ -697,8 +745,9 @@ static void one_step(orc_sim* s, orc_info* info) {
     for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) s->Ub[3 * l + c] = s->bvel[c];
   }
   s->hu = HU; s->hv = HV; s->hw = HW; s->have_hist = true; s->step += 1;
+  s->dt_prev = dt; s->time += dt;
   for (int c = 0; c < 3; ++c) { info->body_force[c] = s->bforce[c]; info->body_disp[c] = s->bdisp[c]; info->body_vel[c] = s->bvel[c]; }
-  info->step = s->step;
+  info->step = s->step; info->dt = dt; info->time = s->time;
 }
 
 // ---- C interface --------------------------------------------------------------------------------
@@ -734,6 +783,7 @@ extern "C" orc_sim* orc_create(const orc_params* p) {
   s->hu = s->u; s->hv = s->v; s->hw = s->w;
   s->have_hist = false; s->step = 0; s->nl = 0; s->nseg = 0; s->has_body = false; s->dof = 0; s->oob = false;
   s->has_mask = false; s->uc[0] = s->uc[1] = s->uc[2] = 0.0;
+  s->dt = s->dt_prev = p->dt; s->time = 0.0;
   for (int c = 0; c < 3; ++c) s->bdisp[c] = s->bvel[c] = s->bforce[c] = 0.0;
   return s;
 }
@@ -804,6 +854,7 @@ extern "C" void orc_momentum_rhs(orc_sim* s, double* hu, double* hv, double* hw)
 }
 extern "C" int orc_predict(orc_sim* s, int stage, double* us, double* vs, double* ws) {
   if (stage < 0 || stage > 2) return 1;
+  s->dt = choose_dt(s);
   vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size()), a, b, c;
   predictor(s, stage, a, b, c, HU, HV, HW);
   std::copy(a.begin(), a.end(), us); std::copy(b.begin(), b.end(), vs); std::copy(c.begin(), c.end(), ws);

@@ -23,7 +23,7 @@ extern "C" {
 #endif
 
 enum { ORC_BC_PERIODIC = 0, ORC_BC_NOSLIP = 1, ORC_BC_SLIP = 2, ORC_BC_INFLOW = 3, ORC_BC_OUTFLOW = 4 };
-enum { ORC_TIME_EULER = 0, ORC_TIME_AB2 = 1 };
+enum { ORC_TIME_EULER = 0, ORC_TIME_AB2 = 1, ORC_TIME_RK3 = 2 };   /* Eq. 4 / configs / "explicit Runge-Kutta" (L100, L431) */
 enum { ORC_PC_NONE = 0, ORC_PC_JACOBI = 1, ORC_PC_GMG = 2 };
 enum { ORC_DELTA_ROMA3 = 0, ORC_DELTA_PESKIN4 = 1 };
 enum { ORC_CONV_CENTRAL = 0, ORC_CONV_UPWIND = 1 };   /* 2nd-order central or 1st-order upwind convection */
@@ -42,6 +42,7 @@ typedef struct {
   int delta;
   uint64_t seed; double inflow_noise;
   int convection;            /* ORC_CONV_* */
+  double cfl;                /* > 0: CFL-adaptive step size, dt = min(dt, cfl h_min / |u|_max) (L431); <= 0: fixed dt */
 } orc_params;
 
 typedef struct {
@@ -49,6 +50,7 @@ typedef struct {
   double rel_residual, true_rel_residual, max_abs_div;
   double body_force[3], body_disp[3], body_vel[3];
   long long step;
+  double dt, time;           /* step size used by the last step, elapsed time */
 } orc_info;
 
 typedef struct orc_sim orc_sim;
