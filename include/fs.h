@@ -54,7 +54,11 @@ typedef enum { FS_F32 = 0, FS_F64 = 1 } fs_dtype;
 /* Boundary types of PAPER.md Table 1 (L429, L454-456). */
 typedef enum { FS_BC_PERIODIC = 0, FS_BC_NOSLIP = 1, FS_BC_SLIP = 2, FS_BC_INFLOW = 3,
                FS_BC_OUTFLOW_CONVECTIVE = 4 } fs_bc;
-typedef enum { FS_TIME_EULER = 0, FS_TIME_AB2 = 1 } fs_time;               /* Eq. 4 / configs */
+typedef enum { FS_TIME_EULER = 0,   /* Eq. 4 as printed (L104) */
+               FS_TIME_AB2 = 1,     /* u~ = u + dt (a0 H^n + a1 H^{n-1}); a0 = 1 + r/2, a1 = -r/2, r = dt_n / dt_{n-1} (configs) */
+               FS_TIME_RK3 = 2      /* "explicit Runge-Kutta" (L100, L431, Table 1): three-stage SSP scheme, each stage a full
+                                       fractional step E(u): u1 = E(u^n), u2 = 3/4 u^n + 1/4 E(u1), u^{n+1} = 1/3 u^n + 2/3 E(u2) */
+             } fs_time;
 typedef enum { FS_PC_NONE = 0, FS_PC_JACOBI = 1, FS_PC_GMG = 2 } fs_precond; /* CG: L449, L686 */
 typedef enum { FS_DELTA_ROMA3 = 0, FS_DELTA_PESKIN4 = 1 } fs_delta;        /* Eq. 21-22 */
 typedef enum { FS_EXEC_GRAPH = 0,   /* one CUDA-graph replay per step, PCG loop = conditional WHILE node */
@@ -92,6 +96,8 @@ typedef struct {
   fs_exec exec_mode;
   fs_conv convection;          /* convective flux scheme of the momentum RHS */
   int solid_mask;              /* != 0: reserve workspace for the eps-mask IBM (fs_set_solid_mask) */
+  double cfl;                  /* > 0: CFL-adaptive step (L431): dt = min(dt, cfl h_min / max|u,v,w|) from the field at the start
+                                  of every step, h_min the smallest cell extent; <= 0: fixed dt */
 } fs_params;
 
 typedef struct {
@@ -103,6 +109,7 @@ typedef struct {
   long long step;
   long long unconverged_steps;  /* sticky, since fs_grid_create: steps whose PCG hit max_iter ...            */
   long long nan_steps;          /* ... and steps whose projected field held a NaN (also seen by async steps) */
+  double dt, time;              /* step size of the last step (CFL-adaptive dt), elapsed time since the grid was created */
 } fs_step_info;
 typedef struct { int iters; int converged; double rel_residual, true_rel_residual; } fs_poisson_info;
 

@@ -25,7 +25,7 @@ FS_ERR_NOT_CONVERGED = 5
 FS_ERR_UNSUPPORTED = 6
 DTYPE = {"f32": 0, "f64": 1}
 BC = {"periodic": 0, "noslip": 1, "slip": 2, "inflow": 3, "outflow": 4}
-TIME = {"euler": 0, "ab2": 1}
+TIME = {"euler": 0, "ab2": 1, "rk3": 2}
 PC = {"none": 0, "jacobi": 1, "gmg": 2}
 DELTA = {"roma3": 0, "peskin4": 1}
 EXEC = {"graph": 0, "stream": 1}
@@ -49,14 +49,15 @@ class fs_params(C.Structure):
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
                 ("delta", C.c_int), ("max_markers", C.c_int),
                 ("seed", C.c_uint64), ("inflow_noise", C.c_double),
-                ("exec_mode", C.c_int), ("convection", C.c_int), ("solid_mask", C.c_int)]
+                ("exec_mode", C.c_int), ("convection", C.c_int), ("solid_mask", C.c_int), ("cfl", C.c_double)]
 
 
 class fs_step_info(C.Structure):
     _fields_ = [("pcg_iters", C.c_int), ("converged", C.c_int), ("nan_flag", C.c_int),
                 ("rel_residual", C.c_double), ("true_rel_residual", C.c_double), ("max_abs_div", C.c_double),
                 ("body_force", C.c_double * 3), ("body_disp", C.c_double * 3), ("body_vel", C.c_double * 3),
-                ("step", C.c_longlong), ("unconverged_steps", C.c_longlong), ("nan_steps", C.c_longlong)]
+                ("step", C.c_longlong), ("unconverged_steps", C.c_longlong), ("nan_steps", C.c_longlong),
+                ("dt", C.c_double), ("time", C.c_double)]
 
 
 class fs_poisson_info(C.Structure):
@@ -155,6 +156,7 @@ def make_params(cfg):
     P.exec_mode = EXEC[cfg.get("exec_mode", "graph")]
     P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
     P.solid_mask = int(cfg.get("solid_mask", 0))
+    P.cfl = float(cfg.get("cfl", 0.0))
     return P, keep
 
 
@@ -162,7 +164,8 @@ def _info_dict(i):
     return dict(pcg_iters=i.pcg_iters, converged=i.converged, nan_flag=i.nan_flag,
                 rel_residual=i.rel_residual, true_rel_residual=i.true_rel_residual,
                 max_abs_div=i.max_abs_div, body_force=list(i.body_force), body_disp=list(i.body_disp),
-                body_vel=list(i.body_vel), step=i.step, unconverged_steps=i.unconverged_steps, nan_steps=i.nan_steps)
+                body_vel=list(i.body_vel), step=i.step, unconverged_steps=i.unconverged_steps, nan_steps=i.nan_steps,
+                dt=i.dt, time=i.time)
 
 
 class Grid:

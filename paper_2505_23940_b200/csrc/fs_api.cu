@@ -119,6 +119,7 @@ fs_status validate(const fs_params* p) {
   if ((long long)((p->nx + 29) / 30) * ((p->ny + 3) / 4) > kMaxPartials) return FS_ERR_UNSUPPORTED;   // one reduction partial per xy tile
   if (p->yf) for (int j = 0; j < p->ny; ++j) if (!(p->yf[j + 1] > p->yf[j])) return FS_ERR_INVALID_ARG;
   if ((int)p->convection < 0 || (int)p->convection > 1) return FS_ERR_INVALID_ARG;
+  if ((int)p->time_scheme < 0 || (int)p->time_scheme > 2) return FS_ERR_INVALID_ARG;
   if ((int)p->precond < 0 || (int)p->precond > 2 || (int)p->delta < 0 || (int)p->delta > 1) return FS_ERR_INVALID_ARG;
   if (p->precond == FS_PC_GMG) {
     const double hx = p->lx / p->nx, hy = p->ly / p->ny, hz = p->lz / p->nz;
@@ -156,6 +157,8 @@ template <class T> size_t carve(fs_grid* g, char* base) {
   c.hu = b.take<T>(g->nU); c.hv = b.take<T>(g->nV); c.hw = b.take<T>(g->nW);
   c.p = b.take<T>(g->nP); c.r = b.take<T>(g->nP); c.d = b.take<T>(g->nP); c.d2 = b.take<T>(g->nP); c.q = b.take<T>(g->nP); c.bh = b.take<T>(g->nP);
   c.z = nullptr; c.r2 = nullptr;
+  c.q0u = c.q0v = c.q0w = nullptr;
+  if (P.time_scheme == FS_TIME_RK3) { c.q0u = b.take<T>(g->nU); c.q0v = b.take<T>(g->nV); c.q0w = b.take<T>(g->nW); }
   mg.nlev = 0;
   if (P.precond == FS_PC_GMG) {
     c.z = b.take<T>(g->nP);
@@ -236,6 +239,7 @@ template <class T> fs_status upload_metrics(fs_grid* g) {
   Scalars hs; std::memset(&hs, 0, sizeof hs);
   hs.sum_dy = sdy * (double)P.nx * (double)P.nz;
   hs.max_iter = P.max_iter; hs.rtol = P.rtol; hs.rho_prev = 1.0; hs.dq = 1.0;
+  hs.dt = hs.dt_prev = P.dt; hs.conv_acc = 1;
   CK(cudaMemcpyAsync(g->S, &hs, sizeof hs, cudaMemcpyHostToDevice, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   // constants
@@ -245,6 +249,8 @@ template <class T> fs_status upload_metrics(fs_grid* g) {
   c.hx = g->hx; c.hy = g->hy; c.hz = g->hz; c.dt = P.dt; c.rho = P.rho; c.nu = P.nu;
   for (int a = 0; a < 3; ++a) c.g[a] = P.body_force[a];
   c.x0 = P.x0; c.y0 = P.y0; c.z0 = P.z0;
+  c.cfl = P.cfl; c.hmin = std::min(g->hx, g->hz);
+  for (int j = 0; j < ny; ++j) c.hmin = std::min(c.hmin, dy[j]);
   c.ihx = (T)(1.0 / g->hx); c.ihz = (T)(1.0 / g->hz);
   c.ihx2 = (T)(1.0 / (g->hx * g->hx)); c.ihz2 = (T)(1.0 / (g->hz * g->hz));
   c.time_scheme = (int)P.time_scheme; c.precond = (int)P.precond; c.warm_start = P.warm_start; c.delta = (int)P.delta;
@@ -282,7 +288,7 @@ template <class T> int enqueue_pre(fs_grid* g, const Launch& L, bool poisson) {
       if (g->ib.has_body || !g->indexed) n += launch_ibm_index<T>(c, g->ib, L);
       n += launch_ibm_interpolate<T>(c, g->ib, c.us, c.vs, c.ws, g->ib.Ul, L);
       n += launch_ibm_force<T>(c, g->ib, L);
-      n += launch_ibm_spread<T>(c, g->ib, g->ib.Fl, c.us, c.vs, c.ws, c.dt, L);
+      n += launch_ibm_spread<T>(c, g->ib, g->ib.Fl, c.us, c.vs, c.ws, -1.0, L);
     }
     n += launch_flux_correction<T>(c, L);
     n += launch_div_rhs<T>(c, L);
@@ -291,41 +297,52 @@ template <class T> int enqueue_pre(fs_grid* g, const Launch& L, bool poisson) {
   return n;
 }
 template <class T> int enqueue_body(fs_grid* g, const Launch& L) { return launch_pcg_body<T>(ctx<T>(g), mgc<T>(g), L); }
-template <class T> int enqueue_post(fs_grid* g, const Launch& L, bool poisson) {
+// stage / nstages: Runge-Kutta (FS_TIME_RK3) runs pre / loop / post three times per step, the other schemes once
+template <class T> int enqueue_post(fs_grid* g, const Launch& L, bool poisson, int stage, int nstages) {
   Ctx<T>& c = ctx<T>(g);
   int n = launch_pcg_finish<T>(c, L);
   if (poisson) n += launch_true_residual<T>(c, L);
-  else { n += launch_project<T>(c, L); n += launch_step_end<T>(c, g->ib, L); }
+  else {
+    n += launch_project<T>(c, L);
+    if (nstages > 1) n += launch_stage_end<T>(c, stage, L);
+    if (stage == nstages - 1) n += launch_step_end<T>(c, g->ib, L);
+  }
   return n;
 }
+inline int num_stages(const fs_grid* g, bool poisson) { return (!poisson && g->P.time_scheme == FS_TIME_RK3) ? 3 : 1; }
 
 template <class T> fs_status build_graph_impl(fs_grid* g, bool poisson, cudaGraphExec_t* out, int* n_fixed, int* n_body, bool* body_open) {
   cudaStream_t s = g->cap;
   cudaStreamCaptureStatus st; cudaGraph_t graph = nullptr; const cudaGraphNode_t* deps = nullptr; size_t nd = 0;
   CK(cudaStreamGetCaptureInfo_v2(s, &st, nullptr, &graph, &deps, &nd));
-  cudaGraphConditionalHandle h;
-  CK(cudaGraphConditionalHandleCreate(&h, graph, 0, cudaGraphCondAssignDefault));
-  Launch L{s, h, 1, nullptr, &g->seen};
-  const int npre = enqueue_pre<T>(g, L, poisson);
-  CK(cudaGetLastError());
-  CK(cudaStreamGetCaptureInfo_v2(s, &st, nullptr, &graph, &deps, &nd));
-  cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
-  np.conditional.handle = h; np.conditional.type = cudaGraphCondTypeWhile; np.conditional.size = 1;
-  cudaGraphNode_t node;
-  CK(cudaGraphAddNode(&node, graph, deps, nd, &np));
-  cudaGraph_t body = np.conditional.phGraph_out[0];
-  CK(cudaStreamBeginCaptureToGraph(g->cap2, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
-  *body_open = true;
-  Launch Lb{g->cap2, h, 1, nullptr, &g->seen};
-  const int nbody = enqueue_body<T>(g, Lb);
-  CK(cudaGetLastError());
-  cudaGraph_t tmp = nullptr;
-  *body_open = false;
-  CK(cudaStreamEndCapture(g->cap2, &tmp));
-  CK(cudaStreamUpdateCaptureDependencies(s, &node, 1, cudaStreamSetCaptureDependencies));
-  const int npost = enqueue_post<T>(g, L, poisson);
-  CK(cudaGetLastError());
-  *n_fixed = npre + npost; *n_body = nbody;
+  const int nst = num_stages(g, poisson);
+  int nfix = 0, nbody = 0;
+  if (!poisson) { Launch L0{s, 0, 0, nullptr, &g->seen}; nfix += launch_step_begin<T>(ctx<T>(g), L0); CK(cudaGetLastError()); }
+  for (int stage = 0; stage < nst; ++stage) {          // one conditional WHILE node (one PCG solve) per stage
+    cudaGraphConditionalHandle h;
+    CK(cudaGraphConditionalHandleCreate(&h, graph, 0, cudaGraphCondAssignDefault));
+    Launch L{s, h, 1, nullptr, &g->seen};
+    nfix += enqueue_pre<T>(g, L, poisson);
+    CK(cudaGetLastError());
+    CK(cudaStreamGetCaptureInfo_v2(s, &st, nullptr, &graph, &deps, &nd));
+    cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+    np.conditional.handle = h; np.conditional.type = cudaGraphCondTypeWhile; np.conditional.size = 1;
+    cudaGraphNode_t node;
+    CK(cudaGraphAddNode(&node, graph, deps, nd, &np));
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    CK(cudaStreamBeginCaptureToGraph(g->cap2, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    *body_open = true;
+    Launch Lb{g->cap2, h, 1, nullptr, &g->seen};
+    nbody = enqueue_body<T>(g, Lb);
+    CK(cudaGetLastError());
+    cudaGraph_t tmp = nullptr;
+    *body_open = false;
+    CK(cudaStreamEndCapture(g->cap2, &tmp));
+    CK(cudaStreamUpdateCaptureDependencies(s, &node, 1, cudaStreamSetCaptureDependencies));
+    nfix += enqueue_post<T>(g, L, poisson, stage, nst);
+    CK(cudaGetLastError());
+  }
+  *n_fixed = nfix; *n_body = nbody;
   return FS_OK;
 }
 
@@ -352,18 +369,22 @@ template <class T> fs_status build_graph(fs_grid* g, bool poisson, cudaGraphExec
 // FS_EXEC_STREAM: same kernels, launched directly; the host polls the done flag between chunks.
 template <class T> fs_status run_stream(fs_grid* g, bool poisson, int* n_fixed, int* n_body) {
   Launch L{g->stream, 0, 0, g->profiling ? &g->prof : nullptr, &g->seen};
-  const int npre = enqueue_pre<T>(g, L, poisson);
-  int nbody = 0;
-  for (;;) {
-    int done = 0;
-    CK(cudaMemcpyAsync(&done, &g->S->done, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
-    CK(cudaStreamSynchronize(g->stream));
-    if (done) break;
-    for (int a = 0; a < 4; ++a) nbody = enqueue_body<T>(g, L);
+  const int nst = num_stages(g, poisson);
+  int nfix = 0, nbody = 0;
+  if (!poisson) nfix += launch_step_begin<T>(ctx<T>(g), L);
+  for (int stage = 0; stage < nst; ++stage) {
+    nfix += enqueue_pre<T>(g, L, poisson);
+    for (;;) {
+      int done = 0;
+      CK(cudaMemcpyAsync(&done, &g->S->done, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
+      CK(cudaStreamSynchronize(g->stream));
+      if (done) break;
+      for (int a = 0; a < 4; ++a) nbody = enqueue_body<T>(g, L);
+    }
+    nfix += enqueue_post<T>(g, L, poisson, stage, nst);
   }
-  const int npost = enqueue_post<T>(g, L, poisson);
   CK(cudaGetLastError());
-  *n_fixed = npre + npost; *n_body = nbody;
+  *n_fixed = nfix; *n_body = nbody;
   return FS_OK;
 }
 
@@ -742,6 +763,7 @@ fs_status fs_step(fs_grid* g, int nsteps, fs_step_info* last) {
   for (int a = 0; a < 3; ++a) { I.body_force[a] = hs.body_force[a]; I.body_disp[a] = hs.body_disp[a]; I.body_vel[a] = hs.body_vel[a]; }
   I.step = hs.step;
   I.unconverged_steps = hs.unconverged_steps; I.nan_steps = hs.nan_steps;
+  I.dt = hs.dt_prev; I.time = hs.time;
   *last = I;                        // valid for FS_OK, FS_ERR_NOT_CONVERGED and FS_ERR_UNSUPPORTED (fs.h)
   if (hs.ibm_oob) return FS_ERR_UNSUPPORTED;
   return (nsteps > 0 && !hs.converged) ? FS_ERR_NOT_CONVERGED : FS_OK;

@@ -32,6 +32,9 @@ struct Scalars {
   int max_iter, pad0;
   double rtol;
   // step control
+  double dt, dt_prev, time;   // step size of the current / previous step (CFL-adaptive dt lives on the device), elapsed time
+  double umax;                // max |u|, |v|, |w| over all stored faces (k_dt_begin)
+  int iter_acc, conv_acc, body_acc, pad4;   // Runge-Kutta: PCG iterations / convergence / body replays summed over the stages
   long long step; int have_hist; int nan_flag;
   double max_div, true_rr;
   long long total_iters, total_body;          // PCG iterations / loop-body replays of all steps so far
@@ -49,7 +52,8 @@ template <class T> struct Ctx {
   int nx, ny, nz, bx, by, bz, nxu, nyv, nzw;
   int bc[6];
   double bcv[6][3];
-  double hx, hy, hz, dt, rho, nu, g[3];
+  double hx, hy, hz, dt, rho, nu, g[3];   // dt: the configured (maximum) step; kernels read the current one from S->dt
+  double cfl, hmin;
   double x0, y0, z0;
   T ihx, ihz, ihx2, ihz2;
   int time_scheme, precond, warm_start, delta, uniform_y, convection;
@@ -65,6 +69,7 @@ template <class T> struct Ctx {
   const double* dy64;  // [ny] fp64 cell heights (reductions, flux areas)
   // fields
   T *u, *v, *w, *p, *us, *vs, *ws, *hu, *hv, *hw;
+  T *q0u, *q0v, *q0w;    // u^n kept for the Runge-Kutta stage combinations (FS_TIME_RK3 only, else nullptr)
   T *r, *r2, *d, *d2, *q, *z, *bh;   // r2: second residual buffer (GMG fused update), else nullptr
   Scalars* S;
   double* partials;     // [kRedSlots][kMaxPartials]
@@ -141,6 +146,8 @@ template <class T> int launch_rhs_from_b(const Ctx<T>& c, const T* b, const Laun
 template <class T> int launch_project(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_divergence(const Ctx<T>& c, const T* u, const T* v, const T* w, T* out, const Launch& L);
 template <class T> int launch_step_end(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
+template <class T> int launch_step_begin(const Ctx<T>& c, const Launch& L);                      // CFL dt, Runge-Kutta u^n copy
+template <class T> int launch_stage_end(const Ctx<T>& c, int stage, const Launch& L);           // Runge-Kutta stage combination
 template <class TS, class TD> void launch_convert(const TS* src, TD* dst, long long n, cudaStream_t s);
 template <class T> void launch_scale(T* x, double a, long long n, cudaStream_t s);
 
@@ -166,6 +173,7 @@ template <class T> cudaError_t mgf_configure_device();
 template <class T> int launch_ibm_index(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
 template <class T> int launch_ibm_interpolate(const Ctx<T>& c, const IbmCtx& ib, const T* u, const T* v, const T* w, double* out, const Launch& L);
 template <class T> int launch_ibm_force(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
+// scale < 0: the field receives (current dt) x the spread force (u* = u~ + dt f, Eq. 4); else scale x
 template <class T> int launch_ibm_spread(const Ctx<T>& c, const IbmCtx& ib, const double* F, T* u, T* v, T* w, double scale, const Launch& L);
 template <class T> int launch_mask_classify(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
 template <class T> int launch_mask_forcing(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);

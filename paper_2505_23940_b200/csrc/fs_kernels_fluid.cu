@@ -44,7 +44,7 @@ template <class T> __device__ __forceinline__ T boundary_normal(const Ctx<T>& c,
   const double dn = d == 0 ? c.hx : (d == 1 ? (double)c.dy64[jedge] : c.hz);
   const double o = (double)old[q], oi = (double)old[qi];
   const double grad = side ? (o - oi) / dn : (oi - o) / dn;
-  return T(o - Ub * c.dt * grad);
+  return T(o - Ub * c.S->dt * grad);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -118,8 +118,9 @@ template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 
   const bool own = tx >= 1 && tx <= kMomTX - 2 && ty >= 1 && ty <= kMomTY - 2 && iu < c.nxu && ju < c.nyv;
   const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nzw);
   const bool ab2 = c.time_scheme == FS_TIME_AB2 && c.S->have_hist;
-  const T a0 = ab2 ? T(1.5) : T(1), a1 = ab2 ? T(-0.5) : T(0);
-  const T dt = T(c.dt), nu = T(c.nu);
+  const double rdt = ab2 ? c.S->dt / c.S->dt_prev : 0.0;       // step-size ratio (1 exactly for a fixed step: a0 = 3/2, a1 = -1/2)
+  const T a0 = ab2 ? T(1.0 + 0.5 * rdt) : T(1), a1 = ab2 ? T(-0.5 * rdt) : T(0);
+  const T dt = T(c.S->dt), nu = T(c.nu);
   constexpr bool upw = UPW;                // convective scheme: compile-time, so the central path carries no selects
   const T* __restrict__ U = c.u; const T* __restrict__ V = c.v; const T* __restrict__ W = c.w;
   const ColRef<T> ru = col_setup<T, 0>(c, i, j), rv = col_setup<T, 1>(c, i, j), rw = col_setup<T, 2>(c, i, j);
@@ -339,7 +340,7 @@ constexpr int kFlatBlocks = 148 * 8;
 template <class T> __global__ void __launch_bounds__(256) k_div_rhs(const Ctx<T> c, const T* __restrict__ bsrc) {
   __shared__ double sh[32]; __shared__ int flag;
   const long long N = (long long)c.nx * c.ny * c.nz;
-  const T sc = T(c.rho / c.dt);
+  const T sc = T(c.rho / c.S->dt);
   double v[1] = {0.0};
   for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
@@ -383,7 +384,7 @@ template <class T> __global__ void __launch_bounds__(256) k_div_rhsv(const Ctx<T
     const unsigned plc = (unsigned)c.nx * c.ny, plv = (unsigned)c.nx * c.nyv;
     const unsigned oc = (unsigned)gx + (unsigned)c.nx * gy, oe = (unsigned)xe + (unsigned)c.nx * gy;
     const unsigned ov = (unsigned)gx + (unsigned)c.nx * gy, ovp = (unsigned)gx + (unsigned)c.nx * jp;
-    const T ihx = c.ihx, ihz = c.ihz, idy = c.idy[gy + 1], sc = T(c.rho / c.dt), mdy = -c.dy[gy + 1];
+    const T ihx = c.ihx, ihz = c.ihz, idy = c.idy[gy + 1], sc = T(c.rho / c.S->dt), mdy = -c.dy[gy + 1];
     W wb = ld16<T>(c.ws + (oc + plc * (unsigned)k0));
 #pragma unroll 2
     for (int k = k0; k < k1; ++k) {
@@ -489,8 +490,8 @@ template <class T> __global__ void __launch_bounds__(256) k_project(const Ctx<T>
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k0 = blockIdx.z * kz;
-  const T dtr = T(c.dt / c.rho);
-  const double sc = c.rho / c.dt, mc = c.S->mean_coef;
+  const T dtr = T(c.S->dt / c.rho);
+  const double sc = c.rho / c.S->dt, mc = c.S->mean_coef;
   double v[1] = {0.0}; double md = 0.0; int nan = 0;
   if (i < c.nxu && j < c.nyv) {
     const int k1 = min(k0 + kz, c.nzw);
@@ -551,9 +552,9 @@ template <class T> __global__ void __launch_bounds__(32 * PjTile<T>::TY, 2) k_pr
   const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nzw);
   const unsigned plc = (unsigned)c.nx * c.ny, plv = (unsigned)c.nx * c.nyv;
   const unsigned rowc_o = (unsigned)sx + (unsigned)c.nx * syc, rowv_o = (unsigned)sx + (unsigned)c.nx * syv;
-  const T dtr = T(c.dt / c.rho), ihx = c.ihx, ihz = c.ihz;
+  const T dtr = T(c.S->dt / c.rho), ihx = c.ihx, ihz = c.ihz;
   const T idycj = c.idyc[syv], idyj = c.idy[syc + 1];
-  const double sc = c.rho / c.dt, mc = c.S->mean_coef, dyj = c.dy64[syc];
+  const double sc = c.rho / c.S->dt, mc = c.S->mean_coef, dyj = c.dy64[syc];
   const int o_own = ty * ROWE + lane * VX;
   const int o_s = (ty > 0 ? ty - 1 : 0) * ROWE + lane * VX, o_n = (ty < kPjTY - 1 ? ty + 1 : ty) * ROWE + lane * VX;
   const int o_w = ty * ROWE + (lane > 0 ? lane * VX - 1 : 0), o_e = ty * ROWE + (lane < 31 ? lane * VX + VX : 32 * VX - 1);
@@ -675,7 +676,7 @@ template <class T> __global__ void k_step_end(const Ctx<T> c, const IbmCtx ib) {
   if (threadIdx.x == 0) {
     for (int a = 0; a < 3; ++a) { dw[a] = 0.0; nv[a] = S->body_vel[a]; }
     if (ib.has_body) {
-      const double dt = c.dt, m = ib.bm, cc = ib.bc, kk = ib.bk;
+      const double dt = S->dt, m = ib.bm, cc = ib.bc, kk = ib.bk;
       for (int a = 0; a < 3; ++a) if (ib.dof & (1 << a)) {
         const double F = S->body_force[a], y0 = S->body_disp[a], y1 = S->body_vel[a];
         const double k1a = y1,                  k1b = body_acc(F, cc, kk, m, y0, y1);
@@ -688,6 +689,10 @@ template <class T> __global__ void k_step_end(const Ctx<T> c, const IbmCtx ib) {
         S->body_disp[a] = w1; S->body_vel[a] = v1;
       }
     }
+    if (c.time_scheme == FS_TIME_RK3) {     // what the step reports: sums over the three stage solves
+      S->iter = S->iter_acc; S->converged = S->conv_acc; S->body_runs = S->body_acc;
+    }
+    S->dt_prev = S->dt; S->time += S->dt;
     S->have_hist = 1; S->step += 1; S->total_iters += S->iter; S->total_body += S->body_runs;
     S->unconverged_steps += S->converged ? 0 : 1; S->nan_steps += S->nan_flag ? 1 : 0;
   }
@@ -702,6 +707,71 @@ template <class T> __global__ void k_step_end(const Ctx<T> c, const IbmCtx ib) {
 }
 template <class T> int launch_step_end(const Ctx<T>& c, const IbmCtx& ib, const Launch& L) {
   FS_LAUNCH(L, "step_end", 0.0, k_step_end<T><<<1, 256, 0, L.s>>>(c, ib));
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Step begin.  CFL-adaptive step size (reading N3-2): dt = min(dt_max, cfl h_min / max|u, v, w|) over all
+// stored faces of the field at time level n; the maximum is order independent (atomicMax on the bit pattern of a
+// non-negative double), the last CTA turns it into S->dt.  Runge-Kutta: u^n is kept for the stage combinations.
+// ---------------------------------------------------------------------------------------------------
+template <class T> __global__ void __launch_bounds__(256) k_dt_begin(const Ctx<T> c) {
+  __shared__ int last;
+  const long long nU = (long long)c.nxu * c.ny * c.nz, nV = (long long)c.nx * c.nyv * c.nz, nW = (long long)c.nx * c.ny * c.nzw;
+  double m = 0.0;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < nU + nV + nW; q += (long long)gridDim.x * blockDim.x) {
+    const T x = q < nU ? c.u[q] : (q < nU + nV ? c.v[q - nU] : c.w[q - nU - nV]);
+    m = fmax(m, fabs((double)x));
+  }
+  m = warp_max(m);
+  if ((threadIdx.x & 31) == 0 && m > 0.0) atomicMax((unsigned long long*)&c.S->umax, (unsigned long long)__double_as_longlong(m));
+  __syncthreads();
+  if (threadIdx.x == 0) { __threadfence(); last = atomicAdd(&c.S->ticket[1], 1u) == gridDim.x - 1; }
+  __syncthreads();
+  if (last && threadIdx.x == 0) {
+    __threadfence();
+    const double um = __longlong_as_double((long long)atomicAdd((unsigned long long*)&c.S->umax, 0ULL));
+    c.S->dt = um > 0.0 ? fmin(c.dt, c.cfl * c.hmin / um) : c.dt;
+    c.S->umax = 0.0; c.S->ticket[1] = 0u;
+  }
+}
+template <class T> __global__ void k_rk_begin(const Ctx<T> c) { c.S->iter_acc = 0; c.S->conv_acc = 1; c.S->body_acc = 0; }
+template <class T> int launch_step_begin(const Ctx<T>& c, const Launch& L) {
+  int n = 0;
+  if (c.cfl > 0.0) {
+    const long long N = (long long)c.nxu * c.ny * c.nz + (long long)c.nx * c.nyv * c.nz + (long long)c.nx * c.ny * c.nzw;
+    FS_LAUNCH(L, "dt_cfl", 3.0 * sizeof(T) * c.nx * c.ny * c.nz, k_dt_begin<T><<<flat_blocks(N), 256, 0, L.s>>>(c)); ++n;
+  }
+  if (c.time_scheme == FS_TIME_RK3) {
+    FS_LAUNCH(L, "rk_save", 6.0 * sizeof(T) * c.nx * c.ny * c.nz, {
+      k_rk_begin<T><<<1, 1, 0, L.s>>>(c);
+      cudaMemcpyAsync(c.q0u, c.u, sizeof(T) * (size_t)c.nxu * c.ny * c.nz, cudaMemcpyDeviceToDevice, L.s);
+      cudaMemcpyAsync(c.q0v, c.v, sizeof(T) * (size_t)c.nx * c.nyv * c.nz, cudaMemcpyDeviceToDevice, L.s);
+      cudaMemcpyAsync(c.q0w, c.w, sizeof(T) * (size_t)c.nx * c.ny * c.nzw, cudaMemcpyDeviceToDevice, L.s);
+    });
+    n += 4;
+  }
+  return n;
+}
+// Runge-Kutta stage end: u <- c0 u^n + c1 u (stages 1, 2; Shu-Osher weights 3/4, 1/4 and 1/3, 2/3), and the per-step sums
+template <class T> __global__ void __launch_bounds__(256) k_rk_combine(const Ctx<T> c, T c0, T c1, int combine) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    Scalars* S = c.S;
+    S->iter_acc += S->iter; S->conv_acc = S->conv_acc && S->converged; S->body_acc += S->body_runs;
+  }
+  if (!combine) return;
+  const long long nU = (long long)c.nxu * c.ny * c.nz, nV = (long long)c.nx * c.nyv * c.nz, nW = (long long)c.nx * c.ny * c.nzw;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < nU + nV + nW; q += (long long)gridDim.x * blockDim.x) {
+    if (q < nU) c.u[q] = c0 * c.q0u[q] + c1 * c.u[q];
+    else if (q < nU + nV) c.v[q - nU] = c0 * c.q0v[q - nU] + c1 * c.v[q - nU];
+    else c.w[q - nU - nV] = c0 * c.q0w[q - nU - nV] + c1 * c.w[q - nU - nV];
+  }
+}
+template <class T> int launch_stage_end(const Ctx<T>& c, int stage, const Launch& L) {
+  const double c0[3] = {0.0, 0.75, 1.0 / 3.0}, c1[3] = {1.0, 0.25, 2.0 / 3.0};
+  const long long N = (long long)c.nxu * c.ny * c.nz + (long long)c.nx * c.nyv * c.nz + (long long)c.nx * c.ny * c.nzw;
+  FS_LAUNCH(L, "rk_combine", (stage > 0 ? 9.0 : 0.0) * sizeof(T) * c.nx * c.ny * c.nz,
+            k_rk_combine<T><<<stage > 0 ? flat_blocks(N) : 1, 256, 0, L.s>>>(c, T(c0[stage]), T(c1[stage]), stage > 0));
   return 1;
 }
 
@@ -731,6 +801,8 @@ template <class T> void launch_scale(T* x, double a, long long n, cudaStream_t s
   template int launch_project<T>(const Ctx<T>&, const Launch&);                                        \
   template int launch_divergence<T>(const Ctx<T>&, const T*, const T*, const T*, T*, const Launch&);   \
   template int launch_step_end<T>(const Ctx<T>&, const IbmCtx&, const Launch&);                        \
+  template int launch_step_begin<T>(const Ctx<T>&, const Launch&);                                     \
+  template int launch_stage_end<T>(const Ctx<T>&, int, const Launch&);                                 \
   template void launch_scale<T>(T*, double, long long, cudaStream_t);
 INST(float)
 INST(double)

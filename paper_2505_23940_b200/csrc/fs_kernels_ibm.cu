@@ -177,7 +177,7 @@ template <class T> __global__ void __launch_bounds__(1024) k_ibm_force(const Ctx
   double v[3] = {0.0, 0.0, 0.0};
   for (int l = threadIdx.x; l < ib.n; l += blockDim.x)
     for (int a = 0; a < 3; ++a) {
-      const double F = (ib.Ub[3 * l + a] - ib.Ul[3 * l + a]) / c.dt;
+      const double F = (ib.Ub[3 * l + a] - ib.Ul[3 * l + a]) / c.S->dt;
       ib.Fl[3 * l + a] = F;
       v[a] += F * ib.dV[l];
     }
@@ -213,6 +213,7 @@ __device__ __forceinline__ int cell_intervals(int m, int n, int bounded, int (&a
 template <class T> __global__ void __launch_bounds__(128) k_ibm_spread(const Ctx<T> c, const IbmCtx ib, const double* __restrict__ F,
                                                                       T* __restrict__ u, T* __restrict__ v, T* __restrict__ w, double scale) {
   const Scalars* S = c.S;
+  if (scale < 0.0) scale = S->dt;          // u* = u~ + dt f with the step size of this step (Eq. 4)
   const int n[3] = {c.nx, c.ny, c.nz}, bd[3] = {c.bx, c.by, c.bz};
   int lo[3], ext[3];
   for (int d = 0; d < 3; ++d) {
@@ -354,7 +355,7 @@ template <class T> __global__ void __launch_bounds__(256) k_mask_apply(const Ctx
     if (cls == 0 || (cls == 2 && !with_ib)) continue;
     T* f = comp == 0 ? c.us : (comp == 1 ? c.vs : c.ws);
     const T target = cls == 1 ? T(uc[comp]) : reinterpret_cast<const T*>(comp == 0 ? ib.ibu : (comp == 1 ? ib.ibv : ib.ibw))[q];
-    v[comp] += ((double)target - (double)f[q]) / c.dt;
+    v[comp] += ((double)target - (double)f[q]) / c.S->dt;
     f[q] = target;
   }
   if (grid_sum<3>(v, c.partials, &c.S->ticket[0], sh, &flag)) {

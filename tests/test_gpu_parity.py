@@ -296,6 +296,57 @@ def test_ibm_empty_and_single_marker(fs):
     g.close()
 
 
+# ------------------------------------------------------------------------------------ NEXT-3: Runge-Kutta, CFL-adaptive dt
+def test_rk3_matches_oracle_and_the_stability_polynomial(fs):
+    cfg = W.taylor_green(n=16, nu=0.1, dt=0.05, time_scheme="rk3", rtol=1e-13)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 5, iters_pm=3)           # iterations are summed over the three stage solves
+    h = 2 * math.pi / 16
+    z = -0.1 * (8.0 / h ** 2 * math.sin(h / 2) ** 2) * 0.05
+    assert abs(np.abs(g.get("u")).max() / np.abs(cfg["init"]["u"]).max() - (1 + z + z * z / 2 + z ** 3 / 6) ** 5) < 1e-12
+    assert abs(ig["time"] - 0.25) < 1e-15 and ig["dt"] == 0.05
+    g.close()
+    # nonlinear cases: GMG-PCG HIT box (fused V-cycle path, three WHILE nodes per graph) and the walled channel
+    for cfg, steps in ((W.hit(n=32, time_scheme="rk3"), 3), (W.channel(n=24, time_scheme="rk3"), 3),
+                       (W.cylinder_fsi(scale=8, per_ring=12, time_scheme="rk3"), 3)):
+        g, o, ig, io, _ = _run_pair(fs, cfg, steps, iters_pm=3)
+        np.testing.assert_allclose(ig["body_disp"], io["body_disp"], rtol=1e-9, atol=1e-15)
+        np.testing.assert_allclose(ig["body_force"], io["body_force"], rtol=1e-9, atol=1e-12)
+        assert "rk_combine" in g.kernels_used()
+        g.close()
+    # graph replay == direct launches, bit for bit; fp32 within 1e-4 of the oracle
+    cfg = W.hit(n=32, time_scheme="rk3")
+    g1 = fs.from_workload(cfg, exec_mode="graph"); g2 = fs.from_workload(cfg, exec_mode="stream")
+    i1 = g1.step(2, per_step=True); i2 = g2.step(2, per_step=True)
+    assert i1["iters_per_step"] == i2["iters_per_step"]
+    for c in "uvwp":
+        assert np.array_equal(g1.get(c), g2.get(c)), c
+    g1.close(); g2.close()
+    o = _oracle(cfg); o.step(3)
+    g = fs.from_workload(cfg, dtype="f32"); g.step(3)
+    errs = {c: relerr(g.get(c), o.get(c)) for c in "uvwp"}
+    assert all(e < TOL32 for e in errs.values()), errs
+    g.close()
+
+
+@pytest.mark.parametrize("scheme", ["ab2", "euler", "rk3"])
+def test_cfl_adaptive_dt_matches_oracle(fs, scheme):
+    # the step size is chosen on the device from max|u| of the current field; same sequence of dt as the oracle
+    for cfg in (W.channel(n=24, cfl=0.35, dt=1e-3, time_scheme=scheme), W.cylinder_fsi(scale=8, per_ring=12, cfl=0.2, dt=2e-2, time_scheme=scheme)):
+        o = _oracle(cfg)
+        g = fs.from_workload(cfg)
+        dts = []
+        for s_ in range(5):
+            io = o.step(1); ig = g.step(1)
+            assert abs(ig["dt"] - io["dt"]) <= 1e-13 * io["dt"], (s_, ig["dt"], io["dt"])
+            assert abs(ig["pcg_iters"] - io["pcg_iters"]) <= (3 if scheme == "rk3" else 1)
+            dts.append(io["dt"])
+        assert abs(ig["time"] - io["time"]) < 1e-12 * io["time"]
+        assert max(dts) < cfg["dt"] and len(set(dts)) > 1            # the CFL limit is active and moves
+        _compare_state(g, o, TOL64)
+        assert "dt_cfl" in g.kernels_used()
+        g.close()
+
+
 # ------------------------------------------------------------------------------------ NEXT-1: the paper's eps-mask IBM
 def _sphere_mask(cfg, centre, radius):
     c = W.coords(cfg)
