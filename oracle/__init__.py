@@ -29,7 +29,7 @@ class _Params(C.Structure):
                 ("precond", C.c_int), ("rtol", C.c_double), ("max_iter", C.c_int), ("warm_start", C.c_int),
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
                 ("delta", C.c_int), ("seed", C.c_uint64), ("inflow_noise", C.c_double), ("convection", C.c_int),
-                ("cfl", C.c_double)]
+                ("cs", C.c_double), ("wall_model", C.c_int), ("cfl", C.c_double)]
 
 
 class _Info(C.Structure):
@@ -53,6 +53,8 @@ def lib():
         L.orc_delta_phi.argtypes = [C.c_int, C.c_double]
         L.orc_inflow_rand.restype = C.c_double
         L.orc_inflow_rand.argtypes = [C.c_uint64, C.c_longlong, C.c_int, C.c_int, C.c_int]
+        L.orc_wall_utau.restype = C.c_double
+        L.orc_wall_utau.argtypes = [C.c_double] * 3
         L.orc_rk4_body.argtypes = [C.c_double] * 5 + [C.POINTER(C.c_double)] * 2
         L.orc_set_body.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_int]
         L.orc_set_history.argtypes = [C.c_void_p, C.c_int, C.c_longlong]
@@ -87,6 +89,10 @@ def inflow_rand(seed, step, face, a, b):
     return lib().orc_inflow_rand(int(seed), int(step), int(face), int(a), int(b))
 
 
+def wall_utau(U, y, nu):
+    return lib().orc_wall_utau(float(U), float(y), float(nu))
+
+
 def rk4_body(m, c, k, F, dt, w, wd):
     a, b = C.c_double(w), C.c_double(wd)
     lib().orc_rk4_body(m, c, k, F, dt, C.byref(a), C.byref(b))
@@ -119,6 +125,8 @@ class Oracle:
         P.delta = DELTA[cfg["delta"]]
         P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
         P.cfl = float(cfg.get("cfl", 0.0))
+        P.cs = float(cfg.get("cs", 0.0))
+        P.wall_model = int(cfg.get("wall_model", 0))
         self.h = L.orc_create(C.byref(P))
         if not self.h:
             raise ValueError("oracle: invalid parameters")
@@ -244,6 +252,9 @@ class Oracle:
         g = [np.empty(self.shape[c]) for c in "uvw"]
         assert lib().orc_predict(self.h, int(stage), _dp(g[0]), _dp(g[1]), _dp(g[2])) == 0
         return g
+
+    def eddy_viscosity(self):
+        out = np.empty(self.shape["p"]); lib().orc_eddy_viscosity(self.h, _dp(out)); return out
 
     def convection(self):
         g = [np.empty(self.shape[c]) for c in "uvw"]

@@ -104,11 +104,85 @@ static inline double interpY(const orc_sim* s, double a, double b, int jf) {
 static inline double TR(const orc_sim* s, double a, double minus, double plus, double central) {
   return s->P.convection == ORC_CONV_UPWIND ? (a > 0.0 ? minus : plus) : central;
 }
+// ---- LES closures (NEXT-4; section 3.4.5) ---------------------------------------------
+// Constant Smagorinsky model (reading N4-1): nu_t = (C_s Delta)^2 |S| at cell centres, Delta = (hx dy_j hz)^(1/3),
+// |S| = sqrt(2 S_ij S_ij) with the diagonal gradients from the cell's own faces and the cross gradients as central
+// differences of the face values averaged to the cell centres (ghost values from the O1 accessors).
+static void eddy_viscosity(const orc_sim* s, const vec& uu, const vec& vv, const vec& ww, vec& nut) {
+  const double hx = s->hx, hz = s->hz, cs = s->P.cs;
+  for (int k = 0; k < s->nz; ++k) for (int j = 0; j < s->ny; ++j) for (int i = 0; i < s->nx; ++i) {
+    auto ux = [&](int jj, int kk) { return 0.5 * (U_(i, jj, kk) + U_(i + 1, jj, kk)); };     // u at the centres of column i
+    auto vy = [&](int ii, int kk) { return 0.5 * (V_(ii, j, kk) + V_(ii, j + 1, kk)); };
+    auto wz = [&](int ii, int jj) { return 0.5 * (W_(ii, jj, k) + W_(ii, jj, k + 1)); };
+    const double dyc2 = DYC(s, j + 1) + DYC(s, j);                                           // y_c(j+1) - y_c(j-1)
+    const double dudx = (U_(i + 1, j, k) - U_(i, j, k)) / hx, dvdy = (V_(i, j + 1, k) - V_(i, j, k)) / s->dy[j];
+    const double dwdz = (W_(i, j, k + 1) - W_(i, j, k)) / hz;
+    const double dudy = (ux(j + 1, k) - ux(j - 1, k)) / dyc2, dudz = (ux(j, k + 1) - ux(j, k - 1)) / (2.0 * hz);
+    const double dvdx = (vy(i + 1, k) - vy(i - 1, k)) / (2.0 * hx), dvdz = (vy(i, k + 1) - vy(i, k - 1)) / (2.0 * hz);
+    const double dwdx = (wz(i + 1, j) - wz(i - 1, j)) / (2.0 * hx), dwdy = (wz(i, j + 1) - wz(i, j - 1)) / dyc2;
+    const double S2 = 2.0 * (dudx * dudx + dvdy * dvdy + dwdz * dwdz)
+                    + (dudy + dvdx) * (dudy + dvdx) + (dudz + dwdx) * (dudz + dwdx) + (dvdz + dwdy) * (dvdz + dwdy);
+    const double delta = std::cbrt(hx * s->dy[j] * hz);
+    nut[IP(s, i, j, k)] = (cs * delta) * (cs * delta) * std::sqrt(S2);
+  }
+}
+// nu_t of cell (i,j,k): wrapped in periodic directions, the boundary cell's value beyond a bounded end
+static inline double NT(const orc_sim* s, const vec& nut, int i, int j, int k) {
+  i = s->bx ? std::min(std::max(i, 0), s->nx - 1) : wrapi(i, s->nx);
+  j = s->by ? std::min(std::max(j, 0), s->ny - 1) : wrapi(j, s->ny);
+  k = s->bz ? std::min(std::max(k, 0), s->nz - 1) : wrapi(k, s->nz);
+  return nut[IP(s, i, j, k)];
+}
+// Equilibrium wall model (Eq. 27, Spalding's law, kappa = 0.4, B = 5): friction velocity u_tau for the wall-parallel
+// speed U at the distance y from the wall, by Newton-Raphson on
+//   g(u_tau) = u+ + e^{-kappa B} [e^{kappa u+} - 1 - kappa u+ - (kappa u+)^2/2 - (kappa u+)^3/6] - y+,  u+ = U/u_tau, y+ = y u_tau/nu.
+// g is convex and decreasing in u_tau, so Newton's iterates rise monotonically to the root from any start on its left
+// (g >= 0).  Start: u+_0 = min( sqrt(Re_y), max(12.5, ln(1.182 Re_y) / kappa) ), Re_y = U y / nu = u+ y+ -- the viscous
+// sublayer value (exact for small Re_y) capped by an upper bound of the root that follows from
+// Re_y >= u+ e^{-kappa B} e^{kappa u+} / 2 for kappa u+ >= 5; both are >= the root's u+, i.e. u_tau,0 <= the root.
+// A fixed 30 iterations (convergence is quadratic after two or three; no data-dependent exit).
+extern "C" double orc_wall_utau(double U, double y, double nu) {
+  if (!(U > 0.0)) return 0.0;
+  const double kap = 0.4, eB = std::exp(-kap * 5.0);
+  const double Rey = U * y / nu;
+  const double up0 = std::min(std::sqrt(Rey), std::max(12.5, std::log(1.182 * Rey) / kap));
+  double ut = U / up0;
+  for (int it = 0; it < 30; ++it) {
+    const double up = U / ut, yp = y * ut / nu, ku = kap * up, e = std::exp(ku);
+    const double gval = up + eB * (e - 1.0 - ku - 0.5 * ku * ku - ku * ku * ku / 6.0) - yp;
+    const double dgdup = 1.0 + eB * kap * (e - 1.0 - ku - 0.5 * ku * ku);
+    const double dg = dgdup * (-up / ut) - y / nu;
+    ut = ut - gval / dg;
+  }
+  return ut;
+}
+// Eq. 28-29: eddy viscosity that makes the wall flux of the tangential component `comp` (velocity rel, other tangential
+// component other, both relative to the wall, at the first off-wall point, distance y) equal to the modelled stress:
+//   tau_w = rho u_tau^2,  tau_wi = tau_w u_i / sqrt(u^2 + w^2),  nu_ti = (tau_wi / rho) / (du_i/dy + eps) - nu,  eps = 1e-6,
+// with du_i/dy = u_i / y (the one-sided gradient the no-slip ghost value produces at the wall face).
+static double wall_nut(const orc_sim* s, double rel, double other, double y) {
+  const double U = std::sqrt(rel * rel + other * other);
+  if (!(U > 0.0)) return 0.0;
+  const double ut = orc_wall_utau(U, y, s->P.nu);
+  const double tau_i = ut * ut * rel / U;                     // tau_wi / rho
+  return tau_i / (rel / y + 1e-6) - s->P.nu;
+}
+
 static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& ww,
                      double nu, const double g[3], vec& HU, vec& HV, vec& HW) {
   const int nx = s->nx, ny = s->ny, nz = s->nz;
   const double hx = s->hx, hz = s->hz;
   std::fill(HU.begin(), HU.end(), 0.0); std::fill(HV.begin(), HV.end(), 0.0); std::fill(HW.begin(), HW.end(), 0.0);
+  // LES: diffusive term div[(nu + nu_t) grad u_i] with nu_t at the flux locations (cell centres natively, edges as the
+  // mean of the four surrounding cells); wall model: nu_t of Eq. 28 on the wall face of no-slip y walls (i = 1, 3)
+  const bool les = nu > 0.0 && (s->P.cs > 0.0 || s->P.wall_model);
+  vec nut;
+  if (les) { nut.assign(s->p.size(), 0.0); if (s->P.cs > 0.0) eddy_viscosity(s, uu, vv, ww, nut); }
+  auto Exy = [&](int i0, int i1, int j0, int j1, int k) { return 0.25 * (NT(s, nut, i0, j0, k) + NT(s, nut, i1, j0, k) + NT(s, nut, i0, j1, k) + NT(s, nut, i1, j1, k)); };
+  auto Exz = [&](int i0, int i1, int j, int k0, int k1) { return 0.25 * (NT(s, nut, i0, j, k0) + NT(s, nut, i1, j, k0) + NT(s, nut, i0, j, k1) + NT(s, nut, i1, j, k1)); };
+  auto Eyz = [&](int i, int j0, int j1, int k0, int k1) { return 0.25 * (NT(s, nut, i, j0, k0) + NT(s, nut, i, j1, k0) + NT(s, nut, i, j0, k1) + NT(s, nut, i, j1, k1)); };
+  const bool wm_lo = les && s->P.wall_model && s->by && s->P.bc[2] == ORC_BC_NOSLIP;
+  const bool wm_hi = les && s->P.wall_model && s->by && s->P.bc[3] == ORC_BC_NOSLIP;
   // u faces (boundary-normal faces i=0, nx of a bounded direction are prescribed, not advanced)
   for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = s->bx; i < nx; ++i) {
     double uc = U_(i, j, k);
@@ -123,7 +197,21 @@ static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& 
     double dxx = (U_(i + 1, j, k) - 2.0 * uc + U_(i - 1, j, k)) / (hx * hx);
     double dyy = ((U_(i, j + 1, k) - uc) / DYC(s, j + 1) - (uc - U_(i, j - 1, k)) / DYC(s, j)) / s->dy[j];
     double dzz = (U_(i, j, k + 1) - 2.0 * uc + U_(i, j, k - 1)) / (hz * hz);
-    HU[IU(s, i, j, k)] = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + g[0];
+    double visc = nu * (dxx + dyy + dzz);
+    if (les) {
+      const double fxe = (nu + NT(s, nut, i, j, k)) * (U_(i + 1, j, k) - uc) / hx, fxw = (nu + NT(s, nut, i - 1, j, k)) * (uc - U_(i - 1, j, k)) / hx;
+      double nn = Exy(i - 1, i, j, j + 1, k), ns = Exy(i - 1, i, j - 1, j, k);
+      if ((wm_lo && j == 0) || (wm_hi && j == ny - 1)) {          // Eq. 28: u is relative to the wall, w interpolated to the u face
+        const int f = j == 0 ? 2 : 3;
+        const double wf = 0.25 * (W_(i - 1, j, k) + W_(i, j, k) + W_(i - 1, j, k + 1) + W_(i, j, k + 1));
+        const double nw = wall_nut(s, uc - s->P.bc_vel[f][0], wf - s->P.bc_vel[f][2], 0.5 * s->dy[j]);
+        if (j == 0) ns = nw; else nn = nw;
+      }
+      const double fyn = (nu + nn) * (U_(i, j + 1, k) - uc) / DYC(s, j + 1), fys = (nu + ns) * (uc - U_(i, j - 1, k)) / DYC(s, j);
+      const double fzt = (nu + Exz(i - 1, i, j, k, k + 1)) * (U_(i, j, k + 1) - uc) / hz, fzb = (nu + Exz(i - 1, i, j, k - 1, k)) * (uc - U_(i, j, k - 1)) / hz;
+      visc = (fxe - fxw) / hx + (fyn - fys) / s->dy[j] + (fzt - fzb) / hz;
+    }
+    HU[IU(s, i, j, k)] = -(cx + cy + cz) + visc + g[0];
   }
   // v faces (control volume between y_c(j-1) and y_c(j), height DYC(j))
   for (int k = 0; k < nz; ++k) for (int j = s->by; j < ny; ++j) for (int i = 0; i < nx; ++i) {
@@ -139,7 +227,14 @@ static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& 
     double dxx = (V_(i + 1, j, k) - 2.0 * vc + V_(i - 1, j, k)) / (hx * hx);
     double dyy = ((V_(i, j + 1, k) - vc) / DY(s, j) - (vc - V_(i, j - 1, k)) / DY(s, j - 1)) / DYC(s, j);
     double dzz = (V_(i, j, k + 1) - 2.0 * vc + V_(i, j, k - 1)) / (hz * hz);
-    HV[IV(s, i, j, k)] = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + g[1];
+    double visc = nu * (dxx + dyy + dzz);
+    if (les) {
+      const double fxe = (nu + Exy(i, i + 1, j - 1, j, k)) * (V_(i + 1, j, k) - vc) / hx, fxw = (nu + Exy(i - 1, i, j - 1, j, k)) * (vc - V_(i - 1, j, k)) / hx;
+      const double fyn = (nu + NT(s, nut, i, j, k)) * (V_(i, j + 1, k) - vc) / DY(s, j), fys = (nu + NT(s, nut, i, j - 1, k)) * (vc - V_(i, j - 1, k)) / DY(s, j - 1);
+      const double fzt = (nu + Eyz(i, j - 1, j, k, k + 1)) * (V_(i, j, k + 1) - vc) / hz, fzb = (nu + Eyz(i, j - 1, j, k - 1, k)) * (vc - V_(i, j, k - 1)) / hz;
+      visc = (fxe - fxw) / hx + (fyn - fys) / DYC(s, j) + (fzt - fzb) / hz;
+    }
+    HV[IV(s, i, j, k)] = -(cx + cy + cz) + visc + g[1];
   }
   // w faces
   for (int k = s->bz; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
@@ -155,7 +250,21 @@ static void momentum(const orc_sim* s, const vec& uu, const vec& vv, const vec& 
     double dxx = (W_(i + 1, j, k) - 2.0 * wc + W_(i - 1, j, k)) / (hx * hx);
     double dyy = ((W_(i, j + 1, k) - wc) / DYC(s, j + 1) - (wc - W_(i, j - 1, k)) / DYC(s, j)) / s->dy[j];
     double dzz = (W_(i, j, k + 1) - 2.0 * wc + W_(i, j, k - 1)) / (hz * hz);
-    HW[IW(s, i, j, k)] = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + g[2];
+    double visc = nu * (dxx + dyy + dzz);
+    if (les) {
+      const double fxe = (nu + Exz(i, i + 1, j, k - 1, k)) * (W_(i + 1, j, k) - wc) / hx, fxw = (nu + Exz(i - 1, i, j, k - 1, k)) * (wc - W_(i - 1, j, k)) / hx;
+      double nn = Eyz(i, j, j + 1, k - 1, k), ns = Eyz(i, j - 1, j, k - 1, k);
+      if ((wm_lo && j == 0) || (wm_hi && j == ny - 1)) {          // Eq. 28 for i = 3: u interpolated to the w face
+        const int f = j == 0 ? 2 : 3;
+        const double uf = 0.25 * (U_(i, j, k - 1) + U_(i + 1, j, k - 1) + U_(i, j, k) + U_(i + 1, j, k));
+        const double nw = wall_nut(s, wc - s->P.bc_vel[f][2], uf - s->P.bc_vel[f][0], 0.5 * s->dy[j]);
+        if (j == 0) ns = nw; else nn = nw;
+      }
+      const double fyn = (nu + nn) * (W_(i, j + 1, k) - wc) / DYC(s, j + 1), fys = (nu + ns) * (wc - W_(i, j - 1, k)) / DYC(s, j);
+      const double fzt = (nu + NT(s, nut, i, j, k)) * (W_(i, j, k + 1) - wc) / hz, fzb = (nu + NT(s, nut, i, j, k - 1)) * (wc - W_(i, j, k - 1)) / hz;
+      visc = (fxe - fxw) / hx + (fyn - fys) / s->dy[j] + (fzt - fzb) / hz;
+    }
+    HW[IW(s, i, j, k)] = -(cx + cy + cz) + visc + g[2];
   }
 }
 
@@ -580,7 +689,7 @@ static void build_face_masks(orc_sim* s) {
 //   u_IB(x) = sum_i (1 / F_Ni) wdot(X_i) delta_h(x - X_i) dV_i,   F_Ni = sum_{x in gamma'} delta_h(x - X_i) dv(x)
 // gamma' = the nodes of marker i's support that are NOT in the solid (Eq. 19 as printed has no dv: it would carry units
 // of 1 / volume); a marker whose support holds no such node contributes nothing.
-static void ib_point_velocity(const orc_sim* s, vec& fu, vec& fv, vec& fw) {
+static void ib_point_velocity(orc_sim* s, vec& fu, vec& fv, vec& fw) {
   const int sw = support_width(s);
   vec G((size_t)3 * s->nl, 0.0);
   for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) {
@@ -593,6 +702,7 @@ static void ib_point_velocity(const orc_sim* s, vec& fu, vec& fv, vec& fw) {
     G[3 * l + c] = FN > 0.0 ? s->Ub[3 * l + c] / FN : 0.0;
   }
   spread(s, G, fu, fv, fw);
+  s->Fl = G;                              // reported as the markers' "force" array: wdot_i / F_Ni
 }
 // Eq. 4 + Eq. 5: with f = eps [ -(explicit right-hand side) + (u_s - u^t) / dt ] the predictor becomes
 //   u* = (1 - eps) u~ + eps u_s,   u_s = u_c in the solid (Eq. 23, third branch), u_IB at the IB points (second branch,
@@ -859,6 +969,11 @@ extern "C" int orc_predict(orc_sim* s, int stage, double* us, double* vs, double
   predictor(s, stage, a, b, c, HU, HV, HW);
   std::copy(a.begin(), a.end(), us); std::copy(b.begin(), b.end(), vs); std::copy(c.begin(), c.end(), ws);
   return 0;
+}
+extern "C" void orc_eddy_viscosity(orc_sim* s, double* out) {
+  vec nut(s->p.size(), 0.0);
+  if (s->P.cs > 0.0) eddy_viscosity(s, s->u, s->v, s->w, nut);
+  std::copy(nut.begin(), nut.end(), out);
 }
 extern "C" void orc_convection(orc_sim* s, double* cu, double* cv, double* cw) {
   vec a(s->u.size()), b(s->v.size()), c(s->w.size()); const double g0[3] = {0, 0, 0};

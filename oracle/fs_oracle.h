@@ -42,6 +42,8 @@ typedef struct {
   int delta;
   uint64_t seed; double inflow_noise;
   int convection;            /* ORC_CONV_* */
+  double cs;                 /* constant Smagorinsky coefficient C_s (L437, L638); 0 = no subgrid model */
+  int wall_model;            /* != 0: equilibrium wall model (Spalding law, Eq. 27-29) on no-slip y walls */
   double cfl;                /* > 0: CFL-adaptive step size, dt = min(dt, cfl h_min / |u|_max) (L431); <= 0: fixed dt */
 } orc_params;
 
@@ -79,6 +81,8 @@ void orc_divergence(orc_sim*, const double* u, const double* v, const double* w,
 void orc_gradient(orc_sim*, const double* p, double* gu, double* gv, double* gw); /* 0 on boundary faces */
 void orc_momentum_rhs(orc_sim*, double* hu, double* hv, double* hw); /* H^n of current u,v,w */
 void orc_convection(orc_sim*, double* cu, double* cv, double* cw);   /* C only (nu=0, g=0) */
+void orc_eddy_viscosity(orc_sim*, double* nut);                  /* Smagorinsky nu_t at the cell centres of the current u, v, w */
+double orc_wall_utau(double U, double y, double nu);             /* u_tau of Spalding's law (Eq. 27) by Newton-Raphson */
 /* The predicted field of the current state without advancing it: stage 0 = after O3 (predictor + prescribed
  * boundary-normal faces, incl. the convective-outflow update), 1 = after O4 (IBM direct forcing, u*),
  * 2 = after O5 (outflow flux correction).  Returns non-zero for an unknown stage. */
