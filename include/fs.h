@@ -96,6 +96,10 @@ typedef struct {
   fs_exec exec_mode;
   fs_conv convection;          /* convective flux scheme of the momentum RHS */
   int solid_mask;              /* != 0: reserve workspace for the eps-mask IBM (fs_set_solid_mask) */
+  double cs;                   /* constant Smagorinsky coefficient C_s (L437, L452, L638): nu_t = (C_s Delta)^2 |S|, Delta = (hx dy hz)^(1/3),
+                                  diffusive term div[(nu + nu_t) grad u_i]; 0 = no subgrid model */
+  int wall_model;              /* != 0: equilibrium wall model on no-slip y walls (Spalding's law, Eq. 27, kappa = 0.4, B = 5, by
+                                  Newton-Raphson; nu_t of Eq. 28-29 on the wall face of the tangential components) */
   double cfl;                  /* > 0: CFL-adaptive step (L431): dt = min(dt, cfl h_min / max|u,v,w|) from the field at the start
                                   of every step, h_min the smallest cell extent; <= 0: fixed dt */
 } fs_params;

@@ -49,7 +49,7 @@ class fs_params(C.Structure):
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
                 ("delta", C.c_int), ("max_markers", C.c_int),
                 ("seed", C.c_uint64), ("inflow_noise", C.c_double),
-                ("exec_mode", C.c_int), ("convection", C.c_int), ("solid_mask", C.c_int), ("cfl", C.c_double)]
+                ("exec_mode", C.c_int), ("convection", C.c_int), ("solid_mask", C.c_int), ("cs", C.c_double), ("wall_model", C.c_int), ("cfl", C.c_double)]
 
 
 class fs_step_info(C.Structure):
@@ -157,6 +157,8 @@ def make_params(cfg):
     P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
     P.solid_mask = int(cfg.get("solid_mask", 0))
     P.cfl = float(cfg.get("cfl", 0.0))
+    P.cs = float(cfg.get("cs", 0.0))
+    P.wall_model = int(cfg.get("wall_model", 0))
     return P, keep
 
 

@@ -120,6 +120,7 @@ fs_status validate(const fs_params* p) {
   if (p->yf) for (int j = 0; j < p->ny; ++j) if (!(p->yf[j + 1] > p->yf[j])) return FS_ERR_INVALID_ARG;
   if ((int)p->convection < 0 || (int)p->convection > 1) return FS_ERR_INVALID_ARG;
   if ((int)p->time_scheme < 0 || (int)p->time_scheme > 2) return FS_ERR_INVALID_ARG;
+  if (!(p->cs >= 0.0)) return FS_ERR_INVALID_ARG;
   if ((int)p->precond < 0 || (int)p->precond > 2 || (int)p->delta < 0 || (int)p->delta > 1) return FS_ERR_INVALID_ARG;
   if (p->precond == FS_PC_GMG) {
     const double hx = p->lx / p->nx, hy = p->ly / p->ny, hz = p->lz / p->nz;
@@ -249,6 +250,7 @@ template <class T> fs_status upload_metrics(fs_grid* g) {
   c.hx = g->hx; c.hy = g->hy; c.hz = g->hz; c.dt = P.dt; c.rho = P.rho; c.nu = P.nu;
   for (int a = 0; a < 3; ++a) c.g[a] = P.body_force[a];
   c.x0 = P.x0; c.y0 = P.y0; c.z0 = P.z0;
+  c.cs = P.cs; c.wall_model = P.wall_model;
   c.cfl = P.cfl; c.hmin = std::min(g->hx, g->hz);
   for (int j = 0; j < ny; ++j) c.hmin = std::min(c.hmin, dy[j]);
   c.ihx = (T)(1.0 / g->hx); c.ihz = (T)(1.0 / g->hz);

@@ -54,6 +54,7 @@ template <class T> struct Ctx {
   double bcv[6][3];
   double hx, hy, hz, dt, rho, nu, g[3];   // dt: the configured (maximum) step; kernels read the current one from S->dt
   double cfl, hmin;
+  double cs; int wall_model;     // LES closures (constant Smagorinsky, Spalding wall model); nu_t lives in q before the Poisson solve
   double x0, y0, z0;
   T ihx, ihz, ihx2, ihz2;
   int time_scheme, precond, warm_start, delta, uniform_y, convection;

@@ -5,6 +5,9 @@
 
 namespace fs {
 
+constexpr int kFlatBlocks = 148 * 8;
+static inline int flat_blocks(long long n) { long long b = (n + 255) / 256; return (int)(b < kFlatBlocks ? (b < 1 ? 1 : b) : kFlatBlocks); }
+
 // ---------------------------------------------------------------------------------------------------
 // Boundary-aware velocity access (S0): see col_setup / col_fix below.
 // Component C at (i,j,k), at most one layer outside the stored range in a direction tangential to C:
@@ -110,8 +113,66 @@ template <class T, int C> __device__ __forceinline__ T col_load(const Ctx<T>& c,
   return col_fix<T, C>(c, r, kk, col_raw<T, C>(c, f, r, kk));
 }
 
-template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 2) k_momentum(const Ctx<T> c, int kz) {
+// ---- LES closures (NEXT-4; section 3.4.5) -------------------------------------------
+// Spalding's law (Eq. 27, kappa = 0.4, B = 5): u_tau for the wall-parallel speed U at distance y, Newton-Raphson on
+// g(u_tau) = u+ + e^{-kappa B}[e^{kappa u+} - 1 - kappa u+ - (kappa u+)^2/2 - (kappa u+)^3/6] - y+ (convex, decreasing:
+// monotone convergence from the left); start u+ = min(sqrt(Re_y), max(12.5, ln(1.182 Re_y)/kappa)), 30 iterations.
+__device__ __forceinline__ double wall_utau(double U, double y, double nu) {
+  if (!(U > 0.0)) return 0.0;
+  const double kap = 0.4, eB = exp(-kap * 5.0);
+  const double Rey = U * y / nu;
+  const double up0 = fmin(sqrt(Rey), fmax(12.5, log(1.182 * Rey) / kap));
+  double ut = U / up0;
+  for (int it = 0; it < 30; ++it) {
+    const double up = U / ut, yp = y * ut / nu, ku = kap * up, e = exp(ku);
+    const double gval = up + eB * (e - 1.0 - ku - 0.5 * ku * ku - ku * ku * ku / 6.0) - yp;
+    const double dgdup = 1.0 + eB * kap * (e - 1.0 - ku - 0.5 * ku * ku);
+    const double dg = dgdup * (-up / ut) - y / nu;
+    ut = ut - gval / dg;
+  }
+  return ut;
+}
+// Eq. 28-29: nu_t on the wall face that makes the flux of the tangential component (rel; the other one: other; both
+// relative to the wall, first off-wall point at distance y) equal to tau_wi / rho = u_tau^2 rel / |U|
+__device__ __forceinline__ double wall_nut(double rel, double other, double y, double nu) {
+  const double U = sqrt(rel * rel + other * other);
+  if (!(U > 0.0)) return 0.0;
+  const double ut = wall_utau(U, y, nu);
+  return (ut * ut * rel / U) / (rel / y + 1e-6) - nu;
+}
+
+// Constant Smagorinsky eddy viscosity at the cell centres (reading N4-1), nu_t = (C_s Delta)^2 sqrt(2 S_ij S_ij): diagonal
+// gradients from the cell's own faces, cross gradients as central differences of face values averaged to the centres.
+// One cell per thread through the boundary-aware accessors (not on the benchmarked path).
+template <class T> __global__ void __launch_bounds__(256) k_eddy_viscosity(const Ctx<T> c, T* __restrict__ nut) {
+  const long long N = (long long)c.nx * c.ny * c.nz;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(q % c.nx); const long long t = q / c.nx; const int j = (int)(t % c.ny), k = (int)(t / c.ny);
+    auto U = [&](int ii, int jj, int kk) { return (double)col_load<T, 0>(c, c.u, col_setup<T, 0>(c, ii, jj), kk); };
+    auto V = [&](int ii, int jj, int kk) { return (double)col_load<T, 1>(c, c.v, col_setup<T, 1>(c, ii, jj), kk); };
+    auto W = [&](int ii, int jj, int kk) { return (double)col_load<T, 2>(c, c.w, col_setup<T, 2>(c, ii, jj), kk); };
+    auto ux = [&](int jj, int kk) { return 0.5 * (U(i, jj, kk) + U(i + 1, jj, kk)); };
+    auto vy = [&](int ii, int kk) { return 0.5 * (V(ii, j, kk) + V(ii, j + 1, kk)); };
+    auto wz = [&](int ii, int jj) { return 0.5 * (W(ii, jj, k) + W(ii, jj, k + 1)); };
+    const double dyj = c.dy64[j];
+    const double dyc2 = 1.0 / (double)c.idyc[j + 1] + 1.0 / (double)c.idyc[j];
+    const double dudx = (U(i + 1, j, k) - U(i, j, k)) / c.hx, dvdy = (V(i, j + 1, k) - V(i, j, k)) / dyj, dwdz = (W(i, j, k + 1) - W(i, j, k)) / c.hz;
+    const double dudy = (ux(j + 1, k) - ux(j - 1, k)) / dyc2, dudz = (ux(j, k + 1) - ux(j, k - 1)) / (2.0 * c.hz);
+    const double dvdx = (vy(i + 1, k) - vy(i - 1, k)) / (2.0 * c.hx), dvdz = (vy(i, k + 1) - vy(i, k - 1)) / (2.0 * c.hz);
+    const double dwdx = (wz(i + 1, j) - wz(i - 1, j)) / (2.0 * c.hx), dwdy = (wz(i, j + 1) - wz(i, j - 1)) / dyc2;
+    const double S2 = 2.0 * (dudx * dudx + dvdy * dvdy + dwdz * dwdz)
+                    + (dudy + dvdx) * (dudy + dvdx) + (dudz + dwdx) * (dudz + dwdx) + (dvdz + dwdy) * (dvdz + dwdy);
+    const double delta = cbrt(c.hx * dyj * c.hz);
+    nut[q] = T((c.cs * delta) * (c.cs * delta) * sqrt(S2));
+  }
+}
+
+// LES variant of the kernel (template flag): the diffusive term becomes div[(nu + nu_t) grad u_i] with nu_t (array `nut`,
+// cell centred) at the flux locations -- cell centres natively, edges as the mean of the four surrounding cells -- through
+// a fourth shared-memory ring; on the wall faces of no-slip y walls nu_t is the wall model's (Eq. 28).
+template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX * kMomTY, LES ? 1 : 2) k_momentum(const Ctx<T> c, int kz, const T* __restrict__ nut) {
   __shared__ T SU[4][kMomTY][kMomTX], SV[4][kMomTY][kMomTX], SW[4][kMomTY][kMomTX];
+  __shared__ T SN[LES ? 4 : 1][LES ? kMomTY : 1][LES ? kMomTX : 1];
   const int tx = threadIdx.x, ty = threadIdx.y;
   const int iu = blockIdx.x * (kMomTX - 2) + tx - 1, ju = blockIdx.y * (kMomTY - 2) + ty - 1;   // may be -1 or past the box
   const int i = min(iu, c.nxu), j = min(ju, c.nyv);
@@ -132,6 +193,16 @@ template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 
                  : tx == 4 ? c.idy + jc + 1 : tx == 5 ? c.idy + jc : tx == 6 ? c.idyc + jc : c.idyc + jc + 1;
     MY[tx][ty] = *tab;
   }
+  // nu_t of the own column: cell index wrapped (periodic) or clamped to the boundary cell (bounded)
+  unsigned nq0 = 0; const unsigned npl = (unsigned)c.nx * (unsigned)c.ny;
+  auto nplane = [&](int kk) { return (unsigned)(c.bz ? min(max(kk, 0), c.nz - 1) : (kk < 0 ? kk + c.nz : (kk >= c.nz ? kk - c.nz : kk))); };
+  if (LES) {
+    const int ic = c.bx ? min(max(iu, 0), c.nx - 1) : wrapi(iu, c.nx), jc = c.by ? min(max(ju, 0), c.ny - 1) : wrapi(ju, c.ny);
+    nq0 = (unsigned)ic + (unsigned)c.nx * (unsigned)jc;
+    SN[(k0 - 1) & 3][ty][tx] = nut[nq0 + npl * nplane(k0 - 1)];
+    SN[k0 & 3][ty][tx] = nut[nq0 + npl * nplane(k0)];
+  }
+  const bool wm_lo = LES && c.wall_model && c.by && c.bc[2] == FS_BC_NOSLIP, wm_hi = LES && c.wall_model && c.by && c.bc[3] == FS_BC_NOSLIP;
   // register queue of the own column: B = k-1, c = k, T = k+1
   T uB = col_load<T, 0>(c, U, ru, k0 - 1), vB = col_load<T, 1>(c, V, rv, k0 - 1), wB = col_load<T, 2>(c, W, rw, k0 - 1);
   T uc = col_load<T, 0>(c, U, ru, k0), vc = col_load<T, 1>(c, V, rv, k0), wc = col_load<T, 2>(c, W, rw, k0);
@@ -157,6 +228,7 @@ template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 
     }
     const int s0 = (k - 1) & 3, s1 = k & 3, s2 = (k + 1) & 3;
     SU[s2][ty][tx] = uT; SV[s2][ty][tx] = vT; SW[s2][ty][tx] = wT;
+    if (LES) SN[s2][ty][tx] = nut[nq0 + npl * nplane(k + 1)];
     if (k + 1 < k1) { un = col_raw<T, 0>(c, U, ru, k + 2); vn = col_raw<T, 1>(c, V, rv, k + 2); wn = col_raw<T, 2>(c, W, rw, k + 2); }
     __syncthreads();
     if (own) {
@@ -183,7 +255,23 @@ template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 
           const T dxx = (uE - T(2) * uc + uW) * c.ihx2;
           const T dyy = ((uN - uc) * idyc1 - (uc - uS) * idyc0) * idyj;
           const T dzz = (uT - T(2) * uc + uB) * c.ihz2;
-          const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[0]);
+          T visc = nu * (dxx + dyy + dzz);
+          if (LES) {
+            const T nC = SN[s1][ty][tx], nW = SN[s1][ty][txm];
+            const T fxe = (nu + nC) * (uE - uc) * c.ihx, fxw = (nu + nW) * (uc - uW) * c.ihx;
+            T nn = T(0.25) * (((nW + nC) + SN[s1][typ][txm]) + SN[s1][typ][tx]), ns = T(0.25) * (((SN[s1][tym][txm] + SN[s1][tym][tx]) + nW) + nC);
+            if ((wm_lo && j == 0) || (wm_hi && j == c.ny - 1)) {     // Eq. 28: u relative to the wall, w interpolated to the u face
+              const int f = j == 0 ? 2 : 3;
+              const double wf = 0.25 * ((((double)SW[s1][ty][txm] + (double)wc) + (double)SW[s2][ty][txm]) + (double)wT);
+              const T nw = T(wall_nut((double)uc - c.bcv[f][0], wf - c.bcv[f][2], 0.5 * c.dy64[j], c.nu));
+              if (j == 0) ns = nw; else nn = nw;
+            }
+            const T fyn = (nu + nn) * (uN - uc) * idyc1, fys = (nu + ns) * (uc - uS) * idyc0;
+            const T nzt = T(0.25) * (((nW + nC) + SN[s2][ty][txm]) + SN[s2][ty][tx]), nzb = T(0.25) * (((SN[s0][ty][txm] + SN[s0][ty][tx]) + nW) + nC);
+            const T fzt = (nu + nzt) * (uT - uc) * c.ihz, fzb = (nu + nzb) * (uc - uB) * c.ihz;
+            visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyj + (fzt - fzb) * c.ihz;
+          }
+          const T H = -(cx + cy + cz) + visc + T(c.g[0]);
           c.us[q] = uc + dt * (a0 * H + a1 * huo);
           c.hu[q] = H;
         }
@@ -210,7 +298,17 @@ template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 
           const T dxx = (vE - T(2) * vc + vW) * c.ihx2;
           const T dyy = ((vN - vc) * idyj - (vc - vS) * idyjm) * idyc0;
           const T dzz = (vT - T(2) * vc + vB) * c.ihz2;
-          const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[1]);
+          T visc = nu * (dxx + dyy + dzz);
+          if (LES) {
+            const T nC = SN[s1][ty][tx], nS = SN[s1][tym][tx];
+            const T fxe = (nu + T(0.25) * (((nS + SN[s1][tym][txp]) + nC) + SN[s1][ty][txp])) * (vE - vc) * c.ihx;
+            const T fxw = (nu + T(0.25) * (((SN[s1][tym][txm] + nS) + SN[s1][ty][txm]) + nC)) * (vc - vW) * c.ihx;
+            const T fyn = (nu + nC) * (vN - vc) * idyj, fys = (nu + nS) * (vc - vS) * idyjm;
+            const T fzt = (nu + T(0.25) * (((nS + nC) + SN[s2][tym][tx]) + SN[s2][ty][tx])) * (vT - vc) * c.ihz;
+            const T fzb = (nu + T(0.25) * (((SN[s0][tym][tx] + SN[s0][ty][tx]) + nS) + nC)) * (vc - vB) * c.ihz;
+            visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyc0 + (fzt - fzb) * c.ihz;
+          }
+          const T H = -(cx + cy + cz) + visc + T(c.g[1]);
           c.vs[q] = vc + dt * (a0 * H + a1 * hvo);
           c.hv[q] = H;
         }
@@ -237,7 +335,23 @@ template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 
           const T dxx = (wE - T(2) * wc + wW) * c.ihx2;
           const T dyy = ((wN - wc) * idyc1 - (wc - wS) * idyc0) * idyj;
           const T dzz = (wT - T(2) * wc + wB) * c.ihz2;
-          const T H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[2]);
+          T visc = nu * (dxx + dyy + dzz);
+          if (LES) {
+            const T nC = SN[s1][ty][tx], nB = SN[s0][ty][tx];
+            const T fxe = (nu + T(0.25) * (((nB + SN[s0][ty][txp]) + nC) + SN[s1][ty][txp])) * (wE - wc) * c.ihx;
+            const T fxw = (nu + T(0.25) * (((SN[s0][ty][txm] + nB) + SN[s1][ty][txm]) + nC)) * (wc - wW) * c.ihx;
+            T nn = T(0.25) * (((nB + SN[s0][typ][tx]) + nC) + SN[s1][typ][tx]), ns = T(0.25) * (((SN[s0][tym][tx] + nB) + SN[s1][tym][tx]) + nC);
+            if ((wm_lo && j == 0) || (wm_hi && j == c.ny - 1)) {     // Eq. 28 for i = 3: u interpolated to the w face
+              const int f = j == 0 ? 2 : 3;
+              const double uf = 0.25 * ((((double)uB + (double)SU[s0][ty][txp]) + (double)uc) + (double)SU[s1][ty][txp]);
+              const T nw = T(wall_nut((double)wc - c.bcv[f][2], uf - c.bcv[f][0], 0.5 * c.dy64[j], c.nu));
+              if (j == 0) ns = nw; else nn = nw;
+            }
+            const T fyn = (nu + nn) * (wN - wc) * idyc1, fys = (nu + ns) * (wc - wS) * idyc0;
+            const T fzt = (nu + nC) * (wT - wc) * c.ihz, fzb = (nu + nB) * (wc - wB) * c.ihz;
+            visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyj + (fzt - fzb) * c.ihz;
+          }
+          const T H = -(cx + cy + cz) + visc + T(c.g[2]);
           c.ws[q] = wc + dt * (a0 * H + a1 * hwo);
           c.hw[q] = H;
         }
@@ -249,11 +363,24 @@ template <class T, bool UPW> __global__ void __launch_bounds__(kMomTX * kMomTY, 
 
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
   const int bxn = (c.nxu + kMomTX - 3) / (kMomTX - 2), byn = (c.nyv + kMomTY - 3) / (kMomTY - 2);
-  // z chunks: >= 4 waves of CTAs (2 CTAs of 320 threads per SM) while chunks stay >= 16 planes
-  const int kz = pick_kz((long long)bxn * byn, c.nzw, 2LL * 148, 2, 16);
+  const bool les = c.nu > 0.0 && (c.cs > 0.0 || c.wall_model);
+  // z chunks: whole waves of resident CTAs (2 CTAs of 320 threads per SM; the LES variant: 1) while chunks stay >= 16 planes
+  const int kz = pick_kz((long long)bxn * byn, c.nzw, (les ? 1LL : 2LL) * 148, 2, 16);
   dim3 b(kMomTX, kMomTY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
-  if (c.convection == FS_CONV_UPWIND) FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,upwind>" : "k_momentum<f32,upwind>", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, true><<<g, b, 0, L.s>>>(c, kz));
-  else FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,central>" : "k_momentum<f32,central>", 12.0 * sizeof(T) * c.nx * c.ny * c.nz, k_momentum<T, false><<<g, b, 0, L.s>>>(c, kz));
+  const double bytes = 12.0 * sizeof(T) * c.nx * c.ny * c.nz;
+  int n = 1;
+  if (les) {
+    const long long N = (long long)c.nx * c.ny * c.nz;
+    T* nut = c.q;                        // PCG scratch, free until the Poisson solve of this step
+    if (c.cs > 0.0) FS_LAUNCH(L, "eddy_viscosity", 4.0 * sizeof(T) * N, k_eddy_viscosity<T><<<flat_blocks(N), 256, 0, L.s>>>(c, nut));
+    else FS_LAUNCH(L, "eddy_viscosity", 1.0 * sizeof(T) * N, cudaMemsetAsync(nut, 0, sizeof(T) * (size_t)N, L.s));
+    ++n;
+    if (c.convection == FS_CONV_UPWIND) FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,upwind,LES>" : "k_momentum<f32,upwind,LES>", bytes + sizeof(T) * N, k_momentum<T, true, true><<<g, b, 0, L.s>>>(c, kz, nut));
+    else FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,central,LES>" : "k_momentum<f32,central,LES>", bytes + sizeof(T) * N, k_momentum<T, false, true><<<g, b, 0, L.s>>>(c, kz, nut));
+    return n;
+  }
+  if (c.convection == FS_CONV_UPWIND) FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,upwind>" : "k_momentum<f32,upwind>", bytes, k_momentum<T, true, false><<<g, b, 0, L.s>>>(c, kz, nullptr));
+  else FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,central>" : "k_momentum<f32,central>", bytes, k_momentum<T, false, false><<<g, b, 0, L.s>>>(c, kz, nullptr));
   return 1;
 }
 
@@ -335,7 +462,6 @@ template <class T> int launch_flux_correction(const Ctx<T>& c, const Launch& L) 
 // S6: raw right-hand side of the symmetrised system, bhat_raw = -dy_j (rho/dt) D(u*)  (Eq. 7;
 // SURVEY O6), and its sum for the compatibility shift.  Written into r; pcg_init finishes the job.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kFlatBlocks = 148 * 8;
 
 template <class T> __global__ void __launch_bounds__(256) k_div_rhs(const Ctx<T> c, const T* __restrict__ bsrc) {
   __shared__ double sh[32]; __shared__ int flag;
@@ -415,7 +541,6 @@ template <class T> __global__ void __launch_bounds__(256) k_div_rhsv(const Ctx<T
     }
   }
 }
-static inline int flat_blocks(long long n) { long long b = (n + 255) / 256; return (int)(b < kFlatBlocks ? (b < 1 ? 1 : b) : kFlatBlocks); }
 
 template <class T> int launch_div_rhs(const Ctx<T>& c, const Launch& L) {
   const long long N = (long long)c.nx * c.ny * c.nz;

@@ -296,6 +296,49 @@ def test_ibm_empty_and_single_marker(fs):
     g.close()
 
 
+# ------------------------------------------------------------------------------------ NEXT-4: LES closures
+@pytest.mark.parametrize("kind", ["periodic", "channel", "open", "channel_upwind_wallonly"])
+def test_les_momentum_rhs_elementwise(fs, kind):
+    # Smagorinsky nu_t + flux-form diffusion (+ the Spalding wall model on the no-slip y walls of the channel), random
+    # fields, ragged tiles; H^n element-wise against the oracle
+    cfg = {"periodic": _cfg_periodic(72, 38, 21, cs=0.17), "channel": _cfg_channel(40, 50, 19, cs=0.12, wall_model=1),
+           "open": _cfg_open(70, 27, 22, inflow_noise=0.05, seed=3, cs=0.2, wall_model=1),
+           "channel_upwind_wallonly": _cfg_channel(36, 30, 17, cs=0.0, wall_model=1, convection="upwind")}[kind]
+    if kind.startswith("channel"):
+        cfg["nu"] = 1.0 / 3000.0
+    cfg["init"] = _rand_fields(cfg, 13)
+    ref = _oracle(cfg).momentum_rhs()
+    g = fs.from_workload(cfg)
+    got = g.momentum_rhs()
+    for c, a, b in zip("uvw", got, ref):
+        assert relerr(a, b) < 1e-12, (kind, c, relerr(a, b))
+    used = g.kernels_used()
+    assert any("LES" in k for k in used), used
+    g.close()
+
+
+def test_wmles_channel_64_runs_and_matches_oracle(fs):
+    # the paper's WMLES workload shape (Table 5: 2 pi x 2 x pi, 64^3), Re_tau-2000-like viscosity, Smagorinsky + wall model
+    # (initial field: the c2 recipe's Poiseuille profile + noise for nu = 1/180, then run at the lower viscosity)
+    def wm(n, **kw):
+        c = W.channel(n=n, cs=0.1, wall_model=1, **kw)
+        c["nu"] = 1.0 / 2000.0
+        return c
+    cfg = wm(64, beta=1e-6, steps=4)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 4)
+    assert ig["max_abs_div"] < 1e-5
+    g.close()
+    cfg = wm(24, time_scheme="rk3", cfl=0.3, dt=1e-3)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 3, iters_pm=3)            # with Runge-Kutta stages and the CFL step on top
+    assert abs(ig["dt"] - io["dt"]) < 1e-13 * io["dt"]
+    g.close()
+    o5 = _oracle(wm(24)); o5.step(5)
+    g = fs.from_workload(wm(24), dtype="f32"); g.step(5)
+    errs = {c: relerr(g.get(c), o5.get(c)) for c in "uvwp"}
+    assert all(e < TOL32 for e in errs.values()), errs
+    g.close()
+
+
 # ------------------------------------------------------------------------------------ NEXT-3: Runge-Kutta, CFL-adaptive dt
 def test_rk3_matches_oracle_and_the_stability_polynomial(fs):
     cfg = W.taylor_green(n=16, nu=0.1, dt=0.05, time_scheme="rk3", rtol=1e-13)
