@@ -29,14 +29,16 @@ class _Params(C.Structure):
                 ("precond", C.c_int), ("rtol", C.c_double), ("max_iter", C.c_int), ("warm_start", C.c_int),
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
                 ("delta", C.c_int), ("seed", C.c_uint64), ("inflow_noise", C.c_double), ("convection", C.c_int),
-                ("cs", C.c_double), ("wall_model", C.c_int), ("cfl", C.c_double)]
+                ("cs", C.c_double), ("wall_model", C.c_int),
+                ("coupling_max_iters", C.c_int), ("coupling_tol", C.c_double), ("cfl", C.c_double)]
 
 
 class _Info(C.Structure):
     _fields_ = [("pcg_iters", C.c_int), ("converged", C.c_int), ("nan_flag", C.c_int),
                 ("rel_residual", C.c_double), ("true_rel_residual", C.c_double), ("max_abs_div", C.c_double),
                 ("body_force", C.c_double * 3), ("body_disp", C.c_double * 3), ("body_vel", C.c_double * 3),
-                ("step", C.c_longlong), ("dt", C.c_double), ("time", C.c_double)]
+                ("step", C.c_longlong), ("dt", C.c_double), ("time", C.c_double),
+                ("coupling_iters", C.c_int), ("coupling_xi", C.c_double)]
 
 
 _lib = None
@@ -78,7 +80,8 @@ def info_dict(i):
     return dict(pcg_iters=i.pcg_iters, converged=i.converged, nan_flag=i.nan_flag,
                 rel_residual=i.rel_residual, true_rel_residual=i.true_rel_residual,
                 max_abs_div=i.max_abs_div, body_force=list(i.body_force), body_disp=list(i.body_disp),
-                body_vel=list(i.body_vel), step=i.step, dt=i.dt, time=i.time)
+                body_vel=list(i.body_vel), step=i.step, dt=i.dt, time=i.time,
+                coupling_iters=i.coupling_iters, coupling_xi=i.coupling_xi)
 
 
 def delta_phi(kind, r):
@@ -125,6 +128,8 @@ class Oracle:
         P.delta = DELTA[cfg["delta"]]
         P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
         P.cfl = float(cfg.get("cfl", 0.0))
+        P.coupling_max_iters = int(cfg.get("coupling_max_iters", 1))
+        P.coupling_tol = float(cfg.get("coupling_tol", 1e-5))
         P.cs = float(cfg.get("cs", 0.0))
         P.wall_model = int(cfg.get("wall_model", 0))
         self.h = L.orc_create(C.byref(P))

@@ -813,11 +813,8 @@ static double choose_dt(const orc_sim* s) {
   return std::min(s->P.dt, s->P.cfl * hmin / umax);
 }
 
-// ---- one fractional step (O1..O9 in order) -----------------------------------------------------
-static void one_step(orc_sim* s, orc_info* info) {
-  s->dt = choose_dt(s);
-  const double dt = s->dt;
-  vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size());
+// ---- the fluid part of one time step: a single fractional step, or the stages of the Runge-Kutta scheme ---------------
+static void fluid_step(orc_sim* s, orc_info* info, vec& HU, vec& HV, vec& HW) {
   if (s->P.time_scheme == ORC_TIME_RK3) {
     // Explicit Runge-Kutta (L100, L431, Table 1; the paper names no tableau -- reading N3-3): the three-stage
     // third-order strong-stability-preserving scheme in Shu-Osher form, every stage a complete fractional step
@@ -841,19 +838,50 @@ static void one_step(orc_sim* s, orc_info* info) {
   } else {
     fluid_substep(s, info, HU, HV, HW);
   }
+}
+
+// ---- one time step (O1..O9 in order), with the strong-coupling loop of Algorithm 1 (L212, L218-237) ------------------
+// Reading N2-1 (the tail of Algorithm 1 is garbled in PAPER.md): sub-iteration k = 1..N restarts the fluid from time level
+// n (u^{t-1}, p^{t-1}) with the structure's latest iterate -- markers at X^n + (w^(k-1) - w^n) moving with wdot^(k-1) --
+// gathers the force, advances the structure from (w^n, wdot^n) with it (RK4, Eq. 12), and stops when
+//   xi = || (w^(k) - w^(k-1)) / w^(k-1) ||_2^2 < tol  (1e-5 in the paper)   or k = N (100 in the paper).
+// N = 1 is the weakly coupled scheme (L212).  A component with w^(k-1) = 0 = w^(k) contributes 0 to xi.
+static void one_step(orc_sim* s, orc_info* info) {
+  s->dt = choose_dt(s);
+  const double dt = s->dt;
+  vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size());
+  const int N = (s->has_body && s->P.coupling_max_iters > 1) ? s->P.coupling_max_iters : 1;
+  vec u0, v0, w0, p0, X0;
+  double d0[3], vel0[3];
+  for (int c = 0; c < 3; ++c) { d0[c] = s->bdisp[c]; vel0[c] = s->bvel[c]; }
+  if (N > 1) { u0 = s->u; v0 = s->v; w0 = s->w; p0 = s->p; X0 = s->X; }
+  int k = 0, iters = 0; double xi = 0.0;
+  for (k = 1; k <= N; ++k) {
+    if (k > 1) { s->u = u0; s->v = v0; s->w = w0; s->p = p0; }
+    fluid_step(s, info, HU, HV, HW);
+    iters += info->pcg_iters;
+    if (s->has_body) {                                                                 // O9
+      xi = 0.0;
+      for (int c = 0; c < 3; ++c) if (s->dof & (1 << c)) {
+        const double prev = s->bdisp[c];                       // w^(k-1): what the markers reflect during this sub-iteration
+        double wn = d0[c], vn = vel0[c];
+        orc_rk4_body(s->bm, s->bc_, s->bk, s->bforce[c], dt, &wn, &vn);
+        const double dw = wn - prev;
+        for (int l = 0; l < s->nl; ++l) s->X[3 * l + c] += dw;
+        s->bdisp[c] = wn; s->bvel[c] = vn;
+        if (!(dw == 0.0 && prev == 0.0)) xi += (dw / prev) * (dw / prev);
+      }
+      for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) s->Ub[3 * l + c] = s->bvel[c];
+    }
+    if (N > 1 && xi < s->P.coupling_tol) break;
+  }
+  if (k > N) k = N;
+  if (N > 1) info->pcg_iters = iters;
+  info->coupling_iters = k; info->coupling_xi = xi;
   divergence(s, s->u, s->v, s->w, s->divu);
   double md = 0.0; int nan = 0;
   for (size_t q = 0; q < s->divu.size(); ++q) { double a = std::fabs(s->divu[q]); if (a > md) md = a; if (a != a) nan = 1; }
   info->max_abs_div = md; info->nan_flag = nan;
-  if (s->has_body) {                                                                   // O9
-    for (int c = 0; c < 3; ++c) if (s->dof & (1 << c)) {
-      double w0 = s->bdisp[c];
-      orc_rk4_body(s->bm, s->bc_, s->bk, s->bforce[c], dt, &s->bdisp[c], &s->bvel[c]);
-      double dw = s->bdisp[c] - w0;
-      for (int l = 0; l < s->nl; ++l) s->X[3 * l + c] += dw;
-    }
-    for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) s->Ub[3 * l + c] = s->bvel[c];
-  }
   s->hu = HU; s->hv = HV; s->hw = HW; s->have_hist = true; s->step += 1;
   s->dt_prev = dt; s->time += dt;
   for (int c = 0; c < 3; ++c) { info->body_force[c] = s->bforce[c]; info->body_disp[c] = s->bdisp[c]; info->body_vel[c] = s->bvel[c]; }

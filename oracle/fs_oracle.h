@@ -44,6 +44,8 @@ typedef struct {
   int convection;            /* ORC_CONV_* */
   double cs;                 /* constant Smagorinsky coefficient C_s (L437, L638); 0 = no subgrid model */
   int wall_model;            /* != 0: equilibrium wall model (Spalding law, Eq. 27-29) on no-slip y walls */
+  int coupling_max_iters;    /* strong FSI coupling (Algorithm 1): at most this many sub-iterations per step; <= 1: weak */
+  double coupling_tol;       /* stop when || (w^k - w^{k-1}) / w^{k-1} ||^2 < tol (paper: 1e-5) */
   double cfl;                /* > 0: CFL-adaptive step size, dt = min(dt, cfl h_min / |u|_max) (L431); <= 0: fixed dt */
 } orc_params;
 
@@ -53,6 +55,7 @@ typedef struct {
   double body_force[3], body_disp[3], body_vel[3];
   long long step;
   double dt, time;           /* step size used by the last step, elapsed time */
+  int coupling_iters; double coupling_xi;   /* Algorithm 1: sub-iterations of the last step and its final xi */
 } orc_info;
 
 typedef struct orc_sim orc_sim;
