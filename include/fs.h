@@ -100,6 +100,9 @@ typedef struct {
                                   diffusive term div[(nu + nu_t) grad u_i]; 0 = no subgrid model */
   int wall_model;              /* != 0: equilibrium wall model on no-slip y walls (Spalding's law, Eq. 27, kappa = 0.4, B = 5, by
                                   Newton-Raphson; nu_t of Eq. 28-29 on the wall face of the tangential components) */
+  int coupling_max_iters;      /* strong FSI coupling (Algorithm 1): up to this many fluid + structure sweeps per step, each
+                                  restarting the fluid from time level n with the structure's latest iterate; <= 1: weak coupling */
+  double coupling_tol;         /* stop when xi = || (w^k - w^{k-1}) / w^{k-1} ||_2^2 < coupling_tol (paper: 1e-5, N <= 100) */
   double cfl;                  /* > 0: CFL-adaptive step (L431): dt = min(dt, cfl h_min / max|u,v,w|) from the field at the start
                                   of every step, h_min the smallest cell extent; <= 0: fixed dt */
 } fs_params;
@@ -114,6 +117,8 @@ typedef struct {
   long long unconverged_steps;  /* sticky, since fs_grid_create: steps whose PCG hit max_iter ...            */
   long long nan_steps;          /* ... and steps whose projected field held a NaN (also seen by async steps) */
   double dt, time;              /* step size of the last step (CFL-adaptive dt), elapsed time since the grid was created */
+  int coupling_iters;           /* Algorithm 1: sweeps of the last step (1 = weak coupling) ... */
+  double coupling_xi;           /* ... and its final xi; pcg_iters is then the sum over the sweeps */
 } fs_step_info;
 typedef struct { int iters; int converged; double rel_residual, true_rel_residual; } fs_poisson_info;
 

@@ -49,7 +49,8 @@ class fs_params(C.Structure):
                 ("mg_nu1", C.c_int), ("mg_nu2", C.c_int), ("mg_coarse_sweeps", C.c_int), ("mg_omega", C.c_double),
                 ("delta", C.c_int), ("max_markers", C.c_int),
                 ("seed", C.c_uint64), ("inflow_noise", C.c_double),
-                ("exec_mode", C.c_int), ("convection", C.c_int), ("solid_mask", C.c_int), ("cs", C.c_double), ("wall_model", C.c_int), ("cfl", C.c_double)]
+                ("exec_mode", C.c_int), ("convection", C.c_int), ("solid_mask", C.c_int), ("cs", C.c_double), ("wall_model", C.c_int),
+                ("coupling_max_iters", C.c_int), ("coupling_tol", C.c_double), ("cfl", C.c_double)]
 
 
 class fs_step_info(C.Structure):
@@ -57,7 +58,7 @@ class fs_step_info(C.Structure):
                 ("rel_residual", C.c_double), ("true_rel_residual", C.c_double), ("max_abs_div", C.c_double),
                 ("body_force", C.c_double * 3), ("body_disp", C.c_double * 3), ("body_vel", C.c_double * 3),
                 ("step", C.c_longlong), ("unconverged_steps", C.c_longlong), ("nan_steps", C.c_longlong),
-                ("dt", C.c_double), ("time", C.c_double)]
+                ("dt", C.c_double), ("time", C.c_double), ("coupling_iters", C.c_int), ("coupling_xi", C.c_double)]
 
 
 class fs_poisson_info(C.Structure):
@@ -157,6 +158,8 @@ def make_params(cfg):
     P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
     P.solid_mask = int(cfg.get("solid_mask", 0))
     P.cfl = float(cfg.get("cfl", 0.0))
+    P.coupling_max_iters = int(cfg.get("coupling_max_iters", 1))
+    P.coupling_tol = float(cfg.get("coupling_tol", 1e-5))
     P.cs = float(cfg.get("cs", 0.0))
     P.wall_model = int(cfg.get("wall_model", 0))
     return P, keep
@@ -167,7 +170,7 @@ def _info_dict(i):
                 rel_residual=i.rel_residual, true_rel_residual=i.true_rel_residual,
                 max_abs_div=i.max_abs_div, body_force=list(i.body_force), body_disp=list(i.body_disp),
                 body_vel=list(i.body_vel), step=i.step, unconverged_steps=i.unconverged_steps, nan_steps=i.nan_steps,
-                dt=i.dt, time=i.time)
+                dt=i.dt, time=i.time, coupling_iters=i.coupling_iters, coupling_xi=i.coupling_xi)
 
 
 class Grid:

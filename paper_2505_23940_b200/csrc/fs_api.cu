@@ -74,6 +74,8 @@ struct fs_grid {
   int step_fixed = 0, step_body = 0, poisson_fixed = 0, poisson_body = 0;
   long long fixed_launches = 0, body_iters_poisson = 0;
   int nl = 0; bool indexed = false;
+  void* bak[7] = {nullptr};           // strong coupling: u, v, w, p, H^{n-1} of time level n (device, T)
+  int last_sweeps = 1; double last_xi = 0.0; long long last_iters = 0;
 };
 
 namespace {
@@ -159,6 +161,11 @@ template <class T> size_t carve(fs_grid* g, char* base) {
   c.p = b.take<T>(g->nP); c.r = b.take<T>(g->nP); c.d = b.take<T>(g->nP); c.d2 = b.take<T>(g->nP); c.q = b.take<T>(g->nP); c.bh = b.take<T>(g->nP);
   c.z = nullptr; c.r2 = nullptr;
   c.q0u = c.q0v = c.q0w = nullptr;
+  for (int a = 0; a < 7; ++a) g->bak[a] = nullptr;
+  if (P.coupling_max_iters > 1) {
+    const size_t nb[7] = {g->nU, g->nV, g->nW, g->nP, g->nU, g->nV, g->nW};
+    for (int a = 0; a < 7; ++a) g->bak[a] = b.take<T>(nb[a]);
+  }
   if (P.time_scheme == FS_TIME_RK3) { c.q0u = b.take<T>(g->nU); c.q0v = b.take<T>(g->nV); c.q0w = b.take<T>(g->nW); }
   mg.nlev = 0;
   if (P.precond == FS_PC_GMG) {
@@ -272,6 +279,7 @@ void init_ibm(fs_grid* g) {
   ib.ivol = 1.0 / (g->hx * g->hy * g->hz);
   ib.has_body = 0; ib.dof = 0; ib.bm = 1.0; ib.bc = 0.0; ib.bk = 0.0;
   ib.has_mask = 0; ib.uc[0] = ib.uc[1] = ib.uc[2] = 0.0;
+  ib.strong = 0;
 }
 
 
@@ -406,6 +414,50 @@ template <class T> fs_status run_once(fs_grid* g, bool poisson) {
   }
   g->fixed_launches += poisson ? g->poisson_fixed : g->step_fixed;
   if (!poisson && g->ib.n > 0) g->indexed = true;
+  return FS_OK;
+}
+
+// One time step.  Weak coupling / no body: one run of the step graph.  Strong coupling (Algorithm 1; reading
+// N2-1): the fluid fields of time level n are kept, every sweep restarts from them with the structure's latest iterate
+// (the markers already reflect it: k_step_end moved them), the structure is advanced from its time-level-n state with the
+// sweep's force, and the host -- the loop is data dependent by nature -- stops on xi = ||(w^k - w^{k-1}) / w^{k-1}||^2.
+template <class T> fs_status advance_step(fs_grid* g) {
+  g->last_sweeps = 1; g->last_xi = 0.0; g->last_iters = -1;
+  const int N = (g->ib.has_body && g->P.coupling_max_iters > 1) ? g->P.coupling_max_iters : 1;
+  if (N == 1) return run_once<T>(g, false);
+  Ctx<T>& c = ctx<T>(g);
+  Scalars h0;
+  CK(cudaMemcpyAsync(&h0, g->S, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  CK(cudaMemcpyAsync(g->S->body_disp0, h0.body_disp, 3 * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(g->S->body_vel0, h0.body_vel, 3 * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  T* fld[7] = {c.u, c.v, c.w, c.p, c.hu, c.hv, c.hw};
+  const size_t nb[7] = {g->nU, g->nV, g->nW, g->nP, g->nU, g->nV, g->nW};
+  for (int a = 0; a < 7; ++a) CK(cudaMemcpyAsync(g->bak[a], fld[a], nb[a] * sizeof(T), cudaMemcpyDeviceToDevice, g->stream));
+  double prev[3] = {h0.body_disp[0], h0.body_disp[1], h0.body_disp[2]};
+  long long iters = 0; double xi = 0.0; int k = 1;
+  for (k = 1; k <= N; ++k) {
+    if (k > 1) {
+      for (int a = 0; a < 7; ++a) CK(cudaMemcpyAsync(fld[a], g->bak[a], nb[a] * sizeof(T), cudaMemcpyDeviceToDevice, g->stream));
+      CK(cudaMemcpyAsync(&g->S->step, &h0.step, sizeof(long long), cudaMemcpyHostToDevice, g->stream));
+      CK(cudaMemcpyAsync(&g->S->have_hist, &h0.have_hist, sizeof(int), cudaMemcpyHostToDevice, g->stream));
+      CK(cudaMemcpyAsync(&g->S->time, &h0.time, sizeof(double), cudaMemcpyHostToDevice, g->stream));
+      CK(cudaMemcpyAsync(&g->S->dt_prev, &h0.dt_prev, sizeof(double), cudaMemcpyHostToDevice, g->stream));
+    }
+    fs_status st = run_once<T>(g, false); if (st != FS_OK) return st;
+    Scalars hs;
+    CK(cudaMemcpyAsync(&hs, g->S, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+    CK(cudaStreamSynchronize(g->stream));
+    iters += hs.iter;
+    xi = 0.0;
+    for (int a = 0; a < 3; ++a) if (g->ib.dof & (1 << a)) {
+      const double dw = hs.body_disp[a] - prev[a];
+      if (!(dw == 0.0 && prev[a] == 0.0)) xi += (dw / prev[a]) * (dw / prev[a]);
+      prev[a] = hs.body_disp[a];
+    }
+    if (xi < g->P.coupling_tol) break;
+  }
+  g->last_sweeps = k > N ? N : k; g->last_xi = xi; g->last_iters = iters;
   return FS_OK;
 }
 
@@ -717,6 +769,7 @@ fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask) {
   if (!g || !(m > 0)) return FS_ERR_INVALID_ARG;
   GUARD(g);
   g->ib.has_body = 1; g->ib.bm = m; g->ib.bc = c; g->ib.bk = k; g->ib.dof = dof_mask;
+  g->ib.strong = g->P.coupling_max_iters > 1;
   invalidate(g);
   return FS_OK;
 }
@@ -752,7 +805,7 @@ fs_status fs_step(fs_grid* g, int nsteps, fs_step_info* last) {
   if (!g || nsteps < 0) return FS_ERR_INVALID_ARG;
   GUARD(g);
   for (int s = 0; s < nsteps; ++s) {
-    fs_status st = g->f64 ? run_once<double>(g, false) : run_once<float>(g, false);
+    fs_status st = g->f64 ? advance_step<double>(g) : advance_step<float>(g);
     if (st != FS_OK) return st;
   }
   if (!last) return FS_OK;
@@ -766,6 +819,8 @@ fs_status fs_step(fs_grid* g, int nsteps, fs_step_info* last) {
   I.step = hs.step;
   I.unconverged_steps = hs.unconverged_steps; I.nan_steps = hs.nan_steps;
   I.dt = hs.dt_prev; I.time = hs.time;
+  I.coupling_iters = g->last_sweeps; I.coupling_xi = g->last_xi;
+  if (g->last_iters >= 0) I.pcg_iters = (int)g->last_iters;
   *last = I;                        // valid for FS_OK, FS_ERR_NOT_CONVERGED and FS_ERR_UNSUPPORTED (fs.h)
   if (hs.ibm_oob) return FS_ERR_UNSUPPORTED;
   return (nsteps > 0 && !hs.converged) ? FS_ERR_NOT_CONVERGED : FS_OK;
@@ -843,7 +898,7 @@ fs_status fs_profile_step(fs_grid* g, int nsteps) {
   g->profiling = true;
   fs_status st = FS_OK;
   for (int s = 0; s < nsteps && st == FS_OK; ++s) {
-    st = g->f64 ? run_once<double>(g, false) : run_once<float>(g, false);
+    st = g->f64 ? advance_step<double>(g) : advance_step<float>(g);
     if (st == FS_OK && cudaStreamSynchronize(g->stream) != cudaSuccess) st = FS_ERR_CUDA;
     prof_collect(&g->prof);
   }

@@ -44,6 +44,7 @@ struct Scalars {
   // IBM
   int nseg; int bbox_lo[3], bbox_hi[3]; int pad1;
   double body_force[3], body_disp[3], body_vel[3];
+  double body_disp0[3], body_vel0[3];   // strong coupling: the body's state at time level n (every sweep's RK4 starts there)
   // tickets for last-block reductions
   unsigned int ticket[8];
 };
@@ -92,6 +93,7 @@ struct IbmCtx {
   int *base, *perm, *keys, *keys_raw, *seg, *flags;
   // body (Eq. 12)
   int has_body, dof; double bm, bc, bk;
+  int strong;                  // strong coupling (Algorithm 1): RK4 starts from body_disp0 / body_vel0
   // eps-mask IBM (Eq. 5, 8-9, 18-19, 23): cell mask, per-face classes (0 fluid, 1 solid, 2 IB point), u_c, scratch for u_IB
   int has_mask; double uc[3];
   unsigned char *eps, *mu, *mv, *mw;

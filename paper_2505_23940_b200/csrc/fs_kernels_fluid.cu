@@ -803,14 +803,15 @@ template <class T> __global__ void k_step_end(const Ctx<T> c, const IbmCtx ib) {
     if (ib.has_body) {
       const double dt = S->dt, m = ib.bm, cc = ib.bc, kk = ib.bk;
       for (int a = 0; a < 3; ++a) if (ib.dof & (1 << a)) {
-        const double F = S->body_force[a], y0 = S->body_disp[a], y1 = S->body_vel[a];
+        // strong coupling: every sweep advances the structure from time level n; the markers reflect the previous iterate
+        const double F = S->body_force[a], y0 = ib.strong ? S->body_disp0[a] : S->body_disp[a], y1 = ib.strong ? S->body_vel0[a] : S->body_vel[a];
         const double k1a = y1,                  k1b = body_acc(F, cc, kk, m, y0, y1);
         const double k2a = y1 + 0.5 * dt * k1b, k2b = body_acc(F, cc, kk, m, y0 + 0.5 * dt * k1a, y1 + 0.5 * dt * k1b);
         const double k3a = y1 + 0.5 * dt * k2b, k3b = body_acc(F, cc, kk, m, y0 + 0.5 * dt * k2a, y1 + 0.5 * dt * k2b);
         const double k4a = y1 + dt * k3b,       k4b = body_acc(F, cc, kk, m, y0 + dt * k3a, y1 + dt * k3b);
         const double w1 = y0 + dt / 6.0 * (k1a + 2.0 * k2a + 2.0 * k3a + k4a);
         const double v1 = y1 + dt / 6.0 * (k1b + 2.0 * k2b + 2.0 * k3b + k4b);
-        dw[a] = w1 - y0; nv[a] = v1;
+        dw[a] = w1 - S->body_disp[a]; nv[a] = v1;
         S->body_disp[a] = w1; S->body_vel[a] = v1;
       }
     }

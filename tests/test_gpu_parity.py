@@ -296,6 +296,40 @@ def test_ibm_empty_and_single_marker(fs):
     g.close()
 
 
+# ------------------------------------------------------------------------------------ NEXT-2: strong coupling (Algorithm 1)
+def test_strong_coupling_matches_oracle(fs):
+    # a light 2-DOF body (added mass matters): same sweeps, same xi, same fields as the oracle's Algorithm 1; N = 1 is the
+    # weak scheme; mask-forced body with strong coupling too (the solid velocity seen by the fluid is the latest iterate)
+    def light(**kw):
+        cfg = W.cylinder_fsi(scale=8, per_ring=16, rtol=1e-10, **kw)
+        m, c, k, dof = cfg["body"]
+        cfg["body"] = (0.25 * m, 0.05, k, 3)
+        return cfg
+    for kw in (dict(coupling_max_iters=30, coupling_tol=1e-12), dict(coupling_max_iters=3, coupling_tol=0.0),
+               dict(coupling_max_iters=30, coupling_tol=1e-10, time_scheme="rk3")):
+        cfg = light(**kw)
+        o = _oracle(cfg); g = fs.from_workload(cfg)
+        for x in (o, g):
+            x.set_body_state([0.02, 0.01, 0.0], [0.0, 0.0, 0.0])
+        for s_ in range(2):
+            io = o.step(1); ig = g.step(1)
+            assert ig["coupling_iters"] == io["coupling_iters"] >= 3, (ig["coupling_iters"], io["coupling_iters"])
+            assert abs(ig["pcg_iters"] - io["pcg_iters"]) <= 3 * io["coupling_iters"]
+            assert abs(ig["coupling_xi"] - io["coupling_xi"]) <= 1e-6 * io["coupling_xi"] + 1e-30
+        _compare_state(g, o, TOL64)
+        for k_ in ("body_force", "body_disp", "body_vel"):
+            np.testing.assert_allclose(ig[k_], io[k_], rtol=1e-9, atol=1e-13)
+        assert relerr(g.get("marker_x"), o.markers()[0]) < 1e-14 and ig["step"] == 2 and abs(ig["time"] - io["time"]) < 1e-15
+        g.close()
+    # weak == coupling_max_iters 1, bitwise on the GPU
+    g1 = fs.from_workload(light()); g2 = fs.from_workload(light(coupling_max_iters=1))
+    g1.step(3); i2 = g2.step(3)
+    assert i2["coupling_iters"] == 1
+    for c in "uvwp":
+        assert np.array_equal(g1.get(c), g2.get(c))
+    g1.close(); g2.close()
+
+
 # ------------------------------------------------------------------------------------ NEXT-4: LES closures
 @pytest.mark.parametrize("kind", ["periodic", "channel", "open", "channel_upwind_wallonly"])
 def test_les_momentum_rhs_elementwise(fs, kind):
