@@ -34,7 +34,7 @@ __device__ __forceinline__ double inflow_rand(uint64_t seed, long long step, int
 // Value of a prescribed boundary-normal face of the predicted field (O1/O3).
 //   old = u^n of that component, q = index of the face, qi = index of its interior neighbour face.
 template <class T> __device__ __forceinline__ T boundary_normal(const Ctx<T>& c, const T* __restrict__ old, int d, int side,
-                                                               int a, int b, size_t q, size_t qi, int jedge) {
+                                                               int a, int b, size_t q, size_t qi, int jedge, double dtc) {
   const int face = 2 * d + side, t = c.bc[face];
   const double Ub = c.bcv[face][d];
   if (t == FS_BC_NOSLIP) return T(Ub);
@@ -47,7 +47,7 @@ template <class T> __device__ __forceinline__ T boundary_normal(const Ctx<T>& c,
   const double dn = d == 0 ? c.hx : (d == 1 ? (double)c.dy64[jedge] : c.hz);
   const double o = (double)old[q], oi = (double)old[qi];
   const double grad = side ? (o - oi) / dn : (oi - o) / dn;
-  return T(o - Ub * c.S->dt * grad);
+  return T(o - Ub * dtc * grad);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -170,7 +170,10 @@ template <class T> __global__ void __launch_bounds__(256) k_eddy_viscosity(const
 // LES variant of the kernel (template flag): the diffusive term becomes div[(nu + nu_t) grad u_i] with nu_t (array `nut`,
 // cell centred) at the flux locations -- cell centres natively, edges as the mean of the four surrounding cells -- through
 // a fourth shared-memory ring; on the wall faces of no-slip y walls nu_t is the wall model's (Eq. 28).
-template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX * kMomTY, LES ? 1 : 2) k_momentum(const Ctx<T> c, int kz, const T* __restrict__ nut) {
+// ADT (CFL-adaptive dt): the step size and the variable-step AB2 coefficients are read from device memory; the fixed-step
+// variant keeps them as constant-bank operands / immediates (the kernel sits at its register limit: three more live
+// doubles cost it a third of its speed).
+template <class T, bool UPW, bool LES, bool ADT> __global__ void __launch_bounds__(kMomTX * kMomTY, LES ? 1 : 2) k_momentum(const Ctx<T> c, int kz, const T* __restrict__ nut) {
   __shared__ T SU[4][kMomTY][kMomTX], SV[4][kMomTY][kMomTX], SW[4][kMomTY][kMomTX];
   __shared__ T SN[LES ? 4 : 1][LES ? kMomTY : 1][LES ? kMomTX : 1];
   const int tx = threadIdx.x, ty = threadIdx.y;
@@ -179,9 +182,10 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
   const bool own = tx >= 1 && tx <= kMomTX - 2 && ty >= 1 && ty <= kMomTY - 2 && iu < c.nxu && ju < c.nyv;
   const int k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nzw);
   const bool ab2 = c.time_scheme == FS_TIME_AB2 && c.S->have_hist;
-  const double rdt = ab2 ? c.S->dt / c.S->dt_prev : 0.0;       // step-size ratio (1 exactly for a fixed step: a0 = 3/2, a1 = -1/2)
-  const T a0 = ab2 ? T(1.0 + 0.5 * rdt) : T(1), a1 = ab2 ? T(-0.5 * rdt) : T(0);
-  const T dt = T(c.S->dt), nu = T(c.nu);
+  // AB2 with the step-size ratio r = dt_n / dt_{n-1}: a0 = 1 + r/2, a1 = -r/2 (3/2, -1/2 for a fixed step)
+  const double rdt = (ADT && ab2) ? c.S->dt / c.S->dt_prev : 1.0;
+  const T a0 = ab2 ? (ADT ? T(1.0 + 0.5 * rdt) : T(1.5)) : T(1), a1 = ab2 ? (ADT ? T(-0.5 * rdt) : T(-0.5)) : T(0);
+  const T dt = ADT ? T(c.S->dt) : T(c.dt), nu = T(c.nu);
   constexpr bool upw = UPW;                // convective scheme: compile-time, so the central path carries no selects
   const T* __restrict__ U = c.u; const T* __restrict__ V = c.v; const T* __restrict__ W = c.w;
   const ColRef<T> ru = col_setup<T, 0>(c, i, j), rv = col_setup<T, 1>(c, i, j), rw = col_setup<T, 2>(c, i, j);
@@ -240,7 +244,7 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
         if (c.bx && (i == 0 || i == c.nx)) {
           const int side = i == 0 ? 0 : 1;
           const size_t qi = side ? q - 1 : q + 1;
-          c.us[q] = boundary_normal<T>(c, U, 0, side, j, k, q, qi, 0);
+          c.us[q] = boundary_normal<T>(c, U, 0, side, j, k, q, qi, 0, (double)dt);
           c.hu[q] = T(0);
         } else {
           const T uE = SU[s1][ty][txp], uW = SU[s1][ty][txm], uN = SU[s1][typ][tx], uS = SU[s1][tym][tx];
@@ -255,7 +259,7 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
           const T dxx = (uE - T(2) * uc + uW) * c.ihx2;
           const T dyy = ((uN - uc) * idyc1 - (uc - uS) * idyc0) * idyj;
           const T dzz = (uT - T(2) * uc + uB) * c.ihz2;
-          T visc = nu * (dxx + dyy + dzz);
+          T H;
           if (LES) {
             const T nC = SN[s1][ty][tx], nW = SN[s1][ty][txm];
             const T fxe = (nu + nC) * (uE - uc) * c.ihx, fxw = (nu + nW) * (uc - uW) * c.ihx;
@@ -269,9 +273,9 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
             const T fyn = (nu + nn) * (uN - uc) * idyc1, fys = (nu + ns) * (uc - uS) * idyc0;
             const T nzt = T(0.25) * (((nW + nC) + SN[s2][ty][txm]) + SN[s2][ty][tx]), nzb = T(0.25) * (((SN[s0][ty][txm] + SN[s0][ty][tx]) + nW) + nC);
             const T fzt = (nu + nzt) * (uT - uc) * c.ihz, fzb = (nu + nzb) * (uc - uB) * c.ihz;
-            visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyj + (fzt - fzb) * c.ihz;
-          }
-          const T H = -(cx + cy + cz) + visc + T(c.g[0]);
+            const T visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyj + (fzt - fzb) * c.ihz;
+            H = -(cx + cy + cz) + visc + T(c.g[0]);
+          } else H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[0]);
           c.us[q] = uc + dt * (a0 * H + a1 * huo);
           c.hu[q] = H;
         }
@@ -282,7 +286,7 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
         if (c.by && (j == 0 || j == c.ny)) {
           const int side = j == 0 ? 0 : 1;
           const size_t qi = side ? q - c.nx : q + c.nx;
-          c.vs[q] = boundary_normal<T>(c, V, 1, side, i, k, q, qi, side ? c.ny - 1 : 0);
+          c.vs[q] = boundary_normal<T>(c, V, 1, side, i, k, q, qi, side ? c.ny - 1 : 0, (double)dt);
           c.hv[q] = T(0);
         } else {
           const T vE = SV[s1][ty][txp], vW = SV[s1][ty][txm], vN = SV[s1][typ][tx], vS = SV[s1][tym][tx];
@@ -298,7 +302,7 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
           const T dxx = (vE - T(2) * vc + vW) * c.ihx2;
           const T dyy = ((vN - vc) * idyj - (vc - vS) * idyjm) * idyc0;
           const T dzz = (vT - T(2) * vc + vB) * c.ihz2;
-          T visc = nu * (dxx + dyy + dzz);
+          T H;
           if (LES) {
             const T nC = SN[s1][ty][tx], nS = SN[s1][tym][tx];
             const T fxe = (nu + T(0.25) * (((nS + SN[s1][tym][txp]) + nC) + SN[s1][ty][txp])) * (vE - vc) * c.ihx;
@@ -306,9 +310,9 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
             const T fyn = (nu + nC) * (vN - vc) * idyj, fys = (nu + nS) * (vc - vS) * idyjm;
             const T fzt = (nu + T(0.25) * (((nS + nC) + SN[s2][tym][tx]) + SN[s2][ty][tx])) * (vT - vc) * c.ihz;
             const T fzb = (nu + T(0.25) * (((SN[s0][tym][tx] + SN[s0][ty][tx]) + nS) + nC)) * (vc - vB) * c.ihz;
-            visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyc0 + (fzt - fzb) * c.ihz;
-          }
-          const T H = -(cx + cy + cz) + visc + T(c.g[1]);
+            const T visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyc0 + (fzt - fzb) * c.ihz;
+            H = -(cx + cy + cz) + visc + T(c.g[1]);
+          } else H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[1]);
           c.vs[q] = vc + dt * (a0 * H + a1 * hvo);
           c.hv[q] = H;
         }
@@ -320,7 +324,7 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
           const int side = k == 0 ? 0 : 1;
           const size_t pl = (size_t)c.nx * c.ny;
           const size_t qi = side ? q - pl : q + pl;
-          c.ws[q] = boundary_normal<T>(c, W, 2, side, i, j, q, qi, 0);
+          c.ws[q] = boundary_normal<T>(c, W, 2, side, i, j, q, qi, 0, (double)dt);
           c.hw[q] = T(0);
         } else {
           const T wE = SW[s1][ty][txp], wW = SW[s1][ty][txm], wN = SW[s1][typ][tx], wS = SW[s1][tym][tx];
@@ -335,7 +339,7 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
           const T dxx = (wE - T(2) * wc + wW) * c.ihx2;
           const T dyy = ((wN - wc) * idyc1 - (wc - wS) * idyc0) * idyj;
           const T dzz = (wT - T(2) * wc + wB) * c.ihz2;
-          T visc = nu * (dxx + dyy + dzz);
+          T H;
           if (LES) {
             const T nC = SN[s1][ty][tx], nB = SN[s0][ty][tx];
             const T fxe = (nu + T(0.25) * (((nB + SN[s0][ty][txp]) + nC) + SN[s1][ty][txp])) * (wE - wc) * c.ihx;
@@ -349,9 +353,9 @@ template <class T, bool UPW, bool LES> __global__ void __launch_bounds__(kMomTX 
             }
             const T fyn = (nu + nn) * (wN - wc) * idyc1, fys = (nu + ns) * (wc - wS) * idyc0;
             const T fzt = (nu + nC) * (wT - wc) * c.ihz, fzb = (nu + nB) * (wc - wB) * c.ihz;
-            visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyj + (fzt - fzb) * c.ihz;
-          }
-          const T H = -(cx + cy + cz) + visc + T(c.g[2]);
+            const T visc = (fxe - fxw) * c.ihx + (fyn - fys) * idyj + (fzt - fzb) * c.ihz;
+            H = -(cx + cy + cz) + visc + T(c.g[2]);
+          } else H = -(cx + cy + cz) + nu * (dxx + dyy + dzz) + T(c.g[2]);
           c.ws[q] = wc + dt * (a0 * H + a1 * hwo);
           c.hw[q] = H;
         }
@@ -369,19 +373,28 @@ template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
   dim3 b(kMomTX, kMomTY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
   const double bytes = 12.0 * sizeof(T) * c.nx * c.ny * c.nz;
   int n = 1;
+  const bool adt = c.cfl > 0.0, upw = c.convection == FS_CONV_UPWIND;
+  T* nut = nullptr;
   if (les) {
     const long long N = (long long)c.nx * c.ny * c.nz;
-    T* nut = c.q;                        // PCG scratch, free until the Poisson solve of this step
+    nut = c.q;                           // PCG scratch, free until the Poisson solve of this step
     if (c.cs > 0.0) FS_LAUNCH(L, "eddy_viscosity", 4.0 * sizeof(T) * N, k_eddy_viscosity<T><<<flat_blocks(N), 256, 0, L.s>>>(c, nut));
     else FS_LAUNCH(L, "eddy_viscosity", 1.0 * sizeof(T) * N, cudaMemsetAsync(nut, 0, sizeof(T) * (size_t)N, L.s));
     ++n;
-    if (c.convection == FS_CONV_UPWIND) FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,upwind,LES>" : "k_momentum<f32,upwind,LES>", bytes + sizeof(T) * N, k_momentum<T, true, true><<<g, b, 0, L.s>>>(c, kz, nut));
-    else FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,central,LES>" : "k_momentum<f32,central,LES>", bytes + sizeof(T) * N, k_momentum<T, false, true><<<g, b, 0, L.s>>>(c, kz, nut));
-    return n;
   }
-  if (c.convection == FS_CONV_UPWIND) FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,upwind>" : "k_momentum<f32,upwind>", bytes, k_momentum<T, true, false><<<g, b, 0, L.s>>>(c, kz, nullptr));
-  else FS_LAUNCHI(L, "momentum_predictor", sizeof(T) == 8 ? "k_momentum<f64,central>" : "k_momentum<f32,central>", bytes, k_momentum<T, false, false><<<g, b, 0, L.s>>>(c, kz, nullptr));
-  return 1;
+  static const char* names[2][2][2] = {{{"k_momentum<f32,central>", "k_momentum<f32,upwind>"}, {"k_momentum<f32,central,LES>", "k_momentum<f32,upwind,LES>"}},
+                                       {{"k_momentum<f64,central>", "k_momentum<f64,upwind>"}, {"k_momentum<f64,central,LES>", "k_momentum<f64,upwind,LES>"}}};
+  const double tot = bytes + (les ? sizeof(T) * (double)c.nx * c.ny * c.nz : 0.0);
+  FS_LAUNCHI(L, "momentum_predictor", names[sizeof(T) == 8][les][upw], tot, {
+    if (les) {
+      if (upw) { if (adt) k_momentum<T, true, true, true><<<g, b, 0, L.s>>>(c, kz, nut); else k_momentum<T, true, true, false><<<g, b, 0, L.s>>>(c, kz, nut); }
+      else { if (adt) k_momentum<T, false, true, true><<<g, b, 0, L.s>>>(c, kz, nut); else k_momentum<T, false, true, false><<<g, b, 0, L.s>>>(c, kz, nut); }
+    } else {
+      if (upw) { if (adt) k_momentum<T, true, false, true><<<g, b, 0, L.s>>>(c, kz, nut); else k_momentum<T, true, false, false><<<g, b, 0, L.s>>>(c, kz, nut); }
+      else { if (adt) k_momentum<T, false, false, true><<<g, b, 0, L.s>>>(c, kz, nut); else k_momentum<T, false, false, false><<<g, b, 0, L.s>>>(c, kz, nut); }
+    }
+  });
+  return n;
 }
 
 // ---------------------------------------------------------------------------------------------------

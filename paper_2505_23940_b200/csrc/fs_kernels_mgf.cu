@@ -14,6 +14,7 @@
 // cell smaller per side (overlapped tiling: 64 x 2TR extended tile -> 60 x (2TR-4) results); the halo
 // re-reads hit L2.  All grids are periodic (GMG is only offered for triply periodic boxes).
 #include "fs_internal.cuh"
+#include <cstdlib>
 
 namespace fs {
 
@@ -278,7 +279,8 @@ k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __rest
 }
 
 // Tile height: TR thread rows (2 TR cell rows; 16 on big levels: fewer halo rows per result, 8 below: more CTAs).
-static int mg_tr(int ny) { return ny >= 384 ? 16 : 8; }
+static int tune_env(const char* n, int d) { const char* e = getenv(n); return e ? atoi(e) : d; }
+static int mg_tr(int ny) { static int thr = tune_env("FS_TUNE_TR16_NY", 384); return ny >= thr ? 16 : 8; }
 template <class T, int TR> static int slots_per_sm() { return (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1); }
 template <class K> static cudaError_t allow_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
