@@ -136,7 +136,15 @@ def _pins(case):
     return P
 
 
-@pytest.mark.parametrize("case", ["c2", "c3", "c4", "c5"])
+def _pin_case(case):
+    # a pin file costs hours of single-threaded oracle time (c4: ~2.5 h); a config whose file has not been written yet
+    # is reported as skipped, never silently passed
+    have = os.path.exists(os.path.join(os.path.dirname(__file__), "golden", "fullsize_%s.txt" % case))
+    return pytest.param(case, marks=pytest.mark.skipif(not have, reason="tests/golden/fullsize_%s.txt not written yet "
+                                                       "(python tests/golden/make_fullsize_pins.py %s)" % (case, case)))
+
+
+@pytest.mark.parametrize("case", [_pin_case(c) for c in ("c2", "c3", "c4", "c5")])
 def test_full_size_full_step_count_against_oracle_pins(fs, case):
     import importlib.util
     spec = importlib.util.spec_from_file_location("make_fullsize_pins", os.path.join(os.path.dirname(__file__), "golden", "make_fullsize_pins.py"))
