@@ -301,11 +301,20 @@ def measure(a, dtype, dev, local, rank, world, dist, with_e2e, with_profile):
         # the first level-0 down launch of every solve has no residual update to do (2.125 words instead of 4.125)
         if "mg_down_l0" in prof and prof["mg_down_l0"]["bytes"] > 4.0 * wbytes * cells * prof["mg_down_l0"]["launches"]:
             prof["mg_down_l0"]["bytes"] -= 2.0 * wbytes * cells * ksteps
+        # the V-cycle levels >= 1 and the one-CTA tail are reported as one entry, "mg_coarse" (per-level times inside it)
+        import re
+        sub = {k: prof.pop(k) for k in list(prof) if re.fullmatch(r"mg_(down|up)_l[1-9][0-9]*|mg_tail", k)}
+        if sub:
+            prof["mg_coarse"] = {"launches": sum(v["launches"] for v in sub.values()) + prof.get("mg_coarse", {}).get("launches", 0),
+                                 "ms": sum(v["ms"] for v in sub.values()) + prof.get("mg_coarse", {}).get("ms", 0.0),
+                                 "bytes": sum(v["bytes"] for v in sub.values()) + prof.get("mg_coarse", {}).get("bytes", 0.0)}
         tot = sum(v["ms"] for v in prof.values())
         kernels = {k: {"launches_per_step": v["launches"] / ksteps, "ms_per_step": v["ms"] / ksteps,
                        "share": v["ms"] / tot if tot else 0.0,
                        "algorithmic_GBps": (v["bytes"] / (v["ms"] * 1e-3) / 1e9) if v["ms"] > 0 else None}
                    for k, v in sorted(prof.items(), key=lambda kv: -kv[1]["ms"])}
+        if sub:
+            kernels["mg_coarse"]["levels_ms_per_step"] = {k: v["ms"] / ksteps for k, v in sorted(sub.items())}
         top = max(prof.items(), key=lambda kv: kv[1]["ms"])
         ach = top[1]["bytes"] / (top[1]["ms"] * 1e-3) / 1e9
         step_bytes = sum(v["bytes"] for v in prof.values()) / ksteps

@@ -37,6 +37,14 @@ struct orc_sim {
   bool oob;                            // a support reached a prescribed face / left a bounded box (unsupported)
   // body (Eq. 12)
   bool has_body; double bm, bc_, bk; int dof; double bdisp[3], bvel[3], bforce[3];
+  // flexible beam (Eq. 11, 13-17, Newmark-beta; reading N2-2 in DESIGN.md 3)
+  bool has_beam; int nb, ndof;         // nodes; degrees of freedom = 2 (nb - 1): (deflection, rotation) of nodes 1..nb-1, node 0 clamped
+  vec bX0; std::vector<int> mnode;     // reference node positions (x, y); node of every marker
+  double bnrm[2];                      // unit normal of the straight reference axis: markers move along it
+  double EI, mus, zeta, ralpha, rbeta, om1, om2;   // Eq. 13-16: stiffness, mass per length, damping ratio, Rayleigh coefficients, omega_1, omega_2
+  vec BK, BM, BC;                      // global matrices (ndof x ndof, dense, row major)
+  vec bw, bv, ba, bQ;                  // displacement, velocity, acceleration of the DOFs; load vector of the last step
+  vec Xref;                            // marker positions of the undeformed beam
   // GMG levels
   int nlev;
   // volume-of-solid mask (eps-mask IBM, Eq. 5, 8-9, 18-19, 23; reading E1 in DESIGN.md 3)
@@ -813,6 +821,126 @@ static double choose_dt(const orc_sim* s) {
   return std::min(s->P.dt, s->P.cfl * hmin / umax);
 }
 
+// ---- flexible beam (NEXT-2; Eq. 11, Eq. 13-17, Newmark-beta L177, Table 1) -------------------
+// Reading N2-2.  A straight beam of nb nodes in the x-y plane, clamped at node 0 (both flexible benchmarks
+// of section 3.3 are clamped plates, L544, L560).  "Only bending deformations are considered, and axial or shear effects
+// are neglected" (L149): every free node carries the two degrees of freedom of the 4 x 4 element matrices of Eq. 13-14,
+// the deflection w along the fixed normal n of the reference axis and the rotation theta; there is no axial motion.
+// Markers sit at the nodes (any number per node, e.g. one per span plane): X_l = X_l^ref + w_node n, U^b_l = wdot_node n.
+// Load: Q_w,i = n . q_i with q_i = -rho sum_{l in node i} F_l dV_l (Eq. 20 gathered per node), no nodal moments.
+// Damping: C = alpha M + beta K (Eq. 15) with alpha, beta from the two LOWEST modal frequencies of Eq. 17 (Eq. 16).
+// Time integration: Newmark-beta in its unconditionally stable second-order form (average acceleration, gamma = 1/2,
+// beta_N = 1/4), started from rest with zero acceleration.
+
+// Solves the dense n x n system A x = b by Gaussian elimination with partial pivoting (A and b by value: overwritten).
+static vec dense_solve(vec A, vec b, int n) {
+  for (int c = 0; c < n; ++c) {
+    int piv = c;
+    for (int r = c + 1; r < n; ++r) if (std::fabs(A[(size_t)r * n + c]) > std::fabs(A[(size_t)piv * n + c])) piv = r;
+    if (piv != c) { for (int k = 0; k < n; ++k) std::swap(A[(size_t)c * n + k], A[(size_t)piv * n + k]); std::swap(b[c], b[piv]); }
+    for (int r = c + 1; r < n; ++r) {
+      const double f = A[(size_t)r * n + c] / A[(size_t)c * n + c];
+      for (int k = c; k < n; ++k) A[(size_t)r * n + k] -= f * A[(size_t)c * n + k];
+      b[r] -= f * b[c];
+    }
+  }
+  vec x(n);
+  for (int r = n - 1; r >= 0; --r) {
+    double t = b[r];
+    for (int k = r + 1; k < n; ++k) t -= A[(size_t)r * n + k] * x[k];
+    x[r] = t / A[(size_t)r * n + r];
+  }
+  return x;
+}
+static vec matvec(const vec& A, const vec& x, int n) {
+  vec y(n, 0.0);
+  for (int r = 0; r < n; ++r) { double t = 0.0; for (int k = 0; k < n; ++k) t += A[(size_t)r * n + k] * x[k]; y[r] = t; }
+  return y;
+}
+static double dotv(const vec& a, const vec& b) { double t = 0.0; for (size_t i = 0; i < a.size(); ++i) t += a[i] * b[i]; return t; }
+
+// Assembles K and M from the element matrices of Eq. 13 and Eq. 14 (local DOF order: w_i, theta_i, w_{i+1}, theta_{i+1}),
+// drops the clamped node's rows and columns, finds omega_1, omega_2 of Eq. 17 by inverse iteration (x <- K^-1 M x, the
+// second vector kept M-orthogonal to the first) and builds C by Eq. 15-16.
+static void beam_assemble(orc_sim* s) {
+  const int nb = s->nb, nfull = 2 * nb, n = s->ndof;
+  vec Kf((size_t)nfull * nfull, 0.0), Mf((size_t)nfull * nfull, 0.0);
+  for (int e = 0; e + 1 < nb; ++e) {
+    const double dx = s->bX0[2 * (e + 1)] - s->bX0[2 * e], dy = s->bX0[2 * (e + 1) + 1] - s->bX0[2 * e + 1];
+    const double L = std::sqrt(dx * dx + dy * dy);
+    const double ke[4][4] = {{12, 6 * L, -12, 6 * L}, {6 * L, 4 * L * L, -6 * L, 2 * L * L}, {-12, -6 * L, 12, -6 * L}, {6 * L, 2 * L * L, -6 * L, 4 * L * L}};
+    const double me[4][4] = {{156, 22 * L, 54, -13 * L}, {22 * L, 4 * L * L, 13 * L, -3 * L * L}, {54, 13 * L, 156, -22 * L}, {-13 * L, -3 * L * L, -22 * L, 4 * L * L}};
+    const double kf = s->EI / (L * L * L), mf = s->mus * L / 420.0;
+    for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+      Kf[(size_t)(2 * e + a) * nfull + (2 * e + b)] += kf * ke[a][b];
+      Mf[(size_t)(2 * e + a) * nfull + (2 * e + b)] += mf * me[a][b];
+    }
+  }
+  s->BK.assign((size_t)n * n, 0.0); s->BM.assign((size_t)n * n, 0.0);
+  for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) {
+    s->BK[(size_t)r * n + c] = Kf[(size_t)(r + 2) * nfull + (c + 2)];
+    s->BM[(size_t)r * n + c] = Mf[(size_t)(r + 2) * nfull + (c + 2)];
+  }
+  vec phi[2]; double lam[2] = {0.0, 0.0};
+  for (int m = 0; m < 2 && m < n; ++m) {
+    vec x(n);
+    for (int i = 0; i < n; ++i) x[i] = 1.0 + 0.37 * i + (m ? ((i / 2) % 2 ? -1.0 : 1.0) : 0.0);   // any start with a component along the mode
+    for (int it = 0; it < 400; ++it) {
+      if (m == 1) { const double c0 = dotv(phi[0], matvec(s->BM, x, n)); for (int i = 0; i < n; ++i) x[i] -= c0 * phi[0][i]; }
+      x = dense_solve(s->BK, matvec(s->BM, x, n), n);
+      if (m == 1) { const double c0 = dotv(phi[0], matvec(s->BM, x, n)); for (int i = 0; i < n; ++i) x[i] -= c0 * phi[0][i]; }
+      const double nm = std::sqrt(dotv(x, matvec(s->BM, x, n)));
+      for (int i = 0; i < n; ++i) x[i] /= nm;
+    }
+    lam[m] = dotv(x, matvec(s->BK, x, n)) / dotv(x, matvec(s->BM, x, n));      // Rayleigh quotient = omega^2
+    phi[m] = x;
+  }
+  s->om1 = std::sqrt(lam[0]); s->om2 = std::sqrt(lam[1]);
+  s->ralpha = 2.0 * s->zeta * s->om1 * s->om2 / (s->om1 + s->om2);              // Eq. 16
+  s->rbeta = 2.0 * s->zeta / (s->om1 + s->om2);
+  s->BC.assign((size_t)n * n, 0.0);
+  for (size_t q = 0; q < s->BC.size(); ++q) s->BC[q] = s->ralpha * s->BM[q] + s->rbeta * s->BK[q];   // Eq. 15
+}
+
+// One Newmark-beta step (gamma = 1/2, beta_N = 1/4) of M a + C v + K w = Q from (w, v, a) with the load Q at the new time.
+static void beam_newmark(const orc_sim* s, const vec& Q, double dt, vec& w, vec& v, vec& a) {
+  const int n = s->ndof;
+  const double gam = 0.5, bet = 0.25;
+  const double a0 = 1.0 / (bet * dt * dt), a1 = gam / (bet * dt), a2 = 1.0 / (bet * dt), a3 = 1.0 / (2.0 * bet) - 1.0;
+  const double a4 = gam / bet - 1.0, a5 = 0.5 * dt * (gam / bet - 2.0);
+  vec Keff((size_t)n * n), tm(n), tc(n);
+  for (size_t q = 0; q < Keff.size(); ++q) Keff[q] = s->BK[q] + a0 * s->BM[q] + a1 * s->BC[q];
+  for (int i = 0; i < n; ++i) { tm[i] = a0 * w[i] + a2 * v[i] + a3 * a[i]; tc[i] = a1 * w[i] + a4 * v[i] + a5 * a[i]; }
+  const vec Mt = matvec(s->BM, tm, n), Ct = matvec(s->BC, tc, n);
+  vec rhs(n);
+  for (int i = 0; i < n; ++i) rhs[i] = Q[i] + Mt[i] + Ct[i];
+  const vec wn = dense_solve(Keff, rhs, n);
+  for (int i = 0; i < n; ++i) {
+    const double an = a0 * (wn[i] - w[i]) - a2 * v[i] - a3 * a[i];
+    v[i] = v[i] + dt * ((1.0 - gam) * a[i] + gam * an);
+    a[i] = an; w[i] = wn[i];
+  }
+}
+// load vector from the marker forces of the last fluid step (Eq. 20 gathered per node, projected on the beam normal)
+static void beam_load(orc_sim* s) {
+  s->bQ.assign(s->ndof, 0.0);
+  for (int l = 0; l < s->nl; ++l) {
+    const int i = s->mnode[l];
+    if (i <= 0) continue;                                      // markers of the clamped node load nothing
+    const double qx = -s->P.rho * s->Fl[3 * l] * s->dV[l], qy = -s->P.rho * s->Fl[3 * l + 1] * s->dV[l];
+    s->bQ[2 * (i - 1)] += qx * s->bnrm[0] + qy * s->bnrm[1];
+  }
+}
+// markers follow their node: X = X^ref + w n, U^b = wdot n
+static void beam_place_markers(orc_sim* s) {
+  for (int l = 0; l < s->nl; ++l) {
+    const int i = s->mnode[l];
+    const double w = i > 0 ? s->bw[2 * (i - 1)] : 0.0, wd = i > 0 ? s->bv[2 * (i - 1)] : 0.0;
+    s->X[3 * l] = s->Xref[3 * l] + w * s->bnrm[0]; s->X[3 * l + 1] = s->Xref[3 * l + 1] + w * s->bnrm[1]; s->X[3 * l + 2] = s->Xref[3 * l + 2];
+    s->Ub[3 * l] = wd * s->bnrm[0]; s->Ub[3 * l + 1] = wd * s->bnrm[1]; s->Ub[3 * l + 2] = 0.0;
+  }
+}
+
 // ---- the fluid part of one time step: a single fractional step, or the stages of the Runge-Kutta scheme ---------------
 static void fluid_step(orc_sim* s, orc_info* info, vec& HU, vec& HV, vec& HW) {
   if (s->P.time_scheme == ORC_TIME_RK3) {
@@ -850,7 +978,8 @@ static void one_step(orc_sim* s, orc_info* info) {
   s->dt = choose_dt(s);
   const double dt = s->dt;
   vec HU(s->u.size()), HV(s->v.size()), HW(s->w.size());
-  const int N = (s->has_body && s->P.coupling_max_iters > 1) ? s->P.coupling_max_iters : 1;
+  const int N = ((s->has_body || s->has_beam) && s->P.coupling_max_iters > 1) ? s->P.coupling_max_iters : 1;
+  const vec bw0 = s->bw, bv0 = s->bv, ba0 = s->ba;             // beam state of time level n
   vec u0, v0, w0, p0, X0;
   double d0[3], vel0[3];
   for (int c = 0; c < 3; ++c) { d0[c] = s->bdisp[c]; vel0[c] = s->bvel[c]; }
@@ -872,6 +1001,19 @@ static void one_step(orc_sim* s, orc_info* info) {
         if (!(dw == 0.0 && prev == 0.0)) xi += (dw / prev) * (dw / prev);
       }
       for (int l = 0; l < s->nl; ++l) for (int c = 0; c < 3; ++c) s->Ub[3 * l + c] = s->bvel[c];
+    }
+    if (s->has_beam) {                                                                 // O9': Newmark-beta on Eq. 11
+      const vec prev = s->bw;                                  // w^(k-1): what the markers reflect during this sub-iteration
+      beam_load(s);
+      vec wn = bw0, vn = bv0, an = ba0;
+      beam_newmark(s, s->bQ, dt, wn, vn, an);
+      xi = 0.0;
+      for (int i = 0; i < s->ndof; ++i) {
+        const double dw = wn[i] - prev[i];
+        if (!(dw == 0.0 && prev[i] == 0.0)) xi += (dw / prev[i]) * (dw / prev[i]);
+      }
+      s->bw = wn; s->bv = vn; s->ba = an;
+      beam_place_markers(s);
     }
     if (N > 1 && xi < s->P.coupling_tol) break;
   }
@@ -919,7 +1061,7 @@ extern "C" orc_sim* orc_create(const orc_params* p) {
   s->u.assign((size_t)s->nxu * s->ny * s->nz, 0.0); s->v.assign((size_t)s->nx * s->nyv * s->nz, 0.0);
   s->w.assign((size_t)s->nx * s->ny * s->nzw, 0.0); s->p.assign(N, 0.0); s->divu.assign(N, 0.0);
   s->hu = s->u; s->hv = s->v; s->hw = s->w;
-  s->have_hist = false; s->step = 0; s->nl = 0; s->nseg = 0; s->has_body = false; s->dof = 0; s->oob = false;
+  s->have_hist = false; s->step = 0; s->nl = 0; s->nseg = 0; s->has_body = false; s->dof = 0; s->oob = false; s->has_beam = false; s->nb = 0; s->ndof = 0;
   s->has_mask = false; s->uc[0] = s->uc[1] = s->uc[2] = 0.0;
   s->dt = s->dt_prev = p->dt; s->time = 0.0;
   for (int c = 0; c < 3; ++c) s->bdisp[c] = s->bvel[c] = s->bforce[c] = 0.0;
@@ -962,6 +1104,51 @@ extern "C" void orc_get_face_masks(orc_sim* s, unsigned char* mu, unsigned char*
 extern "C" int orc_set_body(orc_sim* s, double m, double c, double k, int dof) {
   if (!(m > 0)) return 1;
   s->has_body = true; s->bm = m; s->bc_ = c; s->bk = k; s->dof = dof; return 0;
+}
+extern "C" int orc_set_beam(orc_sim* s, int n_nodes, const double* node_xy, const int* marker_node, double EI, double mu_s, double zeta_s) {
+  if (n_nodes < 2 || !node_xy || !marker_node || !(EI > 0) || !(mu_s > 0) || zeta_s < 0 || s->nl <= 0 || s->has_body || s->has_mask) return 1;
+  const double tx = node_xy[2 * (n_nodes - 1)] - node_xy[0], ty = node_xy[2 * (n_nodes - 1) + 1] - node_xy[1];
+  const double len = std::sqrt(tx * tx + ty * ty);
+  if (!(len > 0)) return 1;
+  for (int i = 1; i < n_nodes; ++i) {                          // straight, ordered along the axis
+    const double ax = node_xy[2 * i] - node_xy[0], ay = node_xy[2 * i + 1] - node_xy[1];
+    const double bx_ = node_xy[2 * i] - node_xy[2 * (i - 1)], by_ = node_xy[2 * i + 1] - node_xy[2 * (i - 1) + 1];
+    if (std::fabs(ax * ty - ay * tx) > 1e-12 * len * len || !(bx_ * tx + by_ * ty > 0)) return 1;
+  }
+  for (int l = 0; l < s->nl; ++l) if (marker_node[l] < 0 || marker_node[l] >= n_nodes) return 1;
+  s->nb = n_nodes; s->ndof = 2 * (n_nodes - 1);
+  s->bX0.assign(node_xy, node_xy + (size_t)2 * n_nodes);
+  s->mnode.assign(marker_node, marker_node + s->nl);
+  s->bnrm[0] = -ty / len; s->bnrm[1] = tx / len;
+  s->EI = EI; s->mus = mu_s; s->zeta = zeta_s;
+  s->bw.assign(s->ndof, 0.0); s->bv.assign(s->ndof, 0.0); s->ba.assign(s->ndof, 0.0); s->bQ.assign(s->ndof, 0.0);
+  s->Xref = s->X;
+  s->has_beam = true;
+  beam_assemble(s);
+  return 0;
+}
+extern "C" int orc_beam_ndof(orc_sim* s) { return s->has_beam ? s->ndof : 0; }
+extern "C" void orc_beam_matrices(orc_sim* s, double* K, double* M, double* C, double* coef /* alpha, beta, omega_1, omega_2 */) {
+  if (K) std::copy(s->BK.begin(), s->BK.end(), K);
+  if (M) std::copy(s->BM.begin(), s->BM.end(), M);
+  if (C) std::copy(s->BC.begin(), s->BC.end(), C);
+  if (coef) { coef[0] = s->ralpha; coef[1] = s->rbeta; coef[2] = s->om1; coef[3] = s->om2; }
+}
+extern "C" void orc_get_beam_state(orc_sim* s, double* w, double* v, double* a, double* Q) {
+  if (w) std::copy(s->bw.begin(), s->bw.end(), w);
+  if (v) std::copy(s->bv.begin(), s->bv.end(), v);
+  if (a) std::copy(s->ba.begin(), s->ba.end(), a);
+  if (Q) std::copy(s->bQ.begin(), s->bQ.end(), Q);
+}
+extern "C" void orc_set_beam_state(orc_sim* s, const double* w, const double* v, const double* a) {
+  s->bw.assign(w, w + s->ndof); s->bv.assign(v, v + s->ndof); s->ba.assign(a, a + s->ndof);
+  beam_place_markers(s);
+}
+extern "C" void orc_beam_newmark(orc_sim* s, const double* Q, double dt) {
+  vec q(Q, Q + s->ndof);
+  beam_newmark(s, q, dt, s->bw, s->bv, s->ba);
+  s->bQ = q;
+  beam_place_markers(s);
 }
 extern "C" int orc_step(orc_sim* s, int nsteps, orc_info* last, int* iters) {
   orc_info info; std::memset(&info, 0, sizeof info);

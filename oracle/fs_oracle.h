@@ -72,6 +72,16 @@ int  orc_set_body(orc_sim*, double m, double c, double k, int dof_mask);
  * the structure velocity to the IB points (Eq. 18-19).  eps_cells == NULL switches back. */
 int  orc_set_solid_mask(orc_sim*, const unsigned char* eps_cells, const double* uc);
 void orc_get_face_masks(orc_sim*, unsigned char* mu, unsigned char* mv, unsigned char* mw);   /* 0 fluid, 1 solid, 2 IB point */
+/* Flexible beam (Eq. 11, 13-17, Newmark-beta; reading N2-2): a straight Euler-Bernoulli beam of n_nodes nodes in the x-y
+ * plane (node_xy: n_nodes * 2), clamped at node 0, two degrees of freedom (deflection along the axis normal, rotation) per
+ * free node; marker_node[l] = the node marker l rides on (call after orc_set_markers).  EI: bending stiffness, mu_s: mass
+ * per unit length, zeta_s: damping ratio of Eq. 16 (Rayleigh damping from omega_1, omega_2 of Eq. 17). */
+int  orc_set_beam(orc_sim*, int n_nodes, const double* node_xy, const int* marker_node, double EI, double mu_s, double zeta_s);
+int  orc_beam_ndof(orc_sim*);                                     /* 2 (n_nodes - 1) */
+void orc_beam_matrices(orc_sim*, double* K, double* M, double* C, double* coef /* alpha, beta, omega_1, omega_2 */);
+void orc_get_beam_state(orc_sim*, double* w, double* v, double* a, double* Q);   /* ndof each; Q = load of the last step */
+void orc_set_beam_state(orc_sim*, const double* w, const double* v, const double* a);
+void orc_beam_newmark(orc_sim*, const double* Q, double dt);      /* one Newmark step with the given load (piece for the pins) */
 int  orc_step(orc_sim*, int nsteps, orc_info* last, int* iters_per_step /* nsteps ints or NULL */);
 int  orc_poisson_solve(orc_sim*, const double* rhs, double* p_inout, orc_info* info);
 int  orc_set_history(orc_sim*, int have_history, long long step);   /* restart support */

@@ -4,6 +4,7 @@
 // Layout in HBM: structure of arrays, x fastest, then y, then z;
 // a velocity component has n+1 entries along its own normal when that direction is bounded.
 #pragma once
+#include <cuda.h>            // CUtensorMap (the type and enums only: the driver entry point is looked up at run time)
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "../../include/fs.h"
@@ -76,6 +77,11 @@ template <class T> struct Ctx {
   Scalars* S;
   double* partials;     // [kRedSlots][kMaxPartials]
 };
+
+// TMA descriptor of a dense (nx, ny, nz) field with a (boxx, boxy, 1) box; passed to kernels as a __grid_constant__ parameter
+struct Tmap { CUtensorMap m; };
+// false when the driver entry point is missing or the field / box does not qualify (then the kernel skips its prefetches)
+bool tmap_encode(Tmap* out, const void* ptr, int esize, int nx, int ny, int nz, int boxx, int boxy);
 
 struct MgLevel { int nx, ny, nz; double h; void *e, *g, *t; };
 template <class T> struct MgCtx {
@@ -190,6 +196,14 @@ template <> struct V2T<float> { using type = float2; };
 template <class T> struct V16T;
 template <> struct V16T<double> { using type = double2; };
 template <> struct V16T<float> { using type = float4; };
+// L2 prefetch of one tile plane of a field through its tensor map (fs_tma.cu): one instruction, no register and no
+// shared memory, so a streaming kernel can run its DRAM fetches several planes ahead of the register loads that
+// follow (those then hit L2) without growing its register queue.  (x, y, z) = element coordinates of the box origin;
+// parts of the box outside the array are skipped.  Called by ONE thread of the CTA.
+__device__ __forceinline__ void tma_prefetch_plane(const Tmap& m, int x, int y, int z) {
+  asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(reinterpret_cast<unsigned long long>(&m)), "r"(x), "r"(y), "r"(z)
+               : "memory");
+}
 template <class T, class V> __device__ __forceinline__ V ldv2(const T* p) { return *reinterpret_cast<const V*>(p); }
 template <class T, class V> __device__ __forceinline__ void stv2(T* p, const V& v) { *reinterpret_cast<V*>(p) = v; }
 

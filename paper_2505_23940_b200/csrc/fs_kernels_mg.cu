@@ -164,6 +164,12 @@ template <class T> cudaError_t mg_configure_device() {
 template cudaError_t mg_configure_device<float>();
 template cudaError_t mg_configure_device<double>();
 
+// profile labels of the fused legs per level (bench.py sums the levels >= 1 and the tail into "mg_coarse")
+static const char* const kDownName[kMaxLevels] = {"mg_down_l0", "mg_down_l1", "mg_down_l2", "mg_down_l3", "mg_down_l4", "mg_down_l5", "mg_down_l6", "mg_down_l7",
+                                                  "mg_down_l8", "mg_down_l9", "mg_down_l10", "mg_down_l11"};
+static const char* const kUpName[kMaxLevels] = {"mg_up_l0", "mg_up_l1", "mg_up_l2", "mg_up_l3", "mg_up_l4", "mg_up_l5", "mg_up_l6", "mg_up_l7",
+                                                "mg_up_l8", "mg_up_l9", "mg_up_l10", "mg_up_l11"};
+
 // Recursion unrolled on the host: emits the kernels of one V-cycle for rhs -> out (out = V(rhs)).
 template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const T* rhs, T* out, const Launch& L, bool* dot_fused, T zs, bool* upd_fused) {
   int n = 0;
@@ -189,7 +195,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     for (int l = 0; l < top; ++l) {
       const MgLevel& V = mg.lev[l];
       const bool upd = l == 0 && upd_fused != nullptr && want_dot && c.r2 != nullptr && rhs == c.r;
-      n += launch_mg_down<T>(c, gl[l], tl[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, V.h, mg.omega, l == 0 ? "mg_down_l0" : "mg_coarse", L,
+      n += launch_mg_down<T>(c, gl[l], tl[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, V.h, mg.omega, kDownName[l], L,
                              upd, upd ? c.r2 : nullptr, upd ? c.q : nullptr);
       if (upd) *upd_fused = true;
     }
@@ -202,7 +208,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
         cells += (size_t)mg.lev[l].nx * mg.lev[l].ny * mg.lev[l].nz;
       }
       const size_t smem = 3 * cells * sizeof(T);
-      FS_LAUNCH(L, "mg_coarse", 2.0 * sizeof(T) * mg.lev[lt].nx * mg.lev[lt].ny * mg.lev[lt].nz,
+      FS_LAUNCH(L, "mg_tail", 2.0 * sizeof(T) * mg.lev[lt].nx * mg.lev[lt].ny * mg.lev[lt].nz,
                 k_mg_tail<T><<<1, 1024, smem, L.s>>>(done, gl[lt], el[lt], a, mg.nu1, mg.nu2, mg.coarse_sweeps, mg.omega)); ++n;
     } else {
       const MgLevel& V = mg.lev[last];
@@ -223,7 +229,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     for (int l = top - 1; l >= 0; --l) {
       const MgLevel& V = mg.lev[l];
       const bool dot = want_dot && l == 0;
-      n += launch_mg_up<T>(c, tl[l], el[l + 1], gl[l], el[l], V.nx, V.ny, V.nz, V.h, mg.omega, dot, zs, l == 0 ? "mg_up_l0" : "mg_coarse", L,
+      n += launch_mg_up<T>(c, tl[l], el[l + 1], gl[l], el[l], V.nx, V.ny, V.nz, V.h, mg.omega, dot, zs, kUpName[l], L,
                            (l == 0 && r_pingpong) ? c.r2 : nullptr);
       if (dot) *dot_fused = true;
     }

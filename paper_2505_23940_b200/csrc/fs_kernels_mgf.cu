@@ -15,10 +15,12 @@
 // re-reads hit L2.  All grids are periodic (GMG is only offered for triply periodic boxes).
 #include "fs_internal.cuh"
 #include <cstdlib>
+#include <cstring>
 
 namespace fs {
 
 constexpr int kMgIX = 60;                 // result columns per tile (extended tile: 64 = 32 lanes x 2)
+constexpr int kMgAhead = 4;               // k_mg_up: planes between an L2 prefetch and the register load of the same data
 template <int TR> struct MgTile { static constexpr int ROWS = 2 * TR, IY = 2 * TR - 4, PL = 2 * TR * 32; };
 
 __device__ __forceinline__ int modp(int a, int n) { a %= n; return a < 0 ? a + n : a; }
@@ -111,27 +113,30 @@ k_mg_down(const int* __restrict__ done, const T* __restrict__ g_a, T* __restrict
   double s2 = 0.0, s1 = 0.0;
   int zl = modp(z0 - 2, nz);              // plane of the youngest load in flight
   int b = 0;                              // buffer of plane t (toggles); plane t-1 lives in PL - b
-  Quad<T> nxt, nx2, qn1, qn2;             // loads in flight: planes t and t+1 (two planes of latency cover)
-  qn1.lo.x = qn1.lo.y = qn1.hi.x = qn1.hi.y = T(0); qn2 = qn1;
+  // Two planes of global loads in flight, in two register buffers that alternate by renaming (the z loop is unrolled
+  // 6 = lcm(3, 2) times): step t consumes the buffer that was filled two steps earlier and refills it with plane t + 2,
+  // so no instruction touches a load before it is two planes old (a register copy between buffers would wait for it).
+  Quad<T> l0g, l0q, l1g, l1q;
+  l0q.lo.x = l0q.lo.y = l0q.hi.x = l0q.hi.y = T(0); l1q = l0q;
   auto fetch = [&](Quad<T>& gq, Quad<T>& qq) {
     const unsigned o = pl * zl;
     gq.lo = ldv2<T, V>(g + (row0 + o)); gq.hi = ldv2<T, V>(g + (row1 + o));
     if (UPD && upd) { qq.lo = ldv2<T, V>(qv + (row0 + o)); qq.hi = ldv2<T, V>(qv + (row1 + o)); }
   };
-  fetch(nxt, qn1);
+  fetch(l0g, l0q);
   zl = zl + 1 == nz ? 0 : zl + 1;
-  fetch(nx2, qn2);
-  // one plane: gA, gB = g(t-2), g(t-1); gC receives g(t).  eA, eB = e(t-3), e(t-2); eC receives e(t-1).
-  auto step = [&](int t, const Quad<T>& gA, const Quad<T>& gB, Quad<T>& gC, const Quad<T>& eA, const Quad<T>& eB, Quad<T>& eC) {
-    gC = nxt;
+  fetch(l1g, l1q);
+  // one plane: gA, gB = g(t-2), g(t-1); gC receives g(t) from the load buffer (lg, lq).  eA, eB = e(t-3), e(t-2); eC receives e(t-1).
+  auto step = [&](int t, const Quad<T>& gA, const Quad<T>& gB, Quad<T>& gC, const Quad<T>& eA, const Quad<T>& eB, Quad<T>& eC,
+                  Quad<T>& lg, Quad<T>& lq) {
+    gC = lg;
     if (UPD && upd) {
-      gC.lo.x = (gC.lo.x - alpha * qn1.lo.x) - rm; gC.lo.y = (gC.lo.y - alpha * qn1.lo.y) - rm;
-      gC.hi.x = (gC.hi.x - alpha * qn1.hi.x) - rm; gC.hi.y = (gC.hi.y - alpha * qn1.hi.y) - rm;
+      gC.lo.x = (gC.lo.x - alpha * lq.lo.x) - rm; gC.lo.y = (gC.lo.y - alpha * lq.lo.y) - rm;
+      gC.hi.x = (gC.hi.x - alpha * lq.hi.x) - rm; gC.hi.y = (gC.hi.y - alpha * lq.hi.y) - rm;
     }
-    nxt = nx2; if (UPD) qn1 = qn2;
     if (t + 1 < tend) {
       zl = zl + 1 == nz ? 0 : zl + 1;
-      fetch(nx2, qn2);
+      fetch(lg, lq);
     }
     const int pb = PL - b;
     if (t >= z0) {            // e(t-1)
@@ -166,9 +171,12 @@ k_mg_down(const int* __restrict__ done, const T* __restrict__ g_a, T* __restrict
   g1 = g0; g2 = g0; e0 = g0; e1 = g0; e2 = g0;
   int t = z0 - 2;
   for (;;) {
-    step(t, g0, g1, g2, e0, e1, e2); if (++t > tend) break;
-    step(t, g1, g2, g0, e1, e2, e0); if (++t > tend) break;
-    step(t, g2, g0, g1, e2, e0, e1); if (++t > tend) break;
+    step(t, g0, g1, g2, e0, e1, e2, l0g, l0q); if (++t > tend) break;
+    step(t, g1, g2, g0, e1, e2, e0, l1g, l1q); if (++t > tend) break;
+    step(t, g2, g0, g1, e2, e0, e1, l0g, l0q); if (++t > tend) break;
+    step(t, g0, g1, g2, e0, e1, e2, l1g, l1q); if (++t > tend) break;
+    step(t, g1, g2, g0, e1, e2, e0, l0g, l0q); if (++t > tend) break;
+    step(t, g2, g0, g1, e2, e0, e1, l1g, l1q); if (++t > tend) break;
   }
   if (UPD && upd) {           // what the last CTA of k_pcg_update does in the unfused path
     double v[2] = {s2, s1};
@@ -200,7 +208,9 @@ template <class T> __device__ __forceinline__ Quad<T> sweepq(const Quad<T>& e, c
 
 template <class T, int TR, bool DOT> __global__ void __launch_bounds__(32 * TR, (sizeof(T) == 4 ? 2 : 1) * (TR == 8 ? 2 : 1))
 k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __restrict__ ec, const T* __restrict__ g_a,
-        const T* __restrict__ g_b, T* __restrict__ eo, int nx, int ny, int nz, T ce, T cw, T cn, T zs, Scalars* S_, double* partials) {
+        const T* __restrict__ g_b, T* __restrict__ eo, int nx, int ny, int nz, T ce, T cw, T cn, T zs, Scalars* S_, double* partials,
+        const __grid_constant__ Tmap tm_e, const __grid_constant__ Tmap tm_c, const __grid_constant__ Tmap tm_ga,
+        const __grid_constant__ Tmap tm_gb, int pf) {
   using V = typename V2T<T>::type;
   constexpr int PL = MgTile<TR>::PL;
   if (done && *done) return;
@@ -225,12 +235,28 @@ k_mg_up(const int* __restrict__ done, const T* __restrict__ ein, const T* __rest
   nxa.lo = ldv2<T, V>(ein + (row0 + pl * zl)); nxa.hi = ldv2<T, V>(ein + (row1 + pl * zl));
   T nxc = ec[crow + cpl * (unsigned)(zl >> 1)];
   nxg.lo.x = nxg.lo.y = nxg.hi.x = nxg.hi.y = T(0);
+  // DRAM fetches run kMgAhead planes ahead of the register loads as L2 prefetches of whole tile planes (one TMA
+  // instruction per field and plane, issued by one thread; fs_tma.cu): the register loads then hit L2, so one plane of
+  // them in flight is enough and the register queue does not grow.
+  constexpr int kAl = 16 / (int)sizeof(T);       // a TMA box must start on 16 bytes: x is rounded down to kAl cells, the box is that much wider
+  const bool pf_on = pf && lane == 0 && ty == 0;
+  const bool g_is_b = g == g_b;
+  const int pf_x = blockIdx.x * kMgIX - 2, pf_y = blockIdx.y * MgTile<TR>::IY - 2;
+  auto prefetch = [&](int t) {             // planes t + kMgAhead of e (and of ec on even planes), t + kMgAhead - 1 of g
+    if (!pf_on || t + kMgAhead > tend) return;
+    const int z = modp(t + kMgAhead, nz);
+    tma_prefetch_plane(tm_e, pf_x & ~(kAl - 1), pf_y, z);
+    tma_prefetch_plane(g_is_b ? tm_gb : tm_ga, pf_x & ~(kAl - 1), pf_y, z == 0 ? nz - 1 : z - 1);
+    if (!(z & 1)) tma_prefetch_plane(tm_c, (pf_x >> 1) & ~(kAl - 1), pf_y >> 1, z >> 1);
+  };
+  for (int tt = z0 - 2 - kMgAhead + 1; tt < z0 - 2; ++tt) prefetch(tt);
   // aA, aB = (e + P ec)(t-2), (t-1); aC receives plane t.  bA, bB = first post-sweep at t-3, t-2; bC receives t-1.
   // gA = g(t-2); gB receives g(t-1).
   auto step = [&](int t, const Quad<T>& aA, const Quad<T>& aB, Quad<T>& aC, const Quad<T>& bA, const Quad<T>& bB, Quad<T>& bC,
                   const Quad<T>& gA, Quad<T>& gB) {
     aC.lo.x = nxa.lo.x + nxc; aC.lo.y = nxa.lo.y + nxc; aC.hi.x = nxa.hi.x + nxc; aC.hi.y = nxa.hi.y + nxc;
     gB = nxg;
+    prefetch(t);
     if (t < tend) {
       const unsigned og = pl * zl;                     // plane t
       nxg.lo = ldv2<T, V>(g + (row0 + og)); nxg.hi = ldv2<T, V>(g + (row1 + og));
@@ -310,7 +336,19 @@ template <class T, int TR, bool DOT> static void up_tr(const Ctx<T>& c, const T*
                                                        T ce, T cw, T cn, T zs, cudaStream_t s) {
   const MgGeom G = mg_geom(nx, ny, nz, MgTile<TR>::IY, slots_per_sm<T, TR>());
   const size_t smem = 8 * (size_t)MgTile<TR>::PL * sizeof(T);
-  k_mg_up<T, TR, DOT><<<G.grid, dim3(32, TR), smem, s>>>(&c.S->done, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, c.S, c.partials);
+  // tensor maps of the fields the kernel streams (extended tile planes: 64 x 2 TR fine cells, 32 x TR coarse cells)
+  Tmap te, tc, tga, tgb;
+  const int ROWS = MgTile<TR>::ROWS;
+  // box origins are rounded down to 16 bytes in the kernel: fine tiles start at 60 bx - 2 (even), coarse ones at 30 bx - 1
+  const int al = 16 / (int)sizeof(T), bxf = 64 + (al > 2 ? al : 0), bxc = 32 + al;
+  int pf = tmap_encode(&te, ein, sizeof(T), nx, ny, nz, bxf, ROWS) && tmap_encode(&tc, ec, sizeof(T), nx / 2, ny / 2, nz / 2, bxc, ROWS / 2) &&
+           tmap_encode(&tga, g, sizeof(T), nx, ny, nz, bxf, ROWS);
+  if (pf && g2) pf = tmap_encode(&tgb, g2, sizeof(T), nx, ny, nz, bxf, ROWS); else if (pf) tgb = tga;
+  if (!pf) { memset(&te, 0, sizeof te); tc = te; tga = te; tgb = te; }
+  // measured at 512^3 / 256^3 (profiles/r2_tma_prefetch.md): removes the long-scoreboard stalls in both precisions, the fp64 leg
+  // gains 0-5 % (it already moves its bytes at 0.88 of the copy rate), the fp32 leg with two CTAs per SM loses 5 %: fp64 only
+  else { static int on = tune_env("FS_TUNE_PF", sizeof(T) == 8 ? 1 : 0); pf = on; }
+  k_mg_up<T, TR, DOT><<<G.grid, dim3(32, TR), smem, s>>>(&c.S->done, ein, ec, g, g2, eo, nx, ny, nz, ce, cw, cn, zs, c.S, c.partials, te, tc, tga, tgb, pf);
 }
 
 // upd: level 0 inside PCG with the residual update of the previous iteration fused in (g2 = the other residual
