@@ -145,6 +145,35 @@ def cylinder_fsi(scale=1, per_ring=75, **kw):
     return cfg
 
 
+# ---------------------------------------------------------------- flexible plate (third item)
+def flexible_plate(scale=4, nodes=17, length=1.0, mass_ratio=10.0, ei=0.5, zeta=0.02, **kw):
+    """A flexible plate clamped at its lower end in a cross flow, spanning the periodic z direction: the shape of the
+    paper's wall-mounted flexible plate (section 3.3.1) on the c4 box.  `nodes` beam nodes along y,
+    one marker per node and span plane; cfg["beam"] = (node_xy, marker_node, EI, mu_s, zeta_s) for set_beam."""
+    nx, ny, nz = 384 // scale, 256 // scale, 32 // max(1, scale // 2)
+    h = 1.0 / 16.0
+    lx, ly, lz = nx * h, ny * h, nz * h
+    cfg = _base(name="flexible_plate", nx=nx, ny=ny, nz=nz, lx=lx, ly=ly, lz=lz, nu=1.0 / 150.0, dt=5e-3, steps=20)
+    cfg["bc"] = ["inflow", "outflow", "slip", "slip", "periodic", "periodic"]
+    cfg["bc_vel"][0] = [1.0, 0.0, 0.0]
+    cfg["bc_vel"][1] = [1.0, 0.0, 0.0]
+    cfg.update(kw)
+    sh = shapes(cfg)
+    cfg["init"] = {"u": np.ones(sh["u"]), "v": np.zeros(sh["v"]), "w": np.zeros(sh["w"])}
+    xp, y0 = lx / 3.0 + 0.013, 0.5 * (ly - length) + 0.007       # off the grid lines
+    s = np.linspace(0.0, length, nodes)
+    node_xy = np.stack([np.full(nodes, xp), y0 + s], axis=1)
+    zc = (np.arange(nz) + 0.5) * h
+    xyz = np.array([[node_xy[i, 0], node_xy[i, 1], z] for z in zc for i in range(nodes)])
+    marker_node = np.array([i for _ in zc for i in range(nodes)], dtype=np.int32)
+    ds = length / (nodes - 1)
+    dvol = np.full(xyz.shape[0], ds * h * h)                    # shell of one grid spacing (L185)
+    cfg["markers"] = (xyz, np.zeros_like(xyz), dvol)
+    cfg["max_markers"] = xyz.shape[0]
+    cfg["beam"] = (node_xy, marker_node, ei, mass_ratio * h * lz, zeta)   # mu_s = density ratio x thickness h x span
+    return cfg
+
+
 # ---------------------------------------------------------------- c5: decaying HIT
 def hit(n=512, seed=777, dtype="f64", device="cpu", **kw):
     """Random-phase solenoidal field, E(k) ~ k^4 exp(-2 (k/4)^2), u_rms = 1.

@@ -60,6 +60,12 @@ def lib():
         L.orc_rk4_body.argtypes = [C.c_double] * 5 + [C.POINTER(C.c_double)] * 2
         L.orc_set_body.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_int]
         L.orc_set_history.argtypes = [C.c_void_p, C.c_int, C.c_longlong]
+        L.orc_set_beam.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_double, C.c_double, C.c_double]
+        L.orc_beam_ndof.argtypes = [C.c_void_p]
+        L.orc_beam_matrices.argtypes = [C.c_void_p] + [C.POINTER(C.c_double)] * 4
+        L.orc_get_beam_state.argtypes = [C.c_void_p] + [C.POINTER(C.c_double)] * 4
+        L.orc_set_beam_state.argtypes = [C.c_void_p] + [C.POINTER(C.c_double)] * 3
+        L.orc_beam_newmark.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.c_double]
         _lib = L
     return _lib
 
@@ -194,6 +200,34 @@ class Oracle:
 
     def set_body(self, m, c, k, dof_mask):
         assert lib().orc_set_body(self.h, m, c, k, dof_mask) == 0
+
+    # ---- flexible beam (Eq. 11, 13-17, Newmark-beta; reading N2-2) -------------
+    def set_beam(self, node_xy, marker_node, EI, mu_s, zeta_s=0.0):
+        xy = _f64(node_xy).reshape(-1, 2)
+        mn = np.ascontiguousarray(marker_node, dtype=np.int32)
+        assert mn.size == self.nl
+        rc = lib().orc_set_beam(self.h, xy.shape[0], _dp(xy), _ip(mn), C.c_double(EI), C.c_double(mu_s), C.c_double(zeta_s))
+        if rc:
+            raise ValueError("oracle: set_beam failed")
+        self.ndof = lib().orc_beam_ndof(self.h)
+
+    def beam_matrices(self):
+        n = self.ndof
+        K, M, Cm, coef = np.empty((n, n)), np.empty((n, n)), np.empty((n, n)), np.empty(4)
+        lib().orc_beam_matrices(self.h, _dp(K), _dp(M), _dp(Cm), _dp(coef))
+        return K, M, Cm, dict(alpha=coef[0], beta=coef[1], omega1=coef[2], omega2=coef[3])
+
+    def beam_state(self):
+        n = self.ndof
+        w, v, a, Q = np.empty(n), np.empty(n), np.empty(n), np.empty(n)
+        lib().orc_get_beam_state(self.h, _dp(w), _dp(v), _dp(a), _dp(Q))
+        return dict(w=w, v=v, a=a, Q=Q)
+
+    def set_beam_state(self, w, v, a):
+        lib().orc_set_beam_state(self.h, _dp(_f64(w)), _dp(_f64(v)), _dp(_f64(a)))
+
+    def beam_newmark(self, Q, dt):
+        lib().orc_beam_newmark(self.h, _dp(_f64(Q)), C.c_double(dt))
 
     def set_body_state(self, disp, vel):
         lib().orc_set_body_state(self.h, _dp(_f64(disp)), _dp(_f64(vel)))
