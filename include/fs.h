@@ -105,6 +105,7 @@ typedef struct {
   double coupling_tol;         /* stop when xi = || (w^k - w^{k-1}) / w^{k-1} ||_2^2 < coupling_tol (paper: 1e-5, N <= 100) */
   double cfl;                  /* > 0: CFL-adaptive step (L431): dt = min(dt, cfl h_min / max|u,v,w|) from the field at the start
                                   of every step, h_min the smallest cell extent; <= 0: fixed dt */
+  int max_beam_nodes;          /* > 0: reserve workspace for a flexible beam of up to this many nodes (fs_set_beam; <= 129) */
 } fs_params;
 
 typedef struct {
@@ -164,6 +165,23 @@ fs_status fs_marker_segments(fs_grid* g, int* nseg);
  * All markers translate with the body. */
 fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask);
 fs_status fs_set_body_state(fs_grid* g, const double* disp3, const double* vel3);   /* HOST */
+
+/* Flexible structure (Eq. 11, Eq. 13-17, Newmark-beta L177): a straight Euler-Bernoulli beam of
+ * n_nodes nodes in the x-y plane, clamped at node 0 (the flexible plates of section 3.3), bending only (L149):
+ * every free node carries the deflection w along the normal n of the reference axis and the rotation theta, the degrees of
+ * freedom of the 4 x 4 element matrices of Eq. 13 (stiffness, EI / L_e^3) and Eq. 14 (consistent mass, mu_s L_e / 420).
+ * Damping C = alpha M + beta K (Eq. 15) with alpha, beta from the two lowest modal frequencies of Eq. 17 and the damping
+ * ratio zeta_s (Eq. 16).  Every step the nodal load Q_i = n . q_i, q_i = -rho sum_{l on node i} F_l dV_l (Eq. 20), drives
+ * one Newmark-beta step (gamma = 1/2, beta = 1/4) of Eq. 11 on the device; markers follow their node, X_l = X_l^ref + w n,
+ * U^b_l = dw/dt n.  With params.coupling_max_iters > 1 the sweeps of Algorithm 1 apply (xi over all degrees of freedom).
+ * node_xy: HOST, n_nodes * 2 fp64, collinear and ordered along the axis; marker_node: HOST, one int per marker (call after
+ * fs_set_ibm_markers; the current marker positions become the reference configuration).  FS_ERR_BAD_STATE without markers
+ * or with params.max_beam_nodes < n_nodes; FS_ERR_UNSUPPORTED together with a rigid body, the eps mask or a CFL-adaptive
+ * step; FS_ERR_INVALID_ARG for nodes that are not collinear / ordered, EI <= 0, mu_s <= 0, zeta_s < 0, a bad node index. */
+fs_status fs_set_beam(fs_grid* g, int n_nodes, const double* node_xy, const int* marker_node, double EI, double mu_s, double zeta_s);
+/* Beam state (HOST, fp64, 2 (n_nodes - 1) values each: w_1, theta_1, w_2, ...; any pointer may be NULL): displacement,
+ * velocity, acceleration, the load vector of the last step; coef (4 values): alpha, beta (Eq. 16), omega_1, omega_2 (Eq. 17). */
+fs_status fs_beam_state(fs_grid* g, double* w, double* v, double* a, double* Q, double* coef);
 
 /* The paper's own IBM: volume-of-solid function eps (1 in solid cells, 0 in fluid cells,
  * L110) instead of marker forcing.  eps_cells: HOST, nz*ny*nx bytes; uc: HOST, 3 fp64, the exact velocity u_c of the

@@ -50,7 +50,8 @@ class fs_params(C.Structure):
                 ("delta", C.c_int), ("max_markers", C.c_int),
                 ("seed", C.c_uint64), ("inflow_noise", C.c_double),
                 ("exec_mode", C.c_int), ("convection", C.c_int), ("solid_mask", C.c_int), ("cs", C.c_double), ("wall_model", C.c_int),
-                ("coupling_max_iters", C.c_int), ("coupling_tol", C.c_double), ("cfl", C.c_double)]
+                ("coupling_max_iters", C.c_int), ("coupling_tol", C.c_double), ("cfl", C.c_double),
+                ("max_beam_nodes", C.c_int)]
 
 
 class fs_step_info(C.Structure):
@@ -68,7 +69,7 @@ class fs_poisson_info(C.Structure):
 
 # every symbol include/fs.h declares (tests check the library exports all of them)
 SYMBOLS = ("fs_workspace_bytes", "fs_grid_create", "fs_grid_destroy", "fs_field_size", "fs_fields_set",
-           "fs_fields_get", "fs_set_history", "fs_set_ibm_markers", "fs_marker_segments", "fs_set_body", "fs_set_solid_mask",
+           "fs_fields_get", "fs_set_history", "fs_set_ibm_markers", "fs_marker_segments", "fs_set_body", "fs_set_solid_mask", "fs_set_beam", "fs_beam_state",
            "fs_set_body_state", "fs_step", "fs_poisson_solve", "fs_ibm_interpolate", "fs_ibm_spread",
            "fs_gmg_vcycle", "fs_momentum_rhs", "fs_profile_step", "fs_profile_count", "fs_profile_entry",
            "fs_profile_reset", "fs_launch_count", "fs_kernels_used", "fs_status_string")
@@ -103,6 +104,8 @@ def lib():
         L.fs_set_body.argtypes = [vp, C.c_double, C.c_double, C.c_double, ip]
         L.fs_set_body_state.argtypes = [vp, dp, dp]
         L.fs_set_solid_mask.argtypes = [vp, C.POINTER(C.c_ubyte), dp]
+        L.fs_set_beam.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_int), C.c_double, C.c_double, C.c_double]
+        L.fs_beam_state.argtypes = [vp, dp, dp, dp, dp, dp]
         L.fs_step.argtypes = [vp, ip, C.POINTER(fs_step_info)]
         L.fs_poisson_solve.argtypes = [vp, vp, vp, ip, ip, C.POINTER(fs_poisson_info)]
         L.fs_ibm_interpolate.argtypes = [vp, dp]
@@ -158,6 +161,7 @@ def make_params(cfg):
     P.convection = {"central": 0, "upwind": 1}[cfg.get("convection", "central")]
     P.solid_mask = int(cfg.get("solid_mask", 0))
     P.cfl = float(cfg.get("cfl", 0.0))
+    P.max_beam_nodes = int(cfg.get("max_beam_nodes", len(cfg["beam"][0]) if cfg.get("beam") is not None else 0))
     P.coupling_max_iters = int(cfg.get("coupling_max_iters", 1))
     P.coupling_tol = float(cfg.get("coupling_tol", 1e-5))
     P.cs = float(cfg.get("cs", 0.0))
@@ -301,6 +305,21 @@ class Grid:
     def set_body(self, m, c, k, dof_mask):
         _check(lib().fs_set_body(self.h, m, c, k, dof_mask), "fs_set_body")
 
+    def set_beam(self, node_xy, marker_node, EI, mu_s, zeta_s=0.0):
+        """fs_set_beam: flexible Euler-Bernoulli beam (Eq. 13-17, Newmark-beta) riding on the current markers."""
+        xy = np.ascontiguousarray(node_xy, dtype=np.float64).reshape(-1, 2)
+        mn = np.ascontiguousarray(marker_node, dtype=np.int32)
+        _check(lib().fs_set_beam(self.h, xy.shape[0], xy.ctypes.data_as(C.POINTER(C.c_double)), mn.ctypes.data_as(C.POINTER(C.c_int)),
+                                 float(EI), float(mu_s), float(zeta_s)), "fs_set_beam")
+        self.beam_ndof = 2 * (xy.shape[0] - 1)
+
+    def beam_state(self):
+        """fs_beam_state: dict(w, v, a, Q, alpha, beta, omega1, omega2)."""
+        dp = C.POINTER(C.c_double)
+        out = [np.empty(self.beam_ndof) for _ in range(4)] + [np.empty(4)]
+        _check(lib().fs_beam_state(self.h, *[a.ctypes.data_as(dp) for a in out]), "fs_beam_state")
+        return dict(w=out[0], v=out[1], a=out[2], Q=out[3], alpha=out[4][0], beta=out[4][1], omega1=out[4][2], omega2=out[4][3])
+
     def set_body_state(self, disp, vel):
         dp = C.POINTER(C.c_double)
         d = np.ascontiguousarray(disp, dtype=np.float64)
@@ -414,4 +433,6 @@ def from_workload(cfg, device="cuda:0", **overrides):
         g.set_body(*c["body"])
     if c.get("mask") is not None:
         g.set_solid_mask(*c["mask"])
+    if c.get("beam") is not None:
+        g.set_beam(*c["beam"])
     return g

@@ -75,6 +75,7 @@ struct fs_grid {
   long long fixed_launches = 0, body_iters_poisson = 0;
   int nl = 0; bool indexed = false;
   void* bak[7] = {nullptr};           // strong coupling: u, v, w, p, H^{n-1} of time level n (device, T)
+  double beam_coef[4] = {0, 0, 0, 0}; // flexible beam: alpha, beta (Eq. 16), omega_1, omega_2 (Eq. 17)
   int last_sweeps = 1; double last_xi = 0.0; long long last_iters = 0;
 };
 
@@ -114,6 +115,7 @@ fs_status validate(const fs_params* p) {
   if (!(p->dt > 0) || !(p->rho > 0) || !(p->lx > 0) || !(p->ly > 0) || !(p->lz > 0) || !(p->nu >= 0)) return FS_ERR_INVALID_ARG;
   if (p->dtype != FS_F32 && p->dtype != FS_F64) return FS_ERR_INVALID_ARG;
   if (p->max_markers < 0 || p->max_iter < 0 || !(p->rtol >= 0)) return FS_ERR_INVALID_ARG;
+  if (p->max_beam_nodes < 0 || p->max_beam_nodes == 1 || p->max_beam_nodes > kMaxBeamNodes) return FS_ERR_INVALID_ARG;
   for (int f = 0; f < 6; ++f) if ((int)p->bc[f] < 0 || (int)p->bc[f] > 4) return FS_ERR_INVALID_ARG;
   for (int d = 0; d < 3; ++d)
     if ((p->bc[2 * d] == FS_BC_PERIODIC) != (p->bc[2 * d + 1] == FS_BC_PERIODIC)) return FS_ERR_INVALID_ARG;
@@ -190,6 +192,14 @@ template <class T> size_t carve(fs_grid* g, char* base) {
   ib.Fl = b.take<double>(3 * M); ib.Ul = b.take<double>(3 * M); ib.wts = b.take<double>(36 * M);
   ib.base = b.take<int>(9 * M); ib.perm = b.take<int>(M); ib.keys = b.take<int>(M); ib.keys_raw = b.take<int>(M);
   ib.seg = b.take<int>(M + 1); ib.flags = b.take<int>(M);
+  ib.bw = ib.bv = ib.ba = ib.bw0 = ib.bv0 = ib.ba0 = ib.bQ = ib.bL = ib.bM = ib.bC = ib.Xref = nullptr; ib.mnode = ib.nstart = ib.nlist = nullptr;
+  if (P.max_beam_nodes > 0) {             // flexible beam: state, band matrices, reference marker positions, node <-> marker maps
+    const size_t nd = 2 * (size_t)(P.max_beam_nodes - 1);
+    ib.bw = b.take<double>(nd); ib.bv = b.take<double>(nd); ib.ba = b.take<double>(nd);
+    ib.bw0 = b.take<double>(nd); ib.bv0 = b.take<double>(nd); ib.ba0 = b.take<double>(nd); ib.bQ = b.take<double>(nd);
+    ib.bL = b.take<double>(4 * nd); ib.bM = b.take<double>(7 * nd); ib.bC = b.take<double>(7 * nd);
+    ib.Xref = b.take<double>(3 * M); ib.mnode = b.take<int>(M); ib.nstart = b.take<int>((size_t)P.max_beam_nodes + 1); ib.nlist = b.take<int>(M);
+  }
   ib.eps = ib.mu = ib.mv = ib.mw = nullptr; ib.ibu = ib.ibv = ib.ibw = nullptr;
   if (P.solid_mask) {                     // eps-mask IBM: cell mask, face classes, and (with markers) the u_IB scratch fields
     ib.eps = b.take<unsigned char>(g->nP);
@@ -280,6 +290,8 @@ void init_ibm(fs_grid* g) {
   ib.has_body = 0; ib.dof = 0; ib.bm = 1.0; ib.bc = 0.0; ib.bk = 0.0;
   ib.has_mask = 0; ib.uc[0] = ib.uc[1] = ib.uc[2] = 0.0;
   ib.strong = 0;
+  ib.has_beam = 0; ib.nbn = 0; ib.ndof = 0; ib.bnrm[0] = ib.bnrm[1] = 0.0;
+  for (int a = 0; a < 6; ++a) ib.nk[a] = 0.0;
 }
 
 
@@ -292,10 +304,10 @@ template <class T> int enqueue_pre(fs_grid* g, const Launch& L, bool poisson) {
   } else {
     n += launch_momentum<T>(c, L);
     if (g->ib.has_mask) {                 // the paper's eps-mask forcing (markers only carry the structure velocity to the IB points)
-      if (g->ib.n > 0 && (g->ib.has_body || !g->indexed)) n += launch_ibm_index<T>(c, g->ib, L);
+      if (g->ib.n > 0 && (g->ib.has_body || g->ib.has_beam || !g->indexed)) n += launch_ibm_index<T>(c, g->ib, L);
       n += launch_mask_forcing<T>(c, g->ib, L);
     } else if (g->ib.n > 0) {
-      if (g->ib.has_body || !g->indexed) n += launch_ibm_index<T>(c, g->ib, L);
+      if (g->ib.has_body || g->ib.has_beam || !g->indexed) n += launch_ibm_index<T>(c, g->ib, L);
       n += launch_ibm_interpolate<T>(c, g->ib, c.us, c.vs, c.ws, g->ib.Ul, L);
       n += launch_ibm_force<T>(c, g->ib, L);
       n += launch_ibm_spread<T>(c, g->ib, g->ib.Fl, c.us, c.vs, c.ws, -1.0, L);
@@ -315,7 +327,10 @@ template <class T> int enqueue_post(fs_grid* g, const Launch& L, bool poisson, i
   else {
     n += launch_project<T>(c, L);
     if (nstages > 1) n += launch_stage_end<T>(c, stage, L);
-    if (stage == nstages - 1) n += launch_step_end<T>(c, g->ib, L);
+    if (stage == nstages - 1) {
+      if (g->ib.has_beam) n += launch_beam_step<T>(c, g->ib, L);
+      n += launch_step_end<T>(c, g->ib, L);
+    }
   }
   return n;
 }
@@ -423,8 +438,14 @@ template <class T> fs_status run_once(fs_grid* g, bool poisson) {
 // sweep's force, and the host -- the loop is data dependent by nature -- stops on xi = ||(w^k - w^{k-1}) / w^{k-1}||^2.
 template <class T> fs_status advance_step(fs_grid* g) {
   g->last_sweeps = 1; g->last_xi = 0.0; g->last_iters = -1;
-  const int N = (g->ib.has_body && g->P.coupling_max_iters > 1) ? g->P.coupling_max_iters : 1;
+  const int N = ((g->ib.has_body || g->ib.has_beam) && g->P.coupling_max_iters > 1) ? g->P.coupling_max_iters : 1;
   if (N == 1) return run_once<T>(g, false);
+  if (g->ib.has_beam) {                   // the beam's state of time level n: every sweep's Newmark step starts there
+    const size_t nb = (size_t)g->ib.ndof * sizeof(double);
+    CK(cudaMemcpyAsync(g->ib.bw0, g->ib.bw, nb, cudaMemcpyDeviceToDevice, g->stream));
+    CK(cudaMemcpyAsync(g->ib.bv0, g->ib.bv, nb, cudaMemcpyDeviceToDevice, g->stream));
+    CK(cudaMemcpyAsync(g->ib.ba0, g->ib.ba, nb, cudaMemcpyDeviceToDevice, g->stream));
+  }
   Ctx<T>& c = ctx<T>(g);
   Scalars h0;
   CK(cudaMemcpyAsync(&h0, g->S, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
@@ -450,11 +471,12 @@ template <class T> fs_status advance_step(fs_grid* g) {
     CK(cudaStreamSynchronize(g->stream));
     iters += hs.iter;
     xi = 0.0;
-    for (int a = 0; a < 3; ++a) if (g->ib.dof & (1 << a)) {
+    for (int a = 0; a < 3; ++a) if (g->ib.has_body && (g->ib.dof & (1 << a))) {
       const double dw = hs.body_disp[a] - prev[a];
       if (!(dw == 0.0 && prev[a] == 0.0)) xi += (dw / prev[a]) * (dw / prev[a]);
       prev[a] = hs.body_disp[a];
     }
+    if (g->ib.has_beam) xi = hs.beam_xi;   // summed over the degrees of freedom by k_beam_step
     if (xi < g->P.coupling_tol) break;
   }
   g->last_sweeps = k > N ? N : k; g->last_xi = xi; g->last_iters = iters;
@@ -721,6 +743,7 @@ fs_status fs_set_ibm_markers(fs_grid* g, int n, const double* xyz, const double*
   if (n > 0 && !g->uniform_y) return FS_ERR_UNSUPPORTED;
   IbmCtx& ib = g->ib;
   ib.n = n; g->nl = n; g->indexed = false;
+  ib.has_beam = 0;                  // a beam rides on a particular marker set: it has to be set again (fs_set_beam)
   invalidate(g);
   if (n == 0) {
     double z[3] = {0, 0, 0};
@@ -768,9 +791,61 @@ fs_status fs_marker_segments(fs_grid* g, int* nseg) {
 fs_status fs_set_body(fs_grid* g, double m, double c, double k, int dof_mask) {
   if (!g || !(m > 0)) return FS_ERR_INVALID_ARG;
   GUARD(g);
+  if (g->ib.has_beam) return FS_ERR_UNSUPPORTED;
   g->ib.has_body = 1; g->ib.bm = m; g->ib.bc = c; g->ib.bk = k; g->ib.dof = dof_mask;
   g->ib.strong = g->P.coupling_max_iters > 1;
   invalidate(g);
+  return FS_OK;
+}
+
+fs_status fs_set_beam(fs_grid* g, int n_nodes, const double* node_xy, const int* marker_node, double EI, double mu_s, double zeta_s) {
+  if (!g || n_nodes < 2 || !node_xy || !marker_node || !(EI > 0) || !(mu_s > 0) || zeta_s < 0) return FS_ERR_INVALID_ARG;
+  GUARD(g);
+  IbmCtx& ib = g->ib;
+  if (ib.n <= 0 || g->P.max_beam_nodes < n_nodes) return FS_ERR_BAD_STATE;
+  if (ib.has_body || ib.has_mask || g->P.cfl > 0.0) return FS_ERR_UNSUPPORTED;
+  const double tx = node_xy[2 * (n_nodes - 1)] - node_xy[0], ty = node_xy[2 * (n_nodes - 1) + 1] - node_xy[1];
+  const double len = std::sqrt(tx * tx + ty * ty);
+  if (!(len > 0)) return FS_ERR_INVALID_ARG;
+  for (int i = 1; i < n_nodes; ++i) {       // collinear and ordered along the axis
+    const double ax = node_xy[2 * i] - node_xy[0], ay = node_xy[2 * i + 1] - node_xy[1];
+    const double ex = node_xy[2 * i] - node_xy[2 * (i - 1)], ey = node_xy[2 * i + 1] - node_xy[2 * (i - 1) + 1];
+    if (std::fabs(ax * ty - ay * tx) > 1e-12 * len * len || !(ex * tx + ey * ty > 0)) return FS_ERR_INVALID_ARG;
+  }
+  std::vector<int> start(n_nodes + 1, 0), list(ib.n);
+  for (int l = 0; l < ib.n; ++l) { if (marker_node[l] < 0 || marker_node[l] >= n_nodes) return FS_ERR_INVALID_ARG; start[marker_node[l] + 1] += 1; }
+  for (int i = 0; i < n_nodes; ++i) start[i + 1] += start[i];
+  { std::vector<int> fill(start.begin(), start.end() - 1); for (int l = 0; l < ib.n; ++l) list[fill[marker_node[l]]++] = l; }
+  const int nd = 2 * (n_nodes - 1);
+  std::vector<double> Lb(4 * (size_t)nd), Mb(7 * (size_t)nd), Cb(7 * (size_t)nd);
+  if (!beam_build(n_nodes, node_xy, EI, mu_s, zeta_s, g->P.dt, Lb.data(), Mb.data(), Cb.data(), ib.nk, g->beam_coef)) return FS_ERR_INVALID_ARG;
+  invalidate(g);
+  ib.has_beam = 1; ib.nbn = n_nodes; ib.ndof = nd; ib.bnrm[0] = -ty / len; ib.bnrm[1] = tx / len;
+  ib.strong = g->P.coupling_max_iters > 1;
+  double* zero7[7] = {ib.bw, ib.bv, ib.ba, ib.bw0, ib.bv0, ib.ba0, ib.bQ};
+  for (double* z : zero7) CK(cudaMemsetAsync(z, 0, (size_t)nd * sizeof(double), g->stream));
+  CK(cudaMemcpyAsync(ib.bL, Lb.data(), Lb.size() * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(ib.bM, Mb.data(), Mb.size() * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(ib.bC, Cb.data(), Cb.size() * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(ib.Xref, ib.X, 3 * (size_t)ib.n * sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
+  CK(cudaMemcpyAsync(ib.mnode, marker_node, (size_t)ib.n * sizeof(int), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(ib.nstart, start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(ib.nlist, list.data(), list.size() * sizeof(int), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return FS_OK;
+}
+
+fs_status fs_beam_state(fs_grid* g, double* w, double* v, double* a, double* Q, double* coef) {
+  if (!g) return FS_ERR_INVALID_ARG;
+  GUARD(g);
+  if (!g->ib.has_beam) return FS_ERR_BAD_STATE;
+  const size_t nb = (size_t)g->ib.ndof * sizeof(double);
+  if (w) CK(cudaMemcpyAsync(w, g->ib.bw, nb, cudaMemcpyDeviceToHost, g->stream));
+  if (v) CK(cudaMemcpyAsync(v, g->ib.bv, nb, cudaMemcpyDeviceToHost, g->stream));
+  if (a) CK(cudaMemcpyAsync(a, g->ib.ba, nb, cudaMemcpyDeviceToHost, g->stream));
+  if (Q) CK(cudaMemcpyAsync(Q, g->ib.bQ, nb, cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  if (coef) for (int i = 0; i < 4; ++i) coef[i] = g->beam_coef[i];
   return FS_OK;
 }
 
@@ -778,7 +853,7 @@ fs_status fs_set_solid_mask(fs_grid* g, const unsigned char* eps_cells, const do
   if (!g) return FS_ERR_INVALID_ARG;
   GUARD(g);
   if (!g->P.solid_mask) return FS_ERR_BAD_STATE;
-  if (!g->uniform_y) return FS_ERR_UNSUPPORTED;
+  if (!g->uniform_y || (eps_cells && g->ib.has_beam)) return FS_ERR_UNSUPPORTED;
   invalidate(g);
   IbmCtx& ib = g->ib;
   if (!eps_cells) { ib.has_mask = 0; return FS_OK; }

@@ -46,6 +46,7 @@ struct Scalars {
   int nseg; int bbox_lo[3], bbox_hi[3]; int pad1;
   double body_force[3], body_disp[3], body_vel[3];
   double body_disp0[3], body_vel0[3];   // strong coupling: the body's state at time level n (every sweep's RK4 starts there)
+  double beam_xi;                       // flexible beam: xi of Algorithm 1 of the last Newmark step
   // tickets for last-block reductions
   unsigned int ticket[8];
 };
@@ -104,7 +105,16 @@ struct IbmCtx {
   int has_mask; double uc[3];
   unsigned char *eps, *mu, *mv, *mw;
   void *ibu, *ibv, *ibw;       // T*: u_IB spread from the markers (Eq. 18), velocity-shaped
+  // flexible beam (Eq. 11, 13-17, Newmark-beta; reading N2-2): ndof = 2 (nodes - 1) degrees of freedom (w, theta per free node)
+  int has_beam, nbn, ndof;
+  double bnrm[2];              // unit normal of the straight reference axis (markers move along it)
+  double nk[6];                // Newmark coefficients a0..a5 for the grid's (fixed) dt
+  double *bw, *bv, *ba, *bw0, *bv0, *ba0, *bQ;   // state, state of time level n (strong coupling), load of the last step
+  double *bL, *bM, *bC;        // band storage: Cholesky factor of K_eff [ndof][4] (columns r-3..r), M and C [ndof][7] (columns r-3..r+3)
+  double *Xref;                // marker positions of the undeformed beam
+  int *mnode, *nstart, *nlist; // node of each marker; markers of node i = nlist[nstart[i] .. nstart[i+1]) in ascending id
 };
+constexpr int kMaxBeamNodes = 129;   // 256 degrees of freedom: the Newmark step runs in one CTA's shared memory
 
 // Per-kernel timing (measurement aid, fs_profile_step): when prof != nullptr every launch is bracketed
 // by a CUDA event pair on the launching stream and tagged with its name and ALGORITHMIC bytes (the
@@ -186,6 +196,11 @@ template <class T> int launch_ibm_force(const Ctx<T>& c, const IbmCtx& ib, const
 template <class T> int launch_ibm_spread(const Ctx<T>& c, const IbmCtx& ib, const double* F, T* u, T* v, T* w, double scale, const Launch& L);
 template <class T> int launch_mask_classify(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
 template <class T> int launch_mask_forcing(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
+template <class T> int launch_beam_step(const Ctx<T>& c, const IbmCtx& ib, const Launch& L);
+// host side of fs_set_beam (fs_beam.cu): assembles Eq. 13-14, finds omega_1, omega_2 of Eq. 17, builds C (Eq. 15-16), factors
+// K_eff = K + a0 M + a1 C; outputs in band storage as IbmCtx describes them.  false: M or K_eff not positive definite.
+bool beam_build(int nb, const double* node_xy, double EI, double mus, double zeta, double dt,
+                double* Lband, double* Mband, double* Cband, double* nk, double* coef /* alpha, beta, omega1, omega2 */);
 
 // ---- device helpers ---------------------------------------------------------------------------------
 #ifdef __CUDACC__

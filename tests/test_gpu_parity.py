@@ -34,6 +34,8 @@ def _oracle(cfg):
         o.set_markers(*cfg["markers"])
     if cfg.get("body") is not None:
         o.set_body(*cfg["body"])
+    if cfg.get("beam") is not None:
+        o.set_beam(*cfg["beam"])
     return o
 
 
@@ -328,6 +330,48 @@ def test_strong_coupling_matches_oracle(fs):
     for c in "uvwp":
         assert np.array_equal(g1.get(c), g2.get(c))
     g1.close(); g2.close()
+
+
+# ------------------------------------------------------------------------------------ NEXT-2: flexible beam (Eq. 13-17, Newmark-beta)
+def test_flexible_beam_matches_oracle(fs):
+    # a clamped flexible plate in a cross flow (the shape of PAPER.md section 3.3.1): beam matrices / frequencies of the host
+    # setup (Cholesky + Jacobi rotations) against the oracle's (inverse iteration), then weak coupling over 10 steps and
+    # strong coupling (Algorithm 1) over 3: state, load vector, markers, fields, sweeps
+    for kw, steps in ((dict(), 10), (dict(coupling_max_iters=25, coupling_tol=1e-12), 3), (dict(coupling_max_iters=4, coupling_tol=0.0, zeta=0.0), 2)):
+        cfg = W.flexible_plate(scale=8, nodes=9, rtol=1e-10, **kw)
+        o = _oracle(cfg); g = fs.from_workload(cfg)
+        co = o.beam_matrices()[3]; sg = g.beam_state()
+        for k_ in ("alpha", "beta", "omega1", "omega2"):
+            assert abs(sg[k_] - co[k_]) <= 1e-10 * abs(co[k_]), (k_, sg[k_], co[k_])
+        for s_ in range(steps):
+            io = o.step(1); ig = g.step(1)
+            assert ig["coupling_iters"] == io["coupling_iters"], (ig["coupling_iters"], io["coupling_iters"])
+            if kw:
+                assert io["coupling_iters"] >= 3 and abs(ig["coupling_xi"] - io["coupling_xi"]) <= 1e-5 * io["coupling_xi"] + 1e-28
+        _compare_state(g, o, TOL64, fields="uvp")
+        # span-uniform flow: w is PCG-residual noise (1e-12) on both sides, compared on the scale of the velocity field (|u| ~ 1)
+        assert np.abs(g.get("w") - o.get("w")).max() < TOL64 * np.abs(o.get("u")).max()
+        so, sg = o.beam_state(), g.beam_state()
+        assert np.abs(so["w"]).max() > 1e-6                                   # the plate did bend
+        for k_ in ("w", "v", "a", "Q"):
+            assert relerr(sg[k_], so[k_]) < 1e-8, (kw, k_, relerr(sg[k_], so[k_]))
+        xo, uo, fo = o.markers()
+        assert relerr(g.get("marker_x"), xo) < 1e-14 and relerr(g.get("marker_u"), uo) < 1e-8 and relerr(g.get("marker_f"), fo) < 1e-8
+        for k_ in ("body_force",):
+            np.testing.assert_allclose(ig[k_], io[k_], rtol=1e-9, atol=1e-13)
+        assert "beam_newmark" in g.kernels_used()
+        g.close()
+    # ABI: a beam needs workspace, markers, and excludes the rigid body
+    cfg = W.flexible_plate(scale=8, nodes=9)
+    g = fs.Grid(dict(cfg, max_beam_nodes=4))
+    for c_, a_ in cfg["init"].items():
+        g.set(c_, a_)
+    with pytest.raises(fs.FsError):
+        g.set_beam(*cfg["beam"])                                              # no markers yet
+    g.set_markers(*cfg["markers"])
+    with pytest.raises(fs.FsError):
+        g.set_beam(*cfg["beam"])                                              # 9 nodes > max_beam_nodes 4
+    g.close()
 
 
 # ------------------------------------------------------------------------------------ NEXT-4: LES closures
