@@ -83,6 +83,9 @@ template <class T> struct Ctx {
 struct Tmap { CUtensorMap m; };
 // false when the driver entry point is missing or the field / box does not qualify (then the kernel skips its prefetches)
 bool tmap_encode(Tmap* out, const void* ptr, int esize, int nx, int ny, int nz, int boxx, int boxy);
+// the fields one streaming kernel prefetches; n = 0: none (some map could not be encoded)
+struct TmapSet { Tmap m[6]; int n; };
+constexpr int kPfAhead = 4;          // planes between the L2 prefetch of a tile plane and the register loads of the same data
 
 struct MgLevel { int nx, ny, nz; double h; void *e, *g, *t; };
 template <class T> struct MgCtx {

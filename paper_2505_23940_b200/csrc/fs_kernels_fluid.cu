@@ -2,8 +2,13 @@
 // Poisson right-hand side (S6), projection + divergence diagnostics (S8), step bookkeeping (S9/S10).
 // Hand-written for sm_100a; shares nothing with oracle/.
 #include "fs_internal.cuh"
+#include <cstring>
+#include <cstdlib>
 
 namespace fs {
+
+static int tune_pf() { const char* e = getenv("FS_TUNE_PF2"); return e ? atoi(e) : 1; }   // experiments: FS_TUNE_PF2=0 turns the TMA prefetches off
+
 
 constexpr int kFlatBlocks = 148 * 8;
 static inline int flat_blocks(long long n) { long long b = (n + 255) / 256; return (int)(b < kFlatBlocks ? (b < 1 ? 1 : b) : kFlatBlocks); }
@@ -673,7 +678,7 @@ template <class T> __global__ void __launch_bounds__(256) k_project(const Ctx<T>
 // rows of the extended tile: 12 in fp32 (80 registers), 8 in fp64 (114 registers, no spills)
 template <class T> struct PjTile { static constexpr int TY = sizeof(T) == 4 ? 12 : 8; };
 
-template <class T> __global__ void __launch_bounds__(32 * PjTile<T>::TY, 2) k_projectv(const Ctx<T> c, int kz) {
+template <class T> __global__ void __launch_bounds__(32 * PjTile<T>::TY, 2) k_projectv(const Ctx<T> c, int kz, const __grid_constant__ TmapSet tm) {
   constexpr int kPjTY = PjTile<T>::TY;
   constexpr int VX = Vec16<T>::VX, ROWE = 32 * VX, PLN = kPjTY * ROWE;
   using W = Vec16<T>;
@@ -706,6 +711,17 @@ template <class T> __global__ void __launch_bounds__(32 * PjTile<T>::TY, 2) k_pr
     r.vs = ld16<T>(c.vs + (rowv_o + plv * kc));
     r.ws = ld16<T>(c.ws + (rowc_o + plc * (unsigned)kwf(k)));
   };
+  // tile planes of p, u*, v*, w* go to L2 kPfAhead planes before the register loads ask for them (one TMA prefetch per field
+  // and plane, issued by one thread; the loads then have L2 latency, which the two planes in flight cover)
+  const bool pf_on = tm.n > 0 && lane == 0 && ty == 0;
+  const int pf_x = (blockIdx.x * 30 - 1) * VX, pf_y = blockIdx.y * (kPjTY - 2) - 1;
+  auto prefetch = [&](int k) {
+    if (!pf_on || k > k1) return;
+    const int kc = kcell(k), kw = kwf(k);
+    tma_prefetch_plane(tm.m[0], pf_x, pf_y, kc); tma_prefetch_plane(tm.m[1], pf_x, pf_y, kc);
+    tma_prefetch_plane(tm.m[2], pf_x, pf_y, kc); tma_prefetch_plane(tm.m[3], pf_x, pf_y, kw);
+  };
+  for (int k = k0 + 2; k < k0 + 2 + kPfAhead; ++k) prefetch(k);
   Raw r0, r1;
   W pB = ld16<T>(c.p + (rowc_o + plc * (unsigned)kcell(k0 - 1)));
   fetch(k0, r0);
@@ -753,6 +769,7 @@ template <class T> __global__ void __launch_bounds__(32 * PjTile<T>::TY, 2) k_pr
     }
     st16<T>(SU + b + o_own, un); st16<T>(SV + b + o_own, vn);
     wnP = wn; pB = r.p;
+    prefetch(k + 2 + kPfAhead);
     if (k + 2 <= k1) fetch(k + 2, r);
     b = PLN - b;
   };
@@ -792,8 +809,13 @@ template <class T> int launch_project(const Ctx<T>& c, const Launch& L) {
   if (!c.bx && c.nx % Vec16<T>::VX == 0) {
     const int bxn = (c.nx + 30 * Vec16<T>::VX - 1) / (30 * Vec16<T>::VX), byn = (c.nyv + PjTile<T>::TY - 3) / (PjTile<T>::TY - 2);
     const int kz = pick_kz((long long)bxn * byn, c.nzw, 2LL * 148, 1, 16);
+    TmapSet tm; memset(&tm, 0, sizeof tm);
+    const int bw = 32 * Vec16<T>::VX, bh = PjTile<T>::TY;
+    static const int pf = tune_pf();
+    if (pf && tmap_encode(&tm.m[0], c.p, sizeof(T), c.nx, c.ny, c.nz, bw, bh) && tmap_encode(&tm.m[1], c.us, sizeof(T), c.nx, c.ny, c.nz, bw, bh) &&
+        tmap_encode(&tm.m[2], c.vs, sizeof(T), c.nx, c.nyv, c.nz, bw, bh) && tmap_encode(&tm.m[3], c.ws, sizeof(T), c.nx, c.ny, c.nzw, bw, bh)) tm.n = 4;
     FS_LAUNCHI(L, "project", sizeof(T) == 8 ? "k_projectv<f64>" : "k_projectv<f32>", 7.0 * sizeof(T) * c.nx * c.ny * c.nz,
-              k_projectv<T><<<dim3(bxn, byn, (c.nzw + kz - 1) / kz), dim3(32, PjTile<T>::TY), 0, L.s>>>(c, kz));
+              k_projectv<T><<<dim3(bxn, byn, (c.nzw + kz - 1) / kz), dim3(32, PjTile<T>::TY), 0, L.s>>>(c, kz, tm));
     return 1;
   }
   ColGeom g = col_geom(c.nxu, c.nyv, c.nzw);
