@@ -5,6 +5,8 @@
 // Loop control lives in device memory: the last block of k_pcg_update decides whether the CUDA-graph
 // WHILE node runs another iteration.
 #include "fs_internal.cuh"
+#include <cstring>
+#include <cstdlib>
 
 namespace fs {
 
@@ -454,7 +456,7 @@ template <class T> static DaGeom dav_geom(int nx, int ny, int nz) {
 // Same start, streaming form of k_pcg_dirapplyv (one 16-byte vector of cells per thread, A applied to x0
 // through a shared plane and a register queue); bhat is only stored when the caller needs it later (WBH:
 // fs_poisson_solve's true residual; fs_step gets that from the projection).
-template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pcg_initv(const Ctx<T> c, int kz, Launch L) {
+template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaTY, 2) k_pcg_initv(const Ctx<T> c, int kz, Launch L, const __grid_constant__ TmapSet tm) {
   constexpr int VX = Vec16<T>::VX;
   constexpr int ROWE = 32 * VX;
   constexpr int PLN = kDaTY * ROWE;
@@ -497,6 +499,15 @@ template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaT
     }
     return d;
   };
+  // tile planes of x0 and of the right-hand side go to L2 kPfAhead planes before the register loads (TMA, one thread)
+  const bool pf_on = tm.n > 0 && lane == 0 && ty == 0;
+  const int pf_x = (blockIdx.x * 30 - 1) * VX, pf_y = blockIdx.y * kDaVIY - 1;
+  auto prefetch = [&](int k) {
+    if (!pf_on || k > k1) return;
+    tma_prefetch_plane(tm.m[0], pf_x, pf_y, c.bz ? min(k, c.nz - 1) : (k >= c.nz ? k - c.nz : k));
+    if (k < k1) tma_prefetch_plane(tm.m[1], pf_x, pf_y, k);
+  };
+  for (int k = k0 + 2; k < k0 + 2 + kPfAhead; ++k) prefetch(k);
   W d0 = fetch(k0 - 1), d1 = fetch(k0), d2, nx1 = fetch(k0 + 1);
   W rb;                                     // raw right-hand side of the plane about to be processed
 #pragma unroll
@@ -508,6 +519,7 @@ template <class T, int PC, bool WBH> __global__ void __launch_bounds__(32 * kDaT
   double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
   auto step = [&](int k, const W& dB, const W& dC, W& dT) {
     dT = nx1;
+    prefetch(k + 2 + kPfAhead);
     if (k + 1 < k1) nx1 = fetch(k + 2);
     const W rcur = rb;
     if (own && k + 1 < k1) rb = ld16<T>(c.r + (row + pl * (unsigned)(k + 1)));
@@ -700,6 +712,17 @@ template <class T> __global__ void __launch_bounds__(256) k_dot_rz(const Ctx<T> 
   }
 }
 
+// tensor maps of n cell-shaped fields with a (boxx, boxy) tile plane box; .n = 0 when prefetching is off, a map cannot be encoded,
+// or the periodic x direction is absent (bounded x: tiles are clamped, not prefetched)
+template <class T> static TmapSet cell_maps(const Ctx<T>& c, const T* const* f, int n, int boxx, int boxy) {
+  static const int on = [] { const char* e = getenv("FS_TUNE_PF2"); return e ? atoi(e) : 1; }();
+  TmapSet tm; memset(&tm, 0, sizeof tm);
+  if (!on || c.bx) return tm;
+  for (int i = 0; i < n; ++i) if (!f[i] || !tmap_encode(&tm.m[i], f[i], sizeof(T), c.nx, c.ny, c.nz, boxx, boxy)) return tm;
+  tm.n = n;
+  return tm;
+}
+
 template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L, bool need_bhat) {
   int n = 0;
   const double N = (double)c.nx * c.ny * c.nz;
@@ -708,9 +731,11 @@ template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L, bool ne
     const DaGeom G = dav_geom<T>(c.nx, c.ny, c.nz);
     const dim3 blk(32, kDaTY);
     const bool jac = c.precond == FS_PC_JACOBI;
+    const T* pf_f[2] = {c.p, c.r};
+    const TmapSet tm = cell_maps<T>(c, pf_f, 2, 32 * Vec16<T>::VX, kDaTY);
     FS_LAUNCHI(L, "pcg_init", sizeof(T) == 8 ? "k_pcg_initv<f64>" : "k_pcg_initv<f32>", (need_bhat ? 4.0 : 3.0) * sizeof(T) * N, {
-      if (jac) { if (need_bhat) k_pcg_initv<T, 1, true><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); else k_pcg_initv<T, 1, false><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); }
-      else { if (need_bhat) k_pcg_initv<T, 0, true><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); else k_pcg_initv<T, 0, false><<<G.grid, blk, 0, L.s>>>(c, G.kz, L); }
+      if (jac) { if (need_bhat) k_pcg_initv<T, 1, true><<<G.grid, blk, 0, L.s>>>(c, G.kz, L, tm); else k_pcg_initv<T, 1, false><<<G.grid, blk, 0, L.s>>>(c, G.kz, L, tm); }
+      else { if (need_bhat) k_pcg_initv<T, 0, true><<<G.grid, blk, 0, L.s>>>(c, G.kz, L, tm); else k_pcg_initv<T, 0, false><<<G.grid, blk, 0, L.s>>>(c, G.kz, L, tm); }
     });
     return n + 1;
   }
