@@ -623,6 +623,10 @@ fs_status fs_grid_create(const fs_params* params, void* workspace, size_t bytes,
     if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) { delete g; return FS_ERR_INVALID_ARG; }
     if (pa.type == cudaMemoryTypeDevice && pa.device != g->device) { delete g; return FS_ERR_INVALID_ARG; }
   }
+  if ((g->f64 ? momv_configure_device<double>() : momv_configure_device<float>()) != cudaSuccess) {
+    std::fprintf(stderr, "libfs: cudaFuncSetAttribute(max dynamic shared memory) failed for the momentum kernel\n");
+    delete g; return FS_ERR_CUDA;
+  }
   if (g->P.precond == FS_PC_GMG) {
     const cudaError_t e1 = g->f64 ? mg_configure_device<double>() : mg_configure_device<float>();
     const cudaError_t e2 = g->f64 ? mgf_configure_device<double>() : mgf_configure_device<float>();

@@ -162,6 +162,10 @@ inline int pick_kz(long long tiles_xy, int nz, long long slots, int halo, int mi
 
 // ---- launchers (one per kernel family; each returns the number of kernels it enqueued) ----------
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L);
+// vectorised S1 kernel (fs_kernels_momv.cu): periodic x, nx a multiple of the vector width, no LES closure, y / z periodic or walls
+template <class T> bool momentumv_applies(const Ctx<T>& c);
+template <class T> int launch_momentumv(const Ctx<T>& c, const Launch& L);
+template <class T> cudaError_t momv_configure_device();
 template <class T> int launch_flux_correction(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_div_rhs(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_rhs_from_b(const Ctx<T>& c, const T* b, const Launch& L);

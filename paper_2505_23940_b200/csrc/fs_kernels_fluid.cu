@@ -371,6 +371,7 @@ template <class T, bool UPW, bool LES, bool ADT> __global__ void __launch_bounds
 }
 
 template <class T> int launch_momentum(const Ctx<T>& c, const Launch& L) {
+  if (momentumv_applies<T>(c)) return launch_momentumv<T>(c, L);
   const int bxn = (c.nxu + kMomTX - 3) / (kMomTX - 2), byn = (c.nyv + kMomTY - 3) / (kMomTY - 2);
   const bool les = c.nu > 0.0 && (c.cs > 0.0 || c.wall_model);
   // z chunks: whole waves of resident CTAs (2 CTAs of 320 threads per SM; the LES variant: 1) while chunks stay >= 16 planes

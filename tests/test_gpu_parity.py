@@ -101,6 +101,44 @@ def test_momentum_rhs_elementwise(fs, kind):
     g.close()
 
 
+@pytest.mark.parametrize("kind", ["periodic", "channel", "zwalls", "channel_upwind", "periodic_adaptive"])
+def test_momentum_vector_kernel_elementwise(fs, kind, monkeypatch):
+    # k_momentumv (one 16-byte vector of faces per thread; periodic x, walls in y / z): H^n element-wise against the oracle
+    # in fp64 at 1e-12 (FS_TUNE_MOMV=2 routes fp64 grids through it; the default uses it for fp32 only, where it is the
+    # faster kernel) and in fp32 on the scale of fp32 rounding; the predicted field through one full step.  Several tiles
+    # (120 x 14 cells in fp32, 60 x 14 in fp64) with ragged tails, several z chunks.
+    def zwalls(**kw):
+        c = _cfg_periodic(136, 34, 40, **kw)
+        c["bc"][4], c["bc"][5] = "noslip", "slip"
+        c["bc_vel"][4] = [0.2, -0.1, 0.0]
+        return c
+    mk = {"periodic": lambda **kw: _cfg_periodic(136, 38, 37, **kw), "channel": lambda **kw: _cfg_channel(128, 50, 35, **kw), "zwalls": zwalls,
+          "channel_upwind": lambda **kw: _cfg_channel(72, 31, 19, convection="upwind", **kw),
+          "periodic_adaptive": lambda **kw: _cfg_periodic(64, 30, 33, cfl=0.3, **kw)}[kind]
+    upw = "upwind" if "upwind" in kind else "central"
+    cfg = mk()
+    cfg["init"] = _rand_fields(cfg, 21)
+    o = _oracle(cfg)
+    ref = o.momentum_rhs()
+    monkeypatch.setenv("FS_TUNE_MOMV", "2")
+    g = fs.from_workload(cfg)
+    got = g.momentum_rhs()
+    assert "k_momentumv<f64,%s>" % upw in g.kernels_used(), g.kernels_used()
+    for c, a, b in zip("uvw", got, ref):
+        assert relerr(a, b) < 1e-12, (kind, c, relerr(a, b))
+    io, ig = o.step(2), g.step(2)                      # second step: AB2 with history (variable step when cfl > 0)
+    _compare_state(g, o, TOL64)
+    assert abs(ig["dt"] - io["dt"]) <= 1e-15 * io["dt"]
+    g.close()
+    monkeypatch.delenv("FS_TUNE_MOMV")
+    g32 = fs.from_workload(dict(cfg, dtype="f32"))
+    got32 = g32.momentum_rhs()
+    assert "k_momentumv<f32,%s>" % upw in g32.kernels_used(), g32.kernels_used()
+    for c, a, b in zip("uvw", got32, ref):
+        assert relerr(a, b) < 2e-5, (kind, c, relerr(a, b))     # fp32: eps32 x the cancellation in the flux differences (|u| / h ~ 50)
+    g32.close()
+
+
 @pytest.mark.parametrize("kind", ["periodic", "channel", "open"])
 def test_momentum_rhs_upwind_elementwise(fs, kind):
     # NEXT-3: first-order upwind convective fluxes (random fields: both signs of every advecting velocity)
