@@ -54,6 +54,7 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-profile", action="store_true")
+    ap.add_argument("--traffic-from", nargs="+", metavar="DTYPE=RAW.CSV", help="write profiles/r2_traffic.csv from ncu raw CSV dumps (no GPU run)")
     return ap.parse_args()
 
 
@@ -141,6 +142,47 @@ def ncu_traffic(dtype, label):
             except ValueError:
                 break
     return None, "kernel not in the committed capture"
+
+
+TRAFFIC_LABELS = (("k_momentum", "momentum_predictor"), ("k_div_rhs", "div_rhs"), ("k_pcg_init", "pcg_init"), ("k_mg_down", "mg_down_l0"),
+                  ("k_mg_up", "mg_up_l0"), ("k_pcg_dirapply", "pcg_dir_apply_dot"), ("k_project", "project"), ("k_pflush", "p_flush_mean"))
+
+
+def traffic_from_ncu(raw_csvs):
+    """`python bench.py --traffic-from f64=<raw.csv> f32=<raw.csv>`: turns `ncu -i <rep> --page raw --csv` dumps of
+    `ncu --set full ... python bench.py --exec stream --single-dtype --dtype <d>` into profiles/r2_traffic.csv: per dtype and
+    profile label the DRAM bytes of the LAST launch of the kernel's largest grid (steady state), stamped with the hash of
+    the sources this checkout holds (ncu_traffic refuses the file when the sources change).  No GPU needed."""
+    import csv
+    out = ["# csrc_sha256=%s" % csrc_hash(),
+           "# dtype,label,kernel,grid,dram_read_bytes,dram_write_bytes,duration_us  (per launch; ncu --set full --clock-control none; see r2_ncu_full.md)"]
+    for spec in raw_csvs:
+        dtype, path = spec.split("=", 1)
+        rows = list(csv.reader(open(path)))
+        h, units = rows[0], rows[1]
+        col = {n: i for i, n in enumerate(h)}
+
+        def val(r, name):
+            v, u = float(r[col[name]].replace(",", "")), units[col[name]]
+            scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "ms": 1e3, "us": 1.0, "ns": 1e-3, "s": 1e6}.get(u, 1.0)
+            return v * scale
+        best = {}
+        for r in rows[2:]:
+            name = r[col["Kernel Name"]]
+            for prefix, label in TRAFFIC_LABELS:
+                if name.split("<")[0].split(" ")[-1].startswith(prefix):
+                    grid = r[col["Grid Size"]]
+                    ncta = 1
+                    for x in grid.strip("()").split(","):
+                        ncta *= int(x)
+                    if label not in best or ncta >= best[label][0]:
+                        best[label] = (ncta, name, grid, val(r, "dram__bytes_read.sum"), val(r, "dram__bytes_write.sum"), val(r, "gpu__time_duration.sum"))
+        for label, (ncta, name, grid, rd, wr, us) in sorted(best.items()):
+            kn = name.replace("void ", "").split("(")[0].replace(",", ";")
+            out.append("%s,%s,%s,%s,%.0f,%.0f,%.1f" % (dtype, label, kn, grid.replace(",", ";"), rd, wr, us))
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    open(path, "w").write("\n".join(out) + "\n")
+    print(path)
 
 
 def peaks():
@@ -425,6 +467,9 @@ def run_ours(a):
 
 def main():
     a = parse()
+    if a.traffic_from:
+        traffic_from_ncu(a.traffic_from)
+        return
     if a.impl == "reference":
         run_reference(a)
     else:

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfs.so")
-SOURCES = ["fs_api.cu", "fs_kernels_fluid.cu", "fs_kernels_pcg.cu", "fs_kernels_mg.cu", "fs_kernels_mgf.cu", "fs_kernels_ibm.cu", "fs_tma.cu", "fs_beam.cu", "fs_kernels_momv.cu"]
+SOURCES = ["fs_api.cu", "fs_kernels_fluid.cu", "fs_kernels_pcg.cu", "fs_kernels_mg.cu", "fs_kernels_mgf.cu", "fs_kernels_ibm.cu", "fs_tma.cu", "fs_beam.cu", "fs_kernels_momv.cu", "fs_kernels_pcgc.cu"]
 HEADERS = [os.path.join(CSRC, "fs_internal.cuh"), os.path.join(HERE, "..", "include", "fs.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -343,7 +343,15 @@ template <class T> fs_status build_graph_impl(fs_grid* g, bool poisson, cudaGrap
   const int nst = num_stages(g, poisson);
   int nfix = 0, nbody = 0;
   if (!poisson) { Launch L0{s, 0, 0, nullptr, &g->seen}; nfix += launch_step_begin<T>(ctx<T>(g), L0); CK(cudaGetLastError()); }
-  for (int stage = 0; stage < nst; ++stage) {          // one conditional WHILE node (one PCG solve) per stage
+  const bool coop = pcg_coop_applies<T>(ctx<T>(g));    // L2-sized grids: the whole solve is one persistent cooperative kernel
+  for (int stage = 0; stage < nst && coop; ++stage) {
+    Launch L{s, 0, 0, nullptr, &g->seen};
+    nfix += enqueue_pre<T>(g, L, poisson);
+    nfix += launch_pcg_coop<T>(ctx<T>(g), L);
+    nfix += enqueue_post<T>(g, L, poisson, stage, nst);
+    CK(cudaGetLastError());
+  }
+  for (int stage = 0; stage < nst && !coop; ++stage) {  // one conditional WHILE node (one PCG solve) per stage
     cudaGraphConditionalHandle h;
     CK(cudaGraphConditionalHandleCreate(&h, graph, 0, cudaGraphCondAssignDefault));
     Launch L{s, h, 1, nullptr, &g->seen};
@@ -397,9 +405,11 @@ template <class T> fs_status run_stream(fs_grid* g, bool poisson, int* n_fixed, 
   const int nst = num_stages(g, poisson);
   int nfix = 0, nbody = 0;
   if (!poisson) nfix += launch_step_begin<T>(ctx<T>(g), L);
+  const bool coop = pcg_coop_applies<T>(ctx<T>(g));
   for (int stage = 0; stage < nst; ++stage) {
     nfix += enqueue_pre<T>(g, L, poisson);
-    for (;;) {
+    if (coop) nfix += launch_pcg_coop<T>(ctx<T>(g), L);
+    else for (;;) {
       int done = 0;
       CK(cudaMemcpyAsync(&done, &g->S->done, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
       CK(cudaStreamSynchronize(g->stream));

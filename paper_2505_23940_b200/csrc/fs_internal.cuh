@@ -7,6 +7,7 @@
 #include <cuda.h>            // CUtensorMap (the type and enums only: the driver entry point is looked up at run time)
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <cstdlib>
 #include "../../include/fs.h"
 
 namespace fs {
@@ -147,6 +148,7 @@ template <class T> constexpr const char* tname() { return sizeof(T) == 8 ? "f64"
 // waves x planes per chunk (a half-empty last wave costs as much as a full one), chunks of at least min_kz
 // planes, at most kMaxPartials CTAs (one reduction partial each).
 inline int pick_kz(long long tiles_xy, int nz, long long slots, int halo, int min_kz) {
+  { static const int ov = [] { const char* e = getenv("FS_TUNE_MINKZ"); return e ? atoi(e) : 0; }(); if (ov > 0) min_kz = ov; }
   int best = nz; double best_cost = 1e300;
   for (int zc = 1; zc <= nz; ++zc) {
     const int kz = (nz + zc - 1) / zc;
@@ -180,6 +182,9 @@ template <class T> void launch_scale(T* x, double a, long long n, cudaStream_t s
 template <class T> int launch_pcg_init(const Ctx<T>& c, const Launch& L, bool need_bhat);
 template <class T> int launch_pcg_body(const Ctx<T>& c, const MgCtx<T>& mg, const Launch& L);
 template <class T> int launch_pcg_finish(const Ctx<T>& c, const Launch& L);
+// the whole solve as one persistent cooperative kernel (fs_kernels_pcgc.cu): point preconditioners, L2-sized grids
+template <class T> bool pcg_coop_applies(const Ctx<T>& c);
+template <class T> int launch_pcg_coop(const Ctx<T>& c, const Launch& L);
 template <class T> int launch_true_residual(const Ctx<T>& c, const Launch& L);
 // dot_fused != nullptr asks for rho_cur = rhs . (zs out) from the last kernel; *dot_fused says whether it was done
 // upd_fused != nullptr additionally asks the level-0 down kernel to perform the residual update of the previous
