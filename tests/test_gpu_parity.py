@@ -194,6 +194,42 @@ def test_poisson_solve_matches_oracle(fs, kind, pc):
     g.close(); g2.close()
 
 
+@pytest.mark.parametrize("path", ["coop", "stream"])
+def test_point_pcg_paths_cooperative_and_streaming(fs, path, monkeypatch):
+    # point-preconditioned PCG runs as one persistent cooperative kernel on L2-sized grids (k_pcg_coop) and as the streaming
+    # kernel pair inside the graph's WHILE node on large ones (k_pcg_dirapply2 + k_pcg_updatev); every parity grid is small,
+    # so FS_TUNE_COOP=0 routes this test through the streaming kernels to keep both paths compared with the oracle
+    if path == "stream":
+        monkeypatch.setenv("FS_TUNE_COOP", "0")
+    want = ("k_pcg_coop<f64>",) if path == "coop" else ("k_pcg_dirapply2<f64>", "k_pcg_updatev<f64>")
+    rng = np.random.default_rng(6)
+    for cfg in (_cfg_periodic(44, 30, 37, precond="jacobi", rtol=1e-10, warm_start=0), _cfg_channel(36, 42, 20, precond="jacobi", rtol=1e-10, warm_start=0),
+                _cfg_open(50, 23, 18, precond="none", rtol=1e-10, warm_start=0), _cfg_open(50, 23, 18, precond="jacobi", rtol=1e-10, warm_start=0)):
+        rhs = rng.standard_normal(W.shapes(cfg)["p"])
+        p_ref, iref = _oracle(cfg).poisson_solve(rhs)
+        g = fs.Grid(cfg)
+        p, info = g.poisson_solve(rhs)
+        assert info["converged"] == 1 and abs(info["iters"] - iref["pcg_iters"]) <= 1, (info, iref)
+        assert relerr(p, p_ref) < TOL64 and info["true_rel_residual"] < 1e-8
+        used = g.kernels_used()
+        assert all(k in used for k in want), (path, used)
+        g.close()
+    # full steps: channel (walls, stretched y) and the FSI cylinder (markers, body, open boundaries), fp64 and fp32
+    g, o, ig, io, _ = _run_pair(fs, W.channel(n=32, steps=4), 4)
+    assert all(k in g.kernels_used() for k in want)
+    g.close()
+    cfg = W.cylinder_fsi(scale=8, per_ring=24)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 4)
+    assert all(k in g.kernels_used() for k in want)
+    g32 = fs.from_workload(dict(cfg, dtype="f32"))
+    i32 = g32.step(4)
+    assert i32["converged"] == 1 and i32["nan_flag"] == 0
+    for c_ in "uvp":
+        assert relerr(g32.get(c_), o.get(c_)) < 1e-4, c_
+    assert ("k_pcg_coop<f32>" if path == "coop" else "k_pcg_updatev<f32>") in g32.kernels_used()
+    g.close(); g32.close()
+
+
 @pytest.mark.parametrize("kind,pc", [("periodic", "jacobi"), ("periodic", "none"), ("channel", "jacobi"), ("open", "jacobi"),
                                      ("periodic", "gmg")])
 def test_poisson_solve_fp32_matches_fp64_oracle(fs, kind, pc):
