@@ -288,3 +288,24 @@ def test_moving_wall_couette_linear_profile_is_steady():
     o.set("w", -1.0 * s[None, :, None] * np.ones(o.shape["w"]))
     hu, hv, hw = o.momentum_rhs()
     assert np.abs(hu).max() < 1e-10 and np.abs(hw).max() < 1e-10 and np.abs(hv).max() < 1e-12
+
+
+def test_oracle_runs_clean_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """SURVEY 5 (sanitizer row; compute-sanitizer is closed on this pool, so the CPU side is what can be checked): the oracle
+    built with -fsanitize=address,undefined runs every branch family (tests/oracle_sanitize_main.cpp) without a report."""
+    import os
+    import shutil
+    import subprocess
+    if shutil.which("g++") is None:
+        pytest.skip("no g++")
+    here = os.path.dirname(os.path.abspath(__file__))
+    exe = str(tmp_path / "orc_san")
+    cmd = ["g++", "-O1", "-g", "-std=c++17", "-ffp-contract=off", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+           os.path.join(here, "oracle_sanitize_main.cpp"), os.path.join(here, "..", "oracle", "fs_oracle.cpp"), "-o", exe]
+    b = subprocess.run(cmd, capture_output=True, text=True)
+    if b.returncode != 0 and "sanitize" in b.stderr and "cannot find" in b.stderr:
+        pytest.skip("sanitizer runtime not installed")
+    assert b.returncode == 0, b.stderr[-2000:]
+    r = subprocess.run([exe], capture_output=True, text=True, env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1"))
+    assert r.returncode == 0 and "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr, (r.stdout[-500:], r.stderr[-3000:])
+    assert "oracle sanitizer run: ok" in r.stdout
