@@ -13,6 +13,9 @@
 // The recurrences, the operator and the order of floating-point operations per cell are those of k_pcg_dirapply /
 // k_pcg_update (and of the oracle); only the partition of the reductions differs.  x is updated in place (no deferred
 // update), so the zero-mean pass after the solve is the plain mean + shift.
+// Tried and dropped (profiles/r2_small_configs.md): merging P1 into P2 by recomputing d on the six neighbours of every cell from r
+// and the old d (10 words, two barriers: the barrier floor drops from 11.4 to 9.9 us per iteration) -- the fourteen loads per
+// vector instead of seven thrash L2 on the 25-34 MB fields of c3 / c4 and the step gets 17-25 % slower.
 #include "fs_internal.cuh"
 #include <cstdlib>
 
