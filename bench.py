@@ -332,6 +332,38 @@ def measure(a, dtype, dev, local, rank, world, dist, with_e2e, with_profile):
                "h2d_bytes_per_step": 3 * cells * wbytes, "d2h_bytes_per_step": 4 * cells * wbytes,
                "steps": ke, "ms_per_step": 1e3 * dt / ke,
                "api": "fs_fields_set(u,v,w: pinned host) -> fs_step(1) -> fs_fields_get(u,v,w,p: pinned host)"}
+        # the same traffic for TWO independent grids (replicas), each on its own stream, through the asynchronous
+        # field calls: one grid's H2D / D2H runs while the other one steps (PCIe is full duplex), per step and grid the same bytes
+        try:
+            s2 = torch.cuda.Stream(device=dev)
+            with torch.cuda.stream(s2):
+                g2 = fs.Grid(dict(cfg, dtype=dtype), device=dev, stream=s2)       # same workload; its fields arrive through the pipeline
+            host2 = {c: torch.empty(g.shape[c], dtype=tdt).pin_memory() for c in "uvwp"}
+            for c in "uvwp":
+                host2[c].copy_(host[c])
+            pairs = ((g, host), (g2, host2))
+
+            def pipe_round():
+                for gg, hh in pairs:
+                    for c in "uvw":
+                        gg.set_async(c, hh[c])
+                    gg.step(1, sync=False)
+                    for c in "uvwp":
+                        gg.get_async(c, hh[c])
+
+            pipe_round(); torch.cuda.synchronize(dev)
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(ke):
+                pipe_round()
+            torch.cuda.synchronize(dev)
+            dtp = max_over_ranks(time.perf_counter() - t0, dist, dev)
+            e2e["pipelined_two_replicas"] = {"value": world * 2 * cells * ke / dtp / 1e6, "unit": UNIT, "ms_per_round": 1e3 * dtp / ke,
+                                             "note": "two independent grids on two streams, fs_fields_set_async / fs_step / fs_fields_get_async: "
+                                                     "the copies of one grid overlap the step and the opposite-direction copies of the other"}
+            g2.close(); del g2, host2
+        except RuntimeError as ex:      # e.g. not enough memory for a second grid: the serial number stands alone
+            e2e["pipelined_two_replicas"] = {"value": None, "note": "skipped: %s" % str(ex)[:120]}
         del host, npv
 
     # ---- per-kernel event timing (same kernels, stream launches) -> roofline of the dominant kernel

@@ -150,6 +150,14 @@ fs_status fs_field_size(fs_grid* g, fs_field f, long long* count);
 fs_status fs_fields_set(fs_grid* g, fs_field f, const void* src, fs_dtype dtype, int src_on_device);
 fs_status fs_fields_get(fs_grid* g, fs_field f, void* dst, fs_dtype dtype, int dst_on_device);
 
+/* Asynchronous variants for pipelines -- e.g. several independent grids, each on its own stream, so that one grid's PCIe
+ * traffic overlaps another grid's step (replicas): as fs_fields_set / fs_fields_get for FS_U .. FS_HW with a HOST
+ * buffer of the GRID's dtype, but the copy is only enqueued on the grid's stream.  The buffer must be page-locked for the copy
+ * to be asynchronous and must stay valid and untouched until the caller has synchronised that stream.  FS_ERR_INVALID_ARG
+ * for other fields. */
+fs_status fs_fields_set_async(fs_grid* g, fs_field f, const void* host_src);
+fs_status fs_fields_get_async(fs_grid* g, fs_field f, void* host_dst);
+
 /* Restart support: whether H^{n-1} is valid (AB2) and the step counter (inflow-noise hash). */
 fs_status fs_set_history(fs_grid* g, int have_history, long long step);
 

@@ -69,7 +69,7 @@ class fs_poisson_info(C.Structure):
 
 # every symbol include/fs.h declares (tests check the library exports all of them)
 SYMBOLS = ("fs_workspace_bytes", "fs_grid_create", "fs_grid_destroy", "fs_field_size", "fs_fields_set",
-           "fs_fields_get", "fs_set_history", "fs_set_ibm_markers", "fs_marker_segments", "fs_set_body", "fs_set_solid_mask", "fs_set_beam", "fs_beam_state",
+           "fs_fields_get", "fs_fields_set_async", "fs_fields_get_async", "fs_set_history", "fs_set_ibm_markers", "fs_marker_segments", "fs_set_body", "fs_set_solid_mask", "fs_set_beam", "fs_beam_state",
            "fs_set_body_state", "fs_step", "fs_poisson_solve", "fs_ibm_interpolate", "fs_ibm_spread",
            "fs_gmg_vcycle", "fs_momentum_rhs", "fs_profile_step", "fs_profile_count", "fs_profile_entry",
            "fs_profile_reset", "fs_launch_count", "fs_kernels_used", "fs_status_string")
@@ -98,6 +98,8 @@ def lib():
         L.fs_field_size.argtypes = [vp, ip, C.POINTER(C.c_longlong)]
         L.fs_fields_set.argtypes = [vp, ip, vp, ip, ip]
         L.fs_fields_get.argtypes = [vp, ip, vp, ip, ip]
+        L.fs_fields_set_async.argtypes = [vp, ip, vp]
+        L.fs_fields_get_async.argtypes = [vp, ip, vp]
         L.fs_set_history.argtypes = [vp, ip, C.c_longlong]
         L.fs_set_ibm_markers.argtypes = [vp, ip, dp, dp, dp]
         L.fs_marker_segments.argtypes = [vp, C.POINTER(C.c_int)]
@@ -269,6 +271,16 @@ class Grid:
             return a.reshape(3, -1, 3)
         return a
 
+    def set_async(self, name, host):
+        """fs_fields_set_async: enqueue host (pinned torch tensor or numpy array of the grid's dtype) -> field on the grid's stream."""
+        ptr = host.data_ptr() if isinstance(host, self._torch.Tensor) else host.ctypes.data
+        _check(lib().fs_fields_set_async(self.h, FIELD[name], C.c_void_p(ptr)), "fs_fields_set_async")
+
+    def get_async(self, name, host):
+        """fs_fields_get_async: enqueue field -> host buffer on the grid's stream (valid after the stream is synchronised)."""
+        ptr = host.data_ptr() if isinstance(host, self._torch.Tensor) else host.ctypes.data
+        _check(lib().fs_fields_get_async(self.h, FIELD[name], C.c_void_p(ptr)), "fs_fields_get_async")
+
     def set_history(self, have, step):
         _check(lib().fs_set_history(self.h, int(have), int(step)), "fs_set_history")
 
@@ -420,11 +432,11 @@ class Grid:
         return n.value
 
 
-def from_workload(cfg, device="cuda:0", **overrides):
+def from_workload(cfg, device="cuda:0", stream=None, **overrides):
     """Grid initialised from an fs_workloads config: fields, markers and body set through the C ABI."""
     c = dict(cfg)
     c.update(overrides)
-    g = Grid(c, device=device)
+    g = Grid(c, device=device, stream=stream)
     for name, arr in c.get("init", {}).items():
         g.set(name, arr)
     if c.get("markers") is not None:

@@ -705,6 +705,20 @@ fs_status fs_fields_set(fs_grid* g, fs_field f, const void* src, fs_dtype dtype,
   return FS_OK;
 }
 
+static fs_status fields_async(fs_grid* g, fs_field f, void* host, bool set) {
+  if (!g || !host || f > FS_HW) return FS_ERR_INVALID_ARG;
+  GUARD(g);
+  size_t n = 0;
+  void* dev = g->f64 ? (void*)field_ptr<double>(g, f, &n) : (void*)field_ptr<float>(g, f, &n);
+  if (!dev) return FS_ERR_INVALID_ARG;
+  const size_t bytes = n * (g->f64 ? sizeof(double) : sizeof(float));
+  if (set) CK(cudaMemcpyAsync(dev, host, bytes, cudaMemcpyHostToDevice, g->stream));
+  else CK(cudaMemcpyAsync(host, dev, bytes, cudaMemcpyDeviceToHost, g->stream));
+  return FS_OK;
+}
+fs_status fs_fields_set_async(fs_grid* g, fs_field f, const void* host_src) { return fields_async(g, f, const_cast<void*>(host_src), true); }
+fs_status fs_fields_get_async(fs_grid* g, fs_field f, void* host_dst) { return fields_async(g, f, host_dst, false); }
+
 fs_status fs_fields_get(fs_grid* g, fs_field f, void* dst, fs_dtype dtype, int dst_on_device) {
   if (!g || !dst) return FS_ERR_INVALID_ARG;
   GUARD(g);

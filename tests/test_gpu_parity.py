@@ -864,6 +864,33 @@ def test_device_pointer_io_and_dtype_conversion(fs):
     g.close()
 
 
+def test_async_field_io_on_two_streams_equals_the_synchronous_calls(fs):
+    # fs_fields_set_async / fs_fields_get_async (pipelines over independent grids): two grids on two streams fed from
+    # pinned host buffers give bit for bit what one grid fed through the synchronous calls gives
+    import torch
+    cfg = W.taylor_green(n=24)
+    ref = fs.from_workload(cfg)
+    ref.step(3)
+    s2 = torch.cuda.Stream()
+    grids = [fs.Grid(cfg), fs.Grid(cfg, stream=s2)]
+    host = [{c: torch.from_numpy(np.ascontiguousarray(cfg["init"][c])).pin_memory() for c in "uvw"} for _ in grids]
+    out = [{c: torch.empty(ref.shape[c], dtype=torch.float64).pin_memory() for c in "uvwp"} for _ in grids]
+    for g_, h_, o_ in zip(grids, host, out):
+        for c in "uvw":
+            g_.set_async(c, h_[c])
+        g_.step(3, sync=False)
+        for c in "uvwp":
+            g_.get_async(c, o_[c])
+    torch.cuda.synchronize()
+    for o_ in out:
+        for c in "uvwp":
+            assert np.array_equal(o_[c].numpy(), ref.get(c)), c
+    with pytest.raises(fs.FsError):
+        grids[0].set_async("marker_x", host[0]["u"])
+    for g_ in grids + [ref]:
+        g_.close()
+
+
 def test_marker_support_touching_a_wall_is_unsupported(fs):
     # same rule, same threshold as the oracle (pin P22): 1.5 h (Roma) from a non-periodic boundary
     cfg = _cfg_open(40, 30, 28, max_markers=4)
