@@ -74,8 +74,18 @@ template <class T> __global__ void __launch_bounds__(256) k_mg_prolong(const int
 constexpr int kTailCells = 4096;
 struct MgTail { int nlev; int nx[kMaxLevels], ny[kMaxLevels], nz[kMaxLevels]; double h[kMaxLevels]; };
 
+// cell index -> (i, j, k): shifts and masks when nx and ny are powers of two (the usual case: 16^3, 8^3, 4^3), two
+// divisions otherwise; the tail runs on ONE SM and is issue bound, and the divisions were most of its instructions
+__device__ __forceinline__ void tail_ijk(int q, int nx, int ny, int& i, int& j, int& k) {
+  if (((nx & (nx - 1)) | (ny & (ny - 1))) == 0) {
+    const int lx = 31 - __clz(nx), ly = 31 - __clz(ny);
+    i = q & (nx - 1); j = (q >> lx) & (ny - 1); k = q >> (lx + ly);
+  } else { i = q % nx; const int t = q / nx; j = t % ny; k = t / ny; }
+}
+
 template <class T> __device__ __forceinline__ T tail_neg_lap(const T* e, int q, int nx, int ny, int nz, T ih2) {
-  const int i = q % nx, t = q / nx, j = t % ny, k = t / ny;
+  int i, j, k;
+  tail_ijk(q, nx, ny, i, j, k);
   const int ip = i + 1 == nx ? 0 : i + 1, im = i == 0 ? nx - 1 : i - 1;
   const int jp = j + 1 == ny ? 0 : j + 1, jm = j == 0 ? ny - 1 : j - 1;
   const int kp = k + 1 == nz ? 0 : k + 1, km = k == 0 ? nz - 1 : k - 1;
@@ -128,7 +138,8 @@ template <class T> __global__ void __launch_bounds__(1024) k_mg_tail(const int* 
     const int nx = a.nx[l], ny = a.ny[l], nz = a.nz[l], cx = nx / 2, cy = ny / 2;
     const T ih2 = T(1.0 / (a.h[l] * a.h[l]));
     for (int q = tid; q < N[l + 1]; q += nth) {
-      const int i = q % cx, t = q / cx, j = t % cy, k = t / cy;
+      int i, j, k;
+      tail_ijk(q, cx, cy, i, j, k);
       T s = T(0);
       for (int dk = 0; dk < 2; ++dk) for (int dj = 0; dj < 2; ++dj) for (int di = 0; di < 2; ++di) {
         const int fq = (2 * i + di) + nx * ((2 * j + dj) + ny * (2 * k + dk));
@@ -146,7 +157,8 @@ template <class T> __global__ void __launch_bounds__(1024) k_mg_tail(const int* 
     const T* ec = cur[l + 1];
     const bool add = cur[l] != nullptr;
     for (int q = tid; q < N[l]; q += nth) {
-      const int i = q % nx, t = q / nx, j = t % ny, k = t / ny;
+      int i, j, k;
+      tail_ijk(q, nx, ny, i, j, k);
       const T cv = ec[(i >> 1) + cx * ((j >> 1) + cy * (k >> 1))];
       x[q] = add ? x[q] + cv : cv;
     }

@@ -33,23 +33,28 @@ def relerr(a, b):
 
 
 # kernel instantiations each full-size case must have exercised (fs_kernels_used): c2 periodic x, stretched y: the
-# vector kernels; c3 / c4 bounded x: the generic one-cell projection / right-hand side, Jacobi PCG in pairs of cells
+# vector kernels; c3 / c4 bounded x: the generic one-cell projection / right-hand side.  The Jacobi-PCG solve runs as the
+# persistent cooperative kernel by default on these L2-sized grids ("coop") and as the streaming pair inside the graph's
+# WHILE node with FS_TUNE_COOP=0 ("stream", the path of larger grids): both against the same oracle step.
 EXPECT = {
-    "c2": ["k_momentum<f64,central>", "k_div_rhsv<f64>", "k_pcg_initv<f64>", "k_pcg_dirapply2<f64>", "k_pcg_updatev<f64>", "k_projectv<f64>"],
-    "c3": ["k_momentum<f64,central>", "k_div_rhs<f64>", "k_pcg_initv<f64>", "k_pcg_dirapply2<f64>", "k_pcg_updatev<f64>", "k_project<f64>",
-           "ibm_interpolate", "ibm_spread", "flux_sum"],
-    "c4": ["k_momentum<f64,central>", "k_div_rhs<f64>", "k_pcg_dirapply2<f64>", "k_project<f64>", "ibm_index", "ibm_spread", "step_end"],
+    "c2": ["k_momentum<f64,central>", "k_div_rhsv<f64>", "k_pcg_initv<f64>", "k_projectv<f64>"],
+    "c3": ["k_momentum<f64,central>", "k_div_rhs<f64>", "k_pcg_initv<f64>", "k_project<f64>", "ibm_interpolate", "ibm_spread", "flux_sum"],
+    "c4": ["k_momentum<f64,central>", "k_div_rhs<f64>", "k_project<f64>", "ibm_index", "ibm_spread", "step_end"],
 }
+PCG = {"coop": ["k_pcg_coop<f64>"], "stream": ["k_pcg_dirapply2<f64>", "k_pcg_updatev<f64>"]}
 
 
+@pytest.mark.parametrize("path", ["coop", "stream"])
 @pytest.mark.parametrize("case", ["c2", "c3", "c4"])
-def test_one_step_at_full_size_matches_oracle(fs, fullsize_oracle, case):
+def test_one_step_at_full_size_matches_oracle(fs, fullsize_oracle, case, path, monkeypatch):
+    if path == "stream":
+        monkeypatch.setenv("FS_TUNE_COOP", "0")
     cfg = W.make(case)
     g = fs.from_workload(cfg)
     ig = g.step(1, per_step=True)
     assert ig["nan_flag"] == 0 and ig["converged"] == 1, ig
     used = g.kernels_used()
-    for k in EXPECT[case]:
+    for k in EXPECT[case] + PCG[path]:
         assert k in used, (k, used)
     d = fullsize_oracle(case)
     io = json.load(open(os.path.join(d, case + "_info.json")))
