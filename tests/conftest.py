@@ -36,7 +36,8 @@ def pytest_collection_finish(session):
     base = "/dev/shm" if os.path.isdir("/dev/shm") and os.access("/dev/shm", os.W_OK) else None
     d = tempfile.mkdtemp(prefix="fs_fullsize_", dir=base)
     _workers["dir"] = d
-    cases = [c for c in FULLSIZE_CASES if any(("[%s]" % c) in it.nodeid or ("_%s_" % c) in it.nodeid for it in want)]
+    import re
+    cases = [c for c in FULLSIZE_CASES if any(re.search(r"[\[-]%s[\]-]" % c, it.nodeid) or ("_%s_" % c) in it.nodeid for it in want)]
     for c in cases:
         log = open(os.path.join(d, c + ".log"), "w")
         _workers["procs"][c] = subprocess.Popen([sys.executable, os.path.join(ROOT, "tests", "fullsize_oracle_worker.py"), c, d],
