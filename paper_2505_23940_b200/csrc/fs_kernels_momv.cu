@@ -10,6 +10,7 @@
 // index arithmetic and predicates, and reads / writes global memory in 16-byte pieces: 18 shared-memory loads per
 // 2 (4) cells instead of 36 per cell, 32 VX x 16 extended tile -> 30 VX x 14 results (82 % instead of 75 %).
 // The arithmetic per face is that of k_momentum, operation for operation (same parity route against the oracle).
+// fp64 feeds the ring with cp.async (ASY): no register holds a load in flight, ghosts are fixed in place after arrival.
 // Boundary types: x periodic; y and z periodic, no-slip or slip (inflow / outflow faces, the LES closures and odd
 // sizes go through k_momentum).
 #include "fs_internal.cuh"
@@ -18,7 +19,6 @@
 
 namespace fs {
 
-constexpr int kMvTY = 16;                 // rows of the extended tile (14 result rows)
 
 template <class T> __device__ __forceinline__ T mv_tr(bool upwind, T a, T minus, T plus, T central) {
   return upwind ? (a > T(0) ? minus : plus) : central;
@@ -60,8 +60,32 @@ template <class T, int C> __device__ __forceinline__ Vec16<T> mv_fix(const Ctx<T
   return o;
 }
 
-template <class T, bool UPW, bool ADT> __global__ void __launch_bounds__(32 * kMvTY, 1)
+// ghost transform of plane kk for a column (the A, B of mv_fix), applied in place to a vector that a cp.async has put in shared memory
+template <class T, int C> __device__ __forceinline__ void mv_fix_smem(const Ctx<T>& c, const MvCol<T>& r, int kk, T* slot) {
+  T A = r.A, B = r.B;
+  if (c.bz && C != 2) {
+    const int face = kk < 0 ? 4 : (kk >= c.nz ? 5 : -1);
+    if (face >= 0 && c.bc[face] == FS_BC_NOSLIP) { B = T(2.0 * c.bcv[face][C]) - B; A = -A; }
+  }
+  if (A != T(1) || B != T(0)) {
+    Vec16<T> v = ld16<T>(slot);
+#pragma unroll
+    for (int a = 0; a < Vec16<T>::VX; ++a) v.a[a] = A * v.a[a] + B;
+    st16<T>(slot, v);
+  }
+}
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// TY: rows of the extended tile.  ASY: planes of u, v, w go from global memory straight into the shared-memory ring with
+// cp.async (no register holds a load in flight; the thread's own values of planes k-1 and k+1 are read back from the ring)
+template <class T, bool UPW, bool ADT, int TY, bool ASY> __global__ void __launch_bounds__(32 * TY, 1)
 k_momentumv(const Ctx<T> c, int kz, const __grid_constant__ TmapSet tm) {
+  constexpr int kMvTY = TY;
   constexpr int VX = Vec16<T>::VX, ROWE = 32 * VX, PLN = kMvTY * ROWE;
   using W = Vec16<T>;
   extern __shared__ __align__(16) unsigned char mv_smem[];
@@ -91,13 +115,34 @@ k_momentumv(const Ctx<T> c, int kz, const __grid_constant__ TmapSet tm) {
   const int o_s = tym * ROWE + lane * VX, o_n = typ * ROWE + lane * VX;
   const int dw = lane > 0 ? -1 : 0, de = lane < 31 ? VX : VX - 1;          // west / east scalar relative to a vector start
   // register queue of the own column: B = k-1, c = k, T = k+1; n = raw loads of plane k+1 (k+2 after the store) in flight
-  W uB = mv_fix<T, 0>(c, ru, k0 - 1, mv_raw<T, 0>(c, U, ru, k0 - 1)), vB = mv_fix<T, 1>(c, rv, k0 - 1, mv_raw<T, 1>(c, V, rv, k0 - 1)),
+  W uB, vB, wB, uc, vc, wc, un, vn, wn, uTq, vTq, wTq;
+  auto issue = [&](int kk) {                // ASY: plane kk of u, v, w -> ring slot kk & 3 (this thread's vector)
+    const int sl = (kk & 3) * PLN + o_own;
+    cp_async16(SU + sl, U + (ru.off + ru.pl * (unsigned)mv_plane<T, 0>(c, kk)));
+    cp_async16(SV + sl, V + (rv.off + rv.pl * (unsigned)mv_plane<T, 1>(c, kk)));
+    cp_async16(SW + sl, Wf + (rw.off + rw.pl * (unsigned)mv_plane<T, 2>(c, kk)));
+    cp_async_commit();
+  };
+  auto fixup = [&](int kk) {
+    const int sl = (kk & 3) * PLN + o_own;
+    mv_fix_smem<T, 0>(c, ru, kk, SU + sl); mv_fix_smem<T, 1>(c, rv, kk, SV + sl); mv_fix_smem<T, 2>(c, rw, kk, SW + sl);
+  };
+  if (ASY) {
+    issue(k0 - 1); issue(k0); issue(k0 + 1);
+    cp_async_wait_all();
+    fixup(k0 - 1); fixup(k0); fixup(k0 + 1);
+    __syncthreads();
+    uc = ld16<T>(SU + (k0 & 3) * PLN + o_own); vc = ld16<T>(SV + (k0 & 3) * PLN + o_own); wc = ld16<T>(SW + (k0 & 3) * PLN + o_own);
+    uTq = ld16<T>(SU + ((k0 + 1) & 3) * PLN + o_own); vTq = ld16<T>(SV + ((k0 + 1) & 3) * PLN + o_own); wTq = ld16<T>(SW + ((k0 + 1) & 3) * PLN + o_own);
+  } else {
+    uB = mv_fix<T, 0>(c, ru, k0 - 1, mv_raw<T, 0>(c, U, ru, k0 - 1)); vB = mv_fix<T, 1>(c, rv, k0 - 1, mv_raw<T, 1>(c, V, rv, k0 - 1));
     wB = mv_fix<T, 2>(c, rw, k0 - 1, mv_raw<T, 2>(c, Wf, rw, k0 - 1));
-  W uc = mv_fix<T, 0>(c, ru, k0, mv_raw<T, 0>(c, U, ru, k0)), vc = mv_fix<T, 1>(c, rv, k0, mv_raw<T, 1>(c, V, rv, k0)),
+    uc = mv_fix<T, 0>(c, ru, k0, mv_raw<T, 0>(c, U, ru, k0)); vc = mv_fix<T, 1>(c, rv, k0, mv_raw<T, 1>(c, V, rv, k0));
     wc = mv_fix<T, 2>(c, rw, k0, mv_raw<T, 2>(c, Wf, rw, k0));
-  W un = mv_raw<T, 0>(c, U, ru, k0 + 1), vn = mv_raw<T, 1>(c, V, rv, k0 + 1), wn = mv_raw<T, 2>(c, Wf, rw, k0 + 1);
-  st16<T>(SU + ((k0 - 1) & 3) * PLN + o_own, uB); st16<T>(SV + ((k0 - 1) & 3) * PLN + o_own, vB); st16<T>(SW + ((k0 - 1) & 3) * PLN + o_own, wB);
-  st16<T>(SU + (k0 & 3) * PLN + o_own, uc); st16<T>(SV + (k0 & 3) * PLN + o_own, vc); st16<T>(SW + (k0 & 3) * PLN + o_own, wc);
+    un = mv_raw<T, 0>(c, U, ru, k0 + 1); vn = mv_raw<T, 1>(c, V, rv, k0 + 1); wn = mv_raw<T, 2>(c, Wf, rw, k0 + 1);
+    st16<T>(SU + ((k0 - 1) & 3) * PLN + o_own, uB); st16<T>(SV + ((k0 - 1) & 3) * PLN + o_own, vB); st16<T>(SW + ((k0 - 1) & 3) * PLN + o_own, wB);
+    st16<T>(SU + (k0 & 3) * PLN + o_own, uc); st16<T>(SV + (k0 & 3) * PLN + o_own, vc); st16<T>(SW + (k0 & 3) * PLN + o_own, wc);
+  }
   // H^{n-1} of the own faces, one plane ahead (zero where the face does not exist)
   const bool hasu = own && j < c.ny, hasv = own, hasw = own && j < c.ny;
   const unsigned qu0 = (unsigned)sx + (unsigned)c.nx * (unsigned)j, plu = (unsigned)c.nx * (unsigned)c.ny;
@@ -105,9 +150,12 @@ k_momentumv(const Ctx<T> c, int kz, const __grid_constant__ TmapSet tm) {
   W zero;
 #pragma unroll
   for (int a = 0; a < VX; ++a) zero.a[a] = T(0);
-  W hun = (hasu && k0 < c.nz) ? ld16<T>(c.hu + (qu0 + plu * k0)) : zero;
-  W hvn = (hasv && k0 < c.nz) ? ld16<T>(c.hv + (qv0 + plv * k0)) : zero;
-  W hwn = hasw ? ld16<T>(c.hw + (qu0 + plu * k0)) : zero;
+  W hun = zero, hvn = zero, hwn = zero;
+  if (!ASY) {
+    hun = (hasu && k0 < c.nz) ? ld16<T>(c.hu + (qu0 + plu * k0)) : zero;
+    hvn = (hasv && k0 < c.nz) ? ld16<T>(c.hv + (qv0 + plv * k0)) : zero;
+    hwn = hasw ? ld16<T>(c.hw + (qu0 + plu * k0)) : zero;
+  }
   // boundary-normal faces of bounded y / z: no-slip keeps the wall velocity, slip has no normal flow
   const bool vwall = c.by && (j == 0 || j == c.ny);
   const T vwv = vwall ? (c.bc[j == 0 ? 2 : 3] == FS_BC_NOSLIP ? T(c.bcv[j == 0 ? 2 : 3][1]) : T(0)) : T(0);
@@ -118,23 +166,35 @@ k_momentumv(const Ctx<T> c, int kz, const __grid_constant__ TmapSet tm) {
     if (!pf_on || k > k1) return;
     tma_prefetch_plane(tm.m[0], pf_x, pf_y, mv_plane<T, 0>(c, k)); tma_prefetch_plane(tm.m[1], pf_x, pf_y, mv_plane<T, 1>(c, k));
     tma_prefetch_plane(tm.m[2], pf_x, pf_y, mv_plane<T, 2>(c, k));
-    if (k < k1 && k < c.nz) { tma_prefetch_plane(tm.m[3], pf_x, pf_y, k); tma_prefetch_plane(tm.m[4], pf_x, pf_y, k); }
-    if (k < k1) tma_prefetch_plane(tm.m[5], pf_x, pf_y, k);
+    // H^{n-1} is only read on the tile's own faces: its boxes are the 30 VX x (TY - 2) interior
+    if (k < k1 && k < c.nz) { tma_prefetch_plane(tm.m[3], pf_x + VX, pf_y + 1, k); tma_prefetch_plane(tm.m[4], pf_x + VX, pf_y + 1, k); }
+    if (k < k1) tma_prefetch_plane(tm.m[5], pf_x + VX, pf_y + 1, k);
   };
   for (int k = k0 + 2; k < k0 + 2 + kPfAhead; ++k) prefetch(k);
   for (int k = k0; k < k1; ++k) {
-    const W uT = mv_fix<T, 0>(c, ru, k + 1, un), vT = mv_fix<T, 1>(c, rv, k + 1, vn), wT = mv_fix<T, 2>(c, rw, k + 1, wn);
-    const W huo = hun, hvo = hvn, hwo = hwn;
-    if (k + 1 < k1) {
-      hun = (hasu && k + 1 < c.nz) ? ld16<T>(c.hu + (qu0 + plu * (k + 1))) : zero;
-      hvn = (hasv && k + 1 < c.nz) ? ld16<T>(c.hv + (qv0 + plv * (k + 1))) : zero;
-      hwn = hasw ? ld16<T>(c.hw + (qu0 + plu * (k + 1))) : zero;
-    }
     const int s0 = ((k - 1) & 3) * PLN, s1 = (k & 3) * PLN, s2 = ((k + 1) & 3) * PLN;
-    st16<T>(SU + s2 + o_own, uT); st16<T>(SV + s2 + o_own, vT); st16<T>(SW + s2 + o_own, wT);
-    prefetch(k + 2 + kPfAhead);
-    if (k + 1 < k1) { un = mv_raw<T, 0>(c, U, ru, k + 2); vn = mv_raw<T, 1>(c, V, rv, k + 2); wn = mv_raw<T, 2>(c, Wf, rw, k + 2); }
-    __syncthreads();
+    W uT, vT, wT, huo, hvo, hwo;
+    if (ASY) {
+      // planes k-1, k, k+1 are in the ring and visible (barrier at the end of the previous plane); plane k+2 starts its way now
+      if (k + 1 < k1) issue(k + 2);
+      prefetch(k + 2 + kPfAhead);
+      uT = uTq; vT = vTq; wT = wTq;
+      huo = (hasu && k < c.nz) ? ld16<T>(c.hu + (qu0 + plu * k)) : zero;
+      hvo = (hasv && k < c.nz) ? ld16<T>(c.hv + (qv0 + plv * k)) : zero;
+      hwo = hasw ? ld16<T>(c.hw + (qu0 + plu * k)) : zero;
+    } else {
+      uT = mv_fix<T, 0>(c, ru, k + 1, un); vT = mv_fix<T, 1>(c, rv, k + 1, vn); wT = mv_fix<T, 2>(c, rw, k + 1, wn);
+      huo = hun; hvo = hvn; hwo = hwn;
+      if (k + 1 < k1) {
+        hun = (hasu && k + 1 < c.nz) ? ld16<T>(c.hu + (qu0 + plu * (k + 1))) : zero;
+        hvn = (hasv && k + 1 < c.nz) ? ld16<T>(c.hv + (qv0 + plv * (k + 1))) : zero;
+        hwn = hasw ? ld16<T>(c.hw + (qu0 + plu * (k + 1))) : zero;
+      }
+      st16<T>(SU + s2 + o_own, uT); st16<T>(SV + s2 + o_own, vT); st16<T>(SW + s2 + o_own, wT);
+      prefetch(k + 2 + kPfAhead);
+      if (k + 1 < k1) { un = mv_raw<T, 0>(c, U, ru, k + 2); vn = mv_raw<T, 1>(c, V, rv, k + 2); wn = mv_raw<T, 2>(c, Wf, rw, k + 2); }
+      __syncthreads();
+    }
     if (own) {
       const T wyl0 = MY[0][ty], wyh0 = MY[1][ty], wyl1 = MY[2][ty], wyh1 = MY[3][ty];
       const T idyj = MY[4][ty], idyjm = MY[5][ty], idyc0 = MY[6][ty], idyc1 = MY[7][ty];
@@ -142,6 +202,7 @@ k_momentumv(const Ctx<T> c, int kz, const __grid_constant__ TmapSet tm) {
       // needs inside its own block (the compiler barriers keep the three blocks' shared-memory loads from being hoisted
       // to the top together: that would hold 8 vectors + 10 scalars live on top of the register queue)
       const bool kin = k < c.nz;
+      if (ASY) { uB = ld16<T>(SU + s0 + o_own); vB = ld16<T>(SV + s0 + o_own); wB = ld16<T>(SW + s0 + o_own); }
       // ---- u faces ----
       if (j < c.ny && kin) {
         const W uN = ld16<T>(SU + s1 + o_n), uS = ld16<T>(SU + s1 + o_s), vN = ld16<T>(SV + s1 + o_n);
@@ -237,50 +298,61 @@ k_momentumv(const Ctx<T> c, int kz, const __grid_constant__ TmapSet tm) {
         st16<T>(c.ws + q, ws); st16<T>(c.hw + q, H);
       }
     }
-    uB = uc; uc = uT; vB = vc; vc = vT; wB = wc; wc = wT;
+    if (ASY) {
+      cp_async_wait_all();
+      if (k + 1 < k1) fixup(k + 2);
+      __syncthreads();
+      uc = uT; vc = vT; wc = wT;
+      const int s3 = ((k + 2) & 3) * PLN + o_own;
+      uTq = ld16<T>(SU + s3); vTq = ld16<T>(SV + s3); wTq = ld16<T>(SW + s3);
+    } else { uB = uc; uc = uT; vB = vc; vc = vT; wB = wc; wc = wT; }
   }
 }
 
-template <class T> static size_t momv_smem() { return 12 * (size_t)kMvTY * 32 * Vec16<T>::VX * sizeof(T); }
+// Load path per precision (profiles/r2_momentum.md, 512^3): fp64 with register loads sat at its 128-register cap with 16 warps
+// per SM (4.25 ms against k_momentum's 3.45); with cp.async the loads in flight and the k-1 / k+1 copies of the own column live
+// in the ring, the kernel needs 121 registers without spills and runs at 3.27 ms.  fp32 (four cells per thread, enough
+// independent work) is faster with register loads: 1.55 ms against 1.76 with cp.async.  Tile heights 14 / 18 / 20 rows were
+// slower in fp64 (3.40 / 4.47 / 3.85 ms: fewer warps, or spills at the lower register caps).
+template <class T> struct MvCfg { static constexpr int TY = 16; static constexpr bool ASY = sizeof(T) == 8; };
+template <class T> static size_t momv_smem() { return 12 * (size_t)MvCfg<T>::TY * 32 * Vec16<T>::VX * sizeof(T); }
 
 template <class T> bool momentumv_applies(const Ctx<T>& c) {
   if (c.bx || c.nx % Vec16<T>::VX != 0) return false;
   if (c.nu > 0.0 && (c.cs > 0.0 || c.wall_model)) return false;
   for (int f = 2; f < 6; ++f) if (c.bc[f] != FS_BC_PERIODIC && c.bc[f] != FS_BC_NOSLIP && c.bc[f] != FS_BC_SLIP) return false;
-  // measured at 512^3 (profiles/r2_momentum.md): fp32 2.63 -> 1.55 ms; in fp64 the two-cell vector leaves half the independent
-  // work per thread at 16 warps per SM (128 registers) and runs at 4.25 ms against k_momentum's 3.45: fp32 only by default.
-  // FS_TUNE_MOMV (read at every launch: tests switch it): 0 = never, 2 = fp64 too (element-wise parity of this kernel at 1e-12)
+  // FS_TUNE_MOMV=0 (read at every launch: a parity test switches it) routes these grids through k_momentum as well
   const char* e = getenv("FS_TUNE_MOMV");
-  const int mode = e ? atoi(e) : 1;
-  return mode == 2 || (mode == 1 && sizeof(T) == 4);
+  return !(e && atoi(e) == 0);
 }
 
 template <class T> cudaError_t momv_configure_device() {
   const int bytes = (int)momv_smem<T>();
+  constexpr int TY = MvCfg<T>::TY; constexpr bool A = MvCfg<T>::ASY;
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(k_momentumv<T, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(k_momentumv<T, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(k_momentumv<T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_momentumv<T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if ((e = cudaFuncSetAttribute(k_momentumv<T, false, false, TY, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(k_momentumv<T, false, true, TY, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(k_momentumv<T, true, false, TY, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_momentumv<T, true, true, TY, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
 
 template <class T> int launch_momentumv(const Ctx<T>& c, const Launch& L) {
-  constexpr int VX = Vec16<T>::VX;
-  const int bxn = (c.nx + 30 * VX - 1) / (30 * VX), byn = (c.nyv + kMvTY - 3) / (kMvTY - 2);
+  constexpr int VX = Vec16<T>::VX, TY = MvCfg<T>::TY; constexpr bool A = MvCfg<T>::ASY;
+  const int bxn = (c.nx + 30 * VX - 1) / (30 * VX), byn = (c.nyv + TY - 3) / (TY - 2);
   const int kz = pick_kz((long long)bxn * byn, c.nzw, 148, 2, 16);
-  const dim3 b(32, kMvTY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
+  const dim3 b(32, TY, 1), g(bxn, byn, (c.nzw + kz - 1) / kz);
   const bool adt = c.cfl > 0.0, upw = c.convection == FS_CONV_UPWIND;
   TmapSet tm; memset(&tm, 0, sizeof tm);
   static const int pf = [] { const char* e = getenv("FS_TUNE_PF2"); return e ? atoi(e) : 1; }();
-  const int bw = 32 * VX, bh = kMvTY;
+  const int bw = 32 * VX, bh = TY;
   if (pf && tmap_encode(&tm.m[0], c.u, sizeof(T), c.nx, c.ny, c.nz, bw, bh) && tmap_encode(&tm.m[1], c.v, sizeof(T), c.nx, c.nyv, c.nz, bw, bh) &&
-      tmap_encode(&tm.m[2], c.w, sizeof(T), c.nx, c.ny, c.nzw, bw, bh) && tmap_encode(&tm.m[3], c.hu, sizeof(T), c.nx, c.ny, c.nz, bw, bh) &&
-      tmap_encode(&tm.m[4], c.hv, sizeof(T), c.nx, c.nyv, c.nz, bw, bh) && tmap_encode(&tm.m[5], c.hw, sizeof(T), c.nx, c.ny, c.nzw, bw, bh)) tm.n = 6;
+      tmap_encode(&tm.m[2], c.w, sizeof(T), c.nx, c.ny, c.nzw, bw, bh) && tmap_encode(&tm.m[3], c.hu, sizeof(T), c.nx, c.ny, c.nz, bw - 2 * VX, bh - 2) &&
+      tmap_encode(&tm.m[4], c.hv, sizeof(T), c.nx, c.nyv, c.nz, bw - 2 * VX, bh - 2) && tmap_encode(&tm.m[5], c.hw, sizeof(T), c.nx, c.ny, c.nzw, bw - 2 * VX, bh - 2)) tm.n = 6;
   static const char* names[2][2] = {{"k_momentumv<f32,central>", "k_momentumv<f32,upwind>"}, {"k_momentumv<f64,central>", "k_momentumv<f64,upwind>"}};
   const size_t smem = momv_smem<T>();
   FS_LAUNCHI(L, "momentum_predictor", names[sizeof(T) == 8][upw], 12.0 * sizeof(T) * c.nx * c.ny * c.nz, {
-    if (upw) { if (adt) k_momentumv<T, true, true><<<g, b, smem, L.s>>>(c, kz, tm); else k_momentumv<T, true, false><<<g, b, smem, L.s>>>(c, kz, tm); }
-    else { if (adt) k_momentumv<T, false, true><<<g, b, smem, L.s>>>(c, kz, tm); else k_momentumv<T, false, false><<<g, b, smem, L.s>>>(c, kz, tm); }
+    if (upw) { if (adt) k_momentumv<T, true, true, TY, A><<<g, b, smem, L.s>>>(c, kz, tm); else k_momentumv<T, true, false, TY, A><<<g, b, smem, L.s>>>(c, kz, tm); }
+    else { if (adt) k_momentumv<T, false, true, TY, A><<<g, b, smem, L.s>>>(c, kz, tm); else k_momentumv<T, false, false, TY, A><<<g, b, smem, L.s>>>(c, kz, tm); }
   });
   return 1;
 }

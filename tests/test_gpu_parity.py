@@ -104,8 +104,9 @@ def test_momentum_rhs_elementwise(fs, kind):
 @pytest.mark.parametrize("kind", ["periodic", "channel", "zwalls", "channel_upwind", "periodic_adaptive"])
 def test_momentum_vector_kernel_elementwise(fs, kind, monkeypatch):
     # k_momentumv (one 16-byte vector of faces per thread; periodic x, walls in y / z): H^n element-wise against the oracle
-    # in fp64 at 1e-12 (FS_TUNE_MOMV=2 routes fp64 grids through it; the default uses it for fp32 only, where it is the
-    # faster kernel) and in fp32 on the scale of fp32 rounding; the predicted field through one full step.  Several tiles
+    # in fp64 at 1e-12 (cp.async ring variant) and in fp32 (register-load variant) on the scale of fp32 rounding; the
+    # predicted field through two full steps; and with FS_TUNE_MOMV=0 the same grid through k_momentum (one face per thread),
+    # which otherwise only serves bounded x, odd nx and the LES closures.  Several tiles
     # (120 x 14 cells in fp32, 60 x 14 in fp64) with ragged tails, several z chunks.
     def zwalls(**kw):
         c = _cfg_periodic(136, 34, 40, **kw)
@@ -120,7 +121,14 @@ def test_momentum_vector_kernel_elementwise(fs, kind, monkeypatch):
     cfg["init"] = _rand_fields(cfg, 21)
     o = _oracle(cfg)
     ref = o.momentum_rhs()
-    monkeypatch.setenv("FS_TUNE_MOMV", "2")
+    monkeypatch.setenv("FS_TUNE_MOMV", "0")
+    g0 = fs.from_workload(cfg)
+    got0 = g0.momentum_rhs()
+    assert "k_momentum<f64,%s>" % upw in g0.kernels_used(), g0.kernels_used()
+    for c, a, b in zip("uvw", got0, ref):
+        assert relerr(a, b) < 1e-12, (kind, c, relerr(a, b))
+    g0.close()
+    monkeypatch.delenv("FS_TUNE_MOMV")
     g = fs.from_workload(cfg)
     got = g.momentum_rhs()
     assert "k_momentumv<f64,%s>" % upw in g.kernels_used(), g.kernels_used()
@@ -130,7 +138,6 @@ def test_momentum_vector_kernel_elementwise(fs, kind, monkeypatch):
     _compare_state(g, o, TOL64)
     assert abs(ig["dt"] - io["dt"]) <= 1e-15 * io["dt"]
     g.close()
-    monkeypatch.delenv("FS_TUNE_MOMV")
     g32 = fs.from_workload(dict(cfg, dtype="f32"))
     got32 = g32.momentum_rhs()
     assert "k_momentumv<f32,%s>" % upw in g32.kernels_used(), g32.kernels_used()

@@ -33,11 +33,11 @@ def relerr(a, b):
 
 
 # kernel instantiations each full-size case must have exercised (fs_kernels_used): c2 periodic x, stretched y: the
-# vector kernels; c3 / c4 bounded x: the generic one-cell projection / right-hand side.  The Jacobi-PCG solve runs as the
+# vector kernels (momentum included); c3 / c4 bounded x: the generic one-cell projection / right-hand side.  The Jacobi-PCG solve runs as the
 # persistent cooperative kernel by default on these L2-sized grids ("coop") and as the streaming pair inside the graph's
 # WHILE node with FS_TUNE_COOP=0 ("stream", the path of larger grids): both against the same oracle step.
 EXPECT = {
-    "c2": ["k_momentum<f64,central>", "k_div_rhsv<f64>", "k_pcg_initv<f64>", "k_projectv<f64>"],
+    "c2": ["k_momentumv<f64,central>", "k_div_rhsv<f64>", "k_pcg_initv<f64>", "k_projectv<f64>"],
     "c3": ["k_momentum<f64,central>", "k_div_rhs<f64>", "k_pcg_initv<f64>", "k_project<f64>", "ibm_interpolate", "ibm_spread", "flux_sum"],
     "c4": ["k_momentum<f64,central>", "k_div_rhs<f64>", "k_project<f64>", "ibm_index", "ibm_spread", "step_end"],
 }
@@ -87,7 +87,7 @@ def test_one_step_of_c5_at_512_matches_oracle_on_every_cell(fs, fullsize_oracle)
     io = json.load(open(os.path.join(d, "c5_info.json")))
     assert abs(ig["pcg_iters"] - io["pcg_iters"]) <= 1, (ig["pcg_iters"], io["pcg_iters"])
     used = g.kernels_used()
-    for k in ("k_momentum<f64,central>", "k_div_rhsv<f64>", "k_pcg_initv<f64>", "k_mg_down<f64,TR16,UPD>", "k_mg_up<f64,TR16,DOT>",
+    for k in ("k_momentumv<f64,central>", "k_div_rhsv<f64>", "k_pcg_initv<f64>", "k_mg_down<f64,TR16,UPD>", "k_mg_up<f64,TR16,DOT>",
               "k_mg_down<f64,TR8>", "k_pcg_dirapply2<f64>", "k_projectv<f64>"):
         assert k in used, (k, used)
     errs = {}
