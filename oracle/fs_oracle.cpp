@@ -521,25 +521,41 @@ static void jacobi_diag(const orc_sim* s, double* dg) {
   }
 }
 
-// ---- O7g: geometric multigrid V-cycle on (-L) e = g, all-periodic uniform isotropic grids --------
-// level arrays are n^3-shaped with spacing h; operator rediscretised on every level.
-static void mg_neg_lap(int nx, int ny, int nz, double h, const vec& e, vec& out) {
+// ---- O7g: geometric multigrid V-cycle on (-L) e = g, uniform isotropic grids -----------------------------------
+// level arrays are nx x ny x nz-shaped with spacing h; operator rediscretised on every level.  bd[d] != 0: direction d is
+// bounded -- the flux through a boundary face is dropped (homogeneous Neumann, as in the fine operator O6), so a cell has
+// nnb <= 6 neighbours and the diagonal is nnb / h^2 (reading G1 in DESIGN.md 3: SURVEY O7g names triply periodic boxes
+// only; restriction, prolongation and the damped-Jacobi smoother with the TRUE diagonal carry over unchanged, and the
+// cycle stays a symmetric operator).  All periodic: nnb = 6 everywhere, the original formulas bit for bit.
+static inline double mg_nnb(int nx, int ny, int nz, const int bd[3], int i, int j, int k) {
+  double n = 6.0;
+  if (bd[0]) n -= (i == 0) + (i == nx - 1);
+  if (bd[1]) n -= (j == 0) + (j == ny - 1);
+  if (bd[2]) n -= (k == 0) + (k == nz - 1);
+  return n;
+}
+static void mg_neg_lap(int nx, int ny, int nz, double h, const int bd[3], const vec& e, vec& out) {
   double ih2 = 1.0 / (h * h);
   for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
     size_t c = (size_t)i + (size_t)nx * (j + (size_t)ny * k);
-    double nb = e[(size_t)wrapi(i + 1, nx) + (size_t)nx * (j + (size_t)ny * k)] + e[(size_t)wrapi(i - 1, nx) + (size_t)nx * (j + (size_t)ny * k)]
-              + e[(size_t)i + (size_t)nx * (wrapi(j + 1, ny) + (size_t)ny * k)] + e[(size_t)i + (size_t)nx * (wrapi(j - 1, ny) + (size_t)ny * k)]
-              + e[(size_t)i + (size_t)nx * (j + (size_t)ny * wrapi(k + 1, nz))] + e[(size_t)i + (size_t)nx * (j + (size_t)ny * wrapi(k - 1, nz))];
-    out[c] = (6.0 * e[c] - nb) * ih2;
+    auto at = [&](int ii, int jj, int kk) -> double {          // neighbour value; 0 beyond a bounded end (counted out by nnb)
+      if (bd[0] ? (ii < 0 || ii >= nx) : false) return 0.0;
+      if (bd[1] ? (jj < 0 || jj >= ny) : false) return 0.0;
+      if (bd[2] ? (kk < 0 || kk >= nz) : false) return 0.0;
+      return e[(size_t)wrapi(ii, nx) + (size_t)nx * (wrapi(jj, ny) + (size_t)ny * wrapi(kk, nz))];
+    };
+    double nb = at(i + 1, j, k) + at(i - 1, j, k) + at(i, j + 1, k) + at(i, j - 1, k) + at(i, j, k + 1) + at(i, j, k - 1);
+    out[c] = (mg_nnb(nx, ny, nz, bd, i, j, k) * e[c] - nb) * ih2;
   }
 }
-// one damped-Jacobi sweep  e <- e + omega D^-1 (g - (-L) e),  D = 6/h^2
-static void mg_sweep(int nx, int ny, int nz, double h, double omega, const vec& g, vec& e, vec& tmp, bool zero_guess) {
-  double c = omega * h * h / 6.0;
-  size_t N = (size_t)nx * ny * nz;
-  if (zero_guess) { for (size_t q = 0; q < N; ++q) e[q] = c * g[q]; return; }
-  mg_neg_lap(nx, ny, nz, h, e, tmp);
-  for (size_t q = 0; q < N; ++q) e[q] = e[q] + c * (g[q] - tmp[q]);
+// one damped-Jacobi sweep  e <- e + omega D^-1 (g - (-L) e),  D = nnb/h^2
+static void mg_sweep(int nx, int ny, int nz, double h, double omega, const int bd[3], const vec& g, vec& e, vec& tmp, bool zero_guess) {
+  if (!zero_guess) mg_neg_lap(nx, ny, nz, h, bd, e, tmp);
+  for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+    size_t q = (size_t)i + (size_t)nx * (j + (size_t)ny * k);
+    double c = omega * h * h / mg_nnb(nx, ny, nz, bd, i, j, k);
+    e[q] = zero_guess ? c * g[q] : e[q] + c * (g[q] - tmp[q]);
+  }
 }
 static int mg_levels(int nx, int ny, int nz) {
   int L = 1;
@@ -548,14 +564,15 @@ static int mg_levels(int nx, int ny, int nz) {
 }
 static void mg_vcycle(const orc_sim* s, int lev, int nx, int ny, int nz, double h, const vec& g, vec& e) {
   size_t N = (size_t)nx * ny * nz; vec tmp(N);
+  const int bd[3] = {s->bx, s->by, s->bz};
   e.assign(N, 0.0);
   if (lev == s->nlev - 1) {                                    // coarsest: fixed sweeps from zero
-    for (int it = 0; it < s->P.mg_coarse_sweeps; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, g, e, tmp, it == 0);
+    for (int it = 0; it < s->P.mg_coarse_sweeps; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, bd, g, e, tmp, it == 0);
     return;
   }
-  for (int it = 0; it < s->P.mg_nu1; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, g, e, tmp, it == 0);
+  for (int it = 0; it < s->P.mg_nu1; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, bd, g, e, tmp, it == 0);
   vec res(N);
-  if (s->P.mg_nu1 > 0) { mg_neg_lap(nx, ny, nz, h, e, tmp); for (size_t q = 0; q < N; ++q) res[q] = g[q] - tmp[q]; }
+  if (s->P.mg_nu1 > 0) { mg_neg_lap(nx, ny, nz, h, bd, e, tmp); for (size_t q = 0; q < N; ++q) res[q] = g[q] - tmp[q]; }
   else res = g;
   int cx = nx / 2, cy = ny / 2, cz = nz / 2; size_t Nc = (size_t)cx * cy * cz;
   vec gc(Nc), ec;
@@ -568,7 +585,7 @@ static void mg_vcycle(const orc_sim* s, int lev, int nx, int ny, int nz, double 
   mg_vcycle(s, lev + 1, cx, cy, cz, 2.0 * h, gc, ec);
   for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i)      // piecewise-constant prolongation
     e[(size_t)i + (size_t)nx * (j + (size_t)ny * k)] += ec[(size_t)(i / 2) + (size_t)cx * ((j / 2) + (size_t)cy * (k / 2))];
-  for (int it = 0; it < s->P.mg_nu2; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, g, e, tmp, false);
+  for (int it = 0; it < s->P.mg_nu2; ++it) mg_sweep(nx, ny, nz, h, s->P.mg_omega, bd, g, e, tmp, false);
 }
 // z = M^-1 r : A = -h L = h(-L)  =>  z = Vcycle(r / h)
 static void precond_gmg(const orc_sim* s, const vec& r, vec& z) {
@@ -1052,8 +1069,7 @@ extern "C" orc_sim* orc_create(const orc_params* p) {
   }
   s->P.yf = nullptr;
   if (p->precond == ORC_PC_GMG) {
-    bool ok = !s->bx && !s->by && !s->bz && s->uniform_y &&
-              std::fabs(s->hx - s->hy) <= 1e-12 * s->hx && std::fabs(s->hx - s->hz) <= 1e-12 * s->hx;
+    bool ok = s->uniform_y && std::fabs(s->hx - s->hy) <= 1e-12 * s->hx && std::fabs(s->hx - s->hz) <= 1e-12 * s->hx;
     if (!ok) { delete s; return nullptr; }
     s->nlev = mg_levels(s->nx, s->ny, s->nz);
   } else s->nlev = 0;
