@@ -134,8 +134,9 @@ fs_status fs_workspace_bytes(const fs_params* params, size_t* bytes);
  * (L429, L454-456).  params: HOST.  workspace: DEVICE memory of the CURRENT device, >= fs_workspace_bytes,
  * 256-byte aligned, owned by the caller, zeroed by this call.  cuda_stream: a cudaStream_t of the current
  * device (NULL = legacy default stream).  FS_ERR_INVALID_ARG: bad parameters, misaligned / too small / non-device
- * workspace or one that belongs to another device.  FS_ERR_UNSUPPORTED: GMG on a grid that is not uniform /
- * isotropic / all-periodic; more than 2^31 - 1 stored values per field. */
+ * workspace or one that belongs to another device.  FS_ERR_UNSUPPORTED: GMG on a grid that is not uniform and
+ * isotropic (periodic and bounded directions may be mixed: on a bounded one the boundary flux is dropped on every level);
+ * more than 2^31 - 1 stored values per field. */
 fs_status fs_grid_create(const fs_params* params, void* workspace, size_t bytes, void* cuda_stream,
                          fs_grid** out);
 fs_status fs_grid_destroy(fs_grid* g);

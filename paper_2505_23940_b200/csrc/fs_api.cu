@@ -128,8 +128,7 @@ fs_status validate(const fs_params* p) {
   if ((int)p->precond < 0 || (int)p->precond > 2 || (int)p->delta < 0 || (int)p->delta > 1) return FS_ERR_INVALID_ARG;
   if (p->precond == FS_PC_GMG) {
     const double hx = p->lx / p->nx, hy = p->ly / p->ny, hz = p->lz / p->nz;
-    const bool periodic = p->bc[0] == FS_BC_PERIODIC && p->bc[2] == FS_BC_PERIODIC && p->bc[4] == FS_BC_PERIODIC;
-    if (!periodic || p->yf || std::fabs(hx - hy) > 1e-12 * hx || std::fabs(hx - hz) > 1e-12 * hx) return FS_ERR_UNSUPPORTED;
+    if (p->yf || std::fabs(hx - hy) > 1e-12 * hx || std::fabs(hx - hz) > 1e-12 * hx) return FS_ERR_UNSUPPORTED;   // uniform, isotropic
     if (p->mg_nu1 < 0 || p->mg_nu2 < 0 || p->mg_coarse_sweeps < 0) return FS_ERR_INVALID_ARG;
     if (mg_levels(p->nx, p->ny, p->nz) > kMaxLevels) return FS_ERR_UNSUPPORTED;
   }
@@ -175,6 +174,7 @@ template <class T> size_t carve(fs_grid* g, char* base) {
     if (P.mg_nu1 == 2 && P.mg_nu2 == 2) c.r2 = b.take<T>(g->nP);   // second residual buffer of the fused update (k_mg_down<UPD>)
     mg.nlev = mg_levels(P.nx, P.ny, P.nz);
     mg.nu1 = P.mg_nu1; mg.nu2 = P.mg_nu2; mg.coarse_sweeps = P.mg_coarse_sweeps; mg.omega = P.mg_omega;
+    mg.bd = (g->bx ? 1 : 0) | (g->by ? 2 : 0) | (g->bz ? 4 : 0);
     int nx = P.nx, nyy = P.ny, nz = P.nz; double h = g->hx;
     for (int l = 0; l < mg.nlev; ++l) {
       MgLevel& V = mg.lev[l];

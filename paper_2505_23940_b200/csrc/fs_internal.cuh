@@ -91,6 +91,7 @@ constexpr int kPfAhead = 4;          // planes between the L2 prefetch of a tile
 struct MgLevel { int nx, ny, nz; double h; void *e, *g, *t; };
 template <class T> struct MgCtx {
   int nlev, nu1, nu2, coarse_sweeps; double omega;
+  int bd;                      // bit d set: direction d is bounded (boundary fluxes dropped on every level, reading G1); 0: triply periodic
   MgLevel lev[kMaxLevels];
 };
 

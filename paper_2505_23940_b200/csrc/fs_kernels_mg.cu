@@ -1,5 +1,5 @@
 // fs_kernels_mg.cu -- geometric-multigrid V-cycle preconditioner (S7g; not in the
-// paper, named by BASELINE.json c5).  Uniform, isotropic, all-periodic grids.  Per level: nu1 damped-
+// paper, named by BASELINE.json c5).  Uniform, isotropic grids; periodic or bounded (reading G1: boundary fluxes dropped).  Per level: nu1 damped-
 // Jacobi sweeps from a zero guess, residual, 8-cell-average restriction, recursion, piecewise-constant
 // prolongation + correction, nu2 sweeps; the coarsest level does a fixed number of sweeps.  The operator
 // on every level is the rediscretised 7-point -L.  Jacobi is order independent, so the result matches
@@ -11,35 +11,69 @@ namespace fs {
 constexpr int kFlatBlocks = 148 * 8;
 static inline int flat_blocks(long long n) { long long b = (n + 255) / 256; return (int)(b < kFlatBlocks ? (b < 1 ? 1 : b) : kFlatBlocks); }
 
-template <class T> __device__ __forceinline__ T neg_lap(const T* __restrict__ e, int i, int j, int k, int nx, int ny, int nz, T ih2) {
+// (-L) e at a cell.  bd: bit d set = direction d is bounded, the flux through a boundary face is dropped (reading G1): the cell
+// then has nnb < 6 neighbours, returned through *nnb for the Jacobi diagonal nnb / h^2.  bd == 0: the periodic formulas.
+template <class T> __device__ __forceinline__ T neg_lap(const T* __restrict__ e, int i, int j, int k, int nx, int ny, int nz, T ih2, int bd = 0, T* nnb = nullptr) {
+  const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
+  if (bd == 0) {
+    const int ip = i + 1 == nx ? 0 : i + 1, im = i == 0 ? nx - 1 : i - 1;
+    const int jp = j + 1 == ny ? 0 : j + 1, jm = j == 0 ? ny - 1 : j - 1;
+    const int kp = k + 1 == nz ? 0 : k + 1, km = k == 0 ? nz - 1 : k - 1;
+    const T nb = e[row + ip] + e[row + im] + e[(size_t)i + (size_t)nx * ((size_t)jp + (size_t)ny * k)] +
+                 e[(size_t)i + (size_t)nx * ((size_t)jm + (size_t)ny * k)] + e[(size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * kp)] +
+                 e[(size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * km)];
+    if (nnb) *nnb = T(6);
+    return (T(6) * e[row + i] - nb) * ih2;
+  }
+  // neighbours in the oracle's order (+x, -x, +y, -y, +z, -z); a missing one adds 0 and is counted out of nnb
+  const bool bx = bd & 1, by = bd & 2, bz = bd & 4;
+  const bool hxp = !(bx && i + 1 == nx), hxm = !(bx && i == 0), hyp = !(by && j + 1 == ny), hym = !(by && j == 0), hzp = !(bz && k + 1 == nz), hzm = !(bz && k == 0);
   const int ip = i + 1 == nx ? 0 : i + 1, im = i == 0 ? nx - 1 : i - 1;
   const int jp = j + 1 == ny ? 0 : j + 1, jm = j == 0 ? ny - 1 : j - 1;
   const int kp = k + 1 == nz ? 0 : k + 1, km = k == 0 ? nz - 1 : k - 1;
-  const size_t row = (size_t)nx * ((size_t)j + (size_t)ny * k);
-  const T nb = e[row + ip] + e[row + im] + e[(size_t)i + (size_t)nx * ((size_t)jp + (size_t)ny * k)] +
-               e[(size_t)i + (size_t)nx * ((size_t)jm + (size_t)ny * k)] + e[(size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * kp)] +
-               e[(size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * km)];
-  return (T(6) * e[row + i] - nb) * ih2;
+  const T xp = hxp ? e[row + ip] : T(0), xm = hxm ? e[row + im] : T(0);
+  const T yp = hyp ? e[(size_t)i + (size_t)nx * ((size_t)jp + (size_t)ny * k)] : T(0), ym = hym ? e[(size_t)i + (size_t)nx * ((size_t)jm + (size_t)ny * k)] : T(0);
+  const T zp = hzp ? e[(size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * kp)] : T(0), zm = hzm ? e[(size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * km)] : T(0);
+  const T nb = xp + xm + yp + ym + zp + zm;
+  const T n = T((int)hxp + (int)hxm + (int)hyp + (int)hym + (int)hzp + (int)hzm);
+  if (nnb) *nnb = n;
+  return (n * e[row + i] - nb) * ih2;
+}
+// number of neighbours of a cell (the Jacobi diagonal is nnb / h^2)
+__device__ __forceinline__ int mg_nnb(int i, int j, int k, int nx, int ny, int nz, int bd) {
+  int n = 6;
+  if (bd & 1) n -= (i == 0) + (i + 1 == nx);
+  if (bd & 2) n -= (j == 0) + (j + 1 == ny);
+  if (bd & 4) n -= (k == 0) + (k + 1 == nz);
+  return n;
 }
 
-// first sweep from a zero guess: e = omega D^-1 g
-template <class T> __global__ void __launch_bounds__(256) k_mg_first(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__ e, T cw, long long N) {
+// first sweep from a zero guess: e = omega D^-1 g   (cw = omega h^2 / 6; bounded grids: wh2 / nnb per cell, wh2 = omega h^2)
+template <class T> __global__ void __launch_bounds__(256) k_mg_first(const int* __restrict__ done, const T* __restrict__ g, T* __restrict__ e, T cw, long long N,
+                                                                    int nx, int ny, int nz, int bd, double wh2) {
   if (done && *done) return;
-  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) e[q] = cw * g[q];
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
+    T c = cw;
+    if (bd) { const int i = (int)(q % nx); const long long t = q / nx; c = T(wh2 / (double)mg_nnb(i, (int)(t % ny), (int)(t / ny), nx, ny, nz, bd)); }
+    e[q] = c * g[q];
+  }
 }
 // damped-Jacobi sweep  dst = src + omega D^-1 (g - (-L) src)
 template <class T> __global__ void __launch_bounds__(256) k_mg_sweep(const int* __restrict__ done, const T* __restrict__ g, const T* __restrict__ src,
-                                                                    T* __restrict__ dst, int nx, int ny, int nz, T ih2, T cw) {
+                                                                    T* __restrict__ dst, int nx, int ny, int nz, T ih2, T cw, int bd, double wh2) {
   if (done && *done) return;
   const long long N = (long long)nx * ny * nz;
   for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < N; q += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(q % nx); const long long t = q / nx; const int j = (int)(t % ny), k = (int)(t / ny);
-    dst[q] = src[q] + cw * (g[q] - neg_lap<T>(src, i, j, k, nx, ny, nz, ih2));
+    T nnb;
+    const T lap = neg_lap<T>(src, i, j, k, nx, ny, nz, ih2, bd, &nnb);
+    const T c = bd ? T(wh2 / (double)nnb) : cw;
+    dst[q] = src[q] + c * (g[q] - lap);
   }
 }
 // residual + restriction: gc = mean over the 8 children of (g - (-L) e); e == nullptr means e = 0
 template <class T> __global__ void __launch_bounds__(256) k_mg_restrict(const int* __restrict__ done, const T* __restrict__ g, const T* __restrict__ e,
-                                                                       T* __restrict__ gc, int nx, int ny, int nz, T ih2) {
+                                                                       T* __restrict__ gc, int nx, int ny, int nz, T ih2, int bd) {
   if (done && *done) return;
   const int cx = nx / 2, cy = ny / 2, cz = nz / 2;
   const long long Nc = (long long)cx * cy * cz;
@@ -49,7 +83,7 @@ template <class T> __global__ void __launch_bounds__(256) k_mg_restrict(const in
     for (int dk = 0; dk < 2; ++dk) for (int dj = 0; dj < 2; ++dj) for (int di = 0; di < 2; ++di) {
       const int fi = 2 * i + di, fj = 2 * j + dj, fk = 2 * k + dk;
       const size_t fq = (size_t)fi + (size_t)nx * ((size_t)fj + (size_t)ny * fk);
-      a += e ? g[fq] - neg_lap<T>(e, fi, fj, fk, nx, ny, nz, ih2) : g[fq];
+      a += e ? g[fq] - neg_lap<T>(e, fi, fj, fk, nx, ny, nz, ih2, bd) : g[fq];
     }
     gc[q] = T(0.125) * a;
   }
@@ -196,7 +230,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
   if (dot_fused) *dot_fused = false;
   if (upd_fused) *upd_fused = false;
   // Fast path, V(2,2) with at least two levels: two fused kernels per level (fs_kernels_mgf.cu).
-  if (mg.nu1 == 2 && mg.nu2 == 2 && mg.nlev >= 2) {
+  if (mg.nu1 == 2 && mg.nu2 == 2 && mg.nlev >= 2 && mg.bd == 0) {     // triply periodic: the fused legs (bounded grids: the per-sweep kernels below)
     const int last = mg.nlev - 1;
     // tail levels (small enough to live in one CTA's shared memory together): from level lt down
     int lt = last;
@@ -231,9 +265,9 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
       else {
         T* a = ((pre - 1) % 2 == 0) ? el[last] : tl[last];
         T* b = ((pre - 1) % 2 == 0) ? tl[last] : el[last];
-        FS_LAUNCH(L, "mg_coarse", 2.0 * sizeof(T) * N, k_mg_first<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[last], a, cw, N)); ++n;
+        FS_LAUNCH(L, "mg_coarse", 2.0 * sizeof(T) * N, k_mg_first<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[last], a, cw, N, V.nx, V.ny, V.nz, 0, 0.0)); ++n;
         for (int it = 1; it < pre; ++it) {
-          FS_LAUNCH(L, "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[last], a, b, V.nx, V.ny, V.nz, ih2, cw)); ++n;
+          FS_LAUNCH(L, "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[last], a, b, V.nx, V.ny, V.nz, ih2, cw, 0, 0.0)); ++n;
           T* t = a; a = b; b = t;
         }
       }
@@ -252,15 +286,16 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     const MgLevel& V = mg.lev[l];
     const long long N = (long long)V.nx * V.ny * V.nz;
     const T ih2 = T(1.0 / (V.h * V.h)), cw = T(mg.omega * V.h * V.h / 6.0);
+    const double wh2 = mg.omega * V.h * V.h;
     const bool coarsest = l == mg.nlev - 1;
     const int pre = coarsest ? mg.coarse_sweeps : mg.nu1;
     const int swaps = coarsest ? (pre > 0 ? pre - 1 : 0) : ((pre > 0 ? pre - 1 : 0) + mg.nu2);
     T* a = (swaps % 2 == 0) ? el[l] : tl[l];          // so that the level's final iterate lands in el[l]
     T* b = (swaps % 2 == 0) ? tl[l] : el[l];
     if (pre > 0) {
-      FS_LAUNCH(L, l == 0 ? "mg_first_l0" : "mg_coarse", 2.0 * sizeof(T) * N, k_mg_first<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, cw, N)); ++n;
+      FS_LAUNCH(L, l == 0 ? "mg_first_l0" : "mg_coarse", 2.0 * sizeof(T) * N, k_mg_first<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, cw, N, V.nx, V.ny, V.nz, mg.bd, wh2)); ++n;
       for (int it = 1; it < pre; ++it) {
-        FS_LAUNCH(L, l == 0 ? "mg_sweep_l0" : "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, b, V.nx, V.ny, V.nz, ih2, cw)); ++n;
+        FS_LAUNCH(L, l == 0 ? "mg_sweep_l0" : "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, b, V.nx, V.ny, V.nz, ih2, cw, mg.bd, wh2)); ++n;
         T* t = a; a = b; b = t;
       }
       cur[l] = a;
@@ -270,7 +305,7 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     }
     if (!coarsest) {
       const long long Nc = N / 8;
-      FS_LAUNCH(L, l == 0 ? "mg_restrict_l0" : "mg_coarse", (cur[l] ? 2.125 : 1.125) * sizeof(T) * N, k_mg_restrict<T><<<flat_blocks(Nc), 256, 0, L.s>>>(done, gl[l], cur[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, ih2)); ++n;
+      FS_LAUNCH(L, l == 0 ? "mg_restrict_l0" : "mg_coarse", (cur[l] ? 2.125 : 1.125) * sizeof(T) * N, k_mg_restrict<T><<<flat_blocks(Nc), 256, 0, L.s>>>(done, gl[l], cur[l], (T*)mg.lev[l + 1].g, V.nx, V.ny, V.nz, ih2, mg.bd)); ++n;
     }
   }
   // upward leg
@@ -278,13 +313,14 @@ template <class T> int launch_vcycle(const Ctx<T>& c, const MgCtx<T>& mg, const 
     const MgLevel& V = mg.lev[l];
     const long long N = (long long)V.nx * V.ny * V.nz;
     const T ih2 = T(1.0 / (V.h * V.h)), cw = T(mg.omega * V.h * V.h / 6.0);
+    const double wh2 = mg.omega * V.h * V.h;
     T* a = cur[l];
     T* dst = a ? a : ((mg.nu2 % 2 == 0) ? el[l] : tl[l]);
     FS_LAUNCH(L, l == 0 ? "mg_prolong_l0" : "mg_coarse", (a ? 2.125 : 1.125) * sizeof(T) * N, k_mg_prolong<T><<<flat_blocks(N), 256, 0, L.s>>>(done, el[l + 1], a, dst, V.nx, V.ny, V.nz)); ++n;
     a = dst;
     T* b = a == el[l] ? tl[l] : el[l];
     for (int it = 0; it < mg.nu2; ++it) {
-      FS_LAUNCH(L, l == 0 ? "mg_sweep_l0" : "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, b, V.nx, V.ny, V.nz, ih2, cw)); ++n;
+      FS_LAUNCH(L, l == 0 ? "mg_sweep_l0" : "mg_coarse", 3.0 * sizeof(T) * N, k_mg_sweep<T><<<flat_blocks(N), 256, 0, L.s>>>(done, gl[l], a, b, V.nx, V.ny, V.nz, ih2, cw, mg.bd, wh2)); ++n;
       T* t = a; a = b; b = t;
     }
     // a == el[l] by construction of the swap parity

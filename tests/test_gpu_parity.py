@@ -295,6 +295,54 @@ def test_gmg_vcycle_elementwise(fs, dims):
     g.close()
 
 
+@pytest.mark.parametrize("bounded", [(1, 1, 1), (0, 1, 0), (1, 0, 1)])
+def test_gmg_on_bounded_grids_matches_oracle(fs, bounded):
+    # reading G1: multigrid on uniform boxes with Neumann pressure faces (boundary fluxes dropped on every level, true-diagonal
+    # Jacobi); per-sweep kernels with the boundary flags.  V-cycle element-wise, V(1,2) too, Poisson solve, fp32 solve
+    h = 1.0 / 16
+    kinds = (("inflow", "outflow"), ("slip", "noslip"), ("noslip", "slip"))
+
+    def mk(**kw):
+        kw.setdefault("rtol", 1e-10)
+        cfg = W._base(nx=48, ny=32, nz=40, lx=48 * h, ly=32 * h, lz=40 * h, nu=0.01, dt=1e-3, precond="gmg", warm_start=0, **kw)
+        cfg["bc"] = [kinds[d][s_] if bounded[d] else "periodic" for d in range(3) for s_ in range(2)]
+        return cfg
+    rng = np.random.default_rng(8)
+    for kw in (dict(), dict(mg_nu1=1, mg_nu2=2, mg_coarse_sweeps=5)):
+        cfg = mk(**kw)
+        r = rng.standard_normal(W.shapes(cfg)["p"])
+        z_ref = _oracle(cfg).vcycle(r)
+        g = fs.Grid(cfg)
+        z = g.gmg_vcycle(r)
+        assert relerr(z, z_ref) < 1e-12, (bounded, kw, relerr(z, z_ref))
+        assert "k_mg_down<f64,TR8>" not in g.kernels_used()            # the fused periodic legs must not run on a bounded grid
+        g.close()
+    cfg = mk()
+    rhs = rng.standard_normal(W.shapes(cfg)["p"])
+    p_ref, iref = _oracle(cfg).poisson_solve(rhs)
+    g = fs.Grid(cfg)
+    p, info = g.poisson_solve(rhs)
+    assert info["converged"] == 1 and abs(info["iters"] - iref["pcg_iters"]) <= 1 and iref["pcg_iters"] < 25, (info, iref)
+    assert relerr(p, p_ref) < TOL64 and info["true_rel_residual"] < 1e-8
+    g.close()
+    g32 = fs.Grid(dict(mk(rtol=1e-6), dtype="f32"))
+    p32, i32 = g32.poisson_solve(rhs)
+    assert i32["converged"] == 1 and relerr(p32, p_ref) < TOL32
+    g32.close()
+
+
+def test_sphere_with_gmg_pcg_full_steps_match_oracle(fs):
+    # the c3 recipe (open box, 400 markers) with the multigrid preconditioner instead of Jacobi: same fields, a tenth of the iterations
+    cfg = W.sphere(scale=4, n_markers=400, precond="gmg", rtol=1e-10)
+    g, o, ig, io, _ = _run_pair(fs, cfg, 5)
+    assert max(io["iters_per_step"]) < 40
+    cj = W.sphere(scale=4, n_markers=400, rtol=1e-10)
+    oj = _oracle(cj); ij = oj.step(5)
+    assert min(ij["iters_per_step"]) > 4 * max(io["iters_per_step"])
+    assert relerr(o.get("u"), oj.get("u")) < 1e-7                     # the preconditioner changes the path to the solution, not the solution
+    g.close()
+
+
 @pytest.mark.parametrize("nu", [(1, 1, 16), (3, 2, 8), (0, 2, 4), (2, 2, 0)])
 def test_gmg_vcycle_other_smoothing_counts(fs, nu):
     # V(nu1, nu2) other than the fused V(2,2) fast path: the generic per-sweep kernels (fs_kernels_mg.cu), incl. nu1 = 0
