@@ -54,6 +54,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-profile", action="store_true")
+    ap.add_argument("--precond", default=None, choices=["none", "jacobi", "gmg"],
+                    help="override the workload's Poisson preconditioner (context runs: e.g. c3 with the multigrid of reading G1)")
     ap.add_argument("--traffic-from", nargs="+", metavar="DTYPE=RAW.CSV", help="write profiles/r2_traffic.csv from ncu raw CSV dumps (no GPU run)")
     return ap.parse_args()
 
@@ -268,7 +270,7 @@ def measure(a, dtype, dev, local, rank, world, dist, with_e2e, with_profile):
     if a.workload == "c5":
         cfg = W.hit(n=n, dtype=dtype, device=dev, exec_mode=a.exec_mode)   # seeded IC, built with torch FFT on the device
     else:
-        cfg = W.make(a.workload, dtype=dtype, exec_mode=a.exec_mode)
+        cfg = W.make(a.workload, dtype=dtype, exec_mode=a.exec_mode, **({"precond": a.precond} if a.precond else {}))
     cells = cfg["nx"] * cfg["ny"] * cfg["nz"]
     g = fs.from_workload(cfg, device=dev)
     cfg["init"] = None
