@@ -176,3 +176,26 @@ def test_full_size_full_step_count_against_oracle_pins(fs, case):
     for k in ("body_force", "body_disp", "body_vel"):
         np.testing.assert_allclose(ig[k], P[k], rtol=1e-9, atol=1e-12)
     g.close()
+
+
+# ---- a property that holds at any size: the path is deterministic.  Every reduction is added in a fixed order (ticketed
+#      partials), the IBM spread walks sorted cell lists, so two runs from the same state agree BIT FOR BIT; a
+#      race in a shared-memory ring, a prefetch that lands late or a barrier that lets a CTA through early shows up as a
+#      differing word.  Run in the launch configurations bench.py times (c5 at 512^3 in both precisions, CUDA-graph steps;
+#      the cooperative whole-solve kernel on c3 / c4 at their stated sizes).
+@pytest.mark.parametrize("case,dtype,steps", [("c5", "f64", 2), ("c5", "f32", 2), ("c3", "f64", 3), ("c4", "f64", 3), ("c2", "f64", 2)])
+def test_two_runs_from_the_same_state_agree_bit_for_bit(fs, case, dtype, steps):
+    runs = []
+    for rep in range(2):
+        cfg = W.make(case, device="cuda:0") if case == "c5" else W.make(case)
+        g = fs.from_workload(cfg, device="cuda:0", dtype=dtype)
+        info = g.step(steps, per_step=True)
+        assert info["nan_flag"] == 0 and info["converged"] == 1, info
+        runs.append((info, {c: g.get(c) for c in "uvwp"}))
+        g.close()
+    (ia, fa), (ib, fb) = runs
+    assert ia["iters_per_step"] == ib["iters_per_step"], (ia["iters_per_step"], ib["iters_per_step"])
+    for k in ("rel_residual", "max_abs_div", "body_force", "body_disp", "body_vel"):
+        assert np.array_equal(np.asarray(ia[k]), np.asarray(ib[k])), (case, k, ia[k], ib[k])
+    for c in "uvwp":
+        assert np.array_equal(fa[c], fb[c]), (case, dtype, c, float(np.abs(fa[c] - fb[c]).max()))
