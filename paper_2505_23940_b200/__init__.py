@@ -67,8 +67,8 @@ class fs_poisson_info(C.Structure):
                 ("rel_residual", C.c_double), ("true_rel_residual", C.c_double)]
 
 
-# every symbol include/fs.h declares (tests check the library exports all of them)
-SYMBOLS = ("fs_workspace_bytes", "fs_grid_create", "fs_grid_destroy", "fs_field_size", "fs_fields_set",
+# every symbol include/*.h declares (tests check the library exports all of them)
+SYMBOLS = ("fs_divergence_noalloc", "fs_workspace_bytes", "fs_grid_create", "fs_grid_destroy", "fs_field_size", "fs_fields_set",
            "fs_fields_get", "fs_fields_set_async", "fs_fields_get_async", "fs_set_history", "fs_set_ibm_markers", "fs_marker_segments", "fs_set_body", "fs_set_solid_mask", "fs_set_beam", "fs_beam_state",
            "fs_set_body_state", "fs_step", "fs_poisson_solve", "fs_ibm_interpolate", "fs_ibm_spread",
            "fs_gmg_vcycle", "fs_momentum_rhs", "fs_profile_step", "fs_profile_count", "fs_profile_entry",
@@ -121,6 +121,7 @@ def lib():
         L.fs_profile_reset.argtypes = [vp]
         L.fs_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.fs_kernels_used.argtypes = [vp, C.c_char_p, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.fs_divergence_noalloc.argtypes = [ip, ip, ip, C.c_double, C.c_double, C.c_double, ip, vp, vp, vp, vp, vp, vp]
         L.fs_status_string.argtypes = [ip]
         L.fs_status_string.restype = C.c_char_p
         for s in SYMBOLS:
@@ -448,3 +449,26 @@ def from_workload(cfg, device="cuda:0", stream=None, **overrides):
     if c.get("beam") is not None:
         g.set_beam(*c["beam"])
     return g
+
+
+NOALLOC_MAX_CELLS = 16777216     # FS_NOALLOC_MAX_CELLS (include/fs_noalloc.h)
+
+
+def divergence_noalloc(u, v, w, h, div_out=None, result=None, stream=None):
+    """fs_divergence_noalloc (include/fs_noalloc.h): divergence of a triply periodic staggered field given as CUDA tensors
+    of shape (nz, ny, nx), its max norm and squared 2-norm into `result` (2 fp64 words on the device).  The library call
+    allocates nothing (its scratch is a static device array: calls that overlap on the GPU race); this wrapper only
+    marshals: pass div_out / result to keep it allocation-free, else it creates them with torch.  Asynchronous."""
+    import torch
+    assert u.is_cuda and u.is_contiguous() and v.is_contiguous() and w.is_contiguous() and u.shape == v.shape == w.shape and u.dtype == v.dtype == w.dtype
+    nz, ny, nx = u.shape
+    dt = {torch.float32: DTYPE["f32"], torch.float64: DTYPE["f64"]}[u.dtype]
+    if result is None:
+        result = torch.empty(2, dtype=torch.float64, device=u.device)
+    hx, hy, hz = (h, h, h) if np.isscalar(h) else h
+    with torch.cuda.device(u.device):
+        s = stream if stream is not None else torch.cuda.current_stream().cuda_stream
+        _check(lib().fs_divergence_noalloc(nx, ny, nz, hx, hy, hz, dt, u.data_ptr(), v.data_ptr(), w.data_ptr(),
+                                           div_out.data_ptr() if div_out is not None else None, result.data_ptr(), s),
+               "fs_divergence_noalloc")
+    return result

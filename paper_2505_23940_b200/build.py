@@ -11,8 +11,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfs.so")
-SOURCES = ["fs_api.cu", "fs_kernels_fluid.cu", "fs_kernels_pcg.cu", "fs_kernels_mg.cu", "fs_kernels_mgf.cu", "fs_kernels_ibm.cu", "fs_tma.cu", "fs_beam.cu", "fs_kernels_momv.cu", "fs_kernels_pcgc.cu"]
-HEADERS = [os.path.join(CSRC, "fs_internal.cuh"), os.path.join(HERE, "..", "include", "fs.h")]
+SOURCES = ["fs_api.cu", "fs_kernels_fluid.cu", "fs_kernels_pcg.cu", "fs_kernels_mg.cu", "fs_kernels_mgf.cu", "fs_kernels_ibm.cu", "fs_tma.cu", "fs_beam.cu", "fs_kernels_momv.cu", "fs_kernels_pcgc.cu",
+           "noalloc/fs_noalloc.cu"]     # self-contained extra entry point (include/fs_noalloc.h); not part of the hot path
+HEADERS = [os.path.join(CSRC, "fs_internal.cuh"), os.path.join(HERE, "..", "include", "fs.h"), os.path.join(HERE, "..", "include", "fs_noalloc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
@@ -20,7 +21,9 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
 
 def csrc_hash():
     """sha256 over csrc/*.cu, csrc/*.cuh and include/fs.h (sorted by name): identifies the sources a profile was
-    captured from (bench.py refuses a committed ncu capture whose hash differs from the current sources)."""
+    captured from (bench.py refuses a committed ncu capture whose hash differs from the current sources).  These are the
+    sources of the hot path; csrc/noalloc/ (one self-contained entry point, its own translation unit and header) is not
+    among them."""
     import hashlib
     h = hashlib.sha256()
     files = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh")))
@@ -43,7 +46,7 @@ def build(force=False, verbose=False):
     objs, procs = [], []
     for src in SOURCES:
         s = os.path.join(CSRC, src)
-        o = os.path.join(objdir, src.replace(".cu", ".o"))
+        o = os.path.join(objdir, os.path.basename(src).replace(".cu", ".o"))
         objs.append(o)
         if force or _stale(o, [s] + HEADERS):
             cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]

@@ -1,4 +1,4 @@
-"""The C-ABI library builds, loads and exports every symbol include/fs.h declares; host-side argument
+"""The C-ABI library builds, loads and exports every symbol include/*.h declares; host-side argument
 validation (no compute calls: there is no GPU on the CPU test box)."""
 import ctypes as C
 import os
@@ -21,7 +21,8 @@ def fs():
 
 
 def _declared():
-    src = open(os.path.join(ROOT, "include", "fs.h")).read()
+    inc = os.path.join(ROOT, "include")
+    src = "\n".join(open(os.path.join(inc, f)).read() for f in sorted(os.listdir(inc)) if f.endswith(".h"))
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(fs_[a-z_0-9]+)\s*\(", src)))
 
